@@ -1,0 +1,157 @@
+/* hawkes.h -- C ABI of the B200-native phylogenetic-Hawkes likelihood library.
+ *
+ * The library evaluates, on one NVIDIA B200 (sm_100a) in fp64, the hot path of the phylogenetic
+ * Hawkes process of Holbrook, Ji & Suchard (arXiv 2103.03348; "PAPER.md" below):
+ *
+ *   lambda_n = sum_{n'} [ B_{nn'} + theta_{n'} k_{nn'} ]                        PAPER.md:60, 78 (Eq. 1)
+ *   B_{nn'}  = mu0 tau_x^-D tau_t^-1 phi_D((x_n-x_n')/tau_x) phi_1((t_n-t_n')/tau_t) I[x_n != x_n']
+ *   k_{nn'}  = xi0 omega h^-D exp(-omega (t_n-t_n')) phi_D((x_n-x_n')/h) I[t_n' < t_n]
+ *   ell      = sum_n log lambda_n - Lambda(t_N)                                  PAPER.md:76 (Eq. 1)
+ *   Lambda   = mu0 sum_n [Phi((t_N-t_n)/tau_t) - Phi(-t_n/tau_t)]
+ *            + xi0 sum_n theta_n (1 - exp(-omega (t_N-t_n)))                     PAPER.md:72; Eq. 7, l.253
+ *   d ell/d theta_m    = sum_{t_m<t_n} k_{nm}/lambda_n - xi0 (1 - e^{-omega (t_N-t_m)})   Eq. 4, l.137
+ *   d2 ell/d theta_m^2 = - sum_{t_m<t_n} (k_{nm}/lambda_n)^2                              Eq. 5, l.143
+ *
+ * plus the gradient and Hessian with respect to the six hyperparameters (mu0, tau_x, tau_t, xi0, h,
+ * omega) -- always in that order -- that BASELINE.json's north_star adds (the paper samples them by
+ * Metropolis-Hastings; the derivative formulas are in DESIGN.md).  phi_D / Phi are the
+ * standard normal pdf in D dimensions / cdf.  The time-Gaussian factor of the background
+ * is north_star's (the paper's background is space-only): DESIGN.md reading R1.
+ *
+ * Conventions (all entry points)
+ *  - Events are time-sorted: t[0] <= t[1] <= ... <= t[n-1]; t_N = t[n-1].  Ties are
+ *    allowed and do not excite each other (strict '<').
+ *  - x is SoA fp64: x[d*n + i] is coordinate d of event i, d < dim, dim in {1,2,3}.  theta[i] >= 0.
+ *  - Unless an entry point says HOST, every data/output pointer is a DEVICE pointer to fp64 memory on
+ *    the context's device, owned by the caller, and is not retained after the work queued on `stream`
+ *    completes.  `p` is always a HOST pointer and is read before the call returns.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls only enqueue
+ *    work; they never synchronise and never allocate.  One context serves one stream at a time.
+ *  - A NULL output pointer means "not wanted".
+ *  - Return value: 0 = HAWKES_OK; < 0 = error detected on the host, nothing was enqueued or written.
+ *    Conditions that depend on the data (unsorted times, non-finite input, a zero rate) are detected
+ *    on the device and reported by hawkes_last_status().
+ *  - Results are bit-identical from run to run for identical inputs (fixed tile -> partial -> reduce
+ *    order, no floating-point atomics).
+ *  - Exponentials whose value is below 2^-1020 are flushed to zero (reading R15), and the
+ *    indicator I[x_n != x_n'] is evaluated as |x_n - x_n'|^2 != 0 in fp64 (reading R3).
+ */
+#ifndef HAWKES_B200_H
+#define HAWKES_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+    double mu0;    /* background weight                        > 0 */
+    double tau_x;  /* background spatial bandwidth             > 0 */
+    double tau_t;  /* background temporal bandwidth            > 0 */
+    double xi0;    /* self-excitation weight (paper: theta_0)  > 0 */
+    double h;      /* self-excitation spatial bandwidth        > 0 */
+    double omega;  /* self-excitation decay rate (1/time)      > 0 */
+} hawkes_params;
+
+typedef struct hawkes_ctx hawkes_ctx; /* opaque; owns device scratch memory only */
+
+/* status codes */
+enum {
+    HAWKES_OK = 0,
+    HAWKES_ERR_ARG = -1,         /* NULL/negative/oversized argument, n > n_max, dim mismatch     */
+    HAWKES_ERR_PARAM = -2,       /* a hyperparameter is not finite and > 0                          */
+    HAWKES_ERR_UNSORTED = -3,    /* device-detected: t is not non-decreasing                        */
+    HAWKES_ERR_CUDA = -4,        /* a CUDA call failed (no device, launch failure, ...)             */
+    HAWKES_ERR_NOMEM = -5,       /* scratch allocation failed                                       */
+    HAWKES_ERR_UNSUPPORTED = -6, /* dim not in {1,2,3}; dense Hessian with n > 4096                 */
+    HAWKES_ERR_NONFINITE = -7,   /* device-detected: NaN/Inf in x, t or theta, or theta < 0         */
+    HAWKES_WARN_ZERO_RATE = 1    /* device-detected: some lambda_n == 0 => ll = -inf, entries that
+                                    divide by that lambda_n are NaN (always so for n == 1)          */
+};
+
+/* `want` bits of hawkes_eval */
+enum {
+    HAWKES_WANT_LL = 1,
+    HAWKES_WANT_GRAD_THETA = 2,
+    HAWKES_WANT_GRAD_HYPER = 4,
+    HAWKES_WANT_HESS_THETA = 8,
+    HAWKES_WANT_HESS_HYPER = 16,
+    HAWKES_WANT_HESS_CROSS = 32
+};
+
+/* Create a context for problems of up to n_max events in `dim` dimensions on CUDA device `device`;
+ * allocates all scratch (about 200 B per event + 60 MB) once.  *out is set only on success. */
+int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device);
+void hawkes_destroy(hawkes_ctx* ctx);
+const char* hawkes_strerror(int status);
+
+/* Synchronises `stream` and returns the data-dependent status of the most recent evaluation queued
+ * on this context: 0, HAWKES_WARN_ZERO_RATE, HAWKES_ERR_UNSORTED or HAWKES_ERR_NONFINITE (errors win
+ * over warnings).  When it returns an error the outputs of that evaluation are unspecified. */
+int hawkes_last_status(hawkes_ctx* ctx, void* stream);
+
+/* ell (Eq. 1).  ll: 1 double. */
+int hawkes_loglik(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                  const hawkes_params* p /*HOST*/, double* ll, void* stream);
+
+/* ell, d ell/d theta (Eq. 4; all n entries, w.r.t. theta itself) and d ell/d(mu0,tau_x,tau_t,xi0,h,omega).
+ * grad_theta: n doubles; grad_hyper: 6 doubles. */
+int hawkes_grad(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                const hawkes_params* p /*HOST*/, double* ll, double* grad_theta, double* grad_hyper,
+                void* stream);
+
+/* Second derivatives of ell (true sign: the theta-diagonal is <= 0; the paper's preconditioner is its
+ * negative).  hess_theta_diag: n doubles, d2 ell/d theta_m^2 (Eq. 5).  hess_hyper: 36
+ * doubles, row-major symmetric 6x6.  hess_cross: n*6 doubles row-major, d2 ell/d theta_m d p. */
+int hawkes_hessian(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                   const hawkes_params* p /*HOST*/, double* hess_theta_diag, double* hess_hyper,
+                   double* hess_cross, void* stream);
+
+/* One fused evaluation sharing the two pairwise passes across all requested outputs (what an HMC
+ * leapfrog step and the benchmark call).  `want` selects outputs; a wanted output whose pointer is
+ * NULL is HAWKES_ERR_ARG.  Outputs not selected are not touched. */
+int hawkes_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                const hawkes_params* p /*HOST*/, uint32_t want, double* ll, double* grad_theta,
+                double* grad_hyper, double* hess_theta_diag, double* hess_hyper, double* hess_cross,
+                void* stream);
+
+/* The same evaluation with HOST buffers on both sides (pinned or pageable): copies x, t, theta to the
+ * device, evaluates, copies the selected outputs back, all on `stream`, and synchronises `stream`
+ * before returning.  Returns the host status or, if that is 0, the device status of the evaluation. */
+int hawkes_eval_host(hawkes_ctx* ctx, int64_t n, const double* x /*HOST*/, const double* t /*HOST*/,
+                     const double* theta /*HOST*/, const hawkes_params* p /*HOST*/, uint32_t want,
+                     double* ll /*HOST*/, double* grad_theta /*HOST*/, double* grad_hyper /*HOST*/,
+                     double* hess_theta_diag /*HOST*/, double* hess_hyper /*HOST*/,
+                     double* hess_cross /*HOST*/, void* stream);
+
+/* Correctness-only, n <= 4096: the dense block d2 ell/d theta_m d theta_m' = - sum_n k_nm k_nm' /
+ * lambda_n^2 (Lambda is linear in theta), row-major n*n doubles.  Uses n*n*8 bytes of caller memory
+ * only (hess_theta itself is the scratch). */
+int hawkes_hessian_theta_dense(hawkes_ctx* ctx, int64_t n, const double* x, const double* t,
+                               const double* theta, const hawkes_params* p /*HOST*/,
+                               double* hess_theta, void* stream);
+
+/* Helper, not on the hot path: stable argsort of the events by time and gather into SoA outputs
+ * (x_out[dim*n], t_out[n], theta_out[n]); perm[i] = input index of output event i (int64).
+ * Inputs and outputs must not alias. */
+int hawkes_sort_events(hawkes_ctx* ctx, int64_t n, int dim, const double* x_in, const double* t_in,
+                       const double* theta_in, double* x_out, double* t_out, double* theta_out,
+                       int64_t* perm, void* stream);
+
+/* After an evaluation queued on this context has been enqueued: copies of the per-event rates
+ * lambda_n (n doubles) into a caller buffer, on `stream`.  For tests and diagnostics. */
+int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stream);
+
+/* Launch bookkeeping for benchmarks: number of kernels this context has launched since creation. */
+int64_t hawkes_launch_count(const hawkes_ctx* ctx);
+
+/* Measures the fp64 FMA issue peak of the device with a register-resident DFMA-chain kernel run for
+ * about `millis` milliseconds on `stream`; returns DFMA TFLOP/s (2 flops per FMA) in *tflops.
+ * Synchronises.  Used by bench.py for the measured roofline denominator. */
+int hawkes_fp64_peak(hawkes_ctx* ctx, double millis, double* tflops /*HOST*/, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HAWKES_B200_H */

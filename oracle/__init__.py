@@ -20,7 +20,7 @@ def lib():
     if _lib is None:
         _lib = ctypes.CDLL(_build.build())
         _lib.hawkes_ref_eval.restype = ctypes.c_int
-        _lib.hawkes_ref_eval.argtypes = [ctypes.c_int64, ctypes.c_int] + [_dp] * 13 + [ctypes.c_int]
+        _lib.hawkes_ref_eval.argtypes = [ctypes.c_int64, ctypes.c_int] + [_dp] * 14 + [ctypes.c_int]
         _lib.hawkes_ref_rows.restype = ctypes.c_int
         _lib.hawkes_ref_rows.argtypes = [ctypes.c_int64, ctypes.c_int, _dp, _dp, _dp, _dp,
                                          ctypes.c_int64, _ip, _dp, _dp, ctypes.c_int]
@@ -51,10 +51,11 @@ class RefResult:
     hess_hyper: np.ndarray | None = None
     hess_cross: np.ndarray | None = None
     hess_theta_dense: np.ndarray | None = None
+    row_d1: np.ndarray | None = None
 
 
 def evaluate(x, t, theta, params, *, grad=True, hess=False, cross=False, dense=False,
-             threads: int = 1) -> RefResult:
+             row_d1=False, threads: int = 1) -> RefResult:
     """x: [dim, n] SoA; t: [n] sorted; theta: [n]; params: 6 floats.  Always returns ll, the
     integral Lambda(t_N) and lambda[n]; gradient / Hessian pieces on request."""
     x = np.ascontiguousarray(x, dtype=np.float64)
@@ -71,15 +72,17 @@ def evaluate(x, t, theta, params, *, grad=True, hess=False, cross=False, dense=F
     hhy = np.zeros(36) if hess else None
     hcr = np.zeros(n * 6) if cross else None
     hde = np.zeros(n * n) if dense else None
+    rd1 = np.zeros(n * 6) if row_d1 else None
     st = lib().hawkes_ref_eval(n, dim, _p(x), _p(t), _p(theta), _p(prm), _p(ll), _p(integ), _p(lam),
-                               _p(gth), _p(ghy), _p(hth), _p(hhy), _p(hcr), _p(hde), threads)
+                               _p(gth), _p(ghy), _p(hth), _p(hhy), _p(hcr), _p(hde), _p(rd1), threads)
     if st < 0:
         raise ValueError(f"hawkes_ref_eval: bad argument (status {st})")
     return RefResult(status=st, ll=float(ll[0]), integral=float(integ[0]), lam=lam, grad_theta=gth,
                      grad_hyper=ghy, hess_theta_diag=hth,
                      hess_hyper=None if hhy is None else hhy.reshape(6, 6),
                      hess_cross=None if hcr is None else hcr.reshape(n, 6),
-                     hess_theta_dense=None if hde is None else hde.reshape(n, n))
+                     hess_theta_dense=None if hde is None else hde.reshape(n, n),
+                     row_d1=None if rd1 is None else rd1.reshape(n, 6))
 
 
 def rows(x, t, theta, params, idx, *, derivs=True, threads: int = 1):

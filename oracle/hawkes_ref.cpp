@@ -164,11 +164,13 @@ extern "C" {
 //   x[dim*n] SoA (x[d*n+i]), t[n] non-decreasing, theta[n], params[6] = (mu0,tau_x,tau_t,xi0,h,omega)
 //   ll[1], integral[1] (= Lambda(t_N)), lambda[n], grad_theta[n], grad_hyper[6],
 //   hess_theta_diag[n], hess_hyper[36] row-major, hess_cross[n*6] row-major (m, p),
-//   hess_theta_dense[n*n] row-major (small n only; O(n^3)).
+//   hess_theta_dense[n*n] row-major (small n only; O(n^3)),
+//   row_d1[n*6] row-major: d lambda_n / dp (intermediate, for error scales in the parity tests).
 int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const double* theta,
                     const double* params, double* ll, double* integral, double* lambda,
                     double* grad_theta, double* grad_hyper, double* hess_theta_diag,
-                    double* hess_hyper, double* hess_cross, double* hess_theta_dense, int threads) {
+                    double* hess_hyper, double* hess_cross, double* hess_theta_dense, double* row_d1,
+                    int threads) {
     if (n < 1 || dim < 1 || dim > 3 || !x || !t || !theta || !params) return -1;
     for (int i = 0; i < 6; ++i)
         if (!(params[i] > 0.0) || !std::isfinite(params[i])) return -2;
@@ -176,7 +178,7 @@ int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const 
         if (t[i] < t[i - 1]) return -3;
     const P p = make_params(params, dim);
     const int64_t N = n;
-    const bool want_hyper = grad_hyper || hess_hyper || hess_cross;
+    const bool want_hyper = grad_hyper || hess_hyper || hess_cross || row_d1;
     const bool want_cols = grad_theta || hess_theta_diag || hess_cross || hess_theta_dense;
     (void)threads;
 #ifdef _OPENMP
@@ -199,6 +201,8 @@ int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const 
     for (int64_t i = 0; i < N; ++i) {
         if (lam[i] == 0) status = 1;
         if (lambda) lambda[i] = (double)lam[i];
+        if (row_d1)
+            for (int a = 0; a < 6; ++a) row_d1[i * 6 + a] = (double)rows[i].d1[a];
     }
 
     // ---- integral Lambda(t_N) and its derivatives ----

@@ -1,0 +1,200 @@
+"""paper_2103_03348_b200 -- thin Python binding of the B200-native phylogenetic-Hawkes likelihood
+library (include/hawkes.h).  Argument marshalling only: every step of the evaluation runs in the
+CUDA kernels of csrc/hawkes.cu; PyTorch supplies device memory and the stream.  There is no CPU
+fallback -- without the CUDA library (or without a GPU) the calls fail."""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+
+from . import synth  # noqa: F401  (seeded inputs; no method arithmetic)
+from ._lib import Params, load, lib_path  # noqa: F401
+
+OK = 0
+ERR_ARG, ERR_PARAM, ERR_UNSORTED, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = -1, -2, -3, -4, -5, -6, -7
+WARN_ZERO_RATE = 1
+WANT_LL, WANT_GRAD_THETA, WANT_GRAD_HYPER, WANT_HESS_THETA, WANT_HESS_HYPER, WANT_HESS_CROSS = 1, 2, 4, 8, 16, 32
+WANT_GRAD = WANT_LL | WANT_GRAD_THETA | WANT_GRAD_HYPER
+WANT_ALL = 63
+
+
+class HawkesError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {load().hawkes_strerror(status).decode()} (status {status})")
+
+
+@dataclasses.dataclass
+class EvalResult:
+    """Device tensors (or host tensors for eval_host) of the requested outputs; None if not wanted."""
+    ll: object = None
+    grad_theta: object = None
+    grad_hyper: object = None
+    hess_theta_diag: object = None
+    hess_hyper: object = None
+    hess_cross: object = None
+    status: int | None = None
+
+
+def _params(p) -> Params:
+    if isinstance(p, Params):
+        return p
+    return Params(*[float(v) for v in p])
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+class HawkesContext:
+    """Owns one hawkes_ctx (device scratch for problems of up to n_max events in `dim` dimensions)."""
+
+    def __init__(self, n_max: int, dim: int = 2, device: int = 0):
+        import torch
+        self._torch = torch
+        self._lib = load()
+        self.n_max, self.dim, self.device = int(n_max), int(dim), int(device)
+        h = ctypes.c_void_p()
+        rc = self._lib.hawkes_create(ctypes.byref(h), self.n_max, self.dim, self.device)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_create")
+        self._h = h
+        self._dev = torch.device("cuda", self.device)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.hawkes_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _stream(self):
+        return ctypes.c_void_p(self._torch.cuda.current_stream(self._dev).cuda_stream)
+
+    def _check_inputs(self, x, t, theta):
+        torch = self._torch
+        for a in (x, t, theta):
+            if a.dtype != torch.float64 or not a.is_contiguous():
+                raise ValueError("x, t, theta must be contiguous float64 tensors")
+        n = t.shape[0]
+        if x.shape != (self.dim, n) or theta.shape != (n,):
+            raise ValueError("expected x [dim, n] (SoA), t [n], theta [n]")
+        return n
+
+    def _outputs(self, n, want, device):
+        torch = self._torch
+        mk = lambda *s: torch.empty(*s, dtype=torch.float64, device=device)
+        return EvalResult(
+            ll=mk(1) if want & WANT_LL else None,
+            grad_theta=mk(n) if want & WANT_GRAD_THETA else None,
+            grad_hyper=mk(6) if want & WANT_GRAD_HYPER else None,
+            hess_theta_diag=mk(n) if want & WANT_HESS_THETA else None,
+            hess_hyper=mk(6, 6) if want & WANT_HESS_HYPER else None,
+            hess_cross=mk(n, 6) if want & WANT_HESS_CROSS else None)
+
+    # -- the C-ABI calls ---------------------------------------------------------------------------
+    def eval(self, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None) -> EvalResult:
+        """hawkes_eval: device tensors in, device tensors out, asynchronous on the current stream."""
+        n = self._check_inputs(x, t, theta)
+        if not x.is_cuda:
+            raise ValueError("eval() takes CUDA tensors; use eval_host() for host buffers")
+        r = out if out is not None else self._outputs(n, want, self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_eval(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want,
+                                   _ptr(r.ll), _ptr(r.grad_theta), _ptr(r.grad_hyper), _ptr(r.hess_theta_diag),
+                                   _ptr(r.hess_hyper), _ptr(r.hess_cross), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_eval")
+        return r
+
+    def loglik(self, x, t, theta, params):
+        n = self._check_inputs(x, t, theta)
+        r = self._outputs(n, WANT_LL, self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_loglik(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), _ptr(r.ll), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_loglik")
+        return r.ll
+
+    def grad(self, x, t, theta, params) -> EvalResult:
+        n = self._check_inputs(x, t, theta)
+        r = self._outputs(n, WANT_GRAD, self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_grad(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), _ptr(r.ll),
+                                   _ptr(r.grad_theta), _ptr(r.grad_hyper), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_grad")
+        return r
+
+    def hessian(self, x, t, theta, params, cross: bool = False) -> EvalResult:
+        n = self._check_inputs(x, t, theta)
+        want = WANT_HESS_THETA | WANT_HESS_HYPER | (WANT_HESS_CROSS if cross else 0)
+        r = self._outputs(n, want, self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_hessian(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p),
+                                      _ptr(r.hess_theta_diag), _ptr(r.hess_hyper), _ptr(r.hess_cross), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_hessian")
+        return r
+
+    def eval_host(self, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None) -> EvalResult:
+        """hawkes_eval_host: HOST tensors (pinned or pageable) in and out; copies run inside the call,
+        which synchronises the stream and returns the evaluation's device status in `.status`."""
+        n = self._check_inputs(x, t, theta)
+        if x.is_cuda:
+            raise ValueError("eval_host() takes host tensors")
+        r = out if out is not None else self._outputs(n, want, "cpu")
+        p = _params(params)
+        rc = self._lib.hawkes_eval_host(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want,
+                                        _ptr(r.ll), _ptr(r.grad_theta), _ptr(r.grad_hyper), _ptr(r.hess_theta_diag),
+                                        _ptr(r.hess_hyper), _ptr(r.hess_cross), self._stream())
+        if rc < 0:
+            raise HawkesError(rc, "hawkes_eval_host")
+        r.status = rc
+        return r
+
+    def hessian_theta_dense(self, x, t, theta, params):
+        n = self._check_inputs(x, t, theta)
+        H = self._torch.empty(n, n, dtype=self._torch.float64, device=self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_hessian_theta_dense(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), _ptr(H), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_hessian_theta_dense")
+        return H
+
+    def sort_events(self, x, t, theta):
+        """Stable sort by time on the device; returns (x_sorted, t_sorted, theta_sorted, perm)."""
+        torch = self._torch
+        n = self._check_inputs(x, t, theta)
+        xo, to, tho = torch.empty_like(x), torch.empty_like(t), torch.empty_like(theta)
+        perm = torch.empty(n, dtype=torch.int64, device=self._dev)
+        rc = self._lib.hawkes_sort_events(self._h, n, self.dim, _ptr(x), _ptr(t), _ptr(theta), _ptr(xo), _ptr(to),
+                                          _ptr(tho), _ptr(perm), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_sort_events")
+        return xo, to, tho, perm
+
+    def get_lambda(self, n: int):
+        lam = self._torch.empty(n, dtype=self._torch.float64, device=self._dev)
+        rc = self._lib.hawkes_get_lambda(self._h, n, _ptr(lam), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_get_lambda")
+        return lam
+
+    def last_status(self) -> int:
+        return int(self._lib.hawkes_last_status(self._h, self._stream()))
+
+    def launch_count(self) -> int:
+        return int(self._lib.hawkes_launch_count(self._h))
+
+    def fp64_peak(self, millis: float = 200.0) -> float:
+        v = ctypes.c_double(0.0)
+        rc = self._lib.hawkes_fp64_peak(self._h, float(millis), ctypes.byref(v), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_fp64_peak")
+        return float(v.value)

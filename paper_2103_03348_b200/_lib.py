@@ -1,0 +1,64 @@
+"""Loader of the in-tree CUDA library.  There is no fallback: if the library cannot be loaded the
+import of the binding fails loudly."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+_dp = ctypes.c_void_p   # device or host pointer to fp64
+_lib = None
+
+# every symbol include/hawkes.h declares: name -> (restype, argtypes)
+i64, cint, u32, vp = ctypes.c_int64, ctypes.c_int, ctypes.c_uint32, ctypes.c_void_p
+
+
+class Params(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_double) for k in ("mu0", "tau_x", "tau_t", "xi0", "h", "omega")]
+
+
+PP = ctypes.POINTER(Params)
+SYMBOLS = {
+    "hawkes_create": (cint, [ctypes.POINTER(vp), i64, cint, cint]),
+    "hawkes_destroy": (None, [vp]),
+    "hawkes_strerror": (ctypes.c_char_p, [cint]),
+    "hawkes_last_status": (cint, [vp, vp]),
+    "hawkes_loglik": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, vp]),
+    "hawkes_grad": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, _dp, _dp, vp]),
+    "hawkes_hessian": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, _dp, _dp, vp]),
+    "hawkes_eval": (cint, [vp, i64, _dp, _dp, _dp, PP, u32, _dp, _dp, _dp, _dp, _dp, _dp, vp]),
+    "hawkes_eval_host": (cint, [vp, i64, _dp, _dp, _dp, PP, u32, _dp, _dp, _dp, _dp, _dp, _dp, vp]),
+    "hawkes_hessian_theta_dense": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, vp]),
+    "hawkes_sort_events": (cint, [vp, i64, cint, _dp, _dp, _dp, _dp, _dp, _dp, vp, vp]),
+    "hawkes_get_lambda": (cint, [vp, i64, _dp, vp]),
+    "hawkes_launch_count": (i64, [vp]),
+    "hawkes_fp64_peak": (cint, [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]),
+}
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load():
+    """Load (building first if the .so is missing or stale and nvcc is available)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not _build.up_to_date():
+        try:
+            _build.build()
+        except Exception as exc:   # no nvcc on this machine, or compile error
+            if not os.path.exists(path):
+                raise ImportError(
+                    f"paper_2103_03348_b200: CUDA library {path} is missing and could not be built "
+                    f"({exc}); run `python -m paper_2103_03348_b200.build` on a machine with nvcc") from exc
+    lib = ctypes.CDLL(path)
+    for name, (res, args) in SYMBOLS.items():
+        fn = getattr(lib, name)   # AttributeError if the symbol is not exported
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib

@@ -1,0 +1,1131 @@
+// hawkes.cu -- B200 (sm_100a) kernels and C ABI of the phylogenetic-Hawkes likelihood library.
+// The contract of every entry point is in include/hawkes.h; the design (data layout, kernels,
+// rooflines, readings of the paper) is in DESIGN.md.  PAPER.md = arXiv 2103.03348.
+//
+// Pipeline of one evaluation (all on the caller's stream, no host synchronisation):
+//   prep      O(N)   validate, pack events into 32-byte records (x, y, t, theta)           [a0]
+//   pass1     O(N^2) per target n: raw moment sums of the background and excitation terms [a1]
+//   reduce1   O(N)   lambda_n, 1/lambda_n, per-event log/gradient/Hessian/integral terms  [a2, a3]
+//   scalars   O(N/256) fixed-order reduction -> ll, grad_hyper, hess_hyper                [a5]
+//   pass2     O(N^2/2) per source m: c_m = sum k_nm/lambda_n, d_m = sum (k_nm/lambda_n)^2  [a4]
+//   theta     O(N)   grad_theta, hess_theta_diag (and the cross block)                    [a5]
+// (step names a0..a5 are SURVEY.md section 8(a)'s).
+//
+// fp64 exp: every kernel term is 2^z with z = -(scaled squared distances); z is split as
+// z = n/128 + f, n integer, |f| <= 1/256;  2^z = 2^(n>>7) * T[n&127] * p(f)  with T a 128-entry table
+// replicated 16x in shared memory (bank-conflict-free for any index pattern) and p a degree-4
+// polynomial: 8 FP64-pipe instructions per exponential instead of the ~15-18 of exp(double).
+#include "../../include/hawkes.h"
+
+#include <cuda_runtime.h>
+#include <cub/device/device_radix_sort.cuh>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <new>
+
+#include "exp2_consts.inc"
+
+namespace {
+
+constexpr int NT = 128;        // threads per CTA in the pairwise kernels
+constexpr int TS = 128;        // events per streamed shared-memory tile
+constexpr int TAB_N = 1 << HAWKES_EXP2_TBITS;
+constexpr int TAB_REP = 16;    // replicas of the exp2 table (one per lane of a half-warp)
+constexpr int RED_T = 256;     // threads per CTA in the O(N) kernels
+constexpr int NRED = 34;       // per-event scalar sums reduced over n (see reduce1_kernel)
+constexpr int P1_ITEMS_TARGET = 148 * 10;   // pass-1 work items aimed for (10 per SM)
+constexpr int P2_SLOTS_MAX = 16;            // pass-2 partial slots per source tile
+
+constexpr double MAGIC = 6755399441055744.0 / TAB_N;   // 1.5 * 2^52 / 128: ulp = 1/128
+
+// constants of one evaluation, passed by value to every kernel
+struct DevConsts {
+    double negcb;   // -log2(e) / (2 tau_x^2)
+    double rho_b;   // tau_x^2 / tau_t^2        : background exponent = negcb * (r2 + rho_b dt^2)
+    double negcs;   // -log2(e) / (2 h^2)
+    double rho_s;   // 2 h^2 omega              : excitation exponent = negcs * (r2 + rho_s dt)
+    double CB;      // mu0 (2 pi)^-(D+1)/2 tau_x^-D tau_t^-1
+    double CS;      // xi0 omega (2 pi)^-D/2 h^-D
+    double mu0, tau_x, tau_t, xi0, h, omega;
+    int lim_b_hi;   // hi word of the smallest argument whose background exponential is flushed to 0
+    int lim_s_hi;
+    int dim;
+};
+
+enum { ST_UNSORTED = 1, ST_NONFINITE = 2, ST_ZERO_RATE = 4 };
+
+// ------------------------------------------------------------------------------------------------
+// fp64 2^(a * negc) for a >= 0 (negc < 0); returns exactly 0 when hi(a) >= lim_hi or `kill`.
+// FP64 pipe: DFMA, DADD, DFMA (reduction), 4 DFMA (polynomial), DMUL = 8.  Everything else (index,
+// table load, exponent insertion, predicate) runs on the integer / load-store pipes:
+//   t = a*negc + MAGIC leaves n = round(128 z) in the low word of t (z = a*negc);  j = n & 127;
+//   the table entry is the bit pattern of 2^(j/128) with (j << 13) subtracted from its high word, so
+//   that adding (n << 13) = (k << 20) + (j << 13) to it multiplies by 2^k, k = n >> 7, in one integer op.
+// A lane whose term must vanish (underflow, coincident location, acausal pair) looks up n = N_DEAD
+// instead: entry 0 is 1.0 (zero mantissa) and k = -1023 cancels its exponent field, so the assembled
+// bit pattern is exactly +0.0 -- no select on the result.
+// `lane_addr` is the shared-space address of this lane's replica of entry 0 (table + 8 * (lane & 15)).
+constexpr int N_DEAD = -1023 * TAB_N;
+// KILL_MODE 0: no extra kill; 1: kill when kv == 0 (kv = r2, the coincident-location indicator);
+// 2: kill unless kv > 0 (kv = dt, the causal indicator; fp64 compare).
+template <int KILL_MODE>
+__device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi, double kv, unsigned lane_addr) {
+    const double t = fma(a, negc, MAGIC);
+    const double nf = t - MAGIC;
+    const double f = fma(a, negc, -nf);
+    double p = fma(f, HAWKES_EXP2_C4, HAWKES_EXP2_C3);
+    p = fma(p, f, HAWKES_EXP2_C2);
+    p = fma(p, f, HAWKES_EXP2_C1);
+    p = fma(p, f, 1.0);
+    double T;
+    if (KILL_MODE == 1) {
+        asm("{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 alo, ahi, n, thi, klo, khi, ne, j, ad, lo, hi;\n\t"
+            "mov.b64 {alo, ahi}, %1;\n\t"
+            "mov.b64 {n, thi}, %2;\n\t"
+            "mov.b64 {klo, khi}, %3;\n\t"
+            "or.b32 klo, klo, khi;\n\t"
+            "setp.ne.s32 p, klo, 0;\n\t"
+            "setp.lt.and.s32 p, ahi, %4, p;\n\t"
+            "selp.s32 ne, n, %5, p;\n\t"
+            "and.b32 j, ne, 127;\n\t"
+            "mad.lo.u32 ad, j, 128, %6;\n\t"
+            "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"
+            "mad.lo.s32 hi, ne, 8192, hi;\n\t"
+            "mov.b64 %0, {lo, hi};\n\t"
+            "}"
+            : "=d"(T) : "d"(a), "d"(t), "d"(kv), "r"(lim_hi), "n"(N_DEAD), "r"(lane_addr));
+    } else if (KILL_MODE == 2) {
+        asm("{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 alo, ahi, n, thi, ne, j, ad, lo, hi;\n\t"
+            "mov.b64 {alo, ahi}, %1;\n\t"
+            "mov.b64 {n, thi}, %2;\n\t"
+            "setp.gt.f64 p, %3, 0d0000000000000000;\n\t"
+            "setp.lt.and.s32 p, ahi, %4, p;\n\t"
+            "selp.s32 ne, n, %5, p;\n\t"
+            "and.b32 j, ne, 127;\n\t"
+            "mad.lo.u32 ad, j, 128, %6;\n\t"
+            "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"
+            "mad.lo.s32 hi, ne, 8192, hi;\n\t"
+            "mov.b64 %0, {lo, hi};\n\t"
+            "}"
+            : "=d"(T) : "d"(a), "d"(t), "d"(kv), "r"(lim_hi), "n"(N_DEAD), "r"(lane_addr));
+    } else {
+        asm("{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 alo, ahi, n, thi, ne, j, ad, lo, hi;\n\t"
+            "mov.b64 {alo, ahi}, %1;\n\t"
+            "mov.b64 {n, thi}, %2;\n\t"
+            "setp.lt.s32 p, ahi, %3;\n\t"
+            "selp.s32 ne, n, %4, p;\n\t"
+            "and.b32 j, ne, 127;\n\t"
+            "mad.lo.u32 ad, j, 128, %5;\n\t"
+            "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"
+            "mad.lo.s32 hi, ne, 8192, hi;\n\t"
+            "mov.b64 %0, {lo, hi};\n\t"
+            "}"
+            : "=d"(T) : "d"(a), "d"(t), "r"(lim_hi), "n"(N_DEAD), "r"(lane_addr));
+    }
+    return T * p;
+}
+
+// fill the 16x replicated table (entry j, replica r at tab[j*16 + r]) with the biased bit patterns
+// and return the table's shared-space address.
+__device__ __forceinline__ unsigned fill_table(double* tab, const double* __restrict__ tab_g) {
+    for (int i = threadIdx.x; i < TAB_N * TAB_REP; i += blockDim.x) {
+        const int j = i / TAB_REP;
+        const double v = tab_g[j];
+        tab[i] = __hiloint2double(__double2hiint(v) - (j << 13), __double2loint(v));
+    }
+    return (unsigned)__cvta_generic_to_shared(tab);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0: validate and pack.  rec[i] = (x0, x1, t, theta) for dim <= 2 (x1 = 0 for dim 1), or
+// (x0, x1, x2, t, theta, 0) for dim 3.
+__global__ void prep_kernel(int64_t n, int dim, const double* __restrict__ x, const double* __restrict__ t,
+                            const double* __restrict__ theta, double* __restrict__ rec,
+                            unsigned* __restrict__ status) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double ti = t[i], th = theta[i];
+    unsigned bad = 0;
+    if (i > 0 && ti < t[i - 1]) bad |= ST_UNSORTED;
+    if (!isfinite(ti) || !isfinite(th) || th < 0.0) bad |= ST_NONFINITE;
+    double xv[3] = {0.0, 0.0, 0.0};
+    for (int d = 0; d < dim; ++d) {
+        xv[d] = x[(int64_t)d * n + i];
+        if (!isfinite(xv[d])) bad |= ST_NONFINITE;
+    }
+    if (dim <= 2) {
+        double4* r4 = reinterpret_cast<double4*>(rec);
+        r4[i] = make_double4(xv[0], xv[1], ti, th);
+    } else {
+        double2* r2 = reinterpret_cast<double2*>(rec) + 3 * i;
+        r2[0] = make_double2(xv[0], xv[1]);
+        r2[1] = make_double2(xv[2], ti);
+        r2[2] = make_double2(th, 0.0);
+    }
+    if (bad) atomicOr(status, bad);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Streamed tile of TS records in shared memory, double-buffered through registers.
+template <bool DIM3>
+struct RecIO {
+    static constexpr int RS = DIM3 ? 6 : 4;                 // doubles per record
+    static constexpr int CH = RS / 2;                       // 16-byte chunks per record
+    static constexpr int PER_THREAD = TS * CH / NT;         // chunks each thread moves per tile
+    double2 v[PER_THREAD];
+    __device__ __forceinline__ void load(const double* __restrict__ src, int64_t first, int cnt) {
+        const double2* g = reinterpret_cast<const double2*>(src) + first * CH;
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int c = threadIdx.x + q * NT;
+            v[q] = (c < cnt * CH) ? __ldg(g + c) : make_double2(0.0, 0.0);
+        }
+    }
+    __device__ __forceinline__ void store(double* buf) const {
+        double2* s = reinterpret_cast<double2*>(buf);
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) s[threadIdx.x + q * NT] = v[q];
+    }
+};
+
+template <bool DIM3>
+struct Ev {   // one event held in registers: coordinates, time, and a weight (theta or 1/lambda)
+    double x, y, z, t, w;
+};
+
+template <bool DIM3>
+__device__ __forceinline__ Ev<DIM3> read_rec(const double* __restrict__ p) {
+    Ev<DIM3> e;
+    if (!DIM3) {
+        const double2 a = reinterpret_cast<const double2*>(p)[0];
+        const double2 b = reinterpret_cast<const double2*>(p)[1];
+        e.x = a.x; e.y = a.y; e.z = 0.0; e.t = b.x; e.w = b.y;
+    } else {
+        const double2 a = reinterpret_cast<const double2*>(p)[0];
+        const double2 b = reinterpret_cast<const double2*>(p)[1];
+        const double2 c = reinterpret_cast<const double2*>(p)[2];
+        e.x = a.x; e.y = a.y; e.z = b.x; e.t = b.y; e.w = c.x;
+    }
+    return e;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1: pass 1.  Thread owns R targets; sources stream through shared memory.
+// LEVEL 0: b0, s0                      (log-likelihood / theta-gradient only)
+// LEVEL 1: + b1, b2, s1, s2            (hyperparameter gradient)
+// LEVEL 2: + b3, b4, b5, s3, s4, s5    (hyperparameter Hessian)
+// with eB = exp(-r2/2tau_x^2 - dt^2/2tau_t^2) I[r2 != 0], eS = theta_n' exp(-omega dt - r2/2h^2) I[dt > 0]:
+//   b0 = sum eB      b1 = sum eB r2    b2 = sum eB dt^2   b3 = sum eB r2^2  b4 = sum eB r2 dt^2  b5 = sum eB dt^4
+//   s0 = sum eS      s1 = sum eS r2    s2 = sum eS dt     s3 = sum eS r2^2  s4 = sum eS r2 dt    s5 = sum eS dt^2
+template <int LEVEL>
+struct Mom {
+    static constexpr int NB = LEVEL == 0 ? 1 : (LEVEL == 1 ? 3 : 6);
+    double b[NB], s[NB];
+};
+
+// MODE 0: background only (all sources at or after the targets); 1: both terms, every pair causal;
+// 2: both terms with the per-pair test dt > 0 (diagonal tiles and tiles a tie straddles).
+template <int R, int LEVEL, int MODE, bool DIM3>
+__device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt, const Ev<DIM3> (&g)[R],
+                                        Mom<LEVEL> (&m)[R], const DevConsts& c,
+                                        unsigned lane_addr) {
+    constexpr int RS = DIM3 ? 6 : 4;
+#pragma unroll 2
+    for (int j = 0; j < cnt; ++j) {
+        const Ev<DIM3> s = read_rec<DIM3>(sbuf + j * RS);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double dx = g[r].x - s.x, dy = g[r].y - s.y, dt = g[r].t - s.t;
+            double u = fma(dy, dy, dx * dx);
+            if (DIM3) { const double dz = g[r].z - s.z; u = fma(dz, dz, u); }
+            const double w = dt * dt;
+            const double ab = fma(c.rho_b, w, u);
+            const double eB = exp2_scaled<1>(ab, c.negcb, c.lim_b_hi, u, lane_addr);
+            m[r].b[0] += eB;
+            if (LEVEL == 1) {
+                m[r].b[1] = fma(eB, u, m[r].b[1]);
+                m[r].b[2] = fma(eB, w, m[r].b[2]);
+            } else if (LEVEL == 2) {
+                const double q1 = eB * u, q2 = eB * w;
+                m[r].b[1] += q1;
+                m[r].b[2] += q2;
+                m[r].b[3] = fma(q1, u, m[r].b[3]);
+                m[r].b[4] = fma(q1, w, m[r].b[4]);
+                m[r].b[5] = fma(q2, w, m[r].b[5]);
+            }
+            if (MODE != 0) {
+                const double as = fma(c.rho_s, dt, u);
+                const double eS = s.w * exp2_scaled<(MODE == 2) ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, lane_addr);
+                m[r].s[0] += eS;
+                if (LEVEL == 1) {
+                    m[r].s[1] = fma(eS, u, m[r].s[1]);
+                    m[r].s[2] = fma(eS, dt, m[r].s[2]);
+                } else if (LEVEL == 2) {
+                    const double q1 = eS * u, q2 = eS * dt;
+                    m[r].s[1] += q1;
+                    m[r].s[2] += q2;
+                    m[r].s[3] = fma(q1, u, m[r].s[3]);
+                    m[r].s[4] = fma(q1, dt, m[r].s[4]);
+                    m[r].s[5] = fma(q2, dt, m[r].s[5]);
+                }
+            }
+        }
+    }
+}
+
+// grid.x = n_ttiles * n_split; item (I, s): target tile I (NT*R targets) x source tiles
+// [s*tps, min((s+1)*tps, n_stiles)).  part[(s*NMOM + k)*ld + n].
+template <int R, int LEVEL, bool DIM3>
+__global__ void __launch_bounds__(NT) pass1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
+                                                   DevConsts c, const double* __restrict__ tab_g,
+                                                   double* __restrict__ part, int n_split, int tps) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    constexpr int NB = Mom<LEVEL>::NB;
+    __shared__ __align__(16) double tab[TAB_N * TAB_REP];
+    __shared__ __align__(16) double sbuf[2][TS * RS];
+
+    const int n_ttiles = gridDim.x / n_split;
+    const int I = n_ttiles - 1 - (int)(blockIdx.x / n_split);   // late (heavier) target tiles first
+    const int sp = blockIdx.x % n_split;
+    const int n_stiles = (int)((n + TS - 1) / TS);
+    const int J0 = sp * tps, J1 = min(J0 + tps, n_stiles);
+    const int64_t i0 = (int64_t)I * (NT * R);
+    const int64_t i1 = min(i0 + (int64_t)NT * R, n);
+
+    const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
+
+    Ev<DIM3> g[R];
+    Mom<LEVEL> m[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t i = min(i0 + r * NT + threadIdx.x, n - 1);
+        g[r] = read_rec<DIM3>(rec + i * RS);
+#pragma unroll
+        for (int k = 0; k < NB; ++k) { m[r].b[k] = 0.0; m[r].s[k] = 0.0; }
+    }
+    const double t_first = rec[i0 * RS + (DIM3 ? 3 : 2)];   // earliest target time of this tile
+
+    RecIO<DIM3> io;
+    if (J0 < J1) {
+        io.load(rec, (int64_t)J0 * TS, (int)min((int64_t)TS, n - (int64_t)J0 * TS));
+        io.store(sbuf[0]);
+    }
+    __syncthreads();
+    for (int J = J0; J < J1; ++J) {
+        const int cur = (J - J0) & 1;
+        const int64_t j0 = (int64_t)J * TS;
+        const int cnt = (int)min((int64_t)TS, n - j0);
+        if (J + 1 < J1) io.load(rec, j0 + TS, (int)min((int64_t)TS, n - j0 - TS));
+        if (j0 >= i1) {
+            p1_tile<R, LEVEL, 0, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+        } else if (j0 + cnt <= i0 && rec[(j0 + cnt - 1) * RS + (DIM3 ? 3 : 2)] < t_first) {
+            p1_tile<R, LEVEL, 1, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+        } else {
+            p1_tile<R, LEVEL, 2, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+        }
+        if (J + 1 < J1) io.store(sbuf[cur ^ 1]);
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t i = i0 + r * NT + threadIdx.x;
+        if (i < n) {
+            double* o = part + (int64_t)sp * (2 * NB) * ld + i;
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                o[(int64_t)k * ld] = m[r].b[k];
+                o[(int64_t)(NB + k) * ld] = m[r].s[k];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// block-wide fixed-order sum of NV values per thread; result valid in threads < NV of warp 0.
+template <int NV>
+__device__ __forceinline__ void block_reduce(double (&v)[NV], double* out /*global, NV*/) {
+    __shared__ double sm[RED_T / 32][NV];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double a = v[k];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
+        if (lane == 0) sm[wid][k] = a;
+    }
+    __syncthreads();
+    if (threadIdx.x < NV) {
+        double a = 0.0;
+#pragma unroll
+        for (int w = 0; w < RED_T / 32; ++w) a += sm[w][threadIdx.x];
+        out[threadIdx.x] = a;
+    }
+}
+
+__device__ __forceinline__ double norm_pdf(double z) { return 0.3989422804014326779399461 * exp(-0.5 * z * z); }
+__device__ __forceinline__ double norm_cdf(double z) { return 0.5 * erfc(-z * 0.7071067811865475244008444); }
+
+// a2 + a3: per event n, sum the pass-1 partials over splits (fixed order), form lambda_n and the
+// per-event terms of every scalar sum, write 1/lambda_n into the pass-2 target record, and reduce the
+// terms over the block.  blockpart[blk*NRED + k]:
+//   k = 0        sum log lambda_n
+//   k = 1..6     sum (d lambda_n/dp) / lambda_n                           (DESIGN: hyper-gradient)
+//   k = 7..27    sum [lambda_pq/lambda - lambda_p lambda_q/lambda^2], upper triangle row-major
+//   k = 28..30   sum [Phi(a)-Phi(b)],  sum [a phi(a) - b phi(b)],  sum [a phi(a)(2-a^2) - b phi(b)(2-b^2)]
+//   k = 31..33   sum theta (1-E),  sum theta T E,  sum theta T^2 E        (T = t_N - t_n, E = e^{-omega T})
+// glam[n*6 + p] = lambda_{n,p} / lambda_n^2 (only when `glam` != NULL; feeds the cross block).
+template <int LEVEL, bool DIM3>
+__global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
+                                                        DevConsts c, const double* __restrict__ part,
+                                                        int n_split, double* __restrict__ lam,
+                                                        double* __restrict__ trec, double* __restrict__ glam,
+                                                        double* __restrict__ blockpart,
+                                                        unsigned* __restrict__ status) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    constexpr int NB = Mom<LEVEL>::NB;
+    const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
+    double v[NRED];
+#pragma unroll
+    for (int k = 0; k < NRED; ++k) v[k] = 0.0;
+    if (i < n) {
+        double b[6] = {0, 0, 0, 0, 0, 0}, s[6] = {0, 0, 0, 0, 0, 0};
+        for (int sp = 0; sp < n_split; ++sp) {
+            const double* o = part + (int64_t)sp * (2 * NB) * ld + i;
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                b[k] += o[(int64_t)k * ld];
+                s[k] += o[(int64_t)(NB + k) * ld];
+            }
+        }
+        const Ev<DIM3> e = read_rec<DIM3>(rec + i * RS);
+        const double D = (double)c.dim;
+        const double SB = c.CB * b[0], SS = c.CS * s[0];
+        const double L = SB + SS;
+        const double iL = 1.0 / L;
+        lam[i] = L;
+        if (L == 0.0) atomicOr(status, (unsigned)ST_ZERO_RATE);
+        // pass-2 target record: (x, y, t, 1/lambda)
+        if (!DIM3) {
+            reinterpret_cast<double4*>(trec)[i] = make_double4(e.x, e.y, e.t, iL);
+        } else {
+            double2* o2 = reinterpret_cast<double2*>(trec) + 3 * i;
+            o2[0] = make_double2(e.x, e.y);
+            o2[1] = make_double2(e.z, e.t);
+            o2[2] = make_double2(iL, 0.0);
+        }
+        v[0] = log(L);
+        double d1[6] = {0, 0, 0, 0, 0, 0};
+        if (LEVEL >= 1) {
+            const double SBr2 = c.CB * b[1], SBd2 = c.CB * b[2], SSr2 = c.CS * s[1], SSd = c.CS * s[2];
+            const double tx = c.tau_x, tt = c.tau_t, h = c.h, om = c.omega;
+            d1[0] = SB / c.mu0;
+            d1[1] = SBr2 / (tx * tx * tx) - D * SB / tx;
+            d1[2] = SBd2 / (tt * tt * tt) - SB / tt;
+            d1[3] = SS / c.xi0;
+            d1[4] = SSr2 / (h * h * h) - D * SS / h;
+            d1[5] = SS / om - SSd;
+#pragma unroll
+            for (int p = 0; p < 6; ++p) v[1 + p] = d1[p] * iL;
+            if (glam != nullptr) {
+#pragma unroll
+                for (int p = 0; p < 6; ++p) glam[i * 6 + p] = d1[p] * iL * iL;
+            }
+            if (LEVEL >= 2) {
+                const double SBr4 = c.CB * b[3], SBr2d2 = c.CB * b[4], SBd4 = c.CB * b[5];
+                const double SSr4 = c.CS * s[3], SSr2d = c.CS * s[4], SSd2 = c.CS * s[5];
+                double d2[6][6];
+#pragma unroll
+                for (int p = 0; p < 6; ++p)
+#pragma unroll
+                    for (int q = 0; q < 6; ++q) d2[p][q] = 0.0;
+                const double tx2 = tx * tx, tt2 = tt * tt, h2 = h * h;
+                d2[0][1] = d1[1] / c.mu0;
+                d2[0][2] = d1[2] / c.mu0;
+                d2[1][1] = SBr4 / (tx2 * tx2 * tx2) - (2.0 * D + 3.0) * SBr2 / (tx2 * tx2) + D * (D + 1.0) * SB / tx2;
+                d2[2][2] = SBd4 / (tt2 * tt2 * tt2) - 5.0 * SBd2 / (tt2 * tt2) + 2.0 * SB / tt2;
+                d2[1][2] = SBr2d2 / (tx2 * tx * tt2 * tt) - SBr2 / (tx2 * tx * tt) - D * SBd2 / (tx * tt2 * tt) + D * SB / (tx * tt);
+                d2[3][4] = d1[4] / c.xi0;
+                d2[3][5] = d1[5] / c.xi0;
+                d2[4][4] = SSr4 / (h2 * h2 * h2) - (2.0 * D + 3.0) * SSr2 / (h2 * h2) + D * (D + 1.0) * SS / h2;
+                d2[5][5] = SSd2 - 2.0 * SSd / om;
+                d2[4][5] = SSr2 / (h2 * h * om) - SSr2d / (h2 * h) - D * SS / (h * om) + D * SSd / h;
+                int k = 7;
+#pragma unroll
+                for (int p = 0; p < 6; ++p)
+#pragma unroll
+                    for (int q = p; q < 6; ++q) {
+                        v[k] = d2[p][q] * iL - (d1[p] * iL) * (d1[q] * iL);
+                        ++k;
+                    }
+            }
+        }
+        // integral terms (a3)
+        const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
+        const double T = tN - e.t;
+        const double a = T / c.tau_t, bb = -e.t / c.tau_t;
+        const double pa = norm_pdf(a), pb = norm_pdf(bb);
+        v[28] = norm_cdf(a) - norm_cdf(bb);
+        v[29] = a * pa - bb * pb;
+        v[30] = a * pa * (2.0 - a * a) - bb * pb * (2.0 - bb * bb);
+        const double E = exp(-c.omega * T);
+        v[31] = e.w * (-expm1(-c.omega * T));
+        v[32] = e.w * T * E;
+        v[33] = e.w * T * T * E;
+    }
+    block_reduce<NRED>(v, blockpart + (int64_t)blockIdx.x * NRED);
+}
+
+// a5 (scalars): fixed-order sum of the block partials, then ll, grad_hyper, hess_hyper.
+__global__ void __launch_bounds__(64) scalars_kernel(const double* __restrict__ blockpart, int nblk, DevConsts c,
+                                                     double* __restrict__ ll, double* __restrict__ grad_hyper,
+                                                     double* __restrict__ hess_hyper, double* __restrict__ scal_out) {
+    __shared__ double r[NRED];
+    if (threadIdx.x < NRED) {
+        double a = 0.0;
+        for (int b = 0; b < nblk; ++b) a += blockpart[(int64_t)b * NRED + threadIdx.x];
+        r[threadIdx.x] = a;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    const double sPhi = r[28], sAphi = r[29], sAphi2 = r[30], sTh = r[31], sThTE = r[32], sThT2E = r[33];
+    const double Lam = c.mu0 * sPhi + c.xi0 * sTh;
+    if (scal_out) { scal_out[0] = r[0]; scal_out[1] = Lam; }
+    if (ll) *ll = r[0] - Lam;
+    if (grad_hyper) {
+        const double L1[6] = {sPhi, 0.0, -c.mu0 / c.tau_t * sAphi, sTh, 0.0, c.xi0 * sThTE};
+        for (int p = 0; p < 6; ++p) grad_hyper[p] = r[1 + p] - L1[p];
+    }
+    if (hess_hyper) {
+        double L2[6][6];
+        for (int p = 0; p < 6; ++p)
+            for (int q = 0; q < 6; ++q) L2[p][q] = 0.0;
+        L2[0][2] = -sAphi / c.tau_t;
+        L2[2][2] = c.mu0 / (c.tau_t * c.tau_t) * sAphi2;
+        L2[3][5] = sThTE;
+        L2[5][5] = -c.xi0 * sThT2E;
+        int k = 7;
+        for (int p = 0; p < 6; ++p)
+            for (int q = p; q < 6; ++q) {
+                const double hv = r[k++] - L2[p][q];
+                hess_hyper[p * 6 + q] = hv;
+                hess_hyper[q * 6 + p] = hv;
+            }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4: pass 2.  Thread owns R sources m; later targets (x, y, t, 1/lambda) stream through shared memory.
+//   c_m = sum_{t_n > t_m} e_nm / lambda_n,   d_m = sum (e_nm / lambda_n)^2,   e = exp(-omega dt - r2/2h^2)
+// (k_nm = CS e_nm; the constant is applied in theta_kernel).  LEVEL 0: c only; 1: c and d.
+template <int R, int LEVEL, bool MASKED, bool DIM3>
+__device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt, const Ev<DIM3> (&g)[R],
+                                        double (&cm)[R], double (&dm)[R], const DevConsts& c,
+                                        unsigned lane_addr) {
+    constexpr int RS = DIM3 ? 6 : 4;
+#pragma unroll 2
+    for (int j = 0; j < cnt; ++j) {
+        const Ev<DIM3> s = read_rec<DIM3>(sbuf + j * RS);   // a target; s.w = 1/lambda_n
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double dx = s.x - g[r].x, dy = s.y - g[r].y, dt = s.t - g[r].t;
+            double u = fma(dy, dy, dx * dx);
+            if (DIM3) { const double dz = s.z - g[r].z; u = fma(dz, dz, u); }
+            const double as = fma(c.rho_s, dt, u);
+            const double e = exp2_scaled<MASKED ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, lane_addr);
+            if (LEVEL == 0) {
+                cm[r] = fma(e, s.w, cm[r]);
+            } else {
+                const double q = e * s.w;
+                cm[r] += q;
+                dm[r] = fma(q, q, dm[r]);
+            }
+        }
+    }
+}
+
+// grid = (P2 slots, n source tiles).  Block (slot, M): sources of tile M (NT*R) x target tiles
+// [Mt0 + slot*tpc, Mt0 + (slot+1)*tpc) where Mt0 is the first streamed tile that can hold a later target.
+// part2[(slot*2 + k)*ld + m], k = 0 (c), 1 (d).
+template <int R, int LEVEL, bool DIM3>
+__global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
+                                                   int64_t n, int64_t ld, DevConsts c,
+                                                   const double* __restrict__ tab_g, double* __restrict__ part2,
+                                                   int tpc) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    __shared__ __align__(16) double tab[TAB_N * TAB_REP];
+    __shared__ __align__(16) double sbuf[2][TS * RS];
+
+    const int Ms = (int)blockIdx.y;   // early source tiles have the most later targets: heaviest first
+    const int slot = blockIdx.x;
+    const int64_t m0 = (int64_t)Ms * (NT * R);
+    const int64_t m1 = min(m0 + (int64_t)NT * R, n);
+    const int n_ttiles = (int)((n + TS - 1) / TS);
+    const int Jfirst = (int)(m0 / TS);                      // streamed tile holding the first own source
+    const int J0 = Jfirst + slot * tpc, J1 = min(J0 + tpc, n_ttiles);
+
+    Ev<DIM3> g[R];
+    double cm[R], dm[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t i = min(m0 + r * NT + threadIdx.x, n - 1);
+        g[r] = read_rec<DIM3>(rec + i * RS);
+        cm[r] = 0.0;
+        dm[r] = 0.0;
+    }
+    if (J0 < J1) {
+        const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
+        const double t_last = rec[(m1 - 1) * RS + (DIM3 ? 3 : 2)];   // latest own source time
+        RecIO<DIM3> io;
+        io.load(trec, (int64_t)J0 * TS, (int)min((int64_t)TS, n - (int64_t)J0 * TS));
+        io.store(sbuf[0]);
+        __syncthreads();
+        for (int J = J0; J < J1; ++J) {
+            const int cur = (J - J0) & 1;
+            const int64_t j0 = (int64_t)J * TS;
+            const int cnt = (int)min((int64_t)TS, n - j0);
+            if (J + 1 < J1) io.load(trec, j0 + TS, (int)min((int64_t)TS, n - j0 - TS));
+            if (j0 >= m1 && trec[j0 * RS + (DIM3 ? 3 : 2)] > t_last) {
+                p2_tile<R, LEVEL, false, DIM3>(sbuf[cur], cnt, g, cm, dm, c, lane_addr);
+            } else {
+                p2_tile<R, LEVEL, true, DIM3>(sbuf[cur], cnt, g, cm, dm, c, lane_addr);
+            }
+            if (J + 1 < J1) io.store(sbuf[cur ^ 1]);
+            __syncthreads();
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t i = m0 + r * NT + threadIdx.x;
+        if (i < n) {
+            part2[(int64_t)(slot * 2 + 0) * ld + i] = cm[r];
+            if (LEVEL >= 1) part2[(int64_t)(slot * 2 + 1) * ld + i] = dm[r];
+        }
+    }
+}
+
+// a5 (theta): grad_theta[m] = CS c_m - xi0 (1 - E_m);  hess_theta_diag[m] = - CS^2 d_m.
+template <bool DIM3>
+__global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
+                                                      DevConsts c, const double* __restrict__ part2, int n_slots,
+                                                      double* __restrict__ grad_theta,
+                                                      double* __restrict__ hess_theta_diag) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
+    if (i >= n) return;
+    double cs = 0.0, ds = 0.0;
+    for (int s = 0; s < n_slots; ++s) {
+        cs += part2[(int64_t)(s * 2 + 0) * ld + i];
+        if (hess_theta_diag) ds += part2[(int64_t)(s * 2 + 1) * ld + i];
+    }
+    if (grad_theta) {
+        const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
+        const double ti = rec[i * RS + (DIM3 ? 3 : 2)];
+        grad_theta[i] = c.CS * cs - c.xi0 * (-expm1(-c.omega * (tN - ti)));
+    }
+    if (hess_theta_diag) hess_theta_diag[i] = -(c.CS * c.CS) * ds;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Cross block (optional output, not tuned): thread per source m loops over all later targets.
+//   cross[m][p] = sum_n k_nm [ (dlog k_nm/dp) / lambda_n - lambda_{n,p} / lambda_n^2 ] - dLambda/(dtheta_m dp)
+template <bool DIM3>
+__global__ void __launch_bounds__(RED_T) cross_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
+                                                      const double* __restrict__ glam, int64_t n, DevConsts c,
+                                                      double* __restrict__ cross) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    const int64_t m = (int64_t)blockIdx.x * RED_T + threadIdx.x;
+    if (m >= n) return;
+    const Ev<DIM3> g = read_rec<DIM3>(rec + m * RS);
+    double acc[6] = {0, 0, 0, 0, 0, 0};
+    const double D = (double)c.dim;
+    for (int64_t i = m + 1; i < n; ++i) {
+        const Ev<DIM3> s = read_rec<DIM3>(trec + i * RS);
+        const double dt = s.t - g.t;
+        if (!(dt > 0.0)) continue;
+        const double dx = s.x - g.x, dy = s.y - g.y, dz = s.z - g.z;
+        const double u = dx * dx + dy * dy + (DIM3 ? dz * dz : 0.0);
+        const double k = c.CS * exp(-c.omega * dt - u / (2.0 * c.h * c.h));
+        const double a = k * s.w;
+        const double gl[3] = {1.0 / c.xi0, u / (c.h * c.h * c.h) - D / c.h, 1.0 / c.omega - dt};
+#pragma unroll
+        for (int p = 0; p < 6; ++p) acc[p] += a * (p >= 3 ? gl[p - 3] : 0.0) - k * glam[i * 6 + p];
+    }
+    const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
+    const double T = tN - g.t;
+    acc[3] -= -expm1(-c.omega * T);
+    acc[5] -= c.xi0 * T * exp(-c.omega * T);
+#pragma unroll
+    for (int p = 0; p < 6; ++p) cross[m * 6 + p] = acc[p];
+}
+
+// Dense theta-theta block (correctness only): H[m][m'] = - sum_n k_nm k_nm' / lambda_n^2.
+template <bool DIM3>
+__global__ void dense_kernel(const double* __restrict__ rec, const double* __restrict__ trec, int64_t n,
+                             DevConsts c, double* __restrict__ H) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    const int64_t m = (int64_t)blockIdx.y * blockDim.y + threadIdx.y;
+    const int64_t m2 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n || m2 >= n) return;
+    const Ev<DIM3> a = read_rec<DIM3>(rec + m * RS), b = read_rec<DIM3>(rec + m2 * RS);
+    double acc = 0.0;
+    for (int64_t i = (m > m2 ? m : m2) + 1; i < n; ++i) {
+        const Ev<DIM3> s = read_rec<DIM3>(trec + i * RS);
+        const double dta = s.t - a.t, dtb = s.t - b.t;
+        if (!(dta > 0.0) || !(dtb > 0.0)) continue;
+        const double ua = (s.x - a.x) * (s.x - a.x) + (s.y - a.y) * (s.y - a.y) + (DIM3 ? (s.z - a.z) * (s.z - a.z) : 0.0);
+        const double ub = (s.x - b.x) * (s.x - b.x) + (s.y - b.y) * (s.y - b.y) + (DIM3 ? (s.z - b.z) * (s.z - b.z) : 0.0);
+        const double ka = c.CS * exp(-c.omega * dta - ua / (2.0 * c.h * c.h));
+        const double kb = c.CS * exp(-c.omega * dtb - ub / (2.0 * c.h * c.h));
+        acc += (ka * s.w) * (kb * s.w);
+    }
+    H[m * n + m2] = -acc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// helpers for hawkes_sort_events
+__global__ void iota_kernel(int64_t n, int64_t* idx) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) idx[i] = i;
+}
+__global__ void gather_kernel(int64_t n, int dim, const int64_t* __restrict__ perm, const double* __restrict__ x_in,
+                              const double* __restrict__ th_in, double* __restrict__ x_out,
+                              double* __restrict__ th_out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int64_t s = perm[i];
+    for (int d = 0; d < dim; ++d) x_out[(int64_t)d * n + i] = x_in[(int64_t)d * n + s];
+    th_out[i] = th_in[s];
+}
+
+// DFMA-chain microbenchmark: 8 independent chains per thread, `iters` x 8 x 8 FMAs.
+__global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, double* out) {
+    double a[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) a[k] = seed + k + threadIdx.x * 1e-3;
+    const double m = 1.0 - 1e-9, b = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = fma(a[k], m, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += a[k];
+    if (s == 123.456) out[0] = s;   // never true; keeps the chains alive
+}
+
+}  // namespace
+
+// =================================================================================================
+// host side
+struct hawkes_ctx {
+    int device;
+    int dim;
+    int64_t n_max;
+    int64_t ld_max;
+    double* d_tab;        // 128 doubles
+    double* d_rec;        // n_max * RS
+    double* d_trec;       // n_max * RS
+    double* d_part1;      // pass-1 partials
+    size_t part1_doubles;
+    double* d_part2;      // P2_SLOTS_MAX * 2 * ld_max
+    double* d_lam;        // n_max
+    double* d_glam;       // n_max * 6
+    double* d_blockpart;  // nblk_max * NRED
+    double* d_scal;       // 2 (sum log lambda, Lambda) + peak scratch
+    double* d_in;         // staging for hawkes_eval_host: x[dim*n_max], t, theta
+    double* d_out;        // staging for outputs: 1 + n + 6 + n + 36 + 6n
+    unsigned* d_status;
+    void* d_cub;          // temp storage for the sort
+    size_t cub_bytes;
+    double* d_sort_keys;  // n_max
+    int64_t* d_sort_idx;  // n_max
+    int64_t launches;
+};
+
+namespace {
+
+#define CK(call)                                   \
+    do {                                           \
+        cudaError_t e_ = (call);                   \
+        if (e_ != cudaSuccess) return HAWKES_ERR_CUDA; \
+    } while (0)
+
+inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+constexpr int P1_R = 2;   // targets per thread in pass 1
+constexpr int P2_R = 2;   // sources per thread in pass 2
+
+struct Plan {
+    int n_ttiles1, n_split, tps;   // pass 1
+    int n_stiles2, n_slots, tpc;   // pass 2
+    int64_t ld;
+    int nblk;                      // O(N) kernels
+};
+
+Plan make_plan(int64_t n) {
+    Plan p;
+    p.ld = round_up(n, 256);
+    const int n_tiles = (int)((n + TS - 1) / TS);   // streamed tiles
+    p.n_ttiles1 = (int)((n + NT * P1_R - 1) / (NT * P1_R));
+    int want = (P1_ITEMS_TARGET + p.n_ttiles1 - 1) / p.n_ttiles1;
+    if (want < 1) want = 1;
+    if (want > n_tiles) want = n_tiles;
+    p.tps = (n_tiles + want - 1) / want;
+    p.n_split = (n_tiles + p.tps - 1) / p.tps;
+    p.n_stiles2 = (int)((n + NT * P2_R - 1) / (NT * P2_R));
+    p.n_slots = n_tiles < P2_SLOTS_MAX ? n_tiles : P2_SLOTS_MAX;
+    p.tpc = (n_tiles + p.n_slots - 1) / p.n_slots;
+    p.n_slots = (n_tiles + p.tpc - 1) / p.tpc;
+    p.nblk = (int)((n + RED_T - 1) / RED_T);
+    return p;
+}
+
+size_t part1_bound(int64_t n_max) {
+    // n_split * ld <= (P1_ITEMS_TARGET / n_ttiles + 1) * ld  <~  P1_ITEMS_TARGET * NT*R * (ld/n) + ld;
+    // generous, and enqueue_eval() re-checks the actual plan against it.
+    return (size_t)12 * ((size_t)2 * P1_ITEMS_TARGET * NT * P1_R + 4 * (size_t)round_up(n_max, 256));
+}
+
+int make_consts(const hawkes_params* p, int dim, DevConsts* c) {
+    const double v[6] = {p->mu0, p->tau_x, p->tau_t, p->xi0, p->h, p->omega};
+    for (int i = 0; i < 6; ++i)
+        if (!(v[i] > 0.0) || !std::isfinite(v[i])) return HAWKES_ERR_PARAM;
+    const long double log2e = 1.442695040888963407359924681001892137L;
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    const long double cb = log2e / (2.0L * p->tau_x * p->tau_x);
+    const long double cs = log2e / (2.0L * p->h * p->h);
+    c->negcb = (double)(-cb);
+    c->rho_b = (double)(((long double)p->tau_x * p->tau_x) / ((long double)p->tau_t * p->tau_t));
+    c->negcs = (double)(-cs);
+    c->rho_s = (double)(2.0L * p->h * p->h * p->omega);
+    c->CB = (double)((long double)p->mu0 * powl(two_pi, -0.5L * (dim + 1)) * powl(p->tau_x, -dim) / p->tau_t);
+    c->CS = (double)((long double)p->xi0 * p->omega * powl(two_pi, -0.5L * dim) * powl(p->h, -dim));
+    c->mu0 = p->mu0; c->tau_x = p->tau_x; c->tau_t = p->tau_t; c->xi0 = p->xi0; c->h = p->h; c->omega = p->omega;
+    c->dim = dim;
+    // flush when the base-2 exponent is below -1020: argument a >= 1020 / c
+    auto hi_of = [](double d) { union { double d; uint64_t u; } q; q.d = d; return (int)(q.u >> 32); };
+    double lb = (double)(1020.0L / cb), ls = (double)(1020.0L / cs);
+    if (!std::isfinite(lb) || !std::isfinite(ls) || !std::isfinite(c->CB) || !std::isfinite(c->CS) ||
+        !std::isfinite(c->rho_b) || !std::isfinite(c->rho_s)) return HAWKES_ERR_PARAM;
+    c->lim_b_hi = hi_of(lb);
+    c->lim_s_hi = hi_of(ls);
+    return HAWKES_OK;
+}
+
+template <bool DIM3>
+int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                 const DevConsts& c, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
+                 double* hess_theta_diag, double* hess_hyper, double* hess_cross, cudaStream_t st) {
+    const Plan pl = make_plan(n);
+    if ((size_t)pl.n_split * 12 * (size_t)pl.ld > ctx->part1_doubles) return HAWKES_ERR_NOMEM;
+    CK(cudaMemsetAsync(ctx->d_status, 0, sizeof(unsigned), st));
+    prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status);
+    ctx->launches++;
+    const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2
+                       : ((want & (HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_CROSS)) ? 1 : 0);
+    const unsigned g1 = (unsigned)(pl.n_ttiles1 * pl.n_split);
+    double* glam = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_glam : nullptr;
+    switch (level1) {
+        case 0:
+            pass1_kernel<P1_R, 0, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            break;
+        case 1:
+            pass1_kernel<P1_R, 1, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            break;
+        default:
+            pass1_kernel<P1_R, 2, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            break;
+    }
+    ctx->launches += 2;
+    if (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) {
+        scalars_kernel<<<1, 64, 0, st>>>(ctx->d_blockpart, pl.nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
+                                         (want & HAWKES_WANT_GRAD_HYPER) ? grad_hyper : nullptr,
+                                         (want & HAWKES_WANT_HESS_HYPER) ? hess_hyper : nullptr, ctx->d_scal);
+        ctx->launches++;
+    }
+    if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
+        const dim3 g2((unsigned)pl.n_slots, (unsigned)pl.n_stiles2);
+        if (want & HAWKES_WANT_HESS_THETA)
+            pass2_kernel<P2_R, 1, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.tpc);
+        else
+            pass2_kernel<P2_R, 0, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.tpc);
+        theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.n_slots,
+                                                      (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
+                                                      (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr);
+        ctx->launches += 2;
+    }
+    if (want & HAWKES_WANT_HESS_CROSS) {
+        cross_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, ctx->d_trec, ctx->d_glam, n, c, hess_cross);
+        ctx->launches++;
+    }
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int check_common(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                 const hawkes_params* p) {
+    if (!ctx || !x || !t || !theta || !p) return HAWKES_ERR_ARG;
+    if (n < 1 || n > ctx->n_max) return HAWKES_ERR_ARG;
+    return HAWKES_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* hawkes_strerror(int status) {
+    switch (status) {
+        case HAWKES_OK: return "ok";
+        case HAWKES_ERR_ARG: return "invalid argument";
+        case HAWKES_ERR_PARAM: return "hyperparameter not finite and positive";
+        case HAWKES_ERR_UNSORTED: return "event times are not non-decreasing";
+        case HAWKES_ERR_CUDA: return "CUDA error";
+        case HAWKES_ERR_NOMEM: return "out of device memory";
+        case HAWKES_ERR_UNSUPPORTED: return "unsupported dimension or size";
+        case HAWKES_ERR_NONFINITE: return "non-finite input or negative theta";
+        case HAWKES_WARN_ZERO_RATE: return "some lambda_n is zero (ll = -inf)";
+        default: return "unknown status";
+    }
+}
+
+int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
+    if (!out || n_max < 1) return HAWKES_ERR_ARG;
+    if (dim < 1 || dim > 3) return HAWKES_ERR_UNSUPPORTED;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return HAWKES_ERR_CUDA;
+    CK(cudaSetDevice(device));
+    hawkes_ctx* c = new (std::nothrow) hawkes_ctx();
+    if (!c) return HAWKES_ERR_NOMEM;
+    c->device = device;
+    c->dim = dim;
+    c->n_max = n_max;
+    c->ld_max = round_up(n_max, 256);
+    c->launches = 0;
+    const int RS = dim == 3 ? 6 : 4;
+    const int nblk = (int)((n_max + RED_T - 1) / RED_T);
+    c->part1_doubles = part1_bound(n_max);
+    c->cub_bytes = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, c->cub_bytes, (const double*)nullptr, (double*)nullptr,
+                                    (const int64_t*)nullptr, (int64_t*)nullptr, (int)n_max);
+    bool ok = true;
+    auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
+    void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_part1, (void**)&c->d_part2,
+                     (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
+                     (void**)&c->d_out, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
+    for (auto p : ptrs) *p = nullptr;
+    alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
+    alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
+    alloc((void**)&c->d_trec, sizeof(double) * RS * (size_t)c->ld_max);
+    alloc((void**)&c->d_part1, sizeof(double) * c->part1_doubles);
+    alloc((void**)&c->d_part2, sizeof(double) * 2 * P2_SLOTS_MAX * (size_t)c->ld_max);
+    alloc((void**)&c->d_lam, sizeof(double) * (size_t)c->ld_max);
+    alloc((void**)&c->d_glam, sizeof(double) * 6 * (size_t)c->ld_max);
+    alloc((void**)&c->d_blockpart, sizeof(double) * NRED * (size_t)nblk);
+    alloc((void**)&c->d_scal, sizeof(double) * 8);
+    alloc((void**)&c->d_in, sizeof(double) * (size_t)(dim + 2) * (size_t)n_max);
+    alloc((void**)&c->d_out, sizeof(double) * (size_t)(43 + 8 * n_max));
+    alloc((void**)&c->d_status, sizeof(unsigned) * 2);
+    alloc(&c->d_cub, c->cub_bytes);
+    alloc((void**)&c->d_sort_keys, sizeof(double) * (size_t)n_max);
+    alloc((void**)&c->d_sort_idx, sizeof(int64_t) * (size_t)n_max);
+    if (ok && cudaMemcpy(c->d_tab, hawkes_exp2_table_host, sizeof(double) * TAB_N, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
+    if (ok && cudaMemset(c->d_status, 0, sizeof(unsigned) * 2) != cudaSuccess) ok = false;
+    if (!ok) {
+        hawkes_destroy(c);
+        cudaGetLastError();
+        return HAWKES_ERR_NOMEM;
+    }
+    *out = c;
+    return HAWKES_OK;
+}
+
+void hawkes_destroy(hawkes_ctx* c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
+                    c->d_scal, c->d_in, c->d_out, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    delete c;
+}
+
+int hawkes_last_status(hawkes_ctx* ctx, void* stream) {
+    if (!ctx) return HAWKES_ERR_ARG;
+    unsigned s = 0;
+    CK(cudaMemcpyAsync(&s, ctx->d_status, sizeof(unsigned), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CK(cudaStreamSynchronize((cudaStream_t)stream));
+    if (s & ST_NONFINITE) return HAWKES_ERR_NONFINITE;
+    if (s & ST_UNSORTED) return HAWKES_ERR_UNSORTED;
+    if (s & ST_ZERO_RATE) return HAWKES_WARN_ZERO_RATE;
+    return HAWKES_OK;
+}
+
+int hawkes_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                const hawkes_params* p, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
+                double* hess_theta_diag, double* hess_hyper, double* hess_cross, void* stream) {
+    int rc = check_common(ctx, n, x, t, theta, p);
+    if (rc) return rc;
+    if (want == 0 || (want & ~63u)) return HAWKES_ERR_ARG;
+    if (((want & HAWKES_WANT_LL) && !ll) || ((want & HAWKES_WANT_GRAD_THETA) && !grad_theta) ||
+        ((want & HAWKES_WANT_GRAD_HYPER) && !grad_hyper) || ((want & HAWKES_WANT_HESS_THETA) && !hess_theta_diag) ||
+        ((want & HAWKES_WANT_HESS_HYPER) && !hess_hyper) || ((want & HAWKES_WANT_HESS_CROSS) && !hess_cross))
+        return HAWKES_ERR_ARG;
+    DevConsts c;
+    rc = make_consts(p, ctx->dim, &c);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    if (ctx->dim == 3)
+        return enqueue_eval<true>(ctx, n, x, t, theta, c, want, ll, grad_theta, grad_hyper, hess_theta_diag, hess_hyper, hess_cross, (cudaStream_t)stream);
+    return enqueue_eval<false>(ctx, n, x, t, theta, c, want, ll, grad_theta, grad_hyper, hess_theta_diag, hess_hyper, hess_cross, (cudaStream_t)stream);
+}
+
+int hawkes_loglik(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                  const hawkes_params* p, double* ll, void* stream) {
+    if (!ll) return HAWKES_ERR_ARG;
+    return hawkes_eval(ctx, n, x, t, theta, p, HAWKES_WANT_LL, ll, nullptr, nullptr, nullptr, nullptr, nullptr, stream);
+}
+
+int hawkes_grad(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                const hawkes_params* p, double* ll, double* grad_theta, double* grad_hyper, void* stream) {
+    uint32_t want = 0;
+    if (ll) want |= HAWKES_WANT_LL;
+    if (grad_theta) want |= HAWKES_WANT_GRAD_THETA;
+    if (grad_hyper) want |= HAWKES_WANT_GRAD_HYPER;
+    return hawkes_eval(ctx, n, x, t, theta, p, want, ll, grad_theta, grad_hyper, nullptr, nullptr, nullptr, stream);
+}
+
+int hawkes_hessian(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                   const hawkes_params* p, double* hess_theta_diag, double* hess_hyper, double* hess_cross,
+                   void* stream) {
+    uint32_t want = 0;
+    if (hess_theta_diag) want |= HAWKES_WANT_HESS_THETA;
+    if (hess_hyper) want |= HAWKES_WANT_HESS_HYPER;
+    if (hess_cross) want |= HAWKES_WANT_HESS_CROSS;
+    return hawkes_eval(ctx, n, x, t, theta, p, want, nullptr, nullptr, nullptr, hess_theta_diag, hess_hyper, hess_cross, stream);
+}
+
+int hawkes_eval_host(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                     const hawkes_params* p, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
+                     double* hess_theta_diag, double* hess_hyper, double* hess_cross, void* stream) {
+    int rc = check_common(ctx, n, x, t, theta, p);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    const int dim = ctx->dim;
+    double* dx = ctx->d_in;
+    double* dt = dx + (size_t)dim * n;
+    double* dth = dt + n;
+    CK(cudaMemcpyAsync(dx, x, sizeof(double) * (size_t)dim * n, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dt, t, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dth, theta, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    double* o_ll = ctx->d_out;
+    double* o_gh = o_ll + 1;
+    double* o_hh = o_gh + 6;
+    double* o_gt = o_hh + 36;
+    double* o_ht = o_gt + n;
+    double* o_hc = o_ht + n;
+    rc = hawkes_eval(ctx, n, dx, dt, dth, p, want, ll ? o_ll : nullptr, grad_theta ? o_gt : nullptr,
+                     grad_hyper ? o_gh : nullptr, hess_theta_diag ? o_ht : nullptr, hess_hyper ? o_hh : nullptr,
+                     hess_cross ? o_hc : nullptr, stream);
+    if (rc) return rc;
+    if (want & HAWKES_WANT_LL) CK(cudaMemcpyAsync(ll, o_ll, sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (want & HAWKES_WANT_GRAD_HYPER) CK(cudaMemcpyAsync(grad_hyper, o_gh, sizeof(double) * 6, cudaMemcpyDeviceToHost, st));
+    if (want & HAWKES_WANT_HESS_HYPER) CK(cudaMemcpyAsync(hess_hyper, o_hh, sizeof(double) * 36, cudaMemcpyDeviceToHost, st));
+    if (want & HAWKES_WANT_GRAD_THETA) CK(cudaMemcpyAsync(grad_theta, o_gt, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (want & HAWKES_WANT_HESS_THETA) CK(cudaMemcpyAsync(hess_theta_diag, o_ht, sizeof(double) * n, cudaMemcpyDeviceToHost, st));
+    if (want & HAWKES_WANT_HESS_CROSS) CK(cudaMemcpyAsync(hess_cross, o_hc, sizeof(double) * 6 * n, cudaMemcpyDeviceToHost, st));
+    return hawkes_last_status(ctx, stream);
+}
+
+int hawkes_hessian_theta_dense(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                               const hawkes_params* p, double* hess_theta, void* stream) {
+    int rc = check_common(ctx, n, x, t, theta, p);
+    if (rc) return rc;
+    if (!hess_theta) return HAWKES_ERR_ARG;
+    if (n > 4096) return HAWKES_ERR_UNSUPPORTED;
+    // lambda via a log-likelihood-level evaluation (writes trec = (x, y, t, 1/lambda))
+    rc = hawkes_eval(ctx, n, x, t, theta, p, HAWKES_WANT_LL, ctx->d_scal + 4, nullptr, nullptr, nullptr, nullptr, nullptr, stream);
+    if (rc) return rc;
+    DevConsts c;
+    make_consts(p, ctx->dim, &c);
+    const dim3 blk(16, 16), grd((unsigned)((n + 15) / 16), (unsigned)((n + 15) / 16));
+    if (ctx->dim == 3) dense_kernel<true><<<grd, blk, 0, (cudaStream_t)stream>>>(ctx->d_rec, ctx->d_trec, n, c, hess_theta);
+    else dense_kernel<false><<<grd, blk, 0, (cudaStream_t)stream>>>(ctx->d_rec, ctx->d_trec, n, c, hess_theta);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_sort_events(hawkes_ctx* ctx, int64_t n, int dim, const double* x_in, const double* t_in,
+                       const double* theta_in, double* x_out, double* t_out, double* theta_out, int64_t* perm,
+                       void* stream) {
+    if (!ctx || !x_in || !t_in || !theta_in || !x_out || !t_out || !theta_out || !perm) return HAWKES_ERR_ARG;
+    if (n < 1 || n > ctx->n_max || dim != ctx->dim) return HAWKES_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    const int nb = (int)((n + 255) / 256);
+    iota_kernel<<<nb, 256, 0, st>>>(n, ctx->d_sort_idx);
+    size_t bytes = ctx->cub_bytes;
+    CK(cub::DeviceRadixSort::SortPairs(ctx->d_cub, bytes, t_in, t_out, (const int64_t*)ctx->d_sort_idx, perm, (int)n, 0, 64, st));
+    gather_kernel<<<nb, 256, 0, st>>>(n, dim, perm, x_in, theta_in, x_out, theta_out);
+    ctx->launches += 2;
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stream) {
+    if (!ctx || !lambda_out || n < 1 || n > ctx->n_max) return HAWKES_ERR_ARG;
+    CK(cudaMemcpyAsync(lambda_out, ctx->d_lam, sizeof(double) * n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return HAWKES_OK;
+}
+
+int64_t hawkes_launch_count(const hawkes_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int hawkes_fp64_peak(hawkes_ctx* ctx, double millis, double* tflops, void* stream) {
+    if (!ctx || !tflops || !(millis > 0.0)) return HAWKES_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, ctx->device));
+    const int blocks = prop.multiProcessorCount * 8;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    int iters = 2000;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CK(cudaEventRecord(e0, st));
+        dfma_peak_kernel<<<blocks, 256, 0, st>>>(iters, 1.0, ctx->d_scal + 6);
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        const double flops = 2.0 * 64.0 * iters * 256.0 * blocks;
+        const double tf = flops / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+        // aim the next repetition at `millis`
+        double scale = millis / (ms > 1e-3 ? ms : 1e-3);
+        if (scale > 50.0) scale = 50.0;
+        iters = (int)(iters * scale) + 1;
+    }
+    ctx->launches += 4;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *tflops = best;
+    return HAWKES_OK;
+}
+
+}  // extern "C"

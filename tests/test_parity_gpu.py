@@ -1,0 +1,268 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the oracle, element by
+element, on the same seeded inputs.  Tolerance 1e-10 relative (BASELINE.json north_star) in the sense
+of tests/parity.py."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2103_03348_b200 as hp
+from paper_2103_03348_b200 import synth
+from parity import TOL, check, hess_hyper_scale, scales
+
+pytestmark = pytest.mark.gpu
+THREADS = max(1, min(os.cpu_count() or 1, 64))
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def dev(torch, ev):
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda")
+    return f(ev.x), f(ev.t), f(ev.theta)
+
+
+def run_gpu(torch, ev, want=hp.WANT_ALL, ctx=None):
+    ctx = ctx or hp.HawkesContext(ev.n, ev.dim)
+    x, t, th = dev(torch, ev)
+    r = ctx.eval(x, t, th, ev.params, want)
+    st = ctx.last_status()
+    lam = ctx.get_lambda(ev.n)
+    torch.cuda.synchronize()
+    return r, st, lam.cpu().numpy(), ctx
+
+
+def compare_all(ev, r, lam, ref, cross=True):
+    s = scales(ev, ref)
+    out = {}
+    out["lambda"] = check("lambda", lam, ref.lam)
+    out["ll"] = check("ll", r.ll.cpu().numpy()[0], ref.ll, s["ll"])
+    out["grad_theta"] = check("grad_theta", r.grad_theta.cpu().numpy(), ref.grad_theta, s["grad_theta"])
+    g, o = r.grad_theta.cpu().numpy(), ref.grad_theta
+    assert np.max(np.abs(g - o)) <= TOL * np.max(np.abs(o))
+    out["grad_hyper"] = check("grad_hyper", r.grad_hyper.cpu().numpy(), ref.grad_hyper, s["grad_hyper"])
+    if r.hess_theta_diag is not None:
+        out["hess_theta_diag"] = check("hess_theta_diag", r.hess_theta_diag.cpu().numpy(), ref.hess_theta_diag, floor=1e-280)
+    if r.hess_hyper is not None:
+        H = r.hess_hyper.cpu().numpy()
+        assert np.array_equal(H, H.T)
+        out["hess_hyper"] = check("hess_hyper", H, ref.hess_hyper, hess_hyper_scale(ref.hess_hyper))
+    if cross and r.hess_cross is not None:
+        C, O = r.hess_cross.cpu().numpy(), ref.hess_cross
+        mu0, tx, tt, xi0, h, om = ev.params
+        T = ev.t[-1] - ev.t
+        c_m = np.abs(ref.grad_theta + xi0 * (-np.expm1(-om * T)))
+        rr = np.max(np.abs(ref.row_d1 / ref.lam[:, None]), axis=0)
+        colB = rr + np.array([0, 0, 0, 1 / xi0, 40 / h, 1 / om + (ev.t[-1] - ev.t[0])])
+        out["hess_cross"] = check("hess_cross", C, O, c_m[:, None] * colB[None, :] + np.array([0, 0, 0, 1, 0, xi0 * np.max(T)])[None, :], floor=1e-280)
+        for p in range(6):
+            assert np.max(np.abs(C[:, p] - O[:, p])) <= TOL * max(np.max(np.abs(O[:, p])), 1e-280)
+    return out
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,seed,dim,regime,ties,dup", [
+    (2, 1, 2, "mixed", False, False), (3, 2, 2, "excite", False, False), (17, 3, 2, "mixed", True, True),
+    (129, 4, 2, "mixed", False, False), (257, 5, 2, "background", True, False), (300, 6, 1, "mixed", False, True),
+    (300, 7, 3, "excite", True, True), (777, 8, 2, "mixed", True, True), (1500, 9, 3, "mixed", False, False)])
+def test_small_dense_problems_all_outputs(torch, n, seed, dim, regime, ties, dup):
+    """Sizes spanning one thread, one tile, several tiles and ragged tails; D = 1, 2, 3; ties in time
+    and duplicated locations (readings R3/R4); both rate components alive."""
+    ev = synth.small_random(n, seed, dim=dim, regime=regime, ties=ties, duplicates=dup)
+    if n > 64:   # spread the points so that tiles see a mix of near and far pairs
+        ev.x *= math.sqrt(n / 16.0)
+        ev.t *= n / 40.0
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev)
+    assert st == ref.status == 0
+    compare_all(ev, r, lam, ref)
+
+
+def test_worked_examples_on_gpu(torch):
+    """The three worked examples of tests/golden/worked_examples.json (SURVEY.md 8(c) P2')."""
+    import json
+    here = os.path.dirname(os.path.abspath(__file__))
+    g = json.load(open(os.path.join(here, "golden", "worked_examples.json")))
+    for name, c in g["cases"].items():
+        ev = synth.Events(x=np.array(c["x"]), t=np.array(c["t"]), theta=np.array(c["theta"]),
+                          free_idx=np.arange(len(c["t"])), params=tuple(g["params"]))
+        r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD | hp.WANT_HESS_THETA)
+        assert st == 0, name
+        assert abs(r.ll.item() - c["ll"]) < 1e-10 * abs(c["ll"]), name
+        assert np.allclose(r.grad_theta.cpu().numpy(), c["grad_theta"], rtol=1e-10, atol=1e-13), name
+        if "hess_theta_diag" in c:
+            assert np.allclose(r.hess_theta_diag.cpu().numpy(), c["hess_theta_diag"], rtol=1e-10, atol=1e-16), name
+        if "grad_hyper" in c:
+            assert np.allclose(r.grad_hyper.cpu().numpy(), c["grad_hyper"], rtol=1e-10), name
+        if "lambda" in c:
+            assert np.allclose(lam, c["lambda"], rtol=1e-12), name
+
+
+def test_config0_n1000_full_gradient_and_hessian(torch):
+    """BASELINE.json configs[0]: N=1,000, all outputs incl. the N x 6 cross block and the dense
+    theta-theta block."""
+    ev = synth.config(0)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, dense=True, row_d1=True, threads=THREADS)
+    r, st, lam, ctx = run_gpu(torch, ev)
+    assert st == ref.status == 0
+    compare_all(ev, r, lam, ref)
+    x, t, th = dev(torch, ev)
+    H = ctx.hessian_theta_dense(x, t, th, ev.params).cpu().numpy()
+    O = ref.hess_theta_dense
+    d = np.sqrt(np.abs(np.diag(O)))
+    check("hess_theta_dense", H, O, np.outer(d, d), floor=1e-280)
+    assert np.allclose(np.diag(H), r.hess_theta_diag.cpu().numpy(), rtol=1e-10, atol=1e-280)
+
+
+def test_config0_table2_scales(torch):
+    """Same events at the paper's posterior scales (Table 2): nothing underflows there."""
+    ev = synth.config(0)
+    ev.params = synth.TABLE2_PARAMS
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev)
+    assert st == 0
+    compare_all(ev, r, lam, ref)
+
+
+@pytest.fixture(scope="module")
+def cfg1_ref():
+    ev = synth.config(1)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+    return ev, ref
+
+
+def test_config1_n23422_loglik_gradient_hessian(torch, cfg1_ref):
+    """BASELINE.json configs[1] (the headline workload), full oracle, in the launch configuration
+    bench.py times (hawkes_eval with LL | GRAD_THETA | GRAD_HYPER), plus the Hessian outputs."""
+    ev, ref = cfg1_ref
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD, ctx)
+    assert st == ref.status == 0
+    res = compare_all(ev, r, lam, ref, cross=False)
+    r2, st2, lam2, _ = run_gpu(torch, ev, hp.WANT_ALL & ~hp.WANT_HESS_CROSS, ctx)
+    assert st2 == 0
+    compare_all(ev, r2, lam2, ref, cross=False)
+    # the two levels of the pass-1 kernel agree on what they share
+    assert np.allclose(lam, lam2, rtol=1e-13, atol=0)
+    print("max scaled errors", res)
+
+
+def test_entry_points_agree_and_are_deterministic(torch, cfg1_ref):
+    """hawkes_loglik / hawkes_grad / hawkes_hessian / hawkes_eval / hawkes_eval_host return the same
+    bits for the same inputs, run to run (fixed-order reductions, no fp atomics)."""
+    ev, _ = cfg1_ref
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    x, t, th = dev(torch, ev)
+    a = ctx.eval(x, t, th, ev.params, hp.WANT_GRAD)
+    b = ctx.eval(x, t, th, ev.params, hp.WANT_GRAD)
+    g = ctx.grad(x, t, th, ev.params)
+    ll = ctx.loglik(x, t, th, ev.params)
+    hs = ctx.hessian(x, t, th, ev.params)
+    al = ctx.eval(x, t, th, ev.params, hp.WANT_ALL & ~hp.WANT_HESS_CROSS)
+    torch.cuda.synchronize()
+    for f in ("ll", "grad_theta", "grad_hyper"):
+        assert torch.equal(getattr(a, f), getattr(b, f)), f
+        assert torch.equal(getattr(a, f), getattr(g, f)), f
+    assert abs(ll.item() - a.ll.item()) <= 1e-12 * abs(a.ll.item())
+    assert torch.equal(hs.hess_theta_diag, al.hess_theta_diag) and torch.equal(hs.hess_hyper, al.hess_hyper)
+    pin = lambda a_: torch.from_numpy(np.ascontiguousarray(a_)).pin_memory()
+    h = ctx.eval_host(pin(ev.x), pin(ev.t), pin(ev.theta), ev.params, hp.WANT_GRAD)
+    assert h.status == 0
+    assert torch.equal(h.ll, a.ll.cpu()) and torch.equal(h.grad_theta, a.grad_theta.cpu()) and torch.equal(h.grad_hyper, a.grad_hyper.cpu())
+
+
+@pytest.mark.parametrize("n", [50000, 250000])
+def test_scaling_sweep_sampled_rows_and_columns(torch, n):
+    """BASELINE.json configs[4] sizes: the oracle evaluates a seeded sample of 1,024 target rows
+    (lambda_n and d lambda_n/dp) and, once those validate the GPU's lambda, 1,024 source columns
+    (c_m, d_m) with that lambda."""
+    ev = synth.config(4, n=n)
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD | hp.WANT_HESS_THETA, ctx)
+    assert st == 0
+    k = 1024
+    idx = np.sort((synth.uniforms(123, 7, k) * n).astype(np.int64))
+    idx[0], idx[-1] = 0, n - 1
+    lam_o, _ = oracle.rows(ev.x, ev.t, ev.theta, ev.params, idx, derivs=False, threads=THREADS)
+    check("lambda rows", lam[idx], lam_o)
+    c_o, d_o = oracle.cols(ev.x, ev.t, ev.params, lam, idx, threads=THREADS)
+    mu0, tx, tt, xi0, h, om = ev.params
+    integ = xi0 * (-np.expm1(-om * (ev.t[-1] - ev.t[idx])))
+    check("grad_theta cols", r.grad_theta.cpu().numpy()[idx], c_o - integ, np.abs(c_o) + integ)
+    check("hess_theta cols", r.hess_theta_diag.cpu().numpy()[idx], -d_o, floor=1e-280)
+    # properties that hold at any size
+    gt = r.grad_theta.cpu().numpy()
+    assert gt[-1] == 0.0 and np.all(np.isfinite(gt)) and np.all(r.hess_theta_diag.cpu().numpy() <= 0)
+    assert np.all(lam > 0) and math.isfinite(r.ll.item())
+
+
+# ---------------------------------------------------------------------------------------------
+def test_degenerate_and_error_cases(torch):
+    # N = 1: lambda_1 = 0 -> ll = -inf and the zero-rate warning (pin P1)
+    ev = synth.Events(x=np.array([[1.0], [2.0]]), t=np.array([3.7]), theta=np.array([1.3]),
+                      free_idx=np.arange(1), params=synth.CONFIG_PARAMS)
+    r, st, lam, ctx = run_gpu(torch, ev, hp.WANT_GRAD)
+    assert st == hp.WARN_ZERO_RATE and lam[0] == 0.0 and r.ll.item() == -math.inf
+    assert r.grad_theta.item() == 0.0
+    # two simultaneous events at one place: both rates exactly zero
+    ev2 = synth.Events(x=np.array([[1.0, 1.0], [2.0, 2.0]]), t=np.array([1.0, 1.0]), theta=np.ones(2),
+                       free_idx=np.arange(2), params=synth.CONFIG_PARAMS)
+    r, st, lam, _ = run_gpu(torch, ev2, hp.WANT_LL)
+    assert st == hp.WARN_ZERO_RATE and np.all(lam == 0.0)
+    # unsorted times / non-finite input are reported by the device status
+    ev3 = synth.small_random(300, 1)
+    x, t, th = dev(torch, ev3)
+    ctx = hp.HawkesContext(300, 2)
+    tt = t.clone(); tt[[10, 200]] = tt[[200, 10]]
+    ctx.eval(x, tt, th, ev3.params, hp.WANT_LL)
+    assert ctx.last_status() == hp.ERR_UNSORTED
+    xx = x.clone(); xx[1, 5] = float("nan")
+    ctx.eval(xx, t, th, ev3.params, hp.WANT_LL)
+    assert ctx.last_status() == hp.ERR_NONFINITE
+    ctx.eval(x, t, th, ev3.params, hp.WANT_LL)
+    assert ctx.last_status() == 0                      # the status is per evaluation
+    # host-detected errors: nothing is enqueued
+    with pytest.raises(hp.HawkesError) as e:
+        ctx.eval(x, t, th, (0.3, -1.0, 14, 0.7, 1, 1 / 3), hp.WANT_LL)
+    assert e.value.status == hp.ERR_PARAM
+    big = synth.small_random(301, 1)
+    with pytest.raises(hp.HawkesError) as e:
+        ctx.eval(*dev(torch, big), big.params, hp.WANT_LL)
+    assert e.value.status == hp.ERR_ARG
+
+
+def test_underflow_regime_and_far_field(torch):
+    """Bandwidths tiny against the point spread: almost every exponential underflows (the regime of
+    the configs' h = 1 km); and a very wide spread where arguments exceed 2^24 in base-2 units."""
+    ev = synth.small_random(400, 11)
+    ev.x *= 5e4
+    ev.t *= 30.0
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD)
+    assert st == ref.status
+    ok = ref.lam > 1e-280     # below that the oracle's gradual underflow and the flush may differ (R15)
+    check("lambda", lam[ok], ref.lam[ok])
+    assert np.all(lam[~ok] < 1e-270)
+    if ref.status == 0 and np.all(ok):
+        check("ll", r.ll.item(), ref.ll, scales(ev, ref)["ll"])
+
+
+def test_sort_events_helper(torch):
+    ev = synth.small_random(1000, 12, ties=True)
+    perm = np.argsort(synth.uniforms(5, 5, ev.n), kind="stable")
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda")
+    ctx = hp.HawkesContext(ev.n, 2)
+    xo, to, tho, p = ctx.sort_events(f(ev.x[:, perm]), f(ev.t[perm]), f(ev.theta[perm]))
+    torch.cuda.synchronize()
+    order = np.argsort(ev.t[perm], kind="stable")
+    assert np.array_equal(p.cpu().numpy(), order)
+    assert np.array_equal(to.cpu().numpy(), ev.t[perm][order])
+    assert np.array_equal(xo.cpu().numpy(), ev.x[:, perm][:, order])
+    assert np.array_equal(tho.cpu().numpy(), ev.theta[perm][order])
