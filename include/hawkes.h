@@ -146,6 +146,15 @@ int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stre
 /* Launch bookkeeping for benchmarks: number of kernels this context has launched since creation. */
 int64_t hawkes_launch_count(const hawkes_ctx* ctx);
 
+/* Per-kernel device timing for benchmarks.  While enabled, every evaluation queued on the context
+ * records CUDA events on its stream around pass 1, pass 2 (a4) and the whole
+ * evaluation; a ring keeps the most recent 256 evaluations.  hawkes_profile_read() waits for those
+ * evaluations, writes out[0] = number of evaluations summed, out[1] = total pass-1 milliseconds,
+ * out[2] = total pass-2 milliseconds, out[3] = total milliseconds from the first to the last kernel
+ * of the evaluation (out: 4 doubles, HOST), and resets the ring.  Enabling/disabling also resets it. */
+int hawkes_profile_enable(hawkes_ctx* ctx, int enable);
+int hawkes_profile_read(hawkes_ctx* ctx, double* out /*HOST*/);
+
 /* Measures the fp64 FMA issue peak of the device with a register-resident DFMA-chain kernel run for
  * about `millis` milliseconds on `stream`; returns DFMA TFLOP/s (2 flops per FMA) in *tflops.
  * Synchronises.  Used by bench.py for the measured roofline denominator. */

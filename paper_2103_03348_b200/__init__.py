@@ -192,6 +192,19 @@ class HawkesContext:
     def launch_count(self) -> int:
         return int(self._lib.hawkes_launch_count(self._h))
 
+    def profile_enable(self, enable: bool = True):
+        rc = self._lib.hawkes_profile_enable(self._h, 1 if enable else 0)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_profile_enable")
+
+    def profile_read(self) -> dict:
+        """Sums over the evaluations recorded since the last read (at most 256)."""
+        out = (ctypes.c_double * 4)()
+        rc = self._lib.hawkes_profile_read(self._h, out)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_profile_read")
+        return {"evals": int(out[0]), "pass1_ms": out[1], "pass2_ms": out[2], "total_ms": out[3]}
+
     def fp64_peak(self, millis: float = 200.0) -> float:
         v = ctypes.c_double(0.0)
         rc = self._lib.hawkes_fp64_peak(self._h, float(millis), ctypes.byref(v), self._stream())

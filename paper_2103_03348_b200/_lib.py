@@ -33,6 +33,8 @@ SYMBOLS = {
     "hawkes_sort_events": (cint, [vp, i64, cint, _dp, _dp, _dp, _dp, _dp, _dp, vp, vp]),
     "hawkes_get_lambda": (cint, [vp, i64, _dp, vp]),
     "hawkes_launch_count": (i64, [vp]),
+    "hawkes_profile_enable": (cint, [vp, cint]),
+    "hawkes_profile_read": (cint, [vp, ctypes.POINTER(ctypes.c_double)]),
     "hawkes_fp64_peak": (cint, [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]),
 }
 

@@ -37,6 +37,7 @@ constexpr int RED_T = 256;     // threads per CTA in the O(N) kernels
 constexpr int NRED = 34;       // per-event scalar sums reduced over n (see reduce1_kernel)
 constexpr int P1_ITEMS_TARGET = 148 * 10;   // pass-1 work items aimed for (10 per SM)
 constexpr int P2_SLOTS_MAX = 16;            // pass-2 partial slots per source tile
+constexpr int PROF_RING = 256;              // evaluations kept by the timing ring
 
 constexpr double MAGIC = 6755399441055744.0 / TAB_N;   // 1.5 * 2^52 / 128: ulp = 1/128
 
@@ -540,10 +541,12 @@ __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt
             if (DIM3) { const double dz = s.z - g[r].z; u = fma(dz, dz, u); }
             const double as = fma(c.rho_s, dt, u);
             const double e = exp2_scaled<MASKED ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, lane_addr);
+            // an acausal pair is no term of the sum: it must add exactly 0 even when 1/lambda_n = inf
+            const double wn = (MASKED && !(dt > 0.0)) ? 0.0 : s.w;
             if (LEVEL == 0) {
-                cm[r] = fma(e, s.w, cm[r]);
+                cm[r] = fma(e, wn, cm[r]);
             } else {
-                const double q = e * s.w;
+                const double q = e * wn;
                 cm[r] += q;
                 dm[r] = fma(q, q, dm[r]);
             }
@@ -750,6 +753,10 @@ struct hawkes_ctx {
     double* d_sort_keys;  // n_max
     int64_t* d_sort_idx;  // n_max
     int64_t launches;
+    // optional per-kernel timing (hawkes_profile_enable): ring of PROF_RING evaluations x 6 events
+    bool prof_on;
+    int64_t prof_count;           // evaluations recorded since the last read
+    cudaEvent_t* prof_ev;         // [PROF_RING * 6] or NULL
 };
 
 namespace {
@@ -828,24 +835,30 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
                  double* hess_theta_diag, double* hess_hyper, double* hess_cross, cudaStream_t st) {
     const Plan pl = make_plan(n);
     if ((size_t)pl.n_split * 12 * (size_t)pl.ld > ctx->part1_doubles) return HAWKES_ERR_NOMEM;
+    cudaEvent_t* pe = ctx->prof_on ? ctx->prof_ev + 6 * (ctx->prof_count % PROF_RING) : nullptr;
     CK(cudaMemsetAsync(ctx->d_status, 0, sizeof(unsigned), st));
+    if (pe) CK(cudaEventRecord(pe[0], st));
     prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status);
     ctx->launches++;
     const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2
                        : ((want & (HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_CROSS)) ? 1 : 0);
     const unsigned g1 = (unsigned)(pl.n_ttiles1 * pl.n_split);
     double* glam = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_glam : nullptr;
+    if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
             pass1_kernel<P1_R, 0, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            if (pe) cudaEventRecord(pe[2], st);
             reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
         case 1:
             pass1_kernel<P1_R, 1, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            if (pe) cudaEventRecord(pe[2], st);
             reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            if (pe) cudaEventRecord(pe[2], st);
             reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
     }
@@ -858,18 +871,27 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     }
     if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
         const dim3 g2((unsigned)pl.n_slots, (unsigned)pl.n_stiles2);
+        if (pe) CK(cudaEventRecord(pe[3], st));
         if (want & HAWKES_WANT_HESS_THETA)
             pass2_kernel<P2_R, 1, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.tpc);
         else
             pass2_kernel<P2_R, 0, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.tpc);
+        if (pe) CK(cudaEventRecord(pe[4], st));
         theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.n_slots,
                                                       (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
                                                       (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr);
         ctx->launches += 2;
+    } else if (pe) {
+        CK(cudaEventRecord(pe[3], st));
+        CK(cudaEventRecord(pe[4], st));
     }
     if (want & HAWKES_WANT_HESS_CROSS) {
         cross_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, ctx->d_trec, ctx->d_glam, n, c, hess_cross);
         ctx->launches++;
+    }
+    if (pe) {
+        CK(cudaEventRecord(pe[5], st));
+        ctx->prof_count++;
     }
     CK(cudaGetLastError());
     return HAWKES_OK;
@@ -914,6 +936,9 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->n_max = n_max;
     c->ld_max = round_up(n_max, 256);
     c->launches = 0;
+    c->prof_on = false;
+    c->prof_count = 0;
+    c->prof_ev = nullptr;
     const int RS = dim == 3 ? 6 : 4;
     const int nblk = (int)((n_max + RED_T - 1) / RED_T);
     c->part1_doubles = part1_bound(n_max);
@@ -959,6 +984,10 @@ void hawkes_destroy(hawkes_ctx* c) {
                     c->d_scal, c->d_in, c->d_out, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
+    if (c->prof_ev) {
+        for (int i = 0; i < PROF_RING * 6; ++i) cudaEventDestroy(c->prof_ev[i]);
+        delete[] c->prof_ev;
+    }
     delete c;
 }
 
@@ -1093,6 +1122,39 @@ int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stre
 }
 
 int64_t hawkes_launch_count(const hawkes_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int hawkes_profile_enable(hawkes_ctx* ctx, int enable) {
+    if (!ctx) return HAWKES_ERR_ARG;
+    CK(cudaSetDevice(ctx->device));
+    if (enable && !ctx->prof_ev) {
+        ctx->prof_ev = new (std::nothrow) cudaEvent_t[PROF_RING * 6];
+        if (!ctx->prof_ev) return HAWKES_ERR_NOMEM;
+        for (int i = 0; i < PROF_RING * 6; ++i)
+            if (cudaEventCreate(&ctx->prof_ev[i]) != cudaSuccess) return HAWKES_ERR_CUDA;
+    }
+    ctx->prof_on = enable != 0;
+    ctx->prof_count = 0;
+    return HAWKES_OK;
+}
+
+int hawkes_profile_read(hawkes_ctx* ctx, double* out) {
+    if (!ctx || !out || !ctx->prof_ev) return HAWKES_ERR_ARG;
+    CK(cudaSetDevice(ctx->device));
+    const int64_t cnt = ctx->prof_count < PROF_RING ? ctx->prof_count : PROF_RING;
+    double p1 = 0.0, p2 = 0.0, tot = 0.0;
+    for (int64_t k = 0; k < cnt; ++k) {
+        cudaEvent_t* e = ctx->prof_ev + 6 * ((ctx->prof_count - 1 - k) % PROF_RING);
+        CK(cudaEventSynchronize(e[5]));
+        float a = 0.f, b = 0.f, t = 0.f;
+        CK(cudaEventElapsedTime(&a, e[1], e[2]));
+        CK(cudaEventElapsedTime(&b, e[3], e[4]));
+        CK(cudaEventElapsedTime(&t, e[0], e[5]));
+        p1 += a; p2 += b; tot += t;
+    }
+    out[0] = (double)cnt; out[1] = p1; out[2] = p2; out[3] = tot;
+    ctx->prof_count = 0;
+    return HAWKES_OK;
+}
 
 int hawkes_fp64_peak(hawkes_ctx* ctx, double millis, double* tflops, void* stream) {
     if (!ctx || !tflops || !(millis > 0.0)) return HAWKES_ERR_ARG;
