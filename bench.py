@@ -1,0 +1,410 @@
+#!/usr/bin/env python
+"""bench.py -- log-lik + gradient evaluations/s of the phylogenetic-Hawkes hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--config 1] [--n N_EVENTS]
+
+One "step" = one pass of the whole hot path through the C-ABI call
+hawkes_grad: log-likelihood, d/dtheta for all N events and d/d(6 hyperparameters), on the seeded
+synthetic events of BASELINE.json configs[1] (N = 23,422).  Rank 0 prints ONE
+JSON line.  Timing is on the device (one CUDA-event pair per step on the launching stream, L2 flushed
+between steps outside the event pairs), maximum over ranks.  With N > 1 (torchrun) every rank
+evaluates its own replica -- the path is single-GPU by design (replicas only),
+so `value` is N replicas' evaluations over the slowest rank's time ("scaling": "weak").
+
+--impl reference times the ORACLE (oracle/, plain CPU fp64) on the host cores on a bounded sample of
+the same workload; it is a deliberately slow baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "loglik_grad_evals_per_s"
+UNIT = "evals/s"
+
+# Algorithmic FP64 work per pair (SURVEY.md 8(d) table with E = the flop
+# count of the exponential actually shipped: 6 DFMA + 1 DADD + 1 DMUL = 8 FP64-pipe instructions, 14 flops).
+EXP_FLOPS, EXP_INSTR = 14, 8
+P1_B_FLOPS, P1_S_FLOPS, P2_FLOPS = 15 + EXP_FLOPS, 9 + EXP_FLOPS, 12 + EXP_FLOPS
+FP64_LANES_PER_SM = 64
+
+
+def pass1_flops(n: int) -> float:
+    """gradient-level pass 1: every ordered pair carries a background term, every causal pair an excitation term"""
+    return float(n) * n * P1_B_FLOPS + 0.5 * n * (n - 1) * P1_S_FLOPS
+
+
+def pass2_flops(n: int) -> float:
+    return 0.5 * n * (n - 1) * P2_FLOPS
+
+
+class ClockSampler:
+    """Samples SM clock, power and throttle reasons of one GPU while the timed region runs
+    (NVML through nvidia_ml_py; falls back to the recipe's nvidia-smi query loop)."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+               0x10: "sync_boost"}
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        self.index, self.period = index, period_s
+        self.sm, self.power, self.reason_bits = [], [], 0
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thr = None
+        self._proc = None
+        self._nvml = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            uuid_index = self._physical_index()
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(uuid_index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        except Exception:
+            self._nvml = None
+            q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+                 "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                 "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+            try:
+                self._proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                               "-lms", "50", "-i", str(self._physical_index())],
+                                              stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            except Exception:
+                self._proc = None
+        return self
+
+    def _physical_index(self) -> int:
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            parts = [p for p in vis.split(",") if p.strip() != ""]
+            if self.index < len(parts) and parts[self.index].strip().isdigit():
+                return int(parts[self.index])
+        return self.index
+
+    def _loop(self):
+        nv = self._nvml
+        while not self._stop.is_set():
+            try:
+                self.sm.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+                self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+            except Exception:
+                try:
+                    self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                except Exception:
+                    pass
+            self._stop.wait(self.period)
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join(timeout=2.0)
+        reasons = [name for bit, name in self.REASONS.items() if self.reason_bits & bit]
+        if self._proc is not None:
+            self._proc.terminate()
+            try:
+                out, _ = self._proc.communicate(timeout=5)
+            except Exception:
+                out = ""
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            seen = set()
+            for line in out.splitlines():
+                f = [s.strip() for s in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    self.sm.append(int(float(f[1])))
+                    self.sm_max = int(float(f[2]))
+                    self.power.append(float(f[3]))
+                except ValueError:
+                    continue
+                for name, val in zip(names, f[5:9]):
+                    if val.lower().startswith("active"):
+                        seen.add(name)
+            reasons = sorted(seen)
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": reasons, "samples": 0}
+        return {"sm_mhz": int(statistics.median(self.sm)), "sm_min_mhz": min(self.sm), "sm_max_mhz": self.sm_max,
+                "power_w_max": round(max(self.power), 1) if self.power else None,
+                "reasons": reasons, "samples": len(self.sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle, timed on the host cores (cpu_baseline leg and --impl reference)
+def oracle_sample_seconds(ev, idx, threads: int) -> float:
+    """Seconds the oracle needs for the sampled target rows (lambda_n and its 6 hyper-derivatives: pass 1)
+    plus the same number of sampled source columns (c_m, d_m: pass 2).  The column routine needs every
+    lambda_n; for timing it is given a vector of ones (same arithmetic, no O(N^2) set-up)."""
+    import numpy as np
+    import oracle
+    t0 = time.perf_counter()
+    oracle.rows(ev.x, ev.t, ev.theta, ev.params, idx, derivs=True, threads=threads)
+    oracle.cols(ev.x, ev.t, ev.params, np.ones(ev.n), idx, threads=threads)
+    return time.perf_counter() - t0
+
+
+def sample_idx(n: int, r: int):
+    import numpy as np
+    r = max(1, min(n, r))
+    return np.unique(np.linspace(0, n - 1, r).astype(np.int64))
+
+
+def cpu_baseline(ev, budget_s: float = 15.0) -> dict:
+    import oracle
+    threads = oracle.max_threads()
+    probe = sample_idx(ev.n, 64)
+    per_row = oracle_sample_seconds(ev, probe, threads) / len(probe)
+    idx = sample_idx(ev.n, int(budget_s / max(per_row, 1e-9)))
+    secs = oracle_sample_seconds(ev, idx, threads)
+    evals_per_s = (len(idx) / ev.n) / secs
+    return {"value": evals_per_s, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{len(idx)} of {ev.n} target rows (lambda_n + 6 hyper-derivatives) and the same {len(idx)} "
+                      f"source columns (c_m), evenly strided, {secs:.1f} s on {threads} OpenMP threads; "
+                      f"evals/s = (rows/N) / seconds",
+            "seconds_per_eval_extrapolated": 1.0 / evals_per_s}
+
+
+def run_reference(args, ev, workload: str) -> dict:
+    """--impl reference: the oracle as it stands, each step a bounded sample of the workload."""
+    import oracle
+    threads = oracle.max_threads()
+    per_row = oracle_sample_seconds(ev, sample_idx(ev.n, 64), threads) / 64.0
+    budget = 150.0 / (args.steps + args.warmup)
+    idx = sample_idx(ev.n, max(16, int(budget / max(per_row, 1e-9))))
+    for _ in range(args.warmup):
+        oracle_sample_seconds(ev, idx, threads)
+    secs = [oracle_sample_seconds(ev, idx, threads) for _ in range(args.steps)]
+    per_eval = (sum(secs) / len(secs)) * ev.n / len(idx)
+    value = 1.0 / per_eval
+    sample = (f"each step = {len(idx)} of {ev.n} target rows + the same source columns, evenly strided, "
+              f"extrapolated by N/rows; {threads} OpenMP threads")
+    return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_eval * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload, "n_events": ev.n, "dim": ev.dim},
+            "gpairs_per_s": ev.n * float(ev.n) * value / 1e9,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA path
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
+
+
+def ncu_traffic(kernel: str):
+    """dram bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.json), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as fh:
+            return json.load(fh).get(kernel)
+    except Exception:
+        return None
+
+
+def run_b200(args, ev, workload: str) -> dict:
+    import numpy as np
+    import torch
+    import paper_2103_03348_b200 as hp
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier(device_ids=[local])
+            torch.cuda.synchronize(dev)
+
+    n, K, W = ev.n, args.steps, args.warmup
+    ctx = hp.HawkesContext(n, ev.dim, local)
+    x = torch.from_numpy(np.ascontiguousarray(ev.x)).to(dev)
+    t = torch.from_numpy(np.ascontiguousarray(ev.t)).to(dev)
+    th = torch.from_numpy(np.ascontiguousarray(ev.theta)).to(dev)
+    out = ctx.new_outputs(n, hp.WANT_GRAD, dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # 2x the 126 MB L2
+
+    def timed(call, steps):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for e0, e1 in evs:
+            flush.zero_()
+            e0.record()
+            call()
+            e1.record()
+        torch.cuda.synchronize(dev)
+        return [e0.elapsed_time(e1) for e0, e1 in evs]
+
+    step = lambda: ctx.grad(x, t, th, ev.params, out=out)
+    # -- device-resident leg ----------------------------------------------------------------------
+    timed(step, W)
+    assert ctx.last_status() == 0, "evaluation reported a data error"
+    barrier()
+    sampler = ClockSampler(local).start()
+    ctx.profile_enable(True)
+    l0 = ctx.launch_count()
+    wall0 = time.perf_counter()
+    ms = timed(step, K)
+    barrier()
+    wall = time.perf_counter() - wall0
+    launches = ctx.launch_count() - l0
+    prof = ctx.profile_read()
+    ctx.profile_enable(False)
+    total_ms = float(sum(ms))
+    # -- end-to-end leg: HOST buffers through hawkes_eval_host (H2D of inputs + D2H of results inside) ----
+    hx, ht, hth = (a.cpu().pin_memory() for a in (x, t, th))
+    hout = ctx.new_outputs(n, hp.WANT_GRAD, "cpu", pinned=True)
+    estep = lambda: ctx.eval_host(hx, ht, hth, ev.params, hp.WANT_GRAD, out=hout)
+    timed(estep, W)
+    barrier()
+    e_ms = timed(estep, K)
+    barrier()
+    e_total = float(sum(e_ms))
+    clocks = sampler.stop()
+    if dist is not None:
+        v = torch.tensor([total_ms, e_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(v, op=dist.ReduceOp.MAX)
+        total_ms, e_total = float(v[0]), float(v[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return {}
+
+    # -- everything below: rank 0 only --------------------------------------------------------------
+    ll_dev = float(out.ll.item())
+    ll_host = float(hout.ll.item())
+    assert ll_dev == ll_host, "device-resident and host-buffer evaluations must be bit-identical"
+    value = world * K / (total_ms * 1e-3)
+    e_value = world * K / (e_total * 1e-3)
+    props = torch.cuda.get_device_properties(dev)
+    sm_max = clocks.get("sm_max_mhz") or 1965
+    peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    peak_dfma = ctx.fp64_peak(200.0)
+    p1_ms = prof["pass1_ms"] / max(prof["evals"], 1)
+    p2_ms = prof["pass2_ms"] / max(prof["evals"], 1)
+    inner_ms = prof["total_ms"] / max(prof["evals"], 1)
+    a1 = pass1_flops(n) / (p1_ms * 1e-3) / 1e12
+    a2 = pass2_flops(n) / (p2_ms * 1e-3) / 1e12
+    # FP64-pipe instructions per pair as the kernels issue them (SASS count): background 18,
+    # excitation 13, pass 2 15
+    p1_instr = float(n) * n * 18 + 0.5 * n * (n - 1) * 13
+    p2_instr = 0.5 * n * (n - 1) * 15
+    instr_peak = props.multi_processor_count * FP64_LANES_PER_SM * sm_max * 1e6
+    res = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload, "n_events": n, "dim": ev.dim, "outputs": "ll + grad_theta[N] + grad_hyper[6]",
+                   "call": "hawkes_grad", "l2": "256 MiB memset between timed steps, outside the per-step event pairs",
+                   "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)"},
+        "gpairs_per_s": float(n) * n * value / 1e9,
+        "kernel_terms_per_s": (float(n) * n + float(n) * (n - 1)) * value,
+        "wall_s_timed_region": wall,
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "e2e": {"value": e_value, "unit": UNIT, "ms_per_step": e_total / K,
+                "h2d_bytes_per_step": int((ev.dim + 2) * n * 8), "d2h_bytes_per_step": int((1 + n + 6) * 8),
+                "call": "hawkes_eval_host (pinned host buffers)"},
+        "roofline": {"bound": "alu", "kernel": "pass1_kernel<R=%d, LEVEL=1>" % 2, "achieved": a1, "peak": peak_nominal,
+                     "unit": "TFLOP/s", "frac": a1 / peak_nominal,
+                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
+                                    f"{sm_max} MHz (clocks.max.sm); MEASURED_PEAKS.json has no FP64 entry",
+                     "peak_measured_dfma": peak_dfma, "frac_of_measured_dfma": a1 / peak_dfma if peak_dfma else None,
+                     "fp64_pipe_issue_frac": p1_instr / (p1_ms * 1e-3) / instr_peak,
+                     "ms_per_launch": p1_ms, "flops_per_launch": pass1_flops(n),
+                     "traffic": ncu_traffic("pass1_kernel")},
+        "roofline_pass2": {"bound": "alu", "kernel": "pass2_kernel", "achieved": a2, "peak": peak_nominal,
+                           "unit": "TFLOP/s", "frac": a2 / peak_nominal,
+                           "frac_of_measured_dfma": a2 / peak_dfma if peak_dfma else None,
+                           "fp64_pipe_issue_frac": p2_instr / (p2_ms * 1e-3) / instr_peak,
+                           "ms_per_launch": p2_ms, "flops_per_launch": pass2_flops(n),
+                           "traffic": ncu_traffic("pass2_kernel")},
+        "kernel_share": {"pass1": p1_ms / inner_ms, "pass2": p2_ms / inner_ms,
+                         "o_n_and_gaps": 1.0 - (p1_ms + p2_ms) / inner_ms, "first_to_last_kernel_ms": inner_ms},
+        "ll": ll_dev,
+    }
+    if args.extras:
+        hout_all = ctx.new_outputs(n, hp.WANT_HESS_THETA | hp.WANT_HESS_HYPER, dev)
+        hstep = lambda: ctx.hessian(x, t, th, ev.params, out=hout_all)
+        timed(hstep, 2)
+        hms = timed(hstep, max(3, K // 4))
+        lstep = lambda: ctx.eval(x, t, th, ev.params, hp.WANT_LL | hp.WANT_GRAD_THETA, out=out)
+        timed(lstep, 2)
+        lms = timed(lstep, max(3, K // 4))
+        res["extras"] = {"hessian_ms": statistics.median(hms), "ll_grad_theta_only_ms": statistics.median(lms),
+                         "step_ms_min": min(ms), "step_ms_median": statistics.median(ms)}
+    if world == 1 and not args.no_cpu_baseline:
+        res["cpu_baseline"] = cpu_baseline(ev, args.cpu_budget)
+    if dist is not None:
+        dist.destroy_process_group()
+    return res
+
+
+def workload_of(args):
+    from paper_2103_03348_b200 import synth
+    if args.n is not None:
+        ev = synth.make_events(args.n, args.seed)
+        return ev, f"BASELINE.json configs[4] generator at N={args.n} (seed {args.seed})"
+    if args.config == 0:
+        return synth.config(0, args.seed), f"BASELINE.json configs[0]: N=1,000 (seed {args.seed})"
+    if args.config == 1:
+        return synth.config(1, args.seed), (f"BASELINE.json configs[1]: N=23,422 events, 60 clusters, 1,610 non-unit "
+                                            f"theta, params (0.3,10,14,0.7,1,1/3), seed {args.seed}")
+    raise SystemExit("bench.py times configs[1] (default), configs[0] or --n N for the scaling sweep")
+
+
+def main() -> int:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--n", type=int, default=None, help="scaling sweep: N events from the same generator")
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--extras", action="store_true", help="also time the Hessian and the theta-only evaluation")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    rank, world, _ = dist_env()
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        ev, workload = workload_of(args)
+        print(json.dumps(run_reference(args, ev, workload)), flush=True)
+        return 0
+    if world != args.gpus and world > 1:
+        args.gpus = world
+    ev, workload = workload_of(args)
+    res = run_b200(args, ev, workload)
+    if rank == 0:
+        print(json.dumps(res), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

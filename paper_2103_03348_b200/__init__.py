@@ -86,9 +86,9 @@ class HawkesContext:
             raise ValueError("expected x [dim, n] (SoA), t [n], theta [n]")
         return n
 
-    def _outputs(self, n, want, device):
+    def _outputs(self, n, want, device, pinned=False):
         torch = self._torch
-        mk = lambda *s: torch.empty(*s, dtype=torch.float64, device=device)
+        mk = lambda *s: torch.empty(*s, dtype=torch.float64, device=device, pin_memory=pinned)
         return EvalResult(
             ll=mk(1) if want & WANT_LL else None,
             grad_theta=mk(n) if want & WANT_GRAD_THETA else None,
@@ -96,6 +96,10 @@ class HawkesContext:
             hess_theta_diag=mk(n) if want & WANT_HESS_THETA else None,
             hess_hyper=mk(6, 6) if want & WANT_HESS_HYPER else None,
             hess_cross=mk(n, 6) if want & WANT_HESS_CROSS else None)
+
+    def new_outputs(self, n, want, device=None, pinned=False) -> EvalResult:
+        """Output buffers for `want`, to be reused across calls through the `out=` arguments."""
+        return self._outputs(n, want, self._dev if device is None else device, pinned)
 
     # -- the C-ABI calls ---------------------------------------------------------------------------
     def eval(self, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None) -> EvalResult:
@@ -121,9 +125,9 @@ class HawkesContext:
             raise HawkesError(rc, "hawkes_loglik")
         return r.ll
 
-    def grad(self, x, t, theta, params) -> EvalResult:
+    def grad(self, x, t, theta, params, out: EvalResult | None = None) -> EvalResult:
         n = self._check_inputs(x, t, theta)
-        r = self._outputs(n, WANT_GRAD, self._dev)
+        r = out if out is not None else self._outputs(n, WANT_GRAD, self._dev)
         p = _params(params)
         rc = self._lib.hawkes_grad(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), _ptr(r.ll),
                                    _ptr(r.grad_theta), _ptr(r.grad_hyper), self._stream())
@@ -131,10 +135,10 @@ class HawkesContext:
             raise HawkesError(rc, "hawkes_grad")
         return r
 
-    def hessian(self, x, t, theta, params, cross: bool = False) -> EvalResult:
+    def hessian(self, x, t, theta, params, cross: bool = False, out: EvalResult | None = None) -> EvalResult:
         n = self._check_inputs(x, t, theta)
         want = WANT_HESS_THETA | WANT_HESS_HYPER | (WANT_HESS_CROSS if cross else 0)
-        r = self._outputs(n, want, self._dev)
+        r = out if out is not None else self._outputs(n, want, self._dev)
         p = _params(params)
         rc = self._lib.hawkes_hessian(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p),
                                       _ptr(r.hess_theta_diag), _ptr(r.hess_hyper), _ptr(r.hess_cross), self._stream())
