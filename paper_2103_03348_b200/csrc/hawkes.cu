@@ -35,8 +35,10 @@ constexpr int TAB_N = 1 << HAWKES_EXP2_TBITS;
 constexpr int TAB_REP = 16;    // replicas of the exp2 table (one per lane of a half-warp)
 constexpr int RED_T = 256;     // threads per CTA in the O(N) kernels
 constexpr int NRED = 34;       // per-event scalar sums reduced over n (see reduce1_kernel)
-constexpr int P1_ITEMS_TARGET = 148 * 10;   // pass-1 work items aimed for (10 per SM)
-constexpr int P2_SLOTS_MAX = 16;            // pass-2 partial slots per source tile
+#ifndef HAWKES_UNROLL
+#define HAWKES_UNROLL 2
+#endif
+constexpr int UNROLL_J = HAWKES_UNROLL;
 constexpr int PROF_RING = 256;              // evaluations kept by the timing ring
 
 constexpr double MAGIC = 6755399441055744.0 / TAB_N;   // 1.5 * 2^52 / 128: ulp = 1/128
@@ -239,7 +241,7 @@ __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt
                                         Mom<LEVEL> (&m)[R], const DevConsts& c,
                                         unsigned lane_addr) {
     constexpr int RS = DIM3 ? 6 : 4;
-#pragma unroll 2
+#pragma unroll UNROLL_J
     for (int j = 0; j < cnt; ++j) {
         const Ev<DIM3> s = read_rec<DIM3>(sbuf + j * RS);
 #pragma unroll
@@ -282,68 +284,130 @@ __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt
     }
 }
 
-// grid.x = n_ttiles * n_split; item (I, s): target tile I (NT*R targets) x source tiles
-// [s*tps, min((s+1)*tps, n_stiles)).  part[(s*NMOM + k)*ld + n].
+// ------------------------------------------------------------------------------------------------
+// Work decomposition of the two pairwise passes ("stream-K" over the linearised pair space).
+// All (tile, streamed event) pairs of a pass are laid out on one cost axis -- tile after tile, and inside
+// a tile its streamed events in index order, each weighted by the FP64 instructions it costs -- and the
+// axis is cut into `P` equal chunks, one per CTA of a single resident wave.  A CTA therefore visits one
+// or a few consecutive tiles and, in each, a contiguous range of streamed events (a "segment"); its
+// accumulators for that segment go to partial slot (cta - first cta of the tile), and the O(N) kernel
+// that follows sums a tile's slots in slot order.  The cut depends only on (n, P), never on timing:
+// results are bit-identical run to run, the wave has no tail, and no atomics are needed.
+struct Split {
+    int64_t n;       // events
+    int64_t chunk;   // cost units per CTA
+    int tile;        // events owned per tile (threads x R)
+    int n_tiles;
+    int w_all;       // cost of a streamed event every owned event pairs with       (pass 1: background)
+    int w_head;      // extra cost of the streamed events with index < tile end     (pass 1: excitation)
+    int tri;         // 1: only streamed events with index >= tile begin are visited (pass 2)
+};
+
+__host__ __device__ inline int64_t split_prefix(const Split& s, int64_t I) {   // cost of tiles [0, I)
+    if (s.tri) return s.n * I - (int64_t)s.tile * (I * (I - 1) / 2);
+    const int64_t nf = s.n / s.tile;                 // full tiles
+    const int64_t If = I < nf ? I : nf;
+    return (int64_t)s.w_all * s.n * I + (int64_t)s.w_head * ((int64_t)s.tile * (If * (If + 1) / 2) + (I > nf ? s.n : 0));
+}
+__host__ __device__ inline int split_tile_of(const Split& s, int64_t c) {      // largest I with prefix(I) <= c
+    int lo = 0, hi = s.n_tiles - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (split_prefix(s, mid) <= c) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+// streamed-event index reached after `c` cost units of tile I (monotone; 0 -> first visited, cost(I) -> n)
+__host__ __device__ inline int64_t split_pos(const Split& s, int64_t I, int64_t c) {
+    if (s.tri) { const int64_t j = I * s.tile + c; return j < s.n ? j : s.n; }
+    int64_t i1 = (I + 1) * s.tile; if (i1 > s.n) i1 = s.n;
+    const int64_t wh = s.w_all + s.w_head;
+    int64_t j = (c < wh * i1) ? c / wh : i1 + (c - wh * i1) / s.w_all;
+    return j < s.n ? j : s.n;
+}
+// first CTA and number of CTAs (= partial slots) that hold a segment of tile I
+__host__ __device__ inline void split_slots(const Split& s, int64_t I, int* first, int* count) {
+    const int64_t a = split_prefix(s, I) / s.chunk, b = (split_prefix(s, I + 1) - 1) / s.chunk;
+    *first = (int)a;
+    *count = (int)(b - a + 1);
+}
+
+// a1: one CTA of the single wave.  part[(slot*NMOM + k)*ld + n], NMOM = 2 NB.
 template <int R, int LEVEL, bool DIM3>
 __global__ void __launch_bounds__(NT) pass1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                    DevConsts c, const double* __restrict__ tab_g,
-                                                   double* __restrict__ part, int n_split, int tps) {
+                                                   double* __restrict__ part, Split sp) {
     constexpr int RS = DIM3 ? 6 : 4;
+    constexpr int TOFF = DIM3 ? 3 : 2;
     constexpr int NB = Mom<LEVEL>::NB;
     __shared__ __align__(16) double tab[TAB_N * TAB_REP];
     __shared__ __align__(16) double sbuf[2][TS * RS];
 
-    const int n_ttiles = gridDim.x / n_split;
-    const int I = n_ttiles - 1 - (int)(blockIdx.x / n_split);   // late (heavier) target tiles first
-    const int sp = blockIdx.x % n_split;
-    const int n_stiles = (int)((n + TS - 1) / TS);
-    const int J0 = sp * tps, J1 = min(J0 + tps, n_stiles);
-    const int64_t i0 = (int64_t)I * (NT * R);
-    const int64_t i1 = min(i0 + (int64_t)NT * R, n);
-
+    const int64_t total = split_prefix(sp, sp.n_tiles);
+    const int64_t lo = (int64_t)blockIdx.x * sp.chunk;
+    if (lo >= total) return;
+    const int64_t hi = min(lo + sp.chunk, total);
     const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
 
-    Ev<DIM3> g[R];
-    Mom<LEVEL> m[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int64_t i = min(i0 + r * NT + threadIdx.x, n - 1);
-        g[r] = read_rec<DIM3>(rec + i * RS);
-#pragma unroll
-        for (int k = 0; k < NB; ++k) { m[r].b[k] = 0.0; m[r].s[k] = 0.0; }
-    }
-    const double t_first = rec[i0 * RS + (DIM3 ? 3 : 2)];   // earliest target time of this tile
+    for (int I = split_tile_of(sp, lo); I < sp.n_tiles; ++I) {
+        const int64_t base = split_prefix(sp, I);
+        if (base >= hi) break;
+        const int64_t cost_I = split_prefix(sp, I + 1) - base;
+        const int64_t jb = split_pos(sp, I, max(lo - base, (int64_t)0));
+        const int64_t je = split_pos(sp, I, min(hi - base, cost_I));
+        const int64_t i0 = (int64_t)I * (NT * R);
+        const int64_t i1 = min(i0 + (int64_t)NT * R, n);
 
-    RecIO<DIM3> io;
-    if (J0 < J1) {
-        io.load(rec, (int64_t)J0 * TS, (int)min((int64_t)TS, n - (int64_t)J0 * TS));
-        io.store(sbuf[0]);
-    }
-    __syncthreads();
-    for (int J = J0; J < J1; ++J) {
-        const int cur = (J - J0) & 1;
-        const int64_t j0 = (int64_t)J * TS;
-        const int cnt = (int)min((int64_t)TS, n - j0);
-        if (J + 1 < J1) io.load(rec, j0 + TS, (int)min((int64_t)TS, n - j0 - TS));
-        if (j0 >= i1) {
-            p1_tile<R, LEVEL, 0, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
-        } else if (j0 + cnt <= i0 && rec[(j0 + cnt - 1) * RS + (DIM3 ? 3 : 2)] < t_first) {
-            p1_tile<R, LEVEL, 1, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
-        } else {
-            p1_tile<R, LEVEL, 2, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+        Ev<DIM3> g[R];
+        Mom<LEVEL> m[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = min(i0 + r * NT + threadIdx.x, n - 1);
+            g[r] = read_rec<DIM3>(rec + i * RS);
+#pragma unroll
+            for (int k = 0; k < NB; ++k) { m[r].b[k] = 0.0; m[r].s[k] = 0.0; }
         }
-        if (J + 1 < J1) io.store(sbuf[cur ^ 1]);
+        const double t_first = rec[i0 * RS + TOFF];   // earliest target time of this tile
+
+        // pieces of the segment [jb, je): cut at multiples of TS so that no piece straddles i0 or i1
+        RecIO<DIM3> io;
+        int64_t a = jb;
+        int64_t b = min(je, (a / TS + 1) * TS);
+        __syncthreads();                               // previous tile's readers are done with sbuf
+        if (a < je) {
+            io.load(rec, a, (int)(b - a));
+            io.store(sbuf[0]);
+        }
         __syncthreads();
-    }
+        int cur = 0;
+        while (a < je) {
+            const int cnt = (int)(b - a);
+            const int64_t a2 = b, b2 = min(je, b + TS);
+            if (a2 < je) io.load(rec, a2, (int)(b2 - a2));
+            if (a >= i1) {
+                p1_tile<R, LEVEL, 0, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+            } else if (b <= i0 && rec[(b - 1) * RS + TOFF] < t_first) {
+                p1_tile<R, LEVEL, 1, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+            } else {
+                p1_tile<R, LEVEL, 2, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+            }
+            if (a2 < je) io.store(sbuf[cur ^ 1]);
+            __syncthreads();
+            cur ^= 1;
+            a = a2;
+            b = b2;
+        }
+        const int slot = (int)((int64_t)blockIdx.x - base / sp.chunk);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int64_t i = i0 + r * NT + threadIdx.x;
-        if (i < n) {
-            double* o = part + (int64_t)sp * (2 * NB) * ld + i;
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = i0 + r * NT + threadIdx.x;
+            if (i < n) {
+                double* o = part + (int64_t)slot * (2 * NB) * ld + i;
 #pragma unroll
-            for (int k = 0; k < NB; ++k) {
-                o[(int64_t)k * ld] = m[r].b[k];
-                o[(int64_t)(NB + k) * ld] = m[r].s[k];
+                for (int k = 0; k < NB; ++k) {
+                    o[(int64_t)k * ld] = m[r].b[k];
+                    o[(int64_t)(NB + k) * ld] = m[r].s[k];
+                }
             }
         }
     }
@@ -386,7 +450,7 @@ __device__ __forceinline__ double norm_cdf(double z) { return 0.5 * erfc(-z * 0.
 template <int LEVEL, bool DIM3>
 __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                         DevConsts c, const double* __restrict__ part,
-                                                        int n_split, double* __restrict__ lam,
+                                                        Split sp, double* __restrict__ lam,
                                                         double* __restrict__ trec, double* __restrict__ glam,
                                                         double* __restrict__ blockpart,
                                                         unsigned* __restrict__ status) {
@@ -398,8 +462,10 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
     for (int k = 0; k < NRED; ++k) v[k] = 0.0;
     if (i < n) {
         double b[6] = {0, 0, 0, 0, 0, 0}, s[6] = {0, 0, 0, 0, 0, 0};
-        for (int sp = 0; sp < n_split; ++sp) {
-            const double* o = part + (int64_t)sp * (2 * NB) * ld + i;
+        int slot0, n_slots;
+        split_slots(sp, i / sp.tile, &slot0, &n_slots);
+        for (int q = 0; q < n_slots; ++q) {
+            const double* o = part + (int64_t)q * (2 * NB) * ld + i;
 #pragma unroll
             for (int k = 0; k < NB; ++k) {
                 b[k] += o[(int64_t)k * ld];
@@ -531,7 +597,7 @@ __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt
                                         double (&cm)[R], double (&dm)[R], const DevConsts& c,
                                         unsigned lane_addr) {
     constexpr int RS = DIM3 ? 6 : 4;
-#pragma unroll 2
+#pragma unroll UNROLL_J
     for (int j = 0; j < cnt; ++j) {
         const Ev<DIM3> s = read_rec<DIM3>(sbuf + j * RS);   // a target; s.w = 1/lambda_n
 #pragma unroll
@@ -554,62 +620,77 @@ __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt
     }
 }
 
-// grid = (P2 slots, n source tiles).  Block (slot, M): sources of tile M (NT*R) x target tiles
-// [Mt0 + slot*tpc, Mt0 + (slot+1)*tpc) where Mt0 is the first streamed tile that can hold a later target.
-// part2[(slot*2 + k)*ld + m], k = 0 (c), 1 (d).
+// a4: one CTA of the single wave (decomposition: see Split above, `tri` form -- the streamed targets of
+// source tile M are those with index >= the tile's first source).  part2[(slot*2 + k)*ld + m], k = 0 (c), 1 (d).
 template <int R, int LEVEL, bool DIM3>
 __global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
                                                    int64_t n, int64_t ld, DevConsts c,
                                                    const double* __restrict__ tab_g, double* __restrict__ part2,
-                                                   int tpc) {
+                                                   Split sp) {
     constexpr int RS = DIM3 ? 6 : 4;
+    constexpr int TOFF = DIM3 ? 3 : 2;
     __shared__ __align__(16) double tab[TAB_N * TAB_REP];
     __shared__ __align__(16) double sbuf[2][TS * RS];
 
-    const int Ms = (int)blockIdx.y;   // early source tiles have the most later targets: heaviest first
-    const int slot = blockIdx.x;
-    const int64_t m0 = (int64_t)Ms * (NT * R);
-    const int64_t m1 = min(m0 + (int64_t)NT * R, n);
-    const int n_ttiles = (int)((n + TS - 1) / TS);
-    const int Jfirst = (int)(m0 / TS);                      // streamed tile holding the first own source
-    const int J0 = Jfirst + slot * tpc, J1 = min(J0 + tpc, n_ttiles);
+    const int64_t total = split_prefix(sp, sp.n_tiles);
+    const int64_t lo = (int64_t)blockIdx.x * sp.chunk;
+    if (lo >= total) return;
+    const int64_t hi = min(lo + sp.chunk, total);
+    const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
 
-    Ev<DIM3> g[R];
-    double cm[R], dm[R];
+    for (int M = split_tile_of(sp, lo); M < sp.n_tiles; ++M) {
+        const int64_t base = split_prefix(sp, M);
+        if (base >= hi) break;
+        const int64_t cost_M = split_prefix(sp, M + 1) - base;
+        const int64_t jb = split_pos(sp, M, max(lo - base, (int64_t)0));
+        const int64_t je = split_pos(sp, M, min(hi - base, cost_M));
+        const int64_t m0 = (int64_t)M * (NT * R);
+        const int64_t m1 = min(m0 + (int64_t)NT * R, n);
+
+        Ev<DIM3> g[R];
+        double cm[R], dm[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int64_t i = min(m0 + r * NT + threadIdx.x, n - 1);
-        g[r] = read_rec<DIM3>(rec + i * RS);
-        cm[r] = 0.0;
-        dm[r] = 0.0;
-    }
-    if (J0 < J1) {
-        const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
-        const double t_last = rec[(m1 - 1) * RS + (DIM3 ? 3 : 2)];   // latest own source time
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = min(m0 + r * NT + threadIdx.x, n - 1);
+            g[r] = read_rec<DIM3>(rec + i * RS);
+            cm[r] = 0.0;
+            dm[r] = 0.0;
+        }
+        const double t_last = rec[(m1 - 1) * RS + TOFF];   // latest own source time
+
         RecIO<DIM3> io;
-        io.load(trec, (int64_t)J0 * TS, (int)min((int64_t)TS, n - (int64_t)J0 * TS));
-        io.store(sbuf[0]);
+        int64_t a = jb;
+        int64_t b = min(je, (a / TS + 1) * TS);
         __syncthreads();
-        for (int J = J0; J < J1; ++J) {
-            const int cur = (J - J0) & 1;
-            const int64_t j0 = (int64_t)J * TS;
-            const int cnt = (int)min((int64_t)TS, n - j0);
-            if (J + 1 < J1) io.load(trec, j0 + TS, (int)min((int64_t)TS, n - j0 - TS));
-            if (j0 >= m1 && trec[j0 * RS + (DIM3 ? 3 : 2)] > t_last) {
+        if (a < je) {
+            io.load(trec, a, (int)(b - a));
+            io.store(sbuf[0]);
+        }
+        __syncthreads();
+        int cur = 0;
+        while (a < je) {
+            const int cnt = (int)(b - a);
+            const int64_t a2 = b, b2 = min(je, b + TS);
+            if (a2 < je) io.load(trec, a2, (int)(b2 - a2));
+            if (a >= m1 && trec[a * RS + TOFF] > t_last) {
                 p2_tile<R, LEVEL, false, DIM3>(sbuf[cur], cnt, g, cm, dm, c, lane_addr);
             } else {
                 p2_tile<R, LEVEL, true, DIM3>(sbuf[cur], cnt, g, cm, dm, c, lane_addr);
             }
-            if (J + 1 < J1) io.store(sbuf[cur ^ 1]);
+            if (a2 < je) io.store(sbuf[cur ^ 1]);
             __syncthreads();
+            cur ^= 1;
+            a = a2;
+            b = b2;
         }
-    }
+        const int slot = (int)((int64_t)blockIdx.x - base / sp.chunk);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int64_t i = m0 + r * NT + threadIdx.x;
-        if (i < n) {
-            part2[(int64_t)(slot * 2 + 0) * ld + i] = cm[r];
-            if (LEVEL >= 1) part2[(int64_t)(slot * 2 + 1) * ld + i] = dm[r];
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = m0 + r * NT + threadIdx.x;
+            if (i < n) {
+                part2[(int64_t)(slot * 2 + 0) * ld + i] = cm[r];
+                if (LEVEL >= 1) part2[(int64_t)(slot * 2 + 1) * ld + i] = dm[r];
+            }
         }
     }
 }
@@ -617,13 +698,15 @@ __global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ re
 // a5 (theta): grad_theta[m] = CS c_m - xi0 (1 - E_m);  hess_theta_diag[m] = - CS^2 d_m.
 template <bool DIM3>
 __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
-                                                      DevConsts c, const double* __restrict__ part2, int n_slots,
+                                                      DevConsts c, const double* __restrict__ part2, Split sp,
                                                       double* __restrict__ grad_theta,
                                                       double* __restrict__ hess_theta_diag) {
     constexpr int RS = DIM3 ? 6 : 4;
     const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
     if (i >= n) return;
     double cs = 0.0, ds = 0.0;
+    int slot0, n_slots;
+    split_slots(sp, i / sp.tile, &slot0, &n_slots);
     for (int s = 0; s < n_slots; ++s) {
         cs += part2[(int64_t)(s * 2 + 0) * ld + i];
         if (hess_theta_diag) ds += part2[(int64_t)(s * 2 + 1) * ld + i];
@@ -728,6 +811,16 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, 
 
 }  // namespace
 
+namespace {
+struct Plan {
+    Split sp1, sp2;   // decomposition of pass 1 / pass 2 (chunk = 0: not planned)
+    int grid1, grid2;
+    int64_t ld;
+    int nblk;         // O(N) kernels
+};
+
+}  // namespace
+
 // =================================================================================================
 // host side
 struct hawkes_ctx {
@@ -740,7 +833,13 @@ struct hawkes_ctx {
     double* d_trec;       // n_max * RS
     double* d_part1;      // pass-1 partials
     size_t part1_doubles;
-    double* d_part2;      // P2_SLOTS_MAX * 2 * ld_max
+    double* d_part2;      // pass-2 partials
+    size_t part2_doubles;
+    int sm_count;
+    int occ1[3], occ2[2];  // resident CTAs per SM of pass1_kernel<LEVEL> / pass2_kernel<LEVEL> for this dim
+    Plan plan;            // cached decomposition of the last (n, level1, level2)
+    int64_t plan_n;
+    int plan_l1, plan_l2;
     double* d_lam;        // n_max
     double* d_glam;       // n_max * 6
     double* d_blockpart;  // nblk_max * NRED
@@ -769,38 +868,52 @@ namespace {
 
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
-constexpr int P1_R = 2;   // targets per thread in pass 1
-constexpr int P2_R = 2;   // sources per thread in pass 2
+#ifndef HAWKES_P1_R
+#define HAWKES_P1_R 2
+#endif
+#ifndef HAWKES_P2_R
+#define HAWKES_P2_R 2
+#endif
+constexpr int P1_R = HAWKES_P1_R;   // targets per thread in pass 1
+constexpr int P2_R = HAWKES_P2_R;   // sources per thread in pass 2
 
-struct Plan {
-    int n_ttiles1, n_split, tps;   // pass 1
-    int n_stiles2, n_slots, tpc;   // pass 2
-    int64_t ld;
-    int nblk;                      // O(N) kernels
-};
+// cost weights of the pass-1 cost axis per LEVEL: 2 x FP64-pipe instructions + other instructions of a
+// background term (every streamed source) and of an excitation term (sources before the tile's end)
+constexpr int W_ALL[3] = {40, 44, 54};
+constexpr int W_HEAD[3] = {29, 33, 43};
 
-Plan make_plan(int64_t n) {
-    Plan p;
-    p.ld = round_up(n, 256);
-    const int n_tiles = (int)((n + TS - 1) / TS);   // streamed tiles
-    p.n_ttiles1 = (int)((n + NT * P1_R - 1) / (NT * P1_R));
-    int want = (P1_ITEMS_TARGET + p.n_ttiles1 - 1) / p.n_ttiles1;
-    if (want < 1) want = 1;
-    if (want > n_tiles) want = n_tiles;
-    p.tps = (n_tiles + want - 1) / want;
-    p.n_split = (n_tiles + p.tps - 1) / p.tps;
-    p.n_stiles2 = (int)((n + NT * P2_R - 1) / (NT * P2_R));
-    p.n_slots = n_tiles < P2_SLOTS_MAX ? n_tiles : P2_SLOTS_MAX;
-    p.tpc = (n_tiles + p.n_slots - 1) / p.n_slots;
-    p.n_slots = (n_tiles + p.tpc - 1) / p.tpc;
-    p.nblk = (int)((n + RED_T - 1) / RED_T);
-    return p;
+// Cut the cost axis of one pass into at most `ctas` chunks whose partial slots fit `cap_doubles`
+// (slots of the fullest tile x moments x ld).  Returns the number of CTAs to launch.
+int plan_split(Split* sp, int64_t n, int tile, int w_all, int w_head, int tri, int ctas, int64_t ld, int n_mom,
+               size_t cap_doubles) {
+    sp->n = n;
+    sp->tile = tile;
+    sp->n_tiles = (int)((n + tile - 1) / tile);
+    sp->w_all = w_all;
+    sp->w_head = w_head;
+    sp->tri = tri;
+    const int64_t total = split_prefix(*sp, sp->n_tiles);
+    const int64_t min_chunk = (int64_t)(tri ? 1 : w_all + w_head) * 32;   // >= ~32 streamed events per CTA
+    int64_t chunk = (total + ctas - 1) / ctas;
+    if (chunk < min_chunk) chunk = min_chunk;
+    for (;;) {
+        sp->chunk = chunk;
+        int worst = 0;
+        for (int I = 0; I < sp->n_tiles; ++I) {
+            int first, count;
+            split_slots(*sp, I, &first, &count);
+            if (count > worst) worst = count;
+        }
+        if ((size_t)worst * n_mom * (size_t)ld <= cap_doubles) break;
+        chunk *= 2;
+    }
+    return (int)((total + sp->chunk - 1) / sp->chunk);
 }
 
-size_t part1_bound(int64_t n_max) {
-    // n_split * ld <= (P1_ITEMS_TARGET / n_ttiles + 1) * ld  <~  P1_ITEMS_TARGET * NT*R * (ld/n) + ld;
-    // generous, and enqueue_eval() re-checks the actual plan against it.
-    return (size_t)12 * ((size_t)2 * P1_ITEMS_TARGET * NT * P1_R + 4 * (size_t)round_up(n_max, 256));
+size_t part_bound(int64_t n_max, int ctas_max, int tile, int n_mom) {
+    // slots x ld  <~  1.3 ctas x tile + 2 ld  (see plan_split); generous, and plan_split() coarsens the cut
+    // if an actual plan would not fit
+    return (size_t)n_mom * ((size_t)2 * ctas_max * tile + 4 * (size_t)round_up(n_max, 256));
 }
 
 int make_consts(const hawkes_params* p, int dim, DevConsts* c) {
@@ -833,33 +946,43 @@ template <bool DIM3>
 int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
                  const DevConsts& c, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
                  double* hess_theta_diag, double* hess_hyper, double* hess_cross, cudaStream_t st) {
-    const Plan pl = make_plan(n);
-    if ((size_t)pl.n_split * 12 * (size_t)pl.ld > ctx->part1_doubles) return HAWKES_ERR_NOMEM;
+    const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2
+                       : ((want & (HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_CROSS)) ? 1 : 0);
+    const int level2 = (want & HAWKES_WANT_HESS_THETA) ? 1 : 0;
+    if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2) {
+        Plan& q = ctx->plan;
+        q.ld = round_up(n, 256);
+        q.nblk = (int)((n + RED_T - 1) / RED_T);
+        q.grid1 = plan_split(&q.sp1, n, NT * P1_R, W_ALL[level1], W_HEAD[level1], 0, ctx->sm_count * ctx->occ1[level1],
+                             q.ld, 12, ctx->part1_doubles);
+        q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, ctx->sm_count * ctx->occ2[level2], q.ld, 2,
+                             ctx->part2_doubles);
+        ctx->plan_n = n; ctx->plan_l1 = level1; ctx->plan_l2 = level2;
+    }
+    const Plan& pl = ctx->plan;
     cudaEvent_t* pe = ctx->prof_on ? ctx->prof_ev + 6 * (ctx->prof_count % PROF_RING) : nullptr;
     CK(cudaMemsetAsync(ctx->d_status, 0, sizeof(unsigned), st));
     if (pe) CK(cudaEventRecord(pe[0], st));
     prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status);
     ctx->launches++;
-    const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2
-                       : ((want & (HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_CROSS)) ? 1 : 0);
-    const unsigned g1 = (unsigned)(pl.n_ttiles1 * pl.n_split);
+    const unsigned g1 = (unsigned)pl.grid1;
     double* glam = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_glam : nullptr;
     if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
-            pass1_kernel<P1_R, 0, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            pass1_kernel<P1_R, 0, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
         case 1:
-            pass1_kernel<P1_R, 1, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            pass1_kernel<P1_R, 1, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
         default:
-            pass1_kernel<P1_R, 2, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.n_split, pl.tps);
+            pass1_kernel<P1_R, 2, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.n_split, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
     }
     ctx->launches += 2;
@@ -870,14 +993,14 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         ctx->launches++;
     }
     if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
-        const dim3 g2((unsigned)pl.n_slots, (unsigned)pl.n_stiles2);
+        const unsigned g2 = (unsigned)pl.grid2;
         if (pe) CK(cudaEventRecord(pe[3], st));
         if (want & HAWKES_WANT_HESS_THETA)
-            pass2_kernel<P2_R, 1, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.tpc);
+            pass2_kernel<P2_R, 1, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
         else
-            pass2_kernel<P2_R, 0, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.tpc);
+            pass2_kernel<P2_R, 0, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
         if (pe) CK(cudaEventRecord(pe[4], st));
-        theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.n_slots,
+        theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.sp2,
                                                       (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
                                                       (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr);
         ctx->launches += 2;
@@ -894,6 +1017,18 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         ctx->prof_count++;
     }
     CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+template <bool DIM3>
+int query_occupancy(hawkes_ctx* ctx) {
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ1[0], pass1_kernel<P1_R, 0, DIM3>, NT, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ1[1], pass1_kernel<P1_R, 1, DIM3>, NT, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ1[2], pass1_kernel<P1_R, 2, DIM3>, NT, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ2[0], pass2_kernel<P2_R, 0, DIM3>, NT, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ2[1], pass2_kernel<P2_R, 1, DIM3>, NT, 0));
+    for (int k = 0; k < 3; ++k) if (ctx->occ1[k] < 1) return HAWKES_ERR_CUDA;
+    for (int k = 0; k < 2; ++k) if (ctx->occ2[k] < 1) return HAWKES_ERR_CUDA;
     return HAWKES_OK;
 }
 
@@ -941,7 +1076,21 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->prof_ev = nullptr;
     const int RS = dim == 3 ? 6 : 4;
     const int nblk = (int)((n_max + RED_T - 1) / RED_T);
-    c->part1_doubles = part1_bound(n_max);
+    c->plan_n = -1;
+    c->plan_l1 = c->plan_l2 = -1;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess ||
+        (dim == 3 ? query_occupancy<true>(c) : query_occupancy<false>(c)) != HAWKES_OK) {
+        delete c;
+        cudaGetLastError();
+        return HAWKES_ERR_CUDA;
+    }
+    c->sm_count = prop.multiProcessorCount;
+    int occ1 = 1, occ2 = 1;
+    for (int k = 0; k < 3; ++k) occ1 = c->occ1[k] > occ1 ? c->occ1[k] : occ1;
+    for (int k = 0; k < 2; ++k) occ2 = c->occ2[k] > occ2 ? c->occ2[k] : occ2;
+    c->part1_doubles = part_bound(n_max, c->sm_count * occ1, NT * P1_R, 12);
+    c->part2_doubles = part_bound(n_max, c->sm_count * occ2, NT * P2_R, 2);
     c->cub_bytes = 0;
     cub::DeviceRadixSort::SortPairs(nullptr, c->cub_bytes, (const double*)nullptr, (double*)nullptr,
                                     (const int64_t*)nullptr, (int64_t*)nullptr, (int)n_max);
@@ -955,7 +1104,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
     alloc((void**)&c->d_trec, sizeof(double) * RS * (size_t)c->ld_max);
     alloc((void**)&c->d_part1, sizeof(double) * c->part1_doubles);
-    alloc((void**)&c->d_part2, sizeof(double) * 2 * P2_SLOTS_MAX * (size_t)c->ld_max);
+    alloc((void**)&c->d_part2, sizeof(double) * c->part2_doubles);
     alloc((void**)&c->d_lam, sizeof(double) * (size_t)c->ld_max);
     alloc((void**)&c->d_glam, sizeof(double) * 6 * (size_t)c->ld_max);
     alloc((void**)&c->d_blockpart, sizeof(double) * NRED * (size_t)nblk);
