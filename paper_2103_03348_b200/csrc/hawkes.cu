@@ -12,9 +12,15 @@
 // (step names a0..a5 are SURVEY.md section 8(a)'s).
 //
 // fp64 exp: every kernel term is 2^z with z = -(scaled squared distances); z is split as
-// z = n/128 + f, n integer, |f| <= 1/256;  2^z = 2^(n>>7) * T[n&127] * p(f)  with T a 128-entry table
-// replicated 16x in shared memory (bank-conflict-free for any index pattern) and p a degree-4
-// polynomial: 8 FP64-pipe instructions per exponential instead of the ~15-18 of exp(double).
+// z = n/256 + f, n integer, |f| <= 1/512;  2^z = 2^(n>>8) * T[n&255] * p(f)  with T a 256-entry table
+// replicated once per lane in shared memory (64 KB, bank-conflict-free for any index pattern) and p a
+// degree-4 polynomial: 8 FP64-pipe instructions per exponential instead of the ~15-18 of exp(double).
+//
+// Issue model (measured on B200): an FP64 instruction holds its scheduler's issue
+// port for 2 cycles and nothing else issues beside it, so a warp-instruction stream costs
+// 2 x (FP64 instructions) + (all other instructions) cycles.  The inner loops are therefore written to
+// minimise the non-FP64 instructions as well: one PRMT forms the table address, one IMAD inserts the
+// exponent, and terms that must vanish are dropped by predicating their accumulation.
 #include "../../include/hawkes.h"
 
 #include <cuda_runtime.h>
@@ -29,19 +35,21 @@
 
 namespace {
 
-constexpr int NT = 128;        // threads per CTA in the pairwise kernels
+constexpr int NT = 128;        // threads per work group in the pairwise kernels (one stream-K worker)
 constexpr int TS = 128;        // events per streamed shared-memory tile
 constexpr int TAB_N = 1 << HAWKES_EXP2_TBITS;
-constexpr int TAB_REP = 16;    // replicas of the exp2 table (one per lane of a half-warp)
+static_assert(TAB_N == 256, "the PRMT addressing below takes the low byte of n as the table row");
+constexpr int TAB_ROW = 256;   // bytes per table row: 32 lane replicas of one fp64 entry
+constexpr unsigned TAB_BYTES = TAB_N * TAB_ROW;   // 64 KB, placed on a 64 KB boundary of the shared window
 constexpr int RED_T = 256;     // threads per CTA in the O(N) kernels
 constexpr int NRED = 34;       // per-event scalar sums reduced over n (see reduce1_kernel)
 #ifndef HAWKES_UNROLL
-#define HAWKES_UNROLL 2
+#define HAWKES_UNROLL 4
 #endif
 constexpr int UNROLL_J = HAWKES_UNROLL;
 constexpr int PROF_RING = 256;              // evaluations kept by the timing ring
 
-constexpr double MAGIC = 6755399441055744.0 / TAB_N;   // 1.5 * 2^52 / 128: ulp = 1/128
+constexpr double MAGIC = 6755399441055744.0 / TAB_N;   // 1.5 * 2^52 / 256: ulp = 1/256
 
 // constants of one evaluation, passed by value to every kernel
 struct DevConsts {
@@ -52,6 +60,8 @@ struct DevConsts {
     double CB;      // mu0 (2 pi)^-(D+1)/2 tau_x^-D tau_t^-1
     double CS;      // xi0 omega (2 pi)^-D/2 h^-D
     double mu0, tau_x, tau_t, xi0, h, omega;
+    double CBS, CSS;         // CB S and CS S: the pairwise kernels sum 2^z / S (S = HAWKES_EXP2_S)
+    double d0, d1, d2, d3;   // monic polynomial q(f) = 2^f / S (uniform-register operands of the Horner steps)
     int lim_b_hi;   // hi word of the smallest argument whose background exponential is flushed to 0
     int lim_s_hi;
     int dim;
@@ -60,91 +70,110 @@ struct DevConsts {
 enum { ST_UNSORTED = 1, ST_NONFINITE = 2, ST_ZERO_RATE = 4 };
 
 // ------------------------------------------------------------------------------------------------
-// fp64 2^(a * negc) for a >= 0 (negc < 0); returns exactly 0 when hi(a) >= lim_hi or `kill`.
-// FP64 pipe: DFMA, DADD, DFMA (reduction), 4 DFMA (polynomial), DMUL = 8.  Everything else (index,
-// table load, exponent insertion, predicate) runs on the integer / load-store pipes:
-//   t = a*negc + MAGIC leaves n = round(128 z) in the low word of t (z = a*negc);  j = n & 127;
-//   the table entry is the bit pattern of 2^(j/128) with (j << 13) subtracted from its high word, so
-//   that adding (n << 13) = (k << 20) + (j << 13) to it multiplies by 2^k, k = n >> 7, in one integer op.
-// A lane whose term must vanish (underflow, coincident location, acausal pair) looks up n = N_DEAD
-// instead: entry 0 is 1.0 (zero mantissa) and k = -1023 cancels its exponent field, so the assembled
-// bit pattern is exactly +0.0 -- no select on the result.
-// `lane_addr` is the shared-space address of this lane's replica of entry 0 (table + 8 * (lane & 15)).
+// fp64 2^(a * negc) / S for a >= 0 (negc < 0); returns exactly 0 when hi(a) >= lim_hi or the pair is killed.
+// FP64 pipe: DFMA, DADD, DFMA (reduction), DADD + 3 DFMA (polynomial), DMUL = 8.  Integer / load-store:
+//   t = a*negc + MAGIC leaves n = round(256 z) in the low word of t (z = a*negc);
+//   ISETP/SEL  a term that must vanish (underflow R15, coincident location R3, acausal pair R4) looks up
+//         n = N_DEAD instead: row 0 is 1.0 (zero mantissa) and k = -1023 cancels its exponent field, so
+//         the assembled bit pattern is exactly +0.0 -- no select on the fp64 result;
+//   PRMT  address = {table base bytes 3,2 | low byte of n | lane*8}: row n&255, this lane's replica;
+//   LDS   the entry: bit pattern of 2^(j/256) with (j << 12) subtracted from its high word, so that
+//   IMAD  hi += n << 12 = (k << 20) + (j << 12) multiplies it by 2^k, k = n >> 8.
+// `lane_base` = shared-space address of the table (64 KB aligned) | lane*8.
 constexpr int N_DEAD = -1023 * TAB_N;
 // KILL_MODE 0: no extra kill; 1: kill when kv == 0 (kv = r2, the coincident-location indicator);
 // 2: kill unless kv > 0 (kv = dt, the causal indicator; fp64 compare).
+struct ExpC {       // loop-invariant operands of the exponential
+    double d0, d1, d2, d3;   // monic polynomial: from the kernel parameters (uniform registers)
+    double magic;            // MAGIC as a run-time value in a vector register (see pinned_consts)
+};
 template <int KILL_MODE>
-__device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi, double kv, unsigned lane_addr) {
-    const double t = fma(a, negc, MAGIC);
-    const double nf = t - MAGIC;
+__device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi, double kv, const ExpC& c,
+                                              unsigned lane_base) {
+    // operand discipline: an FP64 instruction reading three distinct vector registers
+    // issues every 3 cycles, one reading two every 2.  negc and the polynomial constants therefore sit in
+    // uniform registers, MAGIC in a vector register, and the polynomial is monic so that each Horner step has
+    // one constant: q(f) = (((f + d3) f + d2) f + d1) f + d0 = 2^f / S.
+    const double t = fma(a, negc, c.magic);
+    const double nf = t - c.magic;
     const double f = fma(a, negc, -nf);
-    double p = fma(f, HAWKES_EXP2_C4, HAWKES_EXP2_C3);
-    p = fma(p, f, HAWKES_EXP2_C2);
-    p = fma(p, f, HAWKES_EXP2_C1);
-    p = fma(p, f, 1.0);
+    double p = f + c.d3;
+    p = fma(p, f, c.d2);
+    p = fma(p, f, c.d1);
+    p = fma(p, f, c.d0);
     double T;
-    if (KILL_MODE == 1) {
+#define HAWKES_EXP2_TAIL                                 \
+        "selp.s32 ne, n, %4, p;\n\t"                     \
+        "prmt.b32 ad, ne, %5, 0x7604;\n\t"               \
+        "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"           \
+        "mad.lo.s32 hi, ne, 4096, hi;\n\t"               \
+        "mov.b64 %0, {lo, hi};\n\t"                      \
+        "}"                                              \
+        : "=d"(T) : "d"(a), "d"(t), "r"(lim_hi), "n"(N_DEAD), "r"(lane_base), "d"(kv)
+    if constexpr (KILL_MODE == 1) {
         asm("{\n\t"
             ".reg .pred p;\n\t"
-            ".reg .b32 alo, ahi, n, thi, klo, khi, ne, j, ad, lo, hi;\n\t"
+            ".reg .b32 alo, ahi, n, thi, klo, khi, ne, ad, lo, hi;\n\t"
             "mov.b64 {alo, ahi}, %1;\n\t"
             "mov.b64 {n, thi}, %2;\n\t"
-            "mov.b64 {klo, khi}, %3;\n\t"
+            "mov.b64 {klo, khi}, %6;\n\t"
             "or.b32 klo, klo, khi;\n\t"
             "setp.ne.s32 p, klo, 0;\n\t"
-            "setp.lt.and.s32 p, ahi, %4, p;\n\t"
-            "selp.s32 ne, n, %5, p;\n\t"
-            "and.b32 j, ne, 127;\n\t"
-            "mad.lo.u32 ad, j, 128, %6;\n\t"
-            "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"
-            "mad.lo.s32 hi, ne, 8192, hi;\n\t"
-            "mov.b64 %0, {lo, hi};\n\t"
-            "}"
-            : "=d"(T) : "d"(a), "d"(t), "d"(kv), "r"(lim_hi), "n"(N_DEAD), "r"(lane_addr));
-    } else if (KILL_MODE == 2) {
+            "setp.lt.and.s32 p, ahi, %3, p;\n\t"
+            HAWKES_EXP2_TAIL);
+    } else if constexpr (KILL_MODE == 2) {
         asm("{\n\t"
             ".reg .pred p;\n\t"
-            ".reg .b32 alo, ahi, n, thi, ne, j, ad, lo, hi;\n\t"
+            ".reg .b32 alo, ahi, n, thi, ne, ad, lo, hi;\n\t"
             "mov.b64 {alo, ahi}, %1;\n\t"
             "mov.b64 {n, thi}, %2;\n\t"
-            "setp.gt.f64 p, %3, 0d0000000000000000;\n\t"
-            "setp.lt.and.s32 p, ahi, %4, p;\n\t"
-            "selp.s32 ne, n, %5, p;\n\t"
-            "and.b32 j, ne, 127;\n\t"
-            "mad.lo.u32 ad, j, 128, %6;\n\t"
-            "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"
-            "mad.lo.s32 hi, ne, 8192, hi;\n\t"
-            "mov.b64 %0, {lo, hi};\n\t"
-            "}"
-            : "=d"(T) : "d"(a), "d"(t), "d"(kv), "r"(lim_hi), "n"(N_DEAD), "r"(lane_addr));
+            "setp.gt.f64 p, %6, 0d0000000000000000;\n\t"
+            "setp.lt.and.s32 p, ahi, %3, p;\n\t"
+            HAWKES_EXP2_TAIL);
     } else {
         asm("{\n\t"
             ".reg .pred p;\n\t"
-            ".reg .b32 alo, ahi, n, thi, ne, j, ad, lo, hi;\n\t"
+            ".reg .b32 alo, ahi, n, thi, ne, ad, lo, hi;\n\t"
             "mov.b64 {alo, ahi}, %1;\n\t"
             "mov.b64 {n, thi}, %2;\n\t"
             "setp.lt.s32 p, ahi, %3;\n\t"
-            "selp.s32 ne, n, %4, p;\n\t"
-            "and.b32 j, ne, 127;\n\t"
-            "mad.lo.u32 ad, j, 128, %5;\n\t"
-            "ld.shared.v2.b32 {lo, hi}, [ad];\n\t"
-            "mad.lo.s32 hi, ne, 8192, hi;\n\t"
-            "mov.b64 %0, {lo, hi};\n\t"
-            "}"
-            : "=d"(T) : "d"(a), "d"(t), "r"(lim_hi), "n"(N_DEAD), "r"(lane_addr));
+            HAWKES_EXP2_TAIL);
     }
+#undef HAWKES_EXP2_TAIL
     return T * p;
 }
 
-// fill the 16x replicated table (entry j, replica r at tab[j*16 + r]) with the biased bit patterns
-// and return the table's shared-space address.
-__device__ __forceinline__ unsigned fill_table(double* tab, const double* __restrict__ tab_g) {
-    for (int i = threadIdx.x; i < TAB_N * TAB_REP; i += blockDim.x) {
-        const int j = i / TAB_REP;
+// fill the table (entry j, replica r at byte j*256 + r*8) with the biased bit patterns
+__device__ __forceinline__ void fill_table(double* tab, const double* __restrict__ tab_g) {
+    for (int i = threadIdx.x; i < TAB_N * 32; i += blockDim.x) {
+        const int j = i >> 5;
         const double v = tab_g[j];
-        tab[i] = __hiloint2double(__double2hiint(v) - (j << 13), __double2loint(v));
+        tab[i] = __hiloint2double(__double2hiint(v) - (j << 12), __double2loint(v));
     }
-    return (unsigned)__cvta_generic_to_shared(tab);
+}
+
+// shared-memory plan of a pairwise CTA: the 64 KB table on the first 64 KB boundary of the dynamic
+// allocation, the groups' streaming buffers in the gap before it if they fit there, else after it.
+struct SmemPlan {
+    unsigned tab_off;   // byte offsets from the start of the dynamic allocation
+    unsigned buf_off;
+};
+__device__ __forceinline__ SmemPlan smem_plan(unsigned base, unsigned buf_bytes) {
+    SmemPlan sp;
+    sp.tab_off = ((base + 0xffffu) & ~0xffffu) - base;
+    sp.buf_off = (sp.tab_off >= buf_bytes) ? 0u : sp.tab_off + TAB_BYTES;
+    return sp;
+}
+// dynamic shared memory to request.  gap = distance to the boundary (< 64 KB): buffers in the gap need
+// gap + 64 KB <= 128 KB; buffers after the table (gap < buf) need gap + 64 KB + buf < 64 KB + 2 buf.
+constexpr unsigned smem_request(unsigned buf_bytes) {
+    return 2u * buf_bytes > TAB_BYTES ? TAB_BYTES + 2u * buf_bytes : 2u * TAB_BYTES;
+}
+constexpr unsigned SMEM_MAX = 227u * 1024u;
+template <bool DIM3> constexpr unsigned group_buf_bytes() { return 2u * TS * (DIM3 ? 6 : 4) * sizeof(double); }
+
+__device__ __forceinline__ void group_sync(int grp) {
+    asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(NT) : "memory");
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -184,18 +213,18 @@ struct RecIO {
     static constexpr int CH = RS / 2;                       // 16-byte chunks per record
     static constexpr int PER_THREAD = TS * CH / NT;         // chunks each thread moves per tile
     double2 v[PER_THREAD];
-    __device__ __forceinline__ void load(const double* __restrict__ src, int64_t first, int cnt) {
+    __device__ __forceinline__ void load(const double* __restrict__ src, int64_t first, int cnt, int tid) {
         const double2* g = reinterpret_cast<const double2*>(src) + first * CH;
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
-            const int c = threadIdx.x + q * NT;
+            const int c = tid + q * NT;
             v[q] = (c < cnt * CH) ? __ldg(g + c) : make_double2(0.0, 0.0);
         }
     }
-    __device__ __forceinline__ void store(double* buf) const {
+    __device__ __forceinline__ void store(double* buf, int tid) const {
         double2* s = reinterpret_cast<double2*>(buf);
 #pragma unroll
-        for (int q = 0; q < PER_THREAD; ++q) s[threadIdx.x + q * NT] = v[q];
+        for (int q = 0; q < PER_THREAD; ++q) s[tid + q * NT] = v[q];
     }
 };
 
@@ -236,10 +265,23 @@ struct Mom {
 
 // MODE 0: background only (all sources at or after the targets); 1: both terms, every pair causal;
 // 2: both terms with the per-pair test dt > 0 (diagonal tiles and tiles a tie straddles).
+struct P1C {        // loop-invariant operands of the pairwise loops
+    double negcb, negcs, rho_b, rho_s;
+    int lim_b_hi, lim_s_hi;
+    ExpC e;
+};
+// MAGIC takes a round trip through shared memory: as a literal it would be the immediate of t = a negc + MAGIC,
+// which forces negc into a vector register and makes f = a negc - nf a three-register DFMA.
+__device__ __forceinline__ void stash_consts(double& smagic) {
+    if (threadIdx.x == 0) smagic = MAGIC;
+}
+__device__ __forceinline__ P1C pinned_consts(const double& smagic, const DevConsts& c) {   // after the barrier
+    const volatile double& v = smagic;
+    return P1C{c.negcb, c.negcs, c.rho_b, c.rho_s, c.lim_b_hi, c.lim_s_hi, {c.d0, c.d1, c.d2, c.d3, v}};
+}
 template <int R, int LEVEL, int MODE, bool DIM3>
 __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt, const Ev<DIM3> (&g)[R],
-                                        Mom<LEVEL> (&m)[R], const DevConsts& c,
-                                        unsigned lane_addr) {
+                                        Mom<LEVEL> (&m)[R], const P1C& c, unsigned lane_base) {
     constexpr int RS = DIM3 ? 6 : 4;
 #pragma unroll UNROLL_J
     for (int j = 0; j < cnt; ++j) {
@@ -251,7 +293,7 @@ __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt
             if (DIM3) { const double dz = g[r].z - s.z; u = fma(dz, dz, u); }
             const double w = dt * dt;
             const double ab = fma(c.rho_b, w, u);
-            const double eB = exp2_scaled<1>(ab, c.negcb, c.lim_b_hi, u, lane_addr);
+            const double eB = exp2_scaled<1>(ab, c.negcb, c.lim_b_hi, u, c.e, lane_base);
             m[r].b[0] += eB;
             if (LEVEL == 1) {
                 m[r].b[1] = fma(eB, u, m[r].b[1]);
@@ -266,7 +308,7 @@ __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt
             }
             if (MODE != 0) {
                 const double as = fma(c.rho_s, dt, u);
-                const double eS = s.w * exp2_scaled<(MODE == 2) ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, lane_addr);
+                const double eS = s.w * exp2_scaled<(MODE == 2) ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, c.e, lane_base);
                 m[r].s[0] += eS;
                 if (LEVEL == 1) {
                     m[r].s[1] = fma(eS, u, m[r].s[1]);
@@ -332,22 +374,36 @@ __host__ __device__ inline void split_slots(const Split& s, int64_t I, int* firs
     *count = (int)(b - a + 1);
 }
 
-// a1: one CTA of the single wave.  part[(slot*NMOM + k)*ld + n], NMOM = 2 NB.
-template <int R, int LEVEL, bool DIM3>
-__global__ void __launch_bounds__(NT) pass1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
-                                                   DevConsts c, const double* __restrict__ tab_g,
-                                                   double* __restrict__ part, Split sp) {
+// a1: one CTA per SM, G independent work groups of NT threads; group (blockIdx.x * G + g) is worker
+// number `vcta` of the single wave.  part[(slot*NMOM + k)*ld + n], NMOM = 2 NB.
+template <int R, int LEVEL, bool DIM3, int G>
+__global__ void __launch_bounds__(NT * G, 1) pass1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
+                                                          DevConsts c, const double* __restrict__ tab_g,
+                                                          double* __restrict__ part, Split sp) {
     constexpr int RS = DIM3 ? 6 : 4;
     constexpr int TOFF = DIM3 ? 3 : 2;
     constexpr int NB = Mom<LEVEL>::NB;
-    __shared__ __align__(16) double tab[TAB_N * TAB_REP];
-    __shared__ __align__(16) double sbuf[2][TS * RS];
+    constexpr unsigned BUF = group_buf_bytes<DIM3>();   // one group's double buffer
+    static_assert(smem_request(G * BUF) <= SMEM_MAX, "table + streaming buffers must fit shared memory");
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double smagic;
+    const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem);
+    const SmemPlan plan = smem_plan(smem_base, G * BUF);
+    fill_table(reinterpret_cast<double*>(smem + plan.tab_off), tab_g);
+    stash_consts(smagic);
+    __syncthreads();   // the only CTA-wide barrier; the groups are independent from here on
+
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
+    const int64_t vcta = (int64_t)blockIdx.x * G + grp;
+    double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
+    double* const sbuf1 = sbuf0 + TS * RS;
+    const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
 
     const int64_t total = split_prefix(sp, sp.n_tiles);
-    const int64_t lo = (int64_t)blockIdx.x * sp.chunk;
+    const int64_t lo = vcta * sp.chunk;
     if (lo >= total) return;
     const int64_t hi = min(lo + sp.chunk, total);
-    const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
+    const P1C pc = pinned_consts(smagic, c);
 
     for (int I = split_tile_of(sp, lo); I < sp.n_tiles; ++I) {
         const int64_t base = split_prefix(sp, I);
@@ -362,7 +418,7 @@ __global__ void __launch_bounds__(NT) pass1_kernel(const double* __restrict__ re
         Mom<LEVEL> m[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t i = min(i0 + r * NT + threadIdx.x, n - 1);
+            const int64_t i = min(i0 + r * NT + tid, n - 1);
             g[r] = read_rec<DIM3>(rec + i * RS);
 #pragma unroll
             for (int k = 0; k < NB; ++k) { m[r].b[k] = 0.0; m[r].s[k] = 0.0; }
@@ -373,34 +429,35 @@ __global__ void __launch_bounds__(NT) pass1_kernel(const double* __restrict__ re
         RecIO<DIM3> io;
         int64_t a = jb;
         int64_t b = min(je, (a / TS + 1) * TS);
-        __syncthreads();                               // previous tile's readers are done with sbuf
+        group_sync(grp);                               // previous tile's readers are done with the buffers
         if (a < je) {
-            io.load(rec, a, (int)(b - a));
-            io.store(sbuf[0]);
+            io.load(rec, a, (int)(b - a), tid);
+            io.store(sbuf0, tid);
         }
-        __syncthreads();
+        group_sync(grp);
         int cur = 0;
         while (a < je) {
             const int cnt = (int)(b - a);
             const int64_t a2 = b, b2 = min(je, b + TS);
-            if (a2 < je) io.load(rec, a2, (int)(b2 - a2));
+            if (a2 < je) io.load(rec, a2, (int)(b2 - a2), tid);
+            const double* sb = cur ? sbuf1 : sbuf0;
             if (a >= i1) {
-                p1_tile<R, LEVEL, 0, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+                p1_tile<R, LEVEL, 0, DIM3>(sb, cnt, g, m, pc, lane_base);
             } else if (b <= i0 && rec[(b - 1) * RS + TOFF] < t_first) {
-                p1_tile<R, LEVEL, 1, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+                p1_tile<R, LEVEL, 1, DIM3>(sb, cnt, g, m, pc, lane_base);
             } else {
-                p1_tile<R, LEVEL, 2, DIM3>(sbuf[cur], cnt, g, m, c, lane_addr);
+                p1_tile<R, LEVEL, 2, DIM3>(sb, cnt, g, m, pc, lane_base);
             }
-            if (a2 < je) io.store(sbuf[cur ^ 1]);
-            __syncthreads();
+            if (a2 < je) io.store(cur ? sbuf0 : sbuf1, tid);
+            group_sync(grp);
             cur ^= 1;
             a = a2;
             b = b2;
         }
-        const int slot = (int)((int64_t)blockIdx.x - base / sp.chunk);
+        const int slot = (int)(vcta - base / sp.chunk);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t i = i0 + r * NT + threadIdx.x;
+            const int64_t i = i0 + r * NT + tid;
             if (i < n) {
                 double* o = part + (int64_t)slot * (2 * NB) * ld + i;
 #pragma unroll
@@ -474,7 +531,7 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
         }
         const Ev<DIM3> e = read_rec<DIM3>(rec + i * RS);
         const double D = (double)c.dim;
-        const double SB = c.CB * b[0], SS = c.CS * s[0];
+        const double SB = c.CBS * b[0], SS = c.CSS * s[0];
         const double L = SB + SS;
         const double iL = 1.0 / L;
         lam[i] = L;
@@ -491,7 +548,7 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
         v[0] = log(L);
         double d1[6] = {0, 0, 0, 0, 0, 0};
         if (LEVEL >= 1) {
-            const double SBr2 = c.CB * b[1], SBd2 = c.CB * b[2], SSr2 = c.CS * s[1], SSd = c.CS * s[2];
+            const double SBr2 = c.CBS * b[1], SBd2 = c.CBS * b[2], SSr2 = c.CSS * s[1], SSd = c.CSS * s[2];
             const double tx = c.tau_x, tt = c.tau_t, h = c.h, om = c.omega;
             d1[0] = SB / c.mu0;
             d1[1] = SBr2 / (tx * tx * tx) - D * SB / tx;
@@ -506,8 +563,8 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
                 for (int p = 0; p < 6; ++p) glam[i * 6 + p] = d1[p] * iL * iL;
             }
             if (LEVEL >= 2) {
-                const double SBr4 = c.CB * b[3], SBr2d2 = c.CB * b[4], SBd4 = c.CB * b[5];
-                const double SSr4 = c.CS * s[3], SSr2d = c.CS * s[4], SSd2 = c.CS * s[5];
+                const double SBr4 = c.CBS * b[3], SBr2d2 = c.CBS * b[4], SBd4 = c.CBS * b[5];
+                const double SSr4 = c.CSS * s[3], SSr2d = c.CSS * s[4], SSd2 = c.CSS * s[5];
                 double d2[6][6];
 #pragma unroll
                 for (int p = 0; p < 6; ++p)
@@ -591,11 +648,10 @@ __global__ void __launch_bounds__(64) scalars_kernel(const double* __restrict__ 
 // ------------------------------------------------------------------------------------------------
 // a4: pass 2.  Thread owns R sources m; later targets (x, y, t, 1/lambda) stream through shared memory.
 //   c_m = sum_{t_n > t_m} e_nm / lambda_n,   d_m = sum (e_nm / lambda_n)^2,   e = exp(-omega dt - r2/2h^2)
-// (k_nm = CS e_nm; the constant is applied in theta_kernel).  LEVEL 0: c only; 1: c and d.
+// (the kernel sums e_nm / S; k_nm = CS e_nm, and CS S is applied in theta_kernel).  LEVEL 0: c only; 1: c and d.
 template <int R, int LEVEL, bool MASKED, bool DIM3>
 __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt, const Ev<DIM3> (&g)[R],
-                                        double (&cm)[R], double (&dm)[R], const DevConsts& c,
-                                        unsigned lane_addr) {
+                                        double (&cm)[R], double (&dm)[R], const P1C& c, unsigned lane_base) {
     constexpr int RS = DIM3 ? 6 : 4;
 #pragma unroll UNROLL_J
     for (int j = 0; j < cnt; ++j) {
@@ -606,7 +662,7 @@ __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt
             double u = fma(dy, dy, dx * dx);
             if (DIM3) { const double dz = s.z - g[r].z; u = fma(dz, dz, u); }
             const double as = fma(c.rho_s, dt, u);
-            const double e = exp2_scaled<MASKED ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, lane_addr);
+            const double e = exp2_scaled<MASKED ? 2 : 0>(as, c.negcs, c.lim_s_hi, dt, c.e, lane_base);
             // an acausal pair is no term of the sum: it must add exactly 0 even when 1/lambda_n = inf
             const double wn = (MASKED && !(dt > 0.0)) ? 0.0 : s.w;
             if (LEVEL == 0) {
@@ -620,23 +676,37 @@ __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt
     }
 }
 
-// a4: one CTA of the single wave (decomposition: see Split above, `tri` form -- the streamed targets of
-// source tile M are those with index >= the tile's first source).  part2[(slot*2 + k)*ld + m], k = 0 (c), 1 (d).
-template <int R, int LEVEL, bool DIM3>
-__global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
-                                                   int64_t n, int64_t ld, DevConsts c,
-                                                   const double* __restrict__ tab_g, double* __restrict__ part2,
-                                                   Split sp) {
+// a4: G work groups per CTA as in pass 1 (decomposition: see Split above, `tri` form -- the streamed
+// targets of source tile M are those with index >= the tile's first source).
+// part2[(slot*2 + k)*ld + m], k = 0 (c), 1 (d).
+template <int R, int LEVEL, bool DIM3, int G>
+__global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
+                                                          int64_t n, int64_t ld, DevConsts c,
+                                                          const double* __restrict__ tab_g, double* __restrict__ part2,
+                                                          Split sp) {
     constexpr int RS = DIM3 ? 6 : 4;
     constexpr int TOFF = DIM3 ? 3 : 2;
-    __shared__ __align__(16) double tab[TAB_N * TAB_REP];
-    __shared__ __align__(16) double sbuf[2][TS * RS];
+    constexpr unsigned BUF = group_buf_bytes<DIM3>();
+    static_assert(smem_request(G * BUF) <= SMEM_MAX, "table + streaming buffers must fit shared memory");
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double smagic;
+    const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem);
+    const SmemPlan plan = smem_plan(smem_base, G * BUF);
+    fill_table(reinterpret_cast<double*>(smem + plan.tab_off), tab_g);
+    stash_consts(smagic);
+    __syncthreads();
+
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
+    const int64_t vcta = (int64_t)blockIdx.x * G + grp;
+    double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
+    double* const sbuf1 = sbuf0 + TS * RS;
+    const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
 
     const int64_t total = split_prefix(sp, sp.n_tiles);
-    const int64_t lo = (int64_t)blockIdx.x * sp.chunk;
+    const int64_t lo = vcta * sp.chunk;
     if (lo >= total) return;
     const int64_t hi = min(lo + sp.chunk, total);
-    const unsigned lane_addr = fill_table(tab, tab_g) + 8u * (threadIdx.x & (TAB_REP - 1));
+    const P1C pc = pinned_consts(smagic, c);
 
     for (int M = split_tile_of(sp, lo); M < sp.n_tiles; ++M) {
         const int64_t base = split_prefix(sp, M);
@@ -651,7 +721,7 @@ __global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ re
         double cm[R], dm[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t i = min(m0 + r * NT + threadIdx.x, n - 1);
+            const int64_t i = min(m0 + r * NT + tid, n - 1);
             g[r] = read_rec<DIM3>(rec + i * RS);
             cm[r] = 0.0;
             dm[r] = 0.0;
@@ -661,32 +731,33 @@ __global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ re
         RecIO<DIM3> io;
         int64_t a = jb;
         int64_t b = min(je, (a / TS + 1) * TS);
-        __syncthreads();
+        group_sync(grp);
         if (a < je) {
-            io.load(trec, a, (int)(b - a));
-            io.store(sbuf[0]);
+            io.load(trec, a, (int)(b - a), tid);
+            io.store(sbuf0, tid);
         }
-        __syncthreads();
+        group_sync(grp);
         int cur = 0;
         while (a < je) {
             const int cnt = (int)(b - a);
             const int64_t a2 = b, b2 = min(je, b + TS);
-            if (a2 < je) io.load(trec, a2, (int)(b2 - a2));
+            if (a2 < je) io.load(trec, a2, (int)(b2 - a2), tid);
+            const double* sb = cur ? sbuf1 : sbuf0;
             if (a >= m1 && trec[a * RS + TOFF] > t_last) {
-                p2_tile<R, LEVEL, false, DIM3>(sbuf[cur], cnt, g, cm, dm, c, lane_addr);
+                p2_tile<R, LEVEL, false, DIM3>(sb, cnt, g, cm, dm, pc, lane_base);
             } else {
-                p2_tile<R, LEVEL, true, DIM3>(sbuf[cur], cnt, g, cm, dm, c, lane_addr);
+                p2_tile<R, LEVEL, true, DIM3>(sb, cnt, g, cm, dm, pc, lane_base);
             }
-            if (a2 < je) io.store(sbuf[cur ^ 1]);
-            __syncthreads();
+            if (a2 < je) io.store(cur ? sbuf0 : sbuf1, tid);
+            group_sync(grp);
             cur ^= 1;
             a = a2;
             b = b2;
         }
-        const int slot = (int)((int64_t)blockIdx.x - base / sp.chunk);
+        const int slot = (int)(vcta - base / sp.chunk);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t i = m0 + r * NT + threadIdx.x;
+            const int64_t i = m0 + r * NT + tid;
             if (i < n) {
                 part2[(int64_t)(slot * 2 + 0) * ld + i] = cm[r];
                 if (LEVEL >= 1) part2[(int64_t)(slot * 2 + 1) * ld + i] = dm[r];
@@ -695,7 +766,7 @@ __global__ void __launch_bounds__(NT) pass2_kernel(const double* __restrict__ re
     }
 }
 
-// a5 (theta): grad_theta[m] = CS c_m - xi0 (1 - E_m);  hess_theta_diag[m] = - CS^2 d_m.
+// a5 (theta): grad_theta[m] = CS c_m - xi0 (1 - E_m);  hess_theta_diag[m] = - CS^2 d_m  (c, d arrive divided by S, S^2).
 template <bool DIM3>
 __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                       DevConsts c, const double* __restrict__ part2, Split sp,
@@ -714,9 +785,9 @@ __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__
     if (grad_theta) {
         const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
         const double ti = rec[i * RS + (DIM3 ? 3 : 2)];
-        grad_theta[i] = c.CS * cs - c.xi0 * (-expm1(-c.omega * (tN - ti)));
+        grad_theta[i] = c.CSS * cs - c.xi0 * (-expm1(-c.omega * (tN - ti)));
     }
-    if (hess_theta_diag) hess_theta_diag[i] = -(c.CS * c.CS) * ds;
+    if (hess_theta_diag) hess_theta_diag[i] = -(c.CSS * c.CSS) * ds;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -836,7 +907,7 @@ struct hawkes_ctx {
     double* d_part2;      // pass-2 partials
     size_t part2_doubles;
     int sm_count;
-    int occ1[3], occ2[2];  // resident CTAs per SM of pass1_kernel<LEVEL> / pass2_kernel<LEVEL> for this dim
+    int occ1[3], occ2[2];  // work groups per SM (= per CTA, one CTA per SM) of pass1_kernel<LEVEL> / pass2_kernel<LEVEL>
     Plan plan;            // cached decomposition of the last (n, level1, level2)
     int64_t plan_n;
     int plan_l1, plan_l2;
@@ -876,11 +947,29 @@ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 #endif
 constexpr int P1_R = HAWKES_P1_R;   // targets per thread in pass 1
 constexpr int P2_R = HAWKES_P2_R;   // sources per thread in pass 2
+// work groups (of NT threads) per CTA, one CTA per SM: bounded by 65536 registers / (NT x registers per thread)
+#ifndef HAWKES_P1_G0
+#define HAWKES_P1_G0 4
+#endif
+#ifndef HAWKES_P1_G1
+#define HAWKES_P1_G1 4
+#endif
+#ifndef HAWKES_P1_G2
+#define HAWKES_P1_G2 3
+#endif
+#ifndef HAWKES_P2_G0
+#define HAWKES_P2_G0 4
+#endif
+#ifndef HAWKES_P2_G1
+#define HAWKES_P2_G1 4
+#endif
+constexpr int P1_G[3] = {HAWKES_P1_G0, HAWKES_P1_G1, HAWKES_P1_G2};
+constexpr int P2_G[2] = {HAWKES_P2_G0, HAWKES_P2_G1};
 
-// cost weights of the pass-1 cost axis per LEVEL: 2 x FP64-pipe instructions + other instructions of a
+// cost weights of the pass-1 cost axis per LEVEL: modelled issue cycles of a
 // background term (every streamed source) and of an excitation term (sources before the tile's end)
-constexpr int W_ALL[3] = {40, 44, 54};
-constexpr int W_HEAD[3] = {29, 33, 43};
+constexpr int W_ALL[3] = {40, 46, 57};
+constexpr int W_HEAD[3] = {26, 33, 44};
 
 // Cut the cost axis of one pass into at most `ctas` chunks whose partial slots fit `cap_doubles`
 // (slots of the fullest tile x moments x ld).  Returns the number of CTAs to launch.
@@ -931,6 +1020,9 @@ int make_consts(const hawkes_params* p, int dim, DevConsts* c) {
     c->CB = (double)((long double)p->mu0 * powl(two_pi, -0.5L * (dim + 1)) * powl(p->tau_x, -dim) / p->tau_t);
     c->CS = (double)((long double)p->xi0 * p->omega * powl(two_pi, -0.5L * dim) * powl(p->h, -dim));
     c->mu0 = p->mu0; c->tau_x = p->tau_x; c->tau_t = p->tau_t; c->xi0 = p->xi0; c->h = p->h; c->omega = p->omega;
+    c->CBS = (double)((long double)c->CB * (long double)HAWKES_EXP2_S);
+    c->CSS = (double)((long double)c->CS * (long double)HAWKES_EXP2_S);
+    c->d0 = HAWKES_EXP2_D0; c->d1 = HAWKES_EXP2_D1; c->d2 = HAWKES_EXP2_D2; c->d3 = HAWKES_EXP2_D3;
     c->dim = dim;
     // flush when the base-2 exponent is below -1020: argument a >= 1020 / c
     auto hi_of = [](double d) { union { double d; uint64_t u; } q; q.d = d; return (int)(q.u >> 32); };
@@ -965,22 +1057,22 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     if (pe) CK(cudaEventRecord(pe[0], st));
     prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status);
     ctx->launches++;
-    const unsigned g1 = (unsigned)pl.grid1;
+    const unsigned g1 = (unsigned)((pl.grid1 + P1_G[level1] - 1) / P1_G[level1]);
     double* glam = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_glam : nullptr;
     if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
-            pass1_kernel<P1_R, 0, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
+            pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
             reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
         case 1:
-            pass1_kernel<P1_R, 1, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
+            pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
             reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
         default:
-            pass1_kernel<P1_R, 2, DIM3><<<g1, NT, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
+            pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
             reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
             break;
@@ -993,12 +1085,12 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         ctx->launches++;
     }
     if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
-        const unsigned g2 = (unsigned)pl.grid2;
+        const unsigned g2 = (unsigned)((pl.grid2 + P2_G[level2] - 1) / P2_G[level2]);
         if (pe) CK(cudaEventRecord(pe[3], st));
         if (want & HAWKES_WANT_HESS_THETA)
-            pass2_kernel<P2_R, 1, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
+            pass2_kernel<P2_R, 1, DIM3, P2_G[1]><<<g2, NT * P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
         else
-            pass2_kernel<P2_R, 0, DIM3><<<g2, NT, 0, st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
+            pass2_kernel<P2_R, 0, DIM3, P2_G[0]><<<g2, NT * P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
         if (pe) CK(cudaEventRecord(pe[4], st));
         theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.sp2,
                                                       (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
@@ -1020,15 +1112,25 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     return HAWKES_OK;
 }
 
+// opt the pairwise kernels into the large dynamic shared-memory allocation and check each is launchable
+template <typename K>
+int setup_kernel(K kernel, int groups, unsigned smem_bytes, int* out_groups) {
+    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+    int resident = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kernel, NT * groups, smem_bytes));
+    if (resident < 1) return HAWKES_ERR_CUDA;
+    *out_groups = groups;   // one CTA per SM (the shared-memory request allows no second one)
+    return HAWKES_OK;
+}
+
 template <bool DIM3>
 int query_occupancy(hawkes_ctx* ctx) {
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ1[0], pass1_kernel<P1_R, 0, DIM3>, NT, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ1[1], pass1_kernel<P1_R, 1, DIM3>, NT, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ1[2], pass1_kernel<P1_R, 2, DIM3>, NT, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ2[0], pass2_kernel<P2_R, 0, DIM3>, NT, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ2[1], pass2_kernel<P2_R, 1, DIM3>, NT, 0));
-    for (int k = 0; k < 3; ++k) if (ctx->occ1[k] < 1) return HAWKES_ERR_CUDA;
-    for (int k = 0; k < 2; ++k) if (ctx->occ2[k] < 1) return HAWKES_ERR_CUDA;
+    int rc;
+    if ((rc = setup_kernel(pass1_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), &ctx->occ1[0]))) return rc;
+    if ((rc = setup_kernel(pass1_kernel<P1_R, 1, DIM3, P1_G[1]>, P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), &ctx->occ1[1]))) return rc;
+    if ((rc = setup_kernel(pass1_kernel<P1_R, 2, DIM3, P1_G[2]>, P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), &ctx->occ1[2]))) return rc;
+    if ((rc = setup_kernel(pass2_kernel<P2_R, 0, DIM3, P2_G[0]>, P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), &ctx->occ2[0]))) return rc;
+    if ((rc = setup_kernel(pass2_kernel<P2_R, 1, DIM3, P2_G[1]>, P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), &ctx->occ2[1]))) return rc;
     return HAWKES_OK;
 }
 
