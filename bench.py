@@ -210,13 +210,18 @@ def dist_env():
 
 
 def ncu_traffic(kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.json), or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full
+    summary (profiles/traffic.csv: kernel,dram_bytes_per_launch; profiles/traffic.md names the command), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(path) as fh:
-            return json.load(fh).get(kernel)
+            for line in fh:
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) >= 2 and parts[0] == kernel:
+                    return float(parts[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def run_b200(args, ev, workload: str) -> dict:

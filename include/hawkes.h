@@ -151,7 +151,9 @@ int64_t hawkes_launch_count(const hawkes_ctx* ctx);
  * evaluation; a ring keeps the most recent 256 evaluations.  hawkes_profile_read() waits for those
  * evaluations, writes out[0] = number of evaluations summed, out[1] = total pass-1 milliseconds,
  * out[2] = total pass-2 milliseconds, out[3] = total milliseconds from the first to the last kernel
- * of the evaluation (out: 4 doubles, HOST), and resets the ring.  Enabling/disabling also resets it. */
+ * of the evaluation, out[4] = total milliseconds of step a0 (prep), out[5] = of the O(N) kernels between the
+ * two passes (a2 + a3 + scalars, with their launch gaps), out[6] = of those after pass 2 (a5)
+ * (out: 7 doubles, HOST), and resets the ring.  Enabling/disabling also resets it. */
 int hawkes_profile_enable(hawkes_ctx* ctx, int enable);
 int hawkes_profile_read(hawkes_ctx* ctx, double* out /*HOST*/);
 

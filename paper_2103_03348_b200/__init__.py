@@ -203,11 +203,12 @@ class HawkesContext:
 
     def profile_read(self) -> dict:
         """Sums over the evaluations recorded since the last read (at most 256)."""
-        out = (ctypes.c_double * 4)()
+        out = (ctypes.c_double * 7)()
         rc = self._lib.hawkes_profile_read(self._h, out)
         if rc != 0:
             raise HawkesError(rc, "hawkes_profile_read")
-        return {"evals": int(out[0]), "pass1_ms": out[1], "pass2_ms": out[2], "total_ms": out[3]}
+        return {"evals": int(out[0]), "pass1_ms": out[1], "pass2_ms": out[2], "total_ms": out[3],
+                "prep_ms": out[4], "mid_ms": out[5], "tail_ms": out[6]}
 
     def fp64_peak(self, millis: float = 200.0) -> float:
         v = ctypes.c_double(0.0)

@@ -41,7 +41,8 @@ constexpr int TAB_N = 1 << HAWKES_EXP2_TBITS;
 static_assert(TAB_N == 256, "the PRMT addressing below takes the low byte of n as the table row");
 constexpr int TAB_ROW = 256;   // bytes per table row: 32 lane replicas of one fp64 entry
 constexpr unsigned TAB_BYTES = TAB_N * TAB_ROW;   // 64 KB, placed on a 64 KB boundary of the shared window
-constexpr int RED_T = 256;     // threads per CTA in the O(N) kernels
+constexpr int RED_T = 64;      // threads per CTA in the O(N) kernels (small CTAs: N/64 of them spread over the SMs)
+constexpr int SCAL_T = 1024;   // threads of the single scalars CTA
 constexpr int NRED = 34;       // per-event scalar sums reduced over n (see reduce1_kernel)
 #ifndef HAWKES_UNROLL
 #define HAWKES_UNROLL 4
@@ -521,13 +522,28 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
         double b[6] = {0, 0, 0, 0, 0, 0}, s[6] = {0, 0, 0, 0, 0, 0};
         int slot0, n_slots;
         split_slots(sp, i / sp.tile, &slot0, &n_slots);
-        for (int q = 0; q < n_slots; ++q) {
+        // slots in order (fixed summation order); the loads of two slots are all issued before the adds, so
+        // that the loop costs one L2 round trip per two slots instead of one per load
+        int q = 0;
+        for (; q + 2 <= n_slots; q += 2) {
             const double* o = part + (int64_t)q * (2 * NB) * ld + i;
+            double v[2][2 * NB];
 #pragma unroll
-            for (int k = 0; k < NB; ++k) {
-                b[k] += o[(int64_t)k * ld];
-                s[k] += o[(int64_t)(NB + k) * ld];
-            }
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int k = 0; k < 2 * NB; ++k) v[u][k] = o[((int64_t)u * (2 * NB) + k) * ld];
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int k = 0; k < NB; ++k) { b[k] += v[u][k]; s[k] += v[u][NB + k]; }
+        }
+        if (q < n_slots) {
+            const double* o = part + (int64_t)q * (2 * NB) * ld + i;
+            double v[2 * NB];
+#pragma unroll
+            for (int k = 0; k < 2 * NB; ++k) v[k] = o[(int64_t)k * ld];
+#pragma unroll
+            for (int k = 0; k < NB; ++k) { b[k] += v[k]; s[k] += v[NB + k]; }
         }
         const Ev<DIM3> e = read_rec<DIM3>(rec + i * RS);
         const double D = (double)c.dim;
@@ -608,14 +624,18 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
 }
 
 // a5 (scalars): fixed-order sum of the block partials, then ll, grad_hyper, hess_hyper.
-__global__ void __launch_bounds__(64) scalars_kernel(const double* __restrict__ blockpart, int nblk, DevConsts c,
-                                                     double* __restrict__ ll, double* __restrict__ grad_hyper,
-                                                     double* __restrict__ hess_hyper, double* __restrict__ scal_out) {
+__global__ void __launch_bounds__(SCAL_T) scalars_kernel(const double* __restrict__ blockpart, int nblk, DevConsts c,
+                                                         double* __restrict__ ll, double* __restrict__ grad_hyper,
+                                                         double* __restrict__ hess_hyper, double* __restrict__ scal_out) {
     __shared__ double r[NRED];
-    if (threadIdx.x < NRED) {
+    // warp w sums scalars w and w + 32: lane l takes blocks l, l + 32, ... in order, then a fixed shuffle tree
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int k = wid; k < NRED; k += SCAL_T / 32) {
         double a = 0.0;
-        for (int b = 0; b < nblk; ++b) a += blockpart[(int64_t)b * NRED + threadIdx.x];
-        r[threadIdx.x] = a;
+        for (int b = lane; b < nblk; b += 32) a += blockpart[(int64_t)b * NRED + k];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
+        if (lane == 0) r[k] = a;
     }
     __syncthreads();
     if (threadIdx.x != 0) return;
@@ -778,7 +798,18 @@ __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__
     double cs = 0.0, ds = 0.0;
     int slot0, n_slots;
     split_slots(sp, i / sp.tile, &slot0, &n_slots);
-    for (int s = 0; s < n_slots; ++s) {
+    int s = 0;
+    for (; s + 4 <= n_slots; s += 4) {   // four slots' loads in flight, adds in slot order
+        double vc[4], vd[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            vc[u] = part2[(int64_t)((s + u) * 2 + 0) * ld + i];
+            vd[u] = hess_theta_diag ? part2[(int64_t)((s + u) * 2 + 1) * ld + i] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { cs += vc[u]; ds += vd[u]; }
+    }
+    for (; s < n_slots; ++s) {
         cs += part2[(int64_t)(s * 2 + 0) * ld + i];
         if (hess_theta_diag) ds += part2[(int64_t)(s * 2 + 1) * ld + i];
     }
@@ -1079,7 +1110,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     }
     ctx->launches += 2;
     if (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) {
-        scalars_kernel<<<1, 64, 0, st>>>(ctx->d_blockpart, pl.nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
+        scalars_kernel<<<1, SCAL_T, 0, st>>>(ctx->d_blockpart, pl.nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
                                          (want & HAWKES_WANT_GRAD_HYPER) ? grad_hyper : nullptr,
                                          (want & HAWKES_WANT_HESS_HYPER) ? hess_hyper : nullptr, ctx->d_scal);
         ctx->launches++;
@@ -1392,7 +1423,7 @@ int hawkes_profile_read(hawkes_ctx* ctx, double* out) {
     if (!ctx || !out || !ctx->prof_ev) return HAWKES_ERR_ARG;
     CK(cudaSetDevice(ctx->device));
     const int64_t cnt = ctx->prof_count < PROF_RING ? ctx->prof_count : PROF_RING;
-    double p1 = 0.0, p2 = 0.0, tot = 0.0;
+    double p1 = 0.0, p2 = 0.0, tot = 0.0, pre = 0.0, mid = 0.0, tail = 0.0;
     for (int64_t k = 0; k < cnt; ++k) {
         cudaEvent_t* e = ctx->prof_ev + 6 * ((ctx->prof_count - 1 - k) % PROF_RING);
         CK(cudaEventSynchronize(e[5]));
@@ -1401,8 +1432,12 @@ int hawkes_profile_read(hawkes_ctx* ctx, double* out) {
         CK(cudaEventElapsedTime(&b, e[3], e[4]));
         CK(cudaEventElapsedTime(&t, e[0], e[5]));
         p1 += a; p2 += b; tot += t;
+        CK(cudaEventElapsedTime(&a, e[0], e[1]));
+        CK(cudaEventElapsedTime(&b, e[2], e[3]));
+        CK(cudaEventElapsedTime(&t, e[4], e[5]));
+        pre += a; mid += b; tail += t;
     }
-    out[0] = (double)cnt; out[1] = p1; out[2] = p2; out[3] = tot;
+    out[0] = (double)cnt; out[1] = p1; out[2] = p2; out[3] = tot; out[4] = pre; out[5] = mid; out[6] = tail;
     ctx->prof_count = 0;
     return HAWKES_OK;
 }
