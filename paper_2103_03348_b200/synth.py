@@ -133,3 +133,102 @@ def small_random(n: int, seed: int, dim: int = 2, regime: str = "mixed", ties: b
         params = (0.6, 1.7, 4.0, 0.5, 0.9, 0.8)
     return Events(x=np.ascontiguousarray(x), t=np.ascontiguousarray(t), theta=theta,
                   free_idx=np.arange(n, dtype=np.int64), params=params)
+
+
+# ---------------------------------------------------------------------------------------------------
+# Synthetic phylogeny (stands in for the 1,000 posterior trees of Dudas et al. that PAPER.md:196 uses and that
+# are not in the container): a heterochronous Kingman coalescent whose tip dates are the event times of the
+# sequenced subset, and a Brownian draw of the log-rates z along it.  These are INPUT draws; the density of z
+# (Eq. 2) is computed by the CUDA path and, independently, by oracle/tree_ref.cpp.
+@dataclasses.dataclass
+class Tree:
+    """2M-1 nodes; nodes 0..M-1 are the tips (tip i <-> z[i] <-> event free_idx[i]); parent[root] = -1;
+    branch[v] = edge weight between v and parent[v] (branch[root] = 0)."""
+    parent: np.ndarray   # [2M-1] int32
+    branch: np.ndarray   # [2M-1] float64
+
+    @property
+    def n_tips(self) -> int:
+        return (int(self.parent.shape[0]) + 1) // 2
+
+
+def make_tree(tip_times, seed: int = 0, ne: float = 100.0, mean_root_to_tip: float = 1.0) -> Tree:
+    """Coalescent backwards in time from the latest tip: with k active lineages the next merger comes after
+    Exp(rate k(k-1)/(2 ne)) days; a tip joins the active set when its sampling time is passed (the waiting time is
+    then redrawn).  Branch lengths (days) are finally rescaled so that the mean root-to-tip distance equals
+    `mean_root_to_tip`.  Draw order: waiting times (stream 70), merging pairs (streams 71, 72)."""
+    tt = np.asarray(tip_times, dtype=np.float64)
+    M = int(tt.shape[0])
+    if M == 1:
+        return Tree(parent=np.array([-1], dtype=np.int32), branch=np.zeros(1))
+    order = np.argsort(-tt, kind="stable")            # latest tip first
+    u_wait = uniforms(seed, 70, 4 * M)
+    u_a = uniforms(seed, 71, M)
+    u_b = uniforms(seed, 72, M)
+    parent = np.full(2 * M - 1, -1, dtype=np.int32)
+    node_time = np.zeros(2 * M - 1)                   # backwards time (days before the latest tip)
+    node_time[:M] = tt.max() - tt
+    active: list[int] = []
+    nxt, now, draws, merges, new_node = 0, 0.0, 0, 0, M
+    while nxt < M or len(active) > 1:
+        k = len(active)
+        t_next_tip = node_time[order[nxt]] if nxt < M else np.inf
+        if k < 2:
+            now = t_next_tip
+            active.append(int(order[nxt]))
+            nxt += 1
+            continue
+        wait = -np.log1p(-u_wait[draws]) * (2.0 * ne) / (k * (k - 1.0))
+        draws += 1
+        if now + wait >= t_next_tip:
+            now = t_next_tip
+            active.append(int(order[nxt]))
+            nxt += 1
+            continue
+        now += wait
+        ia = min(int(u_a[merges] * k), k - 1)
+        a = active.pop(ia)
+        ib = min(int(u_b[merges] * (k - 1)), k - 2)
+        b = active.pop(ib)
+        merges += 1
+        parent[a] = parent[b] = new_node
+        node_time[new_node] = now
+        active.append(new_node)
+        new_node += 1
+    branch = np.zeros(2 * M - 1)
+    has_parent = parent >= 0
+    branch[has_parent] = node_time[parent[has_parent]] - node_time[has_parent]
+    # root-to-tip distances for the rescaling
+    dist = np.zeros(2 * M - 1)
+    for v in range(2 * M - 3, -1, -1):                # parents have larger indices than their children
+        dist[v] = dist[parent[v]] + branch[v]
+    branch *= mean_root_to_tip / dist[:M].mean()
+    return Tree(parent=parent, branch=branch)
+
+
+def draw_z(tree: Tree, sigma2: float, tau0: float, seed: int = 0) -> np.ndarray:
+    """Root value ~ N(0, tau0 sigma2), each child ~ N(parent, branch sigma2); returns the tip
+    values z [M].  Normal stream 80."""
+    nn = int(tree.parent.shape[0])
+    M = tree.n_tips
+    g = normals(seed, 80, nn)
+    val = np.zeros(nn)
+    val[nn - 1] = np.sqrt(tau0 * sigma2) * g[nn - 1]
+    for v in range(nn - 2, -1, -1):
+        val[v] = val[tree.parent[v]] + np.sqrt(tree.branch[v] * sigma2) * g[v]
+    return val[:M].copy()
+
+
+TREE_SIGMA2, TREE_TAU0 = 0.25, 0.1
+
+
+def config_tree(seed: int = 0, n: int = 23422, n_centres: int = 60, n_free: int = 1610):
+    """BASELINE.json configs[2]: config 1's events, the log-rates of the `n_free` sequenced events drawn by Brownian
+    diffusion (variance 0.25 per unit branch length, tau0 = 0.1) on a coalescent tree over those events' times.
+    Returns (events, tree, z)."""
+    ev = make_events(n, seed, n_centres=n_centres, n_free=n_free)
+    tree = make_tree(ev.t[ev.free_idx], seed)
+    z = draw_z(tree, TREE_SIGMA2, TREE_TAU0, seed)
+    theta = np.ones(ev.n)
+    theta[ev.free_idx] = np.exp(z)
+    return dataclasses.replace(ev, theta=theta), tree, z
