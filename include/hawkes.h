@@ -162,6 +162,63 @@ int hawkes_profile_read(hawkes_ctx* ctx, double* out /*HOST*/);
  * Synchronises.  Used by bench.py for the measured roofline denominator. */
 int hawkes_fp64_peak(hawkes_ctx* ctx, double millis, double* tflops /*HOST*/, void* stream);
 
+/* ------------------------------------------------------------------------------------------------------
+ * Phylogenetic Brownian-diffusion prior on the log-rates and the z-parametrisation of the rates
+ * (BASELINE.json configs[2]).
+ *
+ *   theta_n = exp(z_n + beta f(t_n)) for n in the sequenced set M, theta_n = 1 otherwise; f(t) = t
+ *                                                                             PAPER.md:97, 202
+ *   p(z | V_G, sigma^2, tau0) = (2 pi sigma^2)^(-M/2) |V_G|^(-1/2) exp(-z^T V_G^-1 z / (2 sigma^2))   Eq. 2, l.101
+ *   V_G: v_mm = tau0 + d_F(root, tip m);  v_nm = tau0 + d_F(root, MRCA(tip n, tip m))
+ *
+ * evaluated in O(M) by post-order message passing on the tree (PAPER.md:121 cites the algorithm; DESIGN.md
+ * section 11 states the recursion used), never forming V_G.
+ *
+ * Tree encoding: M tips, 2M-1 nodes.  Nodes 0..M-1 are the tips, tip i carrying z[i]; nodes M..2M-2 are the
+ * internal nodes in any order; parent[v] is the parent of node v, parent[root] = -1; branch[v] >= 0 is the edge
+ * weight w_v between v and its parent (branch[root] is ignored).  Every internal node has exactly two children.
+ */
+typedef struct hawkes_tree hawkes_tree; /* opaque; owns the device copy of the tree and its scratch */
+
+/* Validates the tree (HAWKES_ERR_ARG if it is not a rooted binary tree over tips 0..M-1 or a branch is negative
+ * or non-finite), orders its internal nodes by level and uploads it.  parent, branch: HOST, 2*n_tips-1 entries.
+ * Allocates; synchronises. */
+int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent /*HOST*/,
+                       const double* branch /*HOST*/, int device);
+void hawkes_tree_destroy(hawkes_tree* tree);
+
+/* log p(z | V_G, sigma2, tau0) (Eq. 2) into *logp and d log p / d z into grad_z[M] (either may be NULL, not both).
+ * z, logp, grad_z: DEVICE.  sigma2 > 0, tau0 >= 0 (HAWKES_ERR_PARAM otherwise).  One kernel on `stream`; no sync.
+ * A tree whose V_G is singular (tau0 = 0 with a zero-length path) yields non-finite results, not an error. */
+int hawkes_tree_prior(hawkes_tree* tree, const double* z, double sigma2, double tau0, double* logp,
+                      double* grad_z, void* stream);
+int32_t hawkes_tree_levels(const hawkes_tree* tree);        /* depth of the level schedule (diagnostics) */
+int64_t hawkes_tree_launch_count(const hawkes_tree* tree);  /* kernels launched since creation */
+
+/* theta[i] = 1 for every i < n, then theta[idx[k]] = exp(z[k] + beta * t[idx[k]]) for k < m.
+ * idx: DEVICE int64 [m], distinct, each in [0, n).  z [m], t [n], theta [n]: DEVICE. */
+int hawkes_theta_from_z(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, const double* z, double beta,
+                        const double* t, double* theta, void* stream);
+
+/* Chain rule through theta(z) for the sequenced events k < m, i = idx[k]:
+ *   grad_z[k] = theta[i] grad_theta[i]                       (+ prior_grad_z[k] when that pointer is not NULL)
+ *   hess_z[k] = theta[i]^2 hess_theta_diag[i] + theta[i] grad_theta[i]      (likelihood part of d2/dz_k^2)
+ *   *grad_beta = sum_k t[i] theta[i] grad_theta[i]            (fixed-order sum; f(t) = t)
+ * hess_theta_diag/hess_z and grad_beta are optional (NULL).  All pointers DEVICE. */
+int hawkes_z_chain(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, const double* theta,
+                   const double* t, const double* grad_theta, const double* hess_theta_diag,
+                   const double* prior_grad_z, double* grad_z, double* hess_z, double* grad_beta, void* stream);
+
+/* One fused evaluation of the z-posterior that HMC integrates and that configs[2] times:
+ *   theta(z) -> log-likelihood, d/dtheta (and the theta-Hessian diagonal if hess_z != NULL) -> tree prior ->
+ *   chain rule.  out3[0] = ell, out3[1] = log p(z | V_G, sigma2, tau0), out3[2] = their sum;
+ *   grad_z[m] = d(ell + log p)/dz;  hess_z[m] = likelihood part of the diagonal second derivative (see
+ *   hawkes_z_chain; the prior's Hessian -V_G^-1/sigma2 is not added).  out3, grad_z, hess_z: DEVICE, each optional.
+ * Uses context scratch for theta and the theta-derivatives; enqueues only. */
+int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                       const int64_t* idx, const double* z, double beta, const hawkes_params* p /*HOST*/,
+                       double sigma2, double tau0, double* out3, double* grad_z, double* hess_z, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -183,6 +183,46 @@ class HawkesContext:
             raise HawkesError(rc, "hawkes_sort_events")
         return xo, to, tho, perm
 
+    # -- z-parametrisation and the fused z-posterior (include/hawkes.h, "Phylogenetic ... prior") ------------
+    def theta_from_z(self, n: int, idx, z, beta: float, t, out=None):
+        """hawkes_theta_from_z: idx int64 [m], z [m], t [n] device tensors -> theta [n]."""
+        theta = out if out is not None else self._torch.empty(n, dtype=self._torch.float64, device=self._dev)
+        rc = self._lib.hawkes_theta_from_z(self._h, n, int(idx.shape[0]), _ptr(idx), _ptr(z), float(beta), _ptr(t),
+                                           _ptr(theta), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_theta_from_z")
+        return theta
+
+    def z_chain(self, idx, theta, t, grad_theta, hess_theta_diag=None, prior_grad_z=None, want_beta: bool = False):
+        """hawkes_z_chain: returns (grad_z [m], hess_z [m] or None, grad_beta [1] or None)."""
+        torch = self._torch
+        n, m = int(theta.shape[0]), int(idx.shape[0])
+        gz = torch.empty(m, dtype=torch.float64, device=self._dev)
+        hz = torch.empty(m, dtype=torch.float64, device=self._dev) if hess_theta_diag is not None else None
+        gb = torch.empty(1, dtype=torch.float64, device=self._dev) if want_beta else None
+        rc = self._lib.hawkes_z_chain(self._h, n, m, _ptr(idx), _ptr(theta), _ptr(t), _ptr(grad_theta),
+                                      _ptr(hess_theta_diag), _ptr(prior_grad_z), _ptr(gz), _ptr(hz), _ptr(gb), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_z_chain")
+        return gz, hz, gb
+
+    def posterior_z(self, tree: "HawkesTree", x, t, idx, z, beta: float, params, sigma2: float, tau0: float,
+                    hess: bool = False, out=None):
+        """hawkes_posterior_z: returns (out3 [ell, log prior, sum], grad_z [m], hess_z [m] or None), device tensors;
+        `out` = a previous return value to reuse its buffers."""
+        torch = self._torch
+        n, m = int(t.shape[0]), int(idx.shape[0])
+        if out is None:
+            mk = lambda k: torch.empty(k, dtype=torch.float64, device=self._dev)
+            out = (mk(3), mk(m), mk(m) if hess else None)
+        p = _params(params)
+        rc = self._lib.hawkes_posterior_z(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
+                                          ctypes.byref(p), float(sigma2), float(tau0), _ptr(out[0]), _ptr(out[1]),
+                                          _ptr(out[2]), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_posterior_z")
+        return out
+
     def get_lambda(self, n: int):
         lam = self._torch.empty(n, dtype=self._torch.float64, device=self._dev)
         rc = self._lib.hawkes_get_lambda(self._h, n, _ptr(lam), self._stream())
@@ -216,3 +256,55 @@ class HawkesContext:
         if rc != 0:
             raise HawkesError(rc, "hawkes_fp64_peak")
         return float(v.value)
+
+
+class HawkesTree:
+    """Owns one hawkes_tree: the device copy of a rooted binary tree over M tips (nodes 0..M-1 are the tips;
+    parent[root] = -1; branch[v] = edge weight to the parent), for the O(M) phylogenetic-diffusion prior."""
+
+    def __init__(self, parent, branch, device: int = 0):
+        import numpy as np
+        import torch
+        self._torch = torch
+        self._lib = load()
+        par = np.ascontiguousarray(parent, dtype=np.int32)
+        br = np.ascontiguousarray(branch, dtype=np.float64)
+        if par.shape != br.shape or par.ndim != 1 or par.shape[0] % 2 != 1:
+            raise ValueError("parent and branch must be 1-D arrays of 2M-1 entries")
+        self.n_tips = (par.shape[0] + 1) // 2
+        self.device = int(device)
+        h = ctypes.c_void_p()
+        rc = self._lib.hawkes_tree_create(ctypes.byref(h), self.n_tips, par.ctypes.data_as(ctypes.c_void_p),
+                                          br.ctypes.data_as(ctypes.c_void_p), self.device)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_tree_create")
+        self._h = h
+        self._dev = torch.device("cuda", self.device)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.hawkes_tree_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def prior(self, z, sigma2: float, tau0: float, grad: bool = True):
+        """hawkes_tree_prior: z [M] device tensor -> (log p [1], d log p / d z [M] or None), device tensors."""
+        torch = self._torch
+        lp = torch.empty(1, dtype=torch.float64, device=self._dev)
+        g = torch.empty(self.n_tips, dtype=torch.float64, device=self._dev) if grad else None
+        st = ctypes.c_void_p(torch.cuda.current_stream(self._dev).cuda_stream)
+        rc = self._lib.hawkes_tree_prior(self._h, _ptr(z), float(sigma2), float(tau0), _ptr(lp), _ptr(g), st)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_tree_prior")
+        return lp, g
+
+    def levels(self) -> int:
+        return int(self._lib.hawkes_tree_levels(self._h))
+
+    def launch_count(self) -> int:
+        return int(self._lib.hawkes_tree_launch_count(self._h))

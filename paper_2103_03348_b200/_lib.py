@@ -36,6 +36,15 @@ SYMBOLS = {
     "hawkes_profile_enable": (cint, [vp, cint]),
     "hawkes_profile_read": (cint, [vp, ctypes.POINTER(ctypes.c_double)]),
     "hawkes_fp64_peak": (cint, [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]),
+    "hawkes_tree_create": (cint, [ctypes.POINTER(vp), ctypes.c_int32, vp, vp, cint]),
+    "hawkes_tree_destroy": (None, [vp]),
+    "hawkes_tree_prior": (cint, [vp, _dp, ctypes.c_double, ctypes.c_double, _dp, _dp, vp]),
+    "hawkes_tree_levels": (ctypes.c_int32, [vp]),
+    "hawkes_tree_launch_count": (i64, [vp]),
+    "hawkes_theta_from_z": (cint, [vp, i64, i64, vp, _dp, ctypes.c_double, _dp, _dp, vp]),
+    "hawkes_z_chain": (cint, [vp, i64, i64, vp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, vp]),
+    "hawkes_posterior_z": (cint, [vp, vp, i64, _dp, _dp, i64, vp, _dp, ctypes.c_double, PP, ctypes.c_double,
+                                  ctypes.c_double, _dp, _dp, _dp, vp]),
 }
 
 

@@ -893,6 +893,56 @@ __global__ void gather_kernel(int64_t n, int dim, const int64_t* __restrict__ pe
     th_out[i] = th_in[s];
 }
 
+// z-parametrisation of the rates (f(t) = t)
+__global__ void fill_ones_kernel(int64_t n, double* __restrict__ theta) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) theta[i] = 1.0;
+}
+__global__ void theta_scatter_kernel(int64_t m, const int64_t* __restrict__ idx, const double* __restrict__ z, double beta,
+                                     const double* __restrict__ t, double* __restrict__ theta) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const int64_t i = idx[k];
+    theta[i] = exp(z[k] + beta * t[i]);
+}
+// chain rule through theta(z); optionally adds the prior gradient and writes (ell, log prior, sum)
+__global__ void z_chain_kernel(int64_t m, const int64_t* __restrict__ idx, const double* __restrict__ theta,
+                               const double* __restrict__ grad_theta, const double* __restrict__ hess_theta_diag,
+                               const double* __restrict__ prior_grad_z, double* __restrict__ grad_z,
+                               double* __restrict__ hess_z, const double* __restrict__ ll_lp, double* __restrict__ out3) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k == 0 && out3 != nullptr) {
+        out3[0] = ll_lp[0];
+        out3[1] = ll_lp[1];
+        out3[2] = ll_lp[0] + ll_lp[1];
+    }
+    if (k >= m) return;
+    const int64_t i = idx[k];
+    const double th = theta[i], g = th * grad_theta[i];
+    if (grad_z) grad_z[k] = prior_grad_z ? g + prior_grad_z[k] : g;
+    if (hess_z) hess_z[k] = fma(th * th, hess_theta_diag[i], g);
+}
+// d ell / d beta = sum_k t_i theta_i d ell/d theta_i: one CTA, thread j takes k = j, j + 1024, ... then a fixed tree
+__global__ void __launch_bounds__(1024) grad_beta_kernel(int64_t m, const int64_t* __restrict__ idx,
+                                                         const double* __restrict__ theta, const double* __restrict__ t,
+                                                         const double* __restrict__ grad_theta, double* __restrict__ out) {
+    __shared__ double sm[32];
+    double a = 0.0;
+    for (int64_t k = threadIdx.x; k < m; k += 1024) {
+        const int64_t i = idx[k];
+        a = fma(t[i] * theta[i], grad_theta[i], a);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double r = 0.0;
+        for (int w = 0; w < 32; ++w) r += sm[w];
+        *out = r;
+    }
+}
+
 // DFMA-chain microbenchmark: 8 independent chains per thread, `iters` x 8 x 8 FMAs.
 __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, double* out) {
     double a[8];
@@ -948,6 +998,7 @@ struct hawkes_ctx {
     double* d_scal;       // 2 (sum log lambda, Lambda) + peak scratch
     double* d_in;         // staging for hawkes_eval_host: x[dim*n_max], t, theta
     double* d_out;        // staging for outputs: 1 + n + 6 + n + 36 + 6n
+    double* d_post;       // hawkes_posterior_z scratch: theta, grad_theta, hess_theta_diag, prior grad (n_max each) + 8
     unsigned* d_status;
     void* d_cub;          // temp storage for the sort
     size_t cub_bytes;
@@ -1231,7 +1282,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_part1, (void**)&c->d_part2,
                      (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
-                     (void**)&c->d_out, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
+                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
     alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
@@ -1244,6 +1295,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_scal, sizeof(double) * 8);
     alloc((void**)&c->d_in, sizeof(double) * (size_t)(dim + 2) * (size_t)n_max);
     alloc((void**)&c->d_out, sizeof(double) * (size_t)(43 + 8 * n_max));
+    alloc((void**)&c->d_post, sizeof(double) * (size_t)(8 + 4 * n_max));
     alloc((void**)&c->d_status, sizeof(unsigned) * 2);
     alloc(&c->d_cub, c->cub_bytes);
     alloc((void**)&c->d_sort_keys, sizeof(double) * (size_t)n_max);
@@ -1263,7 +1315,7 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
-                    c->d_scal, c->d_in, c->d_out, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
+                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     if (c->prof_ev) {
@@ -1393,6 +1445,72 @@ int hawkes_sort_events(hawkes_ctx* ctx, int64_t n, int dim, const double* x_in, 
     CK(cub::DeviceRadixSort::SortPairs(ctx->d_cub, bytes, t_in, t_out, (const int64_t*)ctx->d_sort_idx, perm, (int)n, 0, 64, st));
     gather_kernel<<<nb, 256, 0, st>>>(n, dim, perm, x_in, theta_in, x_out, theta_out);
     ctx->launches += 2;
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_theta_from_z(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, const double* z, double beta,
+                        const double* t, double* theta, void* stream) {
+    if (!ctx || !theta || n < 1 || n > ctx->n_max || m < 0 || m > n) return HAWKES_ERR_ARG;
+    if (m > 0 && (!idx || !z || !t)) return HAWKES_ERR_ARG;
+    if (!std::isfinite(beta)) return HAWKES_ERR_PARAM;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    fill_ones_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, theta);
+    ctx->launches++;
+    if (m > 0) {
+        theta_scatter_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(m, idx, z, beta, t, theta);
+        ctx->launches++;
+    }
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_z_chain(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, const double* theta, const double* t,
+                   const double* grad_theta, const double* hess_theta_diag, const double* prior_grad_z,
+                   double* grad_z, double* hess_z, double* grad_beta, void* stream) {
+    if (!ctx || n < 1 || n > ctx->n_max || m < 1 || m > n || !idx || !theta || !grad_theta) return HAWKES_ERR_ARG;
+    if (!grad_z && !hess_z && !grad_beta) return HAWKES_ERR_ARG;
+    if ((hess_z && !hess_theta_diag) || (grad_beta && !t)) return HAWKES_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(ctx->device));
+    if (grad_z || hess_z) {
+        z_chain_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(m, idx, theta, grad_theta, hess_theta_diag,
+                                                                   prior_grad_z, grad_z, hess_z, nullptr, nullptr);
+        ctx->launches++;
+    }
+    if (grad_beta) {
+        grad_beta_kernel<<<1, 1024, 0, st>>>(m, idx, theta, t, grad_theta, grad_beta);
+        ctx->launches++;
+    }
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                       const int64_t* idx, const double* z, double beta, const hawkes_params* p, double sigma2,
+                       double tau0, double* out3, double* grad_z, double* hess_z, void* stream) {
+    if (!ctx || !tree || !x || !t || !idx || !z || !p) return HAWKES_ERR_ARG;
+    if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
+    if (!out3 && !grad_z && !hess_z) return HAWKES_ERR_ARG;
+    double* th = ctx->d_post + 8;
+    double* gt = th + ctx->n_max;
+    double* ht = gt + ctx->n_max;
+    double* pg = ht + ctx->n_max;
+    double* sc = ctx->d_post;   // sc[0] = ell, sc[1] = log prior
+    int rc = hawkes_theta_from_z(ctx, n, m, idx, z, beta, t, th, stream);
+    if (rc) return rc;
+    const uint32_t want = HAWKES_WANT_LL | ((grad_z || hess_z) ? HAWKES_WANT_GRAD_THETA : 0u) |
+                          (hess_z ? HAWKES_WANT_HESS_THETA : 0u);
+    rc = hawkes_eval(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr, hess_z ? ht : nullptr,
+                     nullptr, nullptr, stream);
+    if (rc) return rc;
+    rc = hawkes_tree_prior(tree, z, sigma2, tau0, sc + 1, grad_z ? pg : nullptr, stream);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    z_chain_kernel<<<(unsigned)((m + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        m, idx, th, gt, hess_z ? ht : nullptr, grad_z ? pg : nullptr, grad_z, hess_z, sc, out3);
+    ctx->launches++;
     CK(cudaGetLastError());
     return HAWKES_OK;
 }

@@ -1,0 +1,251 @@
+// tree.cu -- O(M) evaluation of the phylogenetic Brownian-diffusion prior on the log-rates z (section 2.2,
+// Eq. 2) and of its z-gradient, for sm_100a.  Contract: include/hawkes.h (hawkes_tree_*); design: DESIGN.md section 11.
+//
+// PAPER.md:121 cites the linear-time dynamic programme (post-order message passing on the tree) without printing
+// it; what is implemented is the independent-contrasts recursion, which factorises Eq. 2 exactly:
+//   every node carries the message (m, v): the value of the process at that node is, given the tips below it,
+//   normal with mean m and variance sigma^2 v.   Tips: (z_i, 0).   Internal node u with children a, b:
+//     v_a' = v_a + w_a,  v_b' = v_b + w_b,  c = m_a - m_b,  s = v_a' + v_b'
+//     log p += -1/2 [ log(2 pi sigma^2 s) + c^2 / (sigma^2 s) ]          (the contrast c ~ N(0, sigma^2 s))
+//     alpha = v_b' / s,  m_u = alpha m_a + (1 - alpha) m_b,  v_u = v_a' v_b' / s
+//   root:  s = v_root + tau0,  c = m_root,  same term                     (root value ~ N(0, tau0 sigma^2))
+//   M terms in all (M - 1 internal nodes + the root), matching (2 pi sigma^2)^(-M/2) |V_G|^(-1/2) of Eq. 2.
+// Gradient by one reverse sweep (adjoint of m):  mbar_root = -m_root / (sigma^2 s_root);
+//   mbar_a = alpha mbar_u - c / (sigma^2 s),  mbar_b = (1 - alpha) mbar_u + c / (sigma^2 s);  d log p / d z_i = mbar_tip_i.
+//
+// One CTA walks the tree level by level (level = height above the deepest tip below; all nodes of a level are
+// independent), the node messages living in shared memory (two doubles per node) when the tree fits, else in a
+// global scratch.  Sums are accumulated per thread over a fixed node assignment and reduced in a fixed order, so
+// results are bit-identical run to run.
+#include "../../include/hawkes.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <new>
+#include <vector>
+
+namespace {
+
+constexpr int TREE_T = 1024;
+constexpr size_t TREE_SMEM_MAX = 200 * 1024;
+
+#define CKT(call)                                          \
+    do {                                                   \
+        if ((call) != cudaSuccess) return HAWKES_ERR_CUDA; \
+    } while (0)
+
+// fixed-order block sum of two values; result in thread 0
+__device__ __forceinline__ void block_sum2(double& a, double& b, double* red /*[2 * TREE_T / 32]*/) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, off);
+        b += __shfl_down_sync(0xffffffffu, b, off);
+    }
+    if (lane == 0) { red[2 * wid] = a; red[2 * wid + 1] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double sa = 0.0, sb = 0.0;
+        for (int w = 0; w < TREE_T / 32; ++w) { sa += red[2 * w]; sb += red[2 * w + 1]; }
+        a = sa; b = sb;
+    }
+}
+
+// node storage: nm[v], nv[v] (v = node id).  Life of the slots of the children a, b of an internal node u:
+//   up sweep, before u:   nm = message mean, nv = message variance
+//   up sweep, after u:    nm[a] = alpha_u, nm[b] = c_u / (sigma^2 s_u), nv[a] = s_u   (the messages of a, b are dead)
+//   down sweep:           nv[a], nv[b] = adjoints mbar_a, mbar_b (s_u has been consumed by the log pass)
+template <bool SMEM>
+__global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_levels, const int* __restrict__ level_start,
+                                                            const int* __restrict__ order, const int* __restrict__ child_a,
+                                                            const int* __restrict__ child_b, const double* __restrict__ branch,
+                                                            int root, const double* __restrict__ z, double sigma2,
+                                                            double tau0, double* __restrict__ scratch,
+                                                            double* __restrict__ logp, double* __restrict__ grad_z) {
+    extern __shared__ __align__(16) double sm[];
+    __shared__ double red[2 * TREE_T / 32];
+    const int n_nodes = 2 * n_tips - 1;
+    double* nm = SMEM ? sm : scratch;
+    double* nv = nm + n_nodes;
+    for (int i = threadIdx.x; i < n_tips; i += TREE_T) { nm[i] = z[i]; nv[i] = 0.0; }
+    __syncthreads();
+    const double inv_s2 = 1.0 / sigma2;
+    double quad = 0.0;
+    // up sweep: levels 1 .. n_levels (level_start has n_levels + 1 entries; entry l-1 .. l bound level l)
+    for (int l = 0; l < n_levels; ++l) {
+        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) {
+            const int u = order[q], a = child_a[u], b = child_b[u];
+            const double va = nv[a] + branch[a], vb = nv[b] + branch[b];
+            const double ma = nm[a], mb = nm[b];
+            const double c = ma - mb, s = va + vb, inv = 1.0 / s;
+            const double alpha = vb * inv;
+            nm[u] = fma(alpha, c, mb);          // alpha ma + (1 - alpha) mb
+            nv[u] = va * vb * inv;
+            quad = fma(c * c, inv, quad);
+            nm[a] = alpha;
+            nm[b] = c * inv * inv_s2;
+            nv[a] = s;
+        }
+        __syncthreads();
+    }
+    // log pass: sum of log s over the internal nodes (s sits in nv[child_a])
+    double logs = 0.0;
+    for (int q = threadIdx.x; q < n_tips - 1; q += TREE_T) logs += log(nv[child_a[order[q]]]);
+    double mbar_root = 0.0;
+    if (threadIdx.x == 0) {
+        const double s = nv[root] + tau0, c = nm[root];
+        quad = fma(c * c, 1.0 / s, quad);
+        logs += log(s);
+        mbar_root = -c / (sigma2 * s);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) nv[root] = mbar_root;
+    block_sum2(quad, logs, red);   // contains a barrier: nv[root] is visible after it
+    if (threadIdx.x == 0 && logp)
+        *logp = -0.5 * ((double)n_tips * log(6.283185307179586476925286766559 * sigma2) + logs + quad * inv_s2);
+    if (grad_z == nullptr) return;
+    // down sweep
+    for (int l = n_levels - 1; l >= 0; --l) {
+        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) {
+            const int u = order[q], a = child_a[u], b = child_b[u];
+            const double mbar = nv[u], alpha = nm[a], k = nm[b];
+            nv[a] = fma(alpha, mbar, -k);
+            nv[b] = fma(1.0 - alpha, mbar, k);
+        }
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n_tips; i += TREE_T) grad_z[i] = nv[i];
+}
+
+}  // namespace
+
+struct hawkes_tree {
+    int device;
+    int n_tips, n_levels, root;
+    int *d_level_start, *d_order, *d_child_a, *d_child_b;
+    double *d_branch, *d_scratch;
+    bool smem;
+    size_t smem_bytes;
+    int64_t launches;
+};
+
+extern "C" {
+
+int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent, const double* branch, int device) {
+    if (!out || !parent || !branch || n_tips < 1) return HAWKES_ERR_ARG;
+    const int M = n_tips, nn = 2 * M - 1;
+    std::vector<int> ca(nn, -1), cb(nn, -1), level(nn, 0), pending(nn, 0);
+    int root = -1;
+    for (int v = 0; v < nn; ++v) {
+        const int p = parent[v];
+        if (p < 0) {
+            if (root >= 0) return HAWKES_ERR_ARG;   // two roots
+            root = v;
+            continue;
+        }
+        if (p >= nn || p < M || p == v) return HAWKES_ERR_ARG;          // parents are internal nodes
+        if (!(branch[v] >= 0.0) || !std::isfinite(branch[v])) return HAWKES_ERR_ARG;
+        if (ca[p] < 0) ca[p] = v;
+        else if (cb[p] < 0) cb[p] = v;
+        else return HAWKES_ERR_ARG;                                      // more than two children
+    }
+    if (root < 0) return HAWKES_ERR_ARG;
+    for (int v = M; v < nn; ++v)
+        if (ca[v] < 0 || cb[v] < 0) return HAWKES_ERR_ARG;               // internal node without two children
+    // levels by peeling: a node is ready when both children are done (detects cycles / disconnected parts)
+    std::vector<int> ready;
+    for (int v = 0; v < M; ++v) ready.push_back(v);
+    size_t head = 0;
+    int done = 0, n_levels = 0;
+    while (head < ready.size()) {
+        const int v = ready[head++];
+        ++done;
+        const int p = parent[v];
+        if (p < 0) continue;
+        level[p] = level[p] > level[v] + 1 ? level[p] : level[v] + 1;
+        if (++pending[p] == 2) ready.push_back(p);
+    }
+    if (done != nn) return HAWKES_ERR_ARG;
+    for (int v = M; v < nn; ++v) n_levels = level[v] > n_levels ? level[v] : n_levels;
+    std::vector<int> level_start(n_levels + 1, 0), order(M > 1 ? M - 1 : 1, 0);
+    for (int v = M; v < nn; ++v) level_start[level[v]]++;       // count per level l at index l (levels 1..n_levels)
+    // prefix: level l occupies [start[l-1], start[l])
+    {
+        std::vector<int> cnt(level_start);
+        int acc = 0;
+        level_start[0] = 0;
+        for (int l = 1; l <= n_levels; ++l) { acc += cnt[l]; level_start[l] = acc; }
+        std::vector<int> fill(n_levels + 1, 0);
+        for (int v = M; v < nn; ++v) {
+            const int l = level[v];
+            order[level_start[l - 1] + fill[l]++] = v;
+        }
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return HAWKES_ERR_CUDA;
+    CKT(cudaSetDevice(device));
+    hawkes_tree* t = new (std::nothrow) hawkes_tree();
+    if (!t) return HAWKES_ERR_NOMEM;
+    t->device = device; t->n_tips = M; t->n_levels = n_levels; t->root = root; t->launches = 0;
+    t->smem_bytes = sizeof(double) * 2 * (size_t)nn;
+    t->smem = t->smem_bytes <= TREE_SMEM_MAX;
+    t->d_level_start = t->d_order = t->d_child_a = t->d_child_b = nullptr;
+    t->d_branch = t->d_scratch = nullptr;
+    bool ok = true;
+    auto up = [&](void** d, const void* h, size_t bytes) {
+        if (!ok) return;
+        if (cudaMalloc(d, bytes ? bytes : 8) != cudaSuccess) { ok = false; *d = nullptr; return; }
+        if (h && bytes && cudaMemcpy(*d, h, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
+    };
+    up((void**)&t->d_level_start, level_start.data(), sizeof(int) * level_start.size());
+    up((void**)&t->d_order, order.data(), sizeof(int) * order.size());
+    up((void**)&t->d_child_a, ca.data(), sizeof(int) * nn);
+    up((void**)&t->d_child_b, cb.data(), sizeof(int) * nn);
+    up((void**)&t->d_branch, branch, sizeof(double) * nn);
+    up((void**)&t->d_scratch, nullptr, sizeof(double) * 2 * (size_t)nn);
+    if (ok && t->smem &&
+        cudaFuncSetAttribute(tree_prior_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes) != cudaSuccess)
+        ok = false;
+    if (!ok) {
+        hawkes_tree_destroy(t);
+        cudaGetLastError();
+        return HAWKES_ERR_NOMEM;
+    }
+    *out = t;
+    return HAWKES_OK;
+}
+
+void hawkes_tree_destroy(hawkes_tree* t) {
+    if (!t) return;
+    cudaSetDevice(t->device);
+    void* ptrs[] = {t->d_level_start, t->d_order, t->d_child_a, t->d_child_b, t->d_branch, t->d_scratch};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    delete t;
+}
+
+int hawkes_tree_prior(hawkes_tree* t, const double* z, double sigma2, double tau0, double* logp, double* grad_z,
+                      void* stream) {
+    if (!t || !z || (!logp && !grad_z)) return HAWKES_ERR_ARG;
+    if (!(sigma2 > 0.0) || !std::isfinite(sigma2) || !(tau0 >= 0.0) || !std::isfinite(tau0)) return HAWKES_ERR_PARAM;
+    CKT(cudaSetDevice(t->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (t->smem)
+        tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->d_level_start, t->d_order,
+                                                                 t->d_child_a, t->d_child_b, t->d_branch, t->root, z,
+                                                                 sigma2, tau0, t->d_scratch, logp, grad_z);
+    else
+        tree_prior_kernel<false><<<1, TREE_T, 0, st>>>(t->n_tips, t->n_levels, t->d_level_start, t->d_order, t->d_child_a,
+                                                       t->d_child_b, t->d_branch, t->root, z, sigma2, tau0, t->d_scratch,
+                                                       logp, grad_z);
+    t->launches++;
+    CKT(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int32_t hawkes_tree_levels(const hawkes_tree* t) { return t ? t->n_levels : 0; }
+int64_t hawkes_tree_launch_count(const hawkes_tree* t) { return t ? t->launches : 0; }
+
+}  // extern "C"
