@@ -219,6 +219,42 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
                        const int64_t* idx, const double* z, double beta, const hawkes_params* p /*HOST*/,
                        double sigma2, double tau0, double* out3, double* grad_z, double* hess_z, void* stream);
 
+/* ------------------------------------------------------------------------------------------------------
+ * Preconditioned HMC update of the log-rates z with all likelihood work on the GPU (
+ * BASELINE.json configs[3]).  Target: log pi(z) = ell(theta(z)) + log p(z | V_G, sigma2, tau0).
+ *
+ *   H(z, p) = -log pi(z) + 1/2 p^T M^-1 p, M diagonal
+ *   per iteration: p = sqrt(M) * normals[it];  leapfrog: p += eps/2 grad; n_leapfrog times { z += eps M^-1 p;
+ *   p += eps grad } with the last kick eps/2 (the printed 1/2 in dz/dt is a typo, R7);
+ *   accept iff log(uniforms[it]) < H_old - H_new and H_new is finite.
+ *   Preconditioner (R6): at the start of every iteration it with
+ *   it % precond_every == 0, h_m = max(-d2 ell/dz_m^2, mass_floor) is evaluated at the current state and folded
+ *   into the running average  mass += (h - mass) / (number of refreshes so far, this one included).
+ *
+ * The random numbers are inputs.  Everything is enqueued on `stream`; the accept decision is taken on the device,
+ * the call never synchronises.  n_leapfrog posterior evaluations per iteration (the gradient at the current state
+ * is carried over), plus one Hessian-level evaluation per refresh and one evaluation before the first iteration.
+ */
+typedef struct {
+    int32_t n_iter;          /* iterations to run, >= 1 */
+    int32_t n_leapfrog;      /* leapfrog steps per iteration, >= 1 */
+    int32_t precond_every;   /* refresh interval in iterations; 0 = keep `mass` as given */
+    int32_t n_refresh_done;  /* refreshes already averaged into `mass` (0 for a fresh chain) */
+    double step;             /* eps > 0 */
+    double mass_floor;       /* > 0 */
+    int32_t cache_background; /* 1: evaluate the theta-independent background sums of pass 1 once per call and reuse
+                                 them in every later evaluation (same values; pass 1 then visits causal pairs only) */
+    int32_t reserved;
+} hawkes_hmc_opts;
+
+/* z [m] in-out, mass [m] in-out, normals [n_iter*m], uniforms [n_iter], trace [n_iter*4] or NULL
+ * (per iteration: log pi of the state after the iteration, H_old, H_new, accepted 0/1): all DEVICE.
+ * opts: HOST.  Errors as hawkes_eval (HAWKES_ERR_ARG / HAWKES_ERR_PARAM before anything is enqueued). */
+int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                   const int64_t* idx, double* z, double beta, const hawkes_params* p /*HOST*/, double sigma2,
+                   double tau0, const hawkes_hmc_opts* opts /*HOST*/, const double* normals, const double* uniforms,
+                   double* mass, double* trace, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

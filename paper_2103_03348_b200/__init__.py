@@ -8,7 +8,7 @@ import ctypes
 import dataclasses
 
 from . import synth  # noqa: F401  (seeded inputs; no method arithmetic)
-from ._lib import Params, load, lib_path  # noqa: F401
+from ._lib import HmcOpts, Params, load, lib_path  # noqa: F401
 
 OK = 0
 ERR_ARG, ERR_PARAM, ERR_UNSORTED, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = -1, -2, -3, -4, -5, -6, -7
@@ -222,6 +222,27 @@ class HawkesContext:
         if rc != 0:
             raise HawkesError(rc, "hawkes_posterior_z")
         return out
+
+    def hmc_run(self, tree: "HawkesTree", x, t, idx, z, beta: float, params, sigma2: float, tau0: float, *, n_iter: int,
+                n_leapfrog: int, step: float, precond_every: int, mass, mass_floor: float, normals, uniforms,
+                n_refresh_done: int = 0, cache_background: bool = False, trace=None):
+        """hawkes_hmc_run: z [m] and mass [m] are updated in place (device tensors); normals [n_iter, m] and
+        uniforms [n_iter] are device tensors; returns the trace [n_iter, 4] (device)."""
+        torch = self._torch
+        n, m = int(t.shape[0]), int(idx.shape[0])
+        if normals.shape != (n_iter, m) or uniforms.shape != (n_iter,) or not normals.is_contiguous():
+            raise ValueError("normals must be [n_iter, m] contiguous and uniforms [n_iter]")
+        if trace is None:
+            trace = torch.empty(n_iter, 4, dtype=torch.float64, device=self._dev)
+        o = HmcOpts(int(n_iter), int(n_leapfrog), int(precond_every), int(n_refresh_done), float(step),
+                    float(mass_floor), 1 if cache_background else 0, 0)
+        p = _params(params)
+        rc = self._lib.hawkes_hmc_run(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
+                                      ctypes.byref(p), float(sigma2), float(tau0), ctypes.byref(o), _ptr(normals),
+                                      _ptr(uniforms), _ptr(mass), _ptr(trace), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_hmc_run")
+        return trace
 
     def get_lambda(self, n: int):
         lam = self._torch.empty(n, dtype=self._torch.float64, device=self._dev)

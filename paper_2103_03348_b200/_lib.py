@@ -19,6 +19,12 @@ class Params(ctypes.Structure):
 
 
 PP = ctypes.POINTER(Params)
+
+
+class HmcOpts(ctypes.Structure):
+    _fields_ = [("n_iter", ctypes.c_int32), ("n_leapfrog", ctypes.c_int32), ("precond_every", ctypes.c_int32),
+                ("n_refresh_done", ctypes.c_int32), ("step", ctypes.c_double), ("mass_floor", ctypes.c_double),
+                ("cache_background", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 SYMBOLS = {
     "hawkes_create": (cint, [ctypes.POINTER(vp), i64, cint, cint]),
     "hawkes_destroy": (None, [vp]),
@@ -45,6 +51,8 @@ SYMBOLS = {
     "hawkes_z_chain": (cint, [vp, i64, i64, vp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, vp]),
     "hawkes_posterior_z": (cint, [vp, vp, i64, _dp, _dp, i64, vp, _dp, ctypes.c_double, PP, ctypes.c_double,
                                   ctypes.c_double, _dp, _dp, _dp, vp]),
+    "hawkes_hmc_run": (cint, [vp, vp, i64, _dp, _dp, i64, vp, _dp, ctypes.c_double, PP, ctypes.c_double,
+                              ctypes.c_double, ctypes.POINTER(HmcOpts), _dp, _dp, _dp, _dp, vp]),
 }
 
 

@@ -280,7 +280,9 @@ __device__ __forceinline__ P1C pinned_consts(const double& smagic, const DevCons
     const volatile double& v = smagic;
     return P1C{c.negcb, c.negcs, c.rho_b, c.rho_s, c.lim_b_hi, c.lim_s_hi, {c.d0, c.d1, c.d2, c.d3, v}};
 }
-template <int R, int LEVEL, int MODE, bool DIM3>
+// BG = false: the background sums are taken from the cache of an earlier evaluation (they do not depend on
+// theta), so only the excitation term is evaluated.
+template <int R, int LEVEL, int MODE, bool DIM3, bool BG = true>
 __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt, const Ev<DIM3> (&g)[R],
                                         Mom<LEVEL> (&m)[R], const P1C& c, unsigned lane_base) {
     constexpr int RS = DIM3 ? 6 : 4;
@@ -292,20 +294,22 @@ __device__ __forceinline__ void p1_tile(const double* __restrict__ sbuf, int cnt
             const double dx = g[r].x - s.x, dy = g[r].y - s.y, dt = g[r].t - s.t;
             double u = fma(dy, dy, dx * dx);
             if (DIM3) { const double dz = g[r].z - s.z; u = fma(dz, dz, u); }
-            const double w = dt * dt;
-            const double ab = fma(c.rho_b, w, u);
-            const double eB = exp2_scaled<1>(ab, c.negcb, c.lim_b_hi, u, c.e, lane_base);
-            m[r].b[0] += eB;
-            if (LEVEL == 1) {
-                m[r].b[1] = fma(eB, u, m[r].b[1]);
-                m[r].b[2] = fma(eB, w, m[r].b[2]);
-            } else if (LEVEL == 2) {
-                const double q1 = eB * u, q2 = eB * w;
-                m[r].b[1] += q1;
-                m[r].b[2] += q2;
-                m[r].b[3] = fma(q1, u, m[r].b[3]);
-                m[r].b[4] = fma(q1, w, m[r].b[4]);
-                m[r].b[5] = fma(q2, w, m[r].b[5]);
+            if (BG) {
+                const double w = dt * dt;
+                const double ab = fma(c.rho_b, w, u);
+                const double eB = exp2_scaled<1>(ab, c.negcb, c.lim_b_hi, u, c.e, lane_base);
+                m[r].b[0] += eB;
+                if (LEVEL == 1) {
+                    m[r].b[1] = fma(eB, u, m[r].b[1]);
+                    m[r].b[2] = fma(eB, w, m[r].b[2]);
+                } else if (LEVEL == 2) {
+                    const double q1 = eB * u, q2 = eB * w;
+                    m[r].b[1] += q1;
+                    m[r].b[2] += q2;
+                    m[r].b[3] = fma(q1, u, m[r].b[3]);
+                    m[r].b[4] = fma(q1, w, m[r].b[4]);
+                    m[r].b[5] = fma(q2, w, m[r].b[5]);
+                }
             }
             if (MODE != 0) {
                 const double as = fma(c.rho_s, dt, u);
@@ -365,7 +369,8 @@ __host__ __device__ inline int64_t split_pos(const Split& s, int64_t I, int64_t 
     if (s.tri) { const int64_t j = I * s.tile + c; return j < s.n ? j : s.n; }
     int64_t i1 = (I + 1) * s.tile; if (i1 > s.n) i1 = s.n;
     const int64_t wh = s.w_all + s.w_head;
-    int64_t j = (c < wh * i1) ? c / wh : i1 + (c - wh * i1) / s.w_all;
+    int64_t j = (c < wh * i1 || s.w_all == 0) ? c / wh : i1 + (c - wh * i1) / s.w_all;
+    if (s.w_all == 0 && j > i1) j = i1;   // excitation-only pass: nothing is visited past the tile's end
     return j < s.n ? j : s.n;
 }
 // first CTA and number of CTAs (= partial slots) that hold a segment of tile I
@@ -377,7 +382,7 @@ __host__ __device__ inline void split_slots(const Split& s, int64_t I, int* firs
 
 // a1: one CTA per SM, G independent work groups of NT threads; group (blockIdx.x * G + g) is worker
 // number `vcta` of the single wave.  part[(slot*NMOM + k)*ld + n], NMOM = 2 NB.
-template <int R, int LEVEL, bool DIM3, int G>
+template <int R, int LEVEL, bool DIM3, int G, bool BG = true>
 __global__ void __launch_bounds__(NT * G, 1) pass1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                           DevConsts c, const double* __restrict__ tab_g,
                                                           double* __restrict__ part, Split sp) {
@@ -443,11 +448,11 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_kernel(const double* __restri
             if (a2 < je) io.load(rec, a2, (int)(b2 - a2), tid);
             const double* sb = cur ? sbuf1 : sbuf0;
             if (a >= i1) {
-                p1_tile<R, LEVEL, 0, DIM3>(sb, cnt, g, m, pc, lane_base);
+                if (BG) p1_tile<R, LEVEL, 0, DIM3, BG>(sb, cnt, g, m, pc, lane_base);
             } else if (b <= i0 && rec[(b - 1) * RS + TOFF] < t_first) {
-                p1_tile<R, LEVEL, 1, DIM3>(sb, cnt, g, m, pc, lane_base);
+                p1_tile<R, LEVEL, 1, DIM3, BG>(sb, cnt, g, m, pc, lane_base);
             } else {
-                p1_tile<R, LEVEL, 2, DIM3>(sb, cnt, g, m, pc, lane_base);
+                p1_tile<R, LEVEL, 2, DIM3, BG>(sb, cnt, g, m, pc, lane_base);
             }
             if (a2 < je) io.store(cur ? sbuf0 : sbuf1, tid);
             group_sync(grp);
@@ -511,7 +516,8 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
                                                         Split sp, double* __restrict__ lam,
                                                         double* __restrict__ trec, double* __restrict__ glam,
                                                         double* __restrict__ blockpart,
-                                                        unsigned* __restrict__ status) {
+                                                        unsigned* __restrict__ status, double* __restrict__ bgcache,
+                                                        int bg_mode) {
     constexpr int RS = DIM3 ? 6 : 4;
     constexpr int NB = Mom<LEVEL>::NB;
     const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
@@ -545,6 +551,9 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
 #pragma unroll
             for (int k = 0; k < NB; ++k) { b[k] += v[k]; s[k] += v[NB + k]; }
         }
+        // background-sum cache (LEVEL 0 only; the sum does not depend on theta): 1 = store, 2 = use
+        if (bg_mode == 1) bgcache[i] = b[0];
+        else if (bg_mode == 2) b[0] = bgcache[i];
         const Ev<DIM3> e = read_rec<DIM3>(rec + i * RS);
         const double D = (double)c.dim;
         const double SB = c.CBS * b[0], SS = c.CSS * s[0];
@@ -943,6 +952,82 @@ __global__ void __launch_bounds__(1024) grad_beta_kernel(int64_t m, const int64_
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// HMC on z: three single-CTA kernels around the posterior evaluations.  hs = scalar scratch:
+// hs[0] = K_old; state scalars o3c[3] / o3p[3] = (ell, log prior, log pi) of the current / proposed state.
+constexpr int HMC_T = 1024;
+__device__ __forceinline__ double hmc_block_sum(double a, double* sm /*[32]*/) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = a;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < HMC_T / 32; ++w) r += sm[w];
+    return r;   // valid in thread 0
+}
+// p = sqrt(mass) normal;  K_old = 1/2 sum p^2/mass;  zp = z;  p += eps/2 grad;  zp += eps p / mass
+__global__ void __launch_bounds__(HMC_T) hmc_begin_kernel(int64_t m, const double* __restrict__ z, const double* __restrict__ grad,
+                                                          const double* __restrict__ mass, const double* __restrict__ nrm,
+                                                          double eps, double* __restrict__ zp, double* __restrict__ p,
+                                                          double* __restrict__ hs) {
+    __shared__ double sm[32];
+    double k = 0.0;
+    for (int64_t i = threadIdx.x; i < m; i += HMC_T) {
+        const double mi = mass[i];
+        double pi = sqrt(mi) * nrm[i];
+        k += pi * pi / mi;
+        pi = fma(0.5 * eps, grad[i], pi);
+        p[i] = pi;
+        zp[i] = z[i] + eps * pi / mi;
+    }
+    const double ks = hmc_block_sum(k, sm);
+    if (threadIdx.x == 0) hs[0] = 0.5 * ks;
+}
+// p += eps grad;  zp += eps p / mass
+__global__ void hmc_leap_kernel(int64_t m, const double* __restrict__ grad, const double* __restrict__ mass, double eps,
+                                double* __restrict__ zp, double* __restrict__ p) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    const double pi = fma(eps, grad[i], p[i]);
+    p[i] = pi;
+    zp[i] += eps * pi / mass[i];
+}
+// last half kick, energies, accept test, conditional copy of the state, trace
+__global__ void __launch_bounds__(HMC_T) hmc_end_kernel(int64_t m, const double* __restrict__ gradp, const double* __restrict__ mass,
+                                                        double eps, const double* __restrict__ zp, const double* __restrict__ p,
+                                                        const double* __restrict__ o3p, const double* __restrict__ hs,
+                                                        const double* __restrict__ u, double* __restrict__ z,
+                                                        double* __restrict__ grad, double* __restrict__ o3c,
+                                                        double* __restrict__ trace) {
+    __shared__ double sm[32];
+    __shared__ int acc;
+    double k = 0.0;
+    for (int64_t i = threadIdx.x; i < m; i += HMC_T) {
+        const double pi = fma(0.5 * eps, gradp[i], p[i]);
+        k += pi * pi / mass[i];
+    }
+    const double ks = hmc_block_sum(k, sm);
+    if (threadIdx.x == 0) {
+        const double h_old = -o3c[2] + hs[0], h_new = -o3p[2] + 0.5 * ks;
+        const int a = (isfinite(h_new) && log(*u) < h_old - h_new) ? 1 : 0;
+        acc = a;
+        if (a) { o3c[0] = o3p[0]; o3c[1] = o3p[1]; o3c[2] = o3p[2]; }
+        if (trace) { trace[0] = a ? o3p[2] : o3c[2]; trace[1] = h_old; trace[2] = h_new; trace[3] = (double)a; }
+    }
+    __syncthreads();
+    if (acc)
+        for (int64_t i = threadIdx.x; i < m; i += HMC_T) { z[i] = zp[i]; grad[i] = gradp[i]; }
+}
+// running average of the clamped negative Hessian diagonal: mass += (max(-hess_z, floor) - mass) / k
+__global__ void hmc_mass_kernel(int64_t m, const double* __restrict__ hess_z, double floor_, double inv_k,
+                                double* __restrict__ mass) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    const double h = fmax(-hess_z[i], floor_), mi = mass[i];
+    mass[i] = mi + (h - mi) * inv_k;
+}
+
 // DFMA-chain microbenchmark: 8 independent chains per thread, `iters` x 8 x 8 FMAs.
 __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, double* out) {
     double a[8];
@@ -999,6 +1084,10 @@ struct hawkes_ctx {
     double* d_in;         // staging for hawkes_eval_host: x[dim*n_max], t, theta
     double* d_out;        // staging for outputs: 1 + n + 6 + n + 36 + 6n
     double* d_post;       // hawkes_posterior_z scratch: theta, grad_theta, hess_theta_diag, prior grad (n_max each) + 8
+    double* d_bgcache;    // n_max: cached background sums of pass 1 (LEVEL 0)
+    int bg_mode;          // 0 normal, 1 store the cache, 2 use it (set by hawkes_hmc_run only)
+    int plan_bg;
+    double* d_hmc;        // hawkes_hmc_run scratch: z_prop, p, grad_cur, grad_prop, hess_z (n_max each) + 16
     unsigned* d_status;
     void* d_cub;          // temp storage for the sort
     size_t cub_bytes;
@@ -1123,12 +1212,15 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2
                        : ((want & (HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_CROSS)) ? 1 : 0);
     const int level2 = (want & HAWKES_WANT_HESS_THETA) ? 1 : 0;
-    if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2) {
+    const int bg_mode = level1 == 0 ? ctx->bg_mode : 0;   // the cache holds the LEVEL-0 sum only
+    const int no_bg = bg_mode == 2 ? 1 : 0;
+    if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2 || ctx->plan_bg != no_bg) {
         Plan& q = ctx->plan;
         q.ld = round_up(n, 256);
         q.nblk = (int)((n + RED_T - 1) / RED_T);
-        q.grid1 = plan_split(&q.sp1, n, NT * P1_R, W_ALL[level1], W_HEAD[level1], 0, ctx->sm_count * ctx->occ1[level1],
-                             q.ld, 12, ctx->part1_doubles);
+        q.grid1 = plan_split(&q.sp1, n, NT * P1_R, no_bg ? 0 : W_ALL[level1], W_HEAD[level1], 0,
+                             ctx->sm_count * ctx->occ1[level1], q.ld, 12, ctx->part1_doubles);
+        ctx->plan_bg = no_bg;
         q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, ctx->sm_count * ctx->occ2[level2], q.ld, 2,
                              ctx->part2_doubles);
         ctx->plan_n = n; ctx->plan_l1 = level1; ctx->plan_l2 = level2;
@@ -1144,19 +1236,22 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
+            if (no_bg)
+                pass1_kernel<P1_R, 0, DIM3, P1_G[0], false><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
+            else
             pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode);
             break;
         case 1:
             pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode);
             break;
     }
     ctx->launches += 2;
@@ -1209,6 +1304,8 @@ template <bool DIM3>
 int query_occupancy(hawkes_ctx* ctx) {
     int rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), &ctx->occ1[0]))) return rc;
+    int dummy;
+    if ((rc = setup_kernel(pass1_kernel<P1_R, 0, DIM3, P1_G[0], false>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), &dummy))) return rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 1, DIM3, P1_G[1]>, P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), &ctx->occ1[1]))) return rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 2, DIM3, P1_G[2]>, P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), &ctx->occ1[2]))) return rc;
     if ((rc = setup_kernel(pass2_kernel<P2_R, 0, DIM3, P2_G[0]>, P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), &ctx->occ2[0]))) return rc;
@@ -1262,6 +1359,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     const int nblk = (int)((n_max + RED_T - 1) / RED_T);
     c->plan_n = -1;
     c->plan_l1 = c->plan_l2 = -1;
+    c->bg_mode = 0;
+    c->plan_bg = -1;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess ||
         (dim == 3 ? query_occupancy<true>(c) : query_occupancy<false>(c)) != HAWKES_OK) {
@@ -1282,7 +1381,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_part1, (void**)&c->d_part2,
                      (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
-                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
+                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_bgcache, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
     alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
@@ -1296,6 +1395,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_in, sizeof(double) * (size_t)(dim + 2) * (size_t)n_max);
     alloc((void**)&c->d_out, sizeof(double) * (size_t)(43 + 8 * n_max));
     alloc((void**)&c->d_post, sizeof(double) * (size_t)(8 + 4 * n_max));
+    alloc((void**)&c->d_hmc, sizeof(double) * (size_t)(16 + 5 * n_max));
+    alloc((void**)&c->d_bgcache, sizeof(double) * (size_t)n_max);
     alloc((void**)&c->d_status, sizeof(unsigned) * 2);
     alloc(&c->d_cub, c->cub_bytes);
     alloc((void**)&c->d_sort_keys, sizeof(double) * (size_t)n_max);
@@ -1315,7 +1416,7 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
-                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
+                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_bgcache, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     if (c->prof_ev) {
@@ -1511,6 +1612,61 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
     z_chain_kernel<<<(unsigned)((m + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
         m, idx, th, gt, hess_z ? ht : nullptr, grad_z ? pg : nullptr, grad_z, hess_z, sc, out3);
     ctx->launches++;
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                   const int64_t* idx, double* z, double beta, const hawkes_params* p, double sigma2, double tau0,
+                   const hawkes_hmc_opts* o, const double* normals, const double* uniforms, double* mass, double* trace,
+                   void* stream) {
+    if (!ctx || !tree || !x || !t || !idx || !z || !p || !o || !normals || !uniforms || !mass) return HAWKES_ERR_ARG;
+    if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
+    if (o->n_iter < 1 || o->n_leapfrog < 1 || o->precond_every < 0 || o->n_refresh_done < 0) return HAWKES_ERR_ARG;
+    if (!(o->step > 0.0) || !std::isfinite(o->step) || !(o->mass_floor > 0.0) || !std::isfinite(o->mass_floor))
+        return HAWKES_ERR_PARAM;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* hs = ctx->d_hmc;            // [0] K_old, [4..6] o3 current, [8..10] o3 proposal
+    double* o3c = hs + 4;
+    double* o3p = hs + 8;
+    double* zp = hs + 16;
+    double* pm = zp + ctx->n_max;
+    double* gc = pm + ctx->n_max;
+    double* gp = gc + ctx->n_max;
+    double* hz = gp + ctx->n_max;
+    const double eps = o->step;
+    const unsigned mb = (unsigned)((m + 255) / 256);
+    // the first evaluation fills the background cache, every later one (all at LEVEL 0) uses it
+    ctx->bg_mode = o->cache_background ? 1 : 0;
+    int rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, z, beta, p, sigma2, tau0, o3c, gc, nullptr, stream);
+    ctx->bg_mode = o->cache_background ? 2 : 0;
+    struct Reset { hawkes_ctx* c; ~Reset() { c->bg_mode = 0; } } reset{ctx};
+    if (rc) return rc;
+    int n_refresh = o->n_refresh_done;
+    for (int it = 0; it < o->n_iter; ++it) {
+        if (o->precond_every > 0 && it % o->precond_every == 0) {
+            rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, z, beta, p, sigma2, tau0, nullptr, nullptr, hz, stream);
+            if (rc) return rc;
+            ++n_refresh;
+            CK(cudaSetDevice(ctx->device));
+            hmc_mass_kernel<<<mb, 256, 0, st>>>(m, hz, o->mass_floor, 1.0 / (double)n_refresh, mass);
+            ctx->launches++;
+        }
+        CK(cudaSetDevice(ctx->device));
+        hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, normals + (int64_t)it * m, eps, zp, pm, hs);
+        ctx->launches++;
+        for (int s = 0; s < o->n_leapfrog; ++s) {
+            rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, zp, beta, p, sigma2, tau0, o3p, gp, nullptr, stream);
+            if (rc) return rc;
+            if (s + 1 < o->n_leapfrog) {
+                hmc_leap_kernel<<<mb, 256, 0, st>>>(m, gp, mass, eps, zp, pm);
+                ctx->launches++;
+            }
+        }
+        hmc_end_kernel<<<1, HMC_T, 0, st>>>(m, gp, mass, eps, zp, pm, o3p, hs, uniforms + it, z, gc, o3c,
+                                            trace ? trace + (int64_t)it * 4 : nullptr);
+        ctx->launches++;
+    }
     CK(cudaGetLastError());
     return HAWKES_OK;
 }

@@ -1,0 +1,84 @@
+"""GPU parity of hawkes_hmc_run (include/hawkes.h) against the HMC oracle (oracle/hmc.py) driven by the likelihood
+and prior oracles, on the same seeded inputs and the same random numbers."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import hmc as ohmc
+from oracle import tree as otree
+from paper_2103_03348_b200 import synth
+
+pytestmark = pytest.mark.gpu
+THREADS = min(os.cpu_count() or 1, 32)
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+@pytest.mark.parametrize("cache_bg", [False, True])
+def test_hmc_matches_oracle_trajectory(torch, cache_bg):
+    """1,500 events, 90 sequenced; 6 iterations x 5 leapfrog steps, preconditioner refreshed every 3 iterations.
+    Tolerance: the state after 30 leapfrog steps inherits the 1e-10 bar of the gradient through a mildly expanding
+    map; 1e-8 relative to the scale of z and of the energies leaves two orders of margin (measured ~1e-12)."""
+    import paper_2103_03348_b200 as hp
+    ev = synth.make_events(1500, seed=12, n_centres=6, n_free=90)
+    ev.x *= 0.05
+    idx = ev.free_idx
+    M = len(idx)
+    tree = synth.make_tree(ev.t[idx], 12)
+    s2, tau0, beta = 0.25, 0.1, 0.0005
+    z0 = synth.draw_z(tree, s2, tau0, 12)
+    n_iter, L, eps, every, floor = 6, 5, 0.04, 3, 0.5
+    normals = synth.normals(12, 400, n_iter * M).reshape(n_iter, M)
+    uniforms = synth.uniforms(12, 401, n_iter)
+    uniforms[1] = 1.0      # forces a comparison log(1) = 0 < H_old - H_new: rejects whenever the energy went up
+    mass0 = np.ones(M)
+    V = otree.vg(tree.parent, tree.branch, M, tau0)
+    target = ohmc.hawkes_target(ev.x, ev.t, idx, beta, ev.params, V, s2, threads=THREADS)
+    ref = ohmc.run(target, z0, normals, uniforms, n_iter, L, eps, every, mass0, floor)
+
+    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
+    tr = hp.HawkesTree(tree.parent, tree.branch, 0)
+    z = dev(torch, z0.copy())
+    mass = dev(torch, mass0.copy())
+    trace = ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z, beta, ev.params, s2, tau0,
+                        n_iter=n_iter, n_leapfrog=L, step=eps, precond_every=every, mass=mass, mass_floor=floor,
+                        normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=cache_bg)
+    torch.cuda.synchronize()
+    assert ctx.last_status() == 0
+    trace = trace.cpu().numpy()
+    assert np.array_equal(trace[:, 3], ref["trace"][:, 3]), (trace[:, 3], ref["trace"][:, 3])
+    assert 0 < ref["trace"][:, 3].sum()                     # the case exercises accepted proposals ...
+    escale = np.max(np.abs(ref["trace"][:, 1:3]))
+    assert np.max(np.abs(trace[:, :3] - ref["trace"][:, :3])) <= 1e-8 * escale
+    assert np.max(np.abs(z.cpu().numpy() - ref["z"])) <= 1e-8 * np.max(np.abs(ref["z"]))
+    assert np.max(np.abs(mass.cpu().numpy() - ref["mass"]) / ref["mass"]) <= 1e-8
+
+
+def test_hmc_rejects_bad_options(torch):
+    import paper_2103_03348_b200 as hp
+    ev = synth.make_events(300, seed=3, n_centres=3, n_free=20)
+    idx = ev.free_idx
+    M = len(idx)
+    tree = synth.make_tree(ev.t[idx], 3)
+    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
+    tr = hp.HawkesTree(tree.parent, tree.branch, 0)
+    args = (tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), dev(torch, np.zeros(M)), 0.0, ev.params, 0.25, 0.1)
+    kw = dict(n_iter=2, n_leapfrog=2, step=0.1, precond_every=1, mass=dev(torch, np.ones(M)), mass_floor=0.1,
+              normals=dev(torch, np.zeros((2, M))), uniforms=dev(torch, np.full(2, 0.5)))
+    for bad in (dict(step=0.0), dict(step=float("nan")), dict(mass_floor=0.0)):
+        with pytest.raises(hp.HawkesError) as e:
+            ctx.hmc_run(*args, **{**kw, **bad})
+        assert e.value.status == hp.ERR_PARAM
+    with pytest.raises(hp.HawkesError) as e:
+        ctx.hmc_run(*args, **{**kw, "n_leapfrog": 0})
+    assert e.value.status == hp.ERR_ARG
