@@ -192,6 +192,10 @@ void hawkes_tree_destroy(hawkes_tree* tree);
  * A tree whose V_G is singular (tau0 = 0 with a zero-length path) yields non-finite results, not an error. */
 int hawkes_tree_prior(hawkes_tree* tree, const double* z, double sigma2, double tau0, double* logp,
                       double* grad_z, void* stream);
+/* diag(V_G^-1) / sigma2 = -d2 log p / d z_m^2, the prior's own diagonal curvature, into prec_diag[M] (DEVICE), in
+ * O(M) by an upward and a downward sweep over the message variances.  Uses the tree's global scratch: do not run
+ * it concurrently with hawkes_tree_prior on another stream. */
+int hawkes_tree_precision_diag(hawkes_tree* tree, double sigma2, double tau0, double* prec_diag, void* stream);
 int32_t hawkes_tree_levels(const hawkes_tree* tree);        /* depth of the level schedule (diagnostics) */
 int64_t hawkes_tree_launch_count(const hawkes_tree* tree);  /* kernels launched since creation */
 
@@ -230,6 +234,9 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
  *   Preconditioner (R6): at the start of every iteration it with
  *   it % precond_every == 0, h_m = max(-d2 ell/dz_m^2, mass_floor) is evaluated at the current state and folded
  *   into the running average  mass += (h - mass) / (number of refreshes so far, this one included).
+ *   The mass matrix of the dynamics is M = mass + prior_prec, prior_prec = the constant diagonal curvature of the
+ *   prior (hawkes_tree_precision_diag) or NULL for M = mass (reading R20: without it the dynamics are
+ *   unstable on trees with very short branches).
  *
  * The random numbers are inputs.  Everything is enqueued on `stream`; the accept decision is taken on the device,
  * the call never synchronises.  n_leapfrog posterior evaluations per iteration (the gradient at the current state
@@ -253,7 +260,7 @@ typedef struct {
 int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
                    const int64_t* idx, double* z, double beta, const hawkes_params* p /*HOST*/, double sigma2,
                    double tau0, const hawkes_hmc_opts* opts /*HOST*/, const double* normals, const double* uniforms,
-                   double* mass, double* trace, void* stream);
+                   double* mass, const double* prior_prec /*DEVICE [m] or NULL*/, double* trace, void* stream);
 
 #ifdef __cplusplus
 }

@@ -10,9 +10,11 @@ The algorithm, step by step in the paper's notation (numpy fp64; plain Python lo
     leapfrog (Leimkuhler & Reich, cited l.131):  p += eps/2 grad;  L times { z += eps M^-1 p;  p += eps grad }
                                                   with the last kick eps/2
     accept the proposal with probability min(1, exp(H_old - H_new))            (standard HMC, Neal 2011 cited l.117)
-    preconditioner: running average of the negative diagonal Hessian of the log-likelihood in z, refreshed at a
-    fixed interval (l.143-145; reading R6: floor-clamped, likelihood part only) -- the paper gives no
-    step size, averaging weights or floor: those choices are "parity unpinned".
+    preconditioner: M = A + P, A = running average of the negative diagonal Hessian of the log-likelihood in z,
+    refreshed at a fixed interval and floor-clamped (l.143-145; reading R6), P = the prior's own diagonal
+    curvature diag(V_G^-1)/sigma^2 (constant; optional, reading R20: without it the dynamics are unstable on
+    trees with very short branches) -- the paper gives no step size, averaging weights or floor: those choices are
+    "parity unpinned".
 
 Random numbers are INPUTS (normals [n_iter, M] for the momenta, uniforms [n_iter] for the accept test), so that the
 CUDA path and this oracle consume the same draws.
@@ -38,10 +40,13 @@ def leapfrog(target, z, p, grad, mass, eps: float, n_steps: int):
 
 
 def run(target, z0, normals, uniforms, n_iter: int, n_leapfrog: int, eps: float, precond_every: int, mass0,
-        mass_floor: float):
-    """Returns dict(z [M], mass [M], trace [n_iter, 4] = (log pi after the iteration, H_old, H_new, accepted))."""
+        mass_floor: float, prior_prec=None):
+    """Returns dict(z [M], mass [M] (the running average A), trace [n_iter, 4] = (log pi after the iteration, H_old,
+    H_new, accepted)).  The mass matrix used by the dynamics is A + prior_prec."""
     z = np.array(z0, dtype=np.float64)
-    mass = np.array(mass0, dtype=np.float64)
+    avg = np.array(mass0, dtype=np.float64)
+    pp = np.zeros_like(avg) if prior_prec is None else np.asarray(prior_prec, dtype=np.float64)
+    mass = avg + pp
     logpi, grad, _ = target(z, False)
     n_refresh = 0
     trace = np.zeros((n_iter, 4))
@@ -49,7 +54,8 @@ def run(target, z0, normals, uniforms, n_iter: int, n_leapfrog: int, eps: float,
         if precond_every > 0 and it % precond_every == 0:
             _, _, h = target(z, True)
             n_refresh += 1
-            mass = mass + (np.maximum(h, mass_floor) - mass) / n_refresh     # running average of the clamped Hessians
+            avg = avg + (np.maximum(h, mass_floor) - avg) / n_refresh     # running average of the clamped Hessians
+            mass = avg + pp
         p0 = np.sqrt(mass) * normals[it]
         h_old = -logpi + 0.5 * float(np.sum(p0 * p0 / mass))
         z1, p1, logpi1, grad1 = leapfrog(target, z, p0, grad, mass, eps, n_leapfrog)
@@ -59,7 +65,7 @@ def run(target, z0, normals, uniforms, n_iter: int, n_leapfrog: int, eps: float,
         if accept:
             z, logpi, grad = z1, logpi1, grad1
         trace[it] = (logpi, h_old, h_new, 1.0 if accept else 0.0)
-    return {"z": z, "mass": mass, "trace": trace}
+    return {"z": z, "mass": avg, "trace": trace}
 
 
 def hawkes_target(x, t, idx, beta, params, V, sigma2, threads: int = 1):

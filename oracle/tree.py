@@ -31,6 +31,8 @@ def _l():
         l.tree_ref_vg.argtypes = [ctypes.c_int32, _i32p, _dp, ctypes.c_double, _dp]
         l.tree_ref_logp.restype = ctypes.c_int
         l.tree_ref_logp.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, _dp, _dp]
+        l.tree_ref_precision_diag.restype = ctypes.c_int
+        l.tree_ref_precision_diag.argtypes = [ctypes.c_int32, _dp, ctypes.c_double, _dp]
         _ready = True
     return l
 
@@ -59,6 +61,16 @@ def log_prior(V: np.ndarray, z, sigma2: float, grad: bool = True):
     _l().tree_ref_logp(M, V.ctypes.data_as(_dp), z.ctypes.data_as(_dp), float(sigma2), ctypes.byref(lp),
                        g.ctypes.data_as(_dp) if grad else None)
     return float(lp.value), g
+
+
+def precision_diag(V: np.ndarray, sigma2: float) -> np.ndarray:
+    """diag(V_G^-1) / sigma2 = -d2 log p / d z_m^2 of Eq. 2."""
+    V = np.ascontiguousarray(V, dtype=np.float64)
+    M = V.shape[0]
+    out = np.empty(M, dtype=np.float64)
+    if _l().tree_ref_precision_diag(M, V.ctypes.data_as(_dp), float(sigma2), out.ctypes.data_as(_dp)) != 0:
+        raise ValueError("V is not positive definite")
+    return out
 
 
 def theta_from_z(n: int, idx, z, beta: float, t) -> np.ndarray:

@@ -125,4 +125,36 @@ int tree_ref_logp(int32_t n_tips, const double* V, const double* z, double sigma
     return 0;
 }
 
+// diag(V^-1) / sigma2 = - d2 log p / d z_m^2 (the prior's own curvature; used as the constant part of the HMC
+// preconditioner, reading R6): dense, from the Cholesky factor: (V^-1)_ii = sum_k (L^-1)_ki^2.
+int tree_ref_precision_diag(int32_t n_tips, const double* V, double sigma2, double* out) {
+    const int64_t M = n_tips;
+    std::vector<ld> L((size_t)M * M, 0.0L);
+    for (int64_t j = 0; j < M; ++j) {
+        ld s = (ld)V[j * M + j];
+        for (int64_t k = 0; k < j; ++k) s -= L[j * M + k] * L[j * M + k];
+        if (!(s > 0.0L)) return 1;
+        const ld d = sqrtl(s);
+        L[j * M + j] = d;
+        for (int64_t i = j + 1; i < M; ++i) {
+            ld r = (ld)V[i * M + j];
+            for (int64_t k = 0; k < j; ++k) r -= L[i * M + k] * L[j * M + k];
+            L[i * M + j] = r / d;
+        }
+    }
+    std::vector<ld> col(M);
+    for (int64_t i = 0; i < M; ++i) {
+        // column i of L^-1: solve L y = e_i
+        ld acc = 0.0L;
+        for (int64_t r = i; r < M; ++r) {
+            ld v = (r == i) ? 1.0L : 0.0L;
+            for (int64_t k = i; k < r; ++k) v -= L[r * M + k] * col[k];
+            col[r] = v / L[r * M + r];
+            acc += col[r] * col[r];
+        }
+        out[i] = (double)(acc / (ld)sigma2);
+    }
+    return 0;
+}
+
 }  // extern "C"

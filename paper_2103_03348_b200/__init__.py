@@ -225,7 +225,7 @@ class HawkesContext:
 
     def hmc_run(self, tree: "HawkesTree", x, t, idx, z, beta: float, params, sigma2: float, tau0: float, *, n_iter: int,
                 n_leapfrog: int, step: float, precond_every: int, mass, mass_floor: float, normals, uniforms,
-                n_refresh_done: int = 0, cache_background: bool = False, trace=None):
+                n_refresh_done: int = 0, cache_background: bool = False, prior_prec=None, trace=None):
         """hawkes_hmc_run: z [m] and mass [m] are updated in place (device tensors); normals [n_iter, m] and
         uniforms [n_iter] are device tensors; returns the trace [n_iter, 4] (device)."""
         torch = self._torch
@@ -239,7 +239,7 @@ class HawkesContext:
         p = _params(params)
         rc = self._lib.hawkes_hmc_run(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
                                       ctypes.byref(p), float(sigma2), float(tau0), ctypes.byref(o), _ptr(normals),
-                                      _ptr(uniforms), _ptr(mass), _ptr(trace), self._stream())
+                                      _ptr(uniforms), _ptr(mass), _ptr(prior_prec), _ptr(trace), self._stream())
         if rc != 0:
             raise HawkesError(rc, "hawkes_hmc_run")
         return trace
@@ -323,6 +323,16 @@ class HawkesTree:
         if rc != 0:
             raise HawkesError(rc, "hawkes_tree_prior")
         return lp, g
+
+    def precision_diag(self, sigma2: float, tau0: float):
+        """hawkes_tree_precision_diag: diag(V_G^-1)/sigma2 [M] (device tensor)."""
+        torch = self._torch
+        out = torch.empty(self.n_tips, dtype=torch.float64, device=self._dev)
+        st = ctypes.c_void_p(torch.cuda.current_stream(self._dev).cuda_stream)
+        rc = self._lib.hawkes_tree_precision_diag(self._h, float(sigma2), float(tau0), _ptr(out), st)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_tree_precision_diag")
+        return out
 
     def levels(self) -> int:
         return int(self._lib.hawkes_tree_levels(self._h))

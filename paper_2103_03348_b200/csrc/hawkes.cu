@@ -968,13 +968,14 @@ __device__ __forceinline__ double hmc_block_sum(double a, double* sm /*[32]*/) {
 }
 // p = sqrt(mass) normal;  K_old = 1/2 sum p^2/mass;  zp = z;  p += eps/2 grad;  zp += eps p / mass
 __global__ void __launch_bounds__(HMC_T) hmc_begin_kernel(int64_t m, const double* __restrict__ z, const double* __restrict__ grad,
-                                                          const double* __restrict__ mass, const double* __restrict__ nrm,
+                                                          const double* __restrict__ mass, const double* __restrict__ pp,
+                                                          const double* __restrict__ nrm,
                                                           double eps, double* __restrict__ zp, double* __restrict__ p,
                                                           double* __restrict__ hs) {
     __shared__ double sm[32];
     double k = 0.0;
     for (int64_t i = threadIdx.x; i < m; i += HMC_T) {
-        const double mi = mass[i];
+        const double mi = pp ? mass[i] + pp[i] : mass[i];
         double pi = sqrt(mi) * nrm[i];
         k += pi * pi / mi;
         pi = fma(0.5 * eps, grad[i], pi);
@@ -985,17 +986,17 @@ __global__ void __launch_bounds__(HMC_T) hmc_begin_kernel(int64_t m, const doubl
     if (threadIdx.x == 0) hs[0] = 0.5 * ks;
 }
 // p += eps grad;  zp += eps p / mass
-__global__ void hmc_leap_kernel(int64_t m, const double* __restrict__ grad, const double* __restrict__ mass, double eps,
-                                double* __restrict__ zp, double* __restrict__ p) {
+__global__ void hmc_leap_kernel(int64_t m, const double* __restrict__ grad, const double* __restrict__ mass,
+                                const double* __restrict__ pp, double eps, double* __restrict__ zp, double* __restrict__ p) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m) return;
     const double pi = fma(eps, grad[i], p[i]);
     p[i] = pi;
-    zp[i] += eps * pi / mass[i];
+    zp[i] += eps * pi / (pp ? mass[i] + pp[i] : mass[i]);
 }
 // last half kick, energies, accept test, conditional copy of the state, trace
 __global__ void __launch_bounds__(HMC_T) hmc_end_kernel(int64_t m, const double* __restrict__ gradp, const double* __restrict__ mass,
-                                                        double eps, const double* __restrict__ zp, const double* __restrict__ p,
+                                                        const double* __restrict__ pp, double eps, const double* __restrict__ zp, const double* __restrict__ p,
                                                         const double* __restrict__ o3p, const double* __restrict__ hs,
                                                         const double* __restrict__ u, double* __restrict__ z,
                                                         double* __restrict__ grad, double* __restrict__ o3c,
@@ -1005,7 +1006,7 @@ __global__ void __launch_bounds__(HMC_T) hmc_end_kernel(int64_t m, const double*
     double k = 0.0;
     for (int64_t i = threadIdx.x; i < m; i += HMC_T) {
         const double pi = fma(0.5 * eps, gradp[i], p[i]);
-        k += pi * pi / mass[i];
+        k += pi * pi / (pp ? mass[i] + pp[i] : mass[i]);
     }
     const double ks = hmc_block_sum(k, sm);
     if (threadIdx.x == 0) {
@@ -1618,8 +1619,8 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
 
 int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
                    const int64_t* idx, double* z, double beta, const hawkes_params* p, double sigma2, double tau0,
-                   const hawkes_hmc_opts* o, const double* normals, const double* uniforms, double* mass, double* trace,
-                   void* stream) {
+                   const hawkes_hmc_opts* o, const double* normals, const double* uniforms, double* mass,
+                   const double* prior_prec, double* trace, void* stream) {
     if (!ctx || !tree || !x || !t || !idx || !z || !p || !o || !normals || !uniforms || !mass) return HAWKES_ERR_ARG;
     if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
     if (o->n_iter < 1 || o->n_leapfrog < 1 || o->precond_every < 0 || o->n_refresh_done < 0) return HAWKES_ERR_ARG;
@@ -1653,17 +1654,17 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
             ctx->launches++;
         }
         CK(cudaSetDevice(ctx->device));
-        hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, normals + (int64_t)it * m, eps, zp, pm, hs);
+        hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, prior_prec, normals + (int64_t)it * m, eps, zp, pm, hs);
         ctx->launches++;
         for (int s = 0; s < o->n_leapfrog; ++s) {
             rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, zp, beta, p, sigma2, tau0, o3p, gp, nullptr, stream);
             if (rc) return rc;
             if (s + 1 < o->n_leapfrog) {
-                hmc_leap_kernel<<<mb, 256, 0, st>>>(m, gp, mass, eps, zp, pm);
+                hmc_leap_kernel<<<mb, 256, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm);
                 ctx->launches++;
             }
         }
-        hmc_end_kernel<<<1, HMC_T, 0, st>>>(m, gp, mass, eps, zp, pm, o3p, hs, uniforms + it, z, gc, o3c,
+        hmc_end_kernel<<<1, HMC_T, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm, o3p, hs, uniforms + it, z, gc, o3c,
                                             trace ? trace + (int64_t)it * 4 : nullptr);
         ctx->launches++;
     }

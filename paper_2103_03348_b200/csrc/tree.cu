@@ -58,41 +58,71 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double* red /*[
 //   up sweep, after u:    nm[a] = alpha_u, nm[b] = c_u / (sigma^2 s_u), nv[a] = s_u   (the messages of a, b are dead)
 //   down sweep:           nv[a], nv[b] = adjoints mbar_a, mbar_b (s_u has been consumed by the log pass)
 template <bool SMEM>
-__global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_levels, const int* __restrict__ level_start,
-                                                            const int* __restrict__ order, const int* __restrict__ child_a,
-                                                            const int* __restrict__ child_b, const double* __restrict__ branch,
+__global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_levels, int narrow_from,
+                                                            const int* __restrict__ g_level_start,
+                                                            const int* __restrict__ g_order, const int* __restrict__ g_child_a,
+                                                            const int* __restrict__ g_child_b, const double* __restrict__ g_wa,
+                                                            const double* __restrict__ g_wb,
                                                             int root, const double* __restrict__ z, double sigma2,
                                                             double tau0, double* __restrict__ scratch,
                                                             double* __restrict__ logp, double* __restrict__ grad_z) {
     extern __shared__ __align__(16) double sm[];
     __shared__ double red[2 * TREE_T / 32];
-    const int n_nodes = 2 * n_tips - 1;
+    const int n_nodes = 2 * n_tips - 1, n_int = n_tips - 1;
     double* nm = SMEM ? sm : scratch;
     double* nv = nm + n_nodes;
+    // topology in level order (position q = 0 .. M-2): node id, children, the children's branch lengths.  With SMEM
+    // it is copied next to the messages so that a level costs shared-memory latency only.
+    const int *order = g_order, *child_a = g_child_a, *child_b = g_child_b, *level_start = g_level_start;
+    const double *wa = g_wa, *wb = g_wb;
+    if (SMEM) {
+        double* s_wa = nv + n_nodes;
+        double* s_wb = s_wa + n_int;
+        int* s_order = reinterpret_cast<int*>(s_wb + n_int);
+        int* s_a = s_order + n_int;
+        int* s_b = s_a + n_int;
+        int* s_ls = s_b + n_int;
+        for (int q = threadIdx.x; q < n_int; q += TREE_T) {
+            s_wa[q] = g_wa[q]; s_wb[q] = g_wb[q]; s_order[q] = g_order[q]; s_a[q] = g_child_a[q]; s_b[q] = g_child_b[q];
+        }
+        for (int l = threadIdx.x; l <= n_levels; l += TREE_T) s_ls[l] = g_level_start[l];
+        order = s_order; child_a = s_a; child_b = s_b; wa = s_wa; wb = s_wb; level_start = s_ls;
+    }
     for (int i = threadIdx.x; i < n_tips; i += TREE_T) { nm[i] = z[i]; nv[i] = 0.0; }
     __syncthreads();
     const double inv_s2 = 1.0 / sigma2;
     double quad = 0.0;
-    // up sweep: levels 1 .. n_levels (level_start has n_levels + 1 entries; entry l-1 .. l bound level l)
-    for (int l = 0; l < n_levels; ++l) {
-        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) {
-            const int u = order[q], a = child_a[u], b = child_b[u];
-            const double va = nv[a] + branch[a], vb = nv[b] + branch[b];
-            const double ma = nm[a], mb = nm[b];
-            const double c = ma - mb, s = va + vb, inv = 1.0 / s;
-            const double alpha = vb * inv;
-            nm[u] = fma(alpha, c, mb);          // alpha ma + (1 - alpha) mb
-            nv[u] = va * vb * inv;
-            quad = fma(c * c, inv, quad);
-            nm[a] = alpha;
-            nm[b] = c * inv * inv_s2;
-            nv[a] = s;
-        }
+    // up sweep: levels 1 .. n_levels (level_start has n_levels + 1 entries; entry l-1 .. l bound level l).
+    // Levels below `narrow_from` are walked by the whole CTA with a block barrier each; from `narrow_from` on every
+    // level has at most 32 nodes and warp 0 walks them alone, one warp barrier per level.
+    auto up_node = [&](int q) {
+        const int u = order[q], a = child_a[q], b = child_b[q];
+        const double va = nv[a] + wa[q], vb = nv[b] + wb[q];
+        const double ma = nm[a], mb = nm[b];
+        const double c = ma - mb, s = va + vb, inv = 1.0 / s;
+        const double alpha = vb * inv;
+        nm[u] = fma(alpha, c, mb);          // alpha ma + (1 - alpha) mb
+        nv[u] = va * vb * inv;
+        quad = fma(c * c, inv, quad);
+        nm[a] = alpha;
+        nm[b] = c * inv * inv_s2;
+        nv[a] = s;
+    };
+    for (int l = 0; l < narrow_from; ++l) {
+        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) up_node(q);
         __syncthreads();
     }
+    if (threadIdx.x < 32) {
+        for (int l = narrow_from; l < n_levels; ++l) {
+            const int q = level_start[l] + threadIdx.x;
+            if (q < level_start[l + 1]) up_node(q);
+            __syncwarp();
+        }
+    }
+    __syncthreads();
     // log pass: sum of log s over the internal nodes (s sits in nv[child_a])
     double logs = 0.0;
-    for (int q = threadIdx.x; q < n_tips - 1; q += TREE_T) logs += log(nv[child_a[order[q]]]);
+    for (int q = threadIdx.x; q < n_int; q += TREE_T) logs += log(nv[child_a[q]]);
     double mbar_root = 0.0;
     if (threadIdx.x == 0) {
         const double s = nv[root] + tau0, c = nm[root];
@@ -106,25 +136,72 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
     if (threadIdx.x == 0 && logp)
         *logp = -0.5 * ((double)n_tips * log(6.283185307179586476925286766559 * sigma2) + logs + quad * inv_s2);
     if (grad_z == nullptr) return;
-    // down sweep
-    for (int l = n_levels - 1; l >= 0; --l) {
-        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) {
-            const int u = order[q], a = child_a[u], b = child_b[u];
-            const double mbar = nv[u], alpha = nm[a], k = nm[b];
-            nv[a] = fma(alpha, mbar, -k);
-            nv[b] = fma(1.0 - alpha, mbar, k);
+    // down sweep (narrow levels first, by warp 0)
+    auto down_node = [&](int q) {
+        const int u = order[q], a = child_a[q], b = child_b[q];
+        const double mbar = nv[u], alpha = nm[a], k = nm[b];
+        nv[a] = fma(alpha, mbar, -k);
+        nv[b] = fma(1.0 - alpha, mbar, k);
+    };
+    if (threadIdx.x < 32) {
+        for (int l = n_levels - 1; l >= narrow_from; --l) {
+            const int q = level_start[l] + threadIdx.x;
+            if (q < level_start[l + 1]) down_node(q);
+            __syncwarp();
         }
+    }
+    __syncthreads();
+    for (int l = narrow_from - 1; l >= 0; --l) {
+        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) down_node(q);
         __syncthreads();
     }
     for (int i = threadIdx.x; i < n_tips; i += TREE_T) grad_z[i] = nv[i];
+}
+
+// diag(V_G^-1) / sigma^2 by two sweeps over variances only: v_up[u] = variance of the message of u's subtree,
+// v_out[u] = variance of u's value given every tip OUTSIDE its subtree (root: tau0, the root prior); for a tip,
+// v_out is its conditional variance given all other tips (in units of sigma^2), whose reciprocal is the
+// diagonal entry of the precision matrix.  Run once per tree / (sigma^2, tau0): node store in global scratch.
+__global__ void __launch_bounds__(TREE_T) tree_precision_kernel(int n_tips, int n_levels, const int* __restrict__ level_start,
+                                                                const int* __restrict__ order, const int* __restrict__ child_a,
+                                                                const int* __restrict__ child_b, const double* __restrict__ branch,
+                                                                int root, double sigma2, double tau0, double* __restrict__ scratch,
+                                                                double* __restrict__ prec_diag) {
+    const int n_nodes = 2 * n_tips - 1;
+    double* vup = scratch;
+    double* vout = scratch + n_nodes;
+    for (int i = threadIdx.x; i < n_tips; i += TREE_T) vup[i] = 0.0;
+    __syncthreads();
+    for (int l = 0; l < n_levels; ++l) {
+        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) {
+            const int u = order[q], a = child_a[u], b = child_b[u];
+            const double va = vup[a] + branch[a], vb = vup[b] + branch[b];
+            vup[u] = va * vb / (va + vb);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) vout[root] = tau0;
+    __syncthreads();
+    for (int l = n_levels - 1; l >= 0; --l) {
+        for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) {
+            const int u = order[q], a = child_a[u], b = child_b[u];
+            const double va = vup[a] + branch[a], vb = vup[b] + branch[b], o = vout[u];
+            vout[a] = ((o + vb > 0.0) ? o * vb / (o + vb) : 0.0) + branch[a];
+            vout[b] = ((o + va > 0.0) ? o * va / (o + va) : 0.0) + branch[b];
+        }
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n_tips; i += TREE_T) prec_diag[i] = 1.0 / (sigma2 * vout[i]);
 }
 
 }  // namespace
 
 struct hawkes_tree {
     int device;
-    int n_tips, n_levels, root;
-    int *d_level_start, *d_order, *d_child_a, *d_child_b;
+    int n_tips, n_levels, narrow_from, root;
+    int *d_level_start, *d_order, *d_child_a, *d_child_b;   // child_a/b: by node id (precision kernel)
+    int *d_qa, *d_qb;                                       // children by level-order position (prior kernel)
+    double *d_qwa, *d_qwb;                                  // their branch lengths, same order
     double *d_branch, *d_scratch;
     bool smem;
     size_t smem_bytes;
@@ -189,9 +266,22 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
     hawkes_tree* t = new (std::nothrow) hawkes_tree();
     if (!t) return HAWKES_ERR_NOMEM;
     t->device = device; t->n_tips = M; t->n_levels = n_levels; t->root = root; t->launches = 0;
-    t->smem_bytes = sizeof(double) * 2 * (size_t)nn;
+    // first level from which every level holds at most 32 nodes (walked by a single warp)
+    t->narrow_from = n_levels;
+    while (t->narrow_from > 0 && level_start[t->narrow_from] - level_start[t->narrow_from - 1] <= 32) t->narrow_from--;
+    // shared memory of the prior kernel: 2 message doubles per node + per internal node 2 doubles and 3 ints + the level offsets
+    t->smem_bytes = sizeof(double) * 2 * (size_t)nn + (size_t)(M - 1) * (2 * sizeof(double) + 3 * sizeof(int)) +
+                    (size_t)(n_levels + 1) * sizeof(int) + 16;
+    std::vector<int> qa(M > 1 ? M - 1 : 1, 0), qb(M > 1 ? M - 1 : 1, 0);
+    std::vector<double> qwa(M > 1 ? M - 1 : 1, 0.0), qwb(M > 1 ? M - 1 : 1, 0.0);
+    for (int q = 0; q < M - 1; ++q) {
+        const int u = order[q];
+        qa[q] = ca[u]; qb[q] = cb[u];
+        qwa[q] = branch[ca[u]]; qwb[q] = branch[cb[u]];
+    }
     t->smem = t->smem_bytes <= TREE_SMEM_MAX;
-    t->d_level_start = t->d_order = t->d_child_a = t->d_child_b = nullptr;
+    t->d_level_start = t->d_order = t->d_child_a = t->d_child_b = t->d_qa = t->d_qb = nullptr;
+    t->d_qwa = t->d_qwb = nullptr;
     t->d_branch = t->d_scratch = nullptr;
     bool ok = true;
     auto up = [&](void** d, const void* h, size_t bytes) {
@@ -204,6 +294,10 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
     up((void**)&t->d_child_a, ca.data(), sizeof(int) * nn);
     up((void**)&t->d_child_b, cb.data(), sizeof(int) * nn);
     up((void**)&t->d_branch, branch, sizeof(double) * nn);
+    up((void**)&t->d_qa, qa.data(), sizeof(int) * qa.size());
+    up((void**)&t->d_qb, qb.data(), sizeof(int) * qb.size());
+    up((void**)&t->d_qwa, qwa.data(), sizeof(double) * qwa.size());
+    up((void**)&t->d_qwb, qwb.data(), sizeof(double) * qwb.size());
     up((void**)&t->d_scratch, nullptr, sizeof(double) * 2 * (size_t)nn);
     if (ok && t->smem &&
         cudaFuncSetAttribute(tree_prior_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes) != cudaSuccess)
@@ -220,7 +314,8 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
 void hawkes_tree_destroy(hawkes_tree* t) {
     if (!t) return;
     cudaSetDevice(t->device);
-    void* ptrs[] = {t->d_level_start, t->d_order, t->d_child_a, t->d_child_b, t->d_branch, t->d_scratch};
+    void* ptrs[] = {t->d_level_start, t->d_order, t->d_child_a, t->d_child_b, t->d_branch, t->d_scratch,
+                    t->d_qa, t->d_qb, t->d_qwa, t->d_qwb};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     delete t;
@@ -233,13 +328,25 @@ int hawkes_tree_prior(hawkes_tree* t, const double* z, double sigma2, double tau
     CKT(cudaSetDevice(t->device));
     cudaStream_t st = (cudaStream_t)stream;
     if (t->smem)
-        tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->d_level_start, t->d_order,
-                                                                 t->d_child_a, t->d_child_b, t->d_branch, t->root, z,
+        tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_order,
+                                                                 t->d_qa, t->d_qb, t->d_qwa, t->d_qwb, t->root, z,
                                                                  sigma2, tau0, t->d_scratch, logp, grad_z);
     else
-        tree_prior_kernel<false><<<1, TREE_T, 0, st>>>(t->n_tips, t->n_levels, t->d_level_start, t->d_order, t->d_child_a,
-                                                       t->d_child_b, t->d_branch, t->root, z, sigma2, tau0, t->d_scratch,
+        tree_prior_kernel<false><<<1, TREE_T, 0, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_order, t->d_qa,
+                                                       t->d_qb, t->d_qwa, t->d_qwb, t->root, z, sigma2, tau0, t->d_scratch,
                                                        logp, grad_z);
+    t->launches++;
+    CKT(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_tree_precision_diag(hawkes_tree* t, double sigma2, double tau0, double* prec_diag, void* stream) {
+    if (!t || !prec_diag) return HAWKES_ERR_ARG;
+    if (!(sigma2 > 0.0) || !std::isfinite(sigma2) || !(tau0 >= 0.0) || !std::isfinite(tau0)) return HAWKES_ERR_PARAM;
+    CKT(cudaSetDevice(t->device));
+    tree_precision_kernel<<<1, TREE_T, 0, (cudaStream_t)stream>>>(t->n_tips, t->n_levels, t->d_level_start, t->d_order,
+                                                                 t->d_child_a, t->d_child_b, t->d_branch, t->root, sigma2,
+                                                                 tau0, t->d_scratch, prec_diag);
     t->launches++;
     CKT(cudaGetLastError());
     return HAWKES_OK;

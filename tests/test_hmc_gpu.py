@@ -24,8 +24,8 @@ def dev(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
 
 
-@pytest.mark.parametrize("cache_bg", [False, True])
-def test_hmc_matches_oracle_trajectory(torch, cache_bg):
+@pytest.mark.parametrize("cache_bg,with_prior_prec", [(False, False), (True, False), (True, True)])
+def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     """1,500 events, 90 sequenced; 6 iterations x 5 leapfrog steps, preconditioner refreshed every 3 iterations.
     Tolerance: the state after 30 leapfrog steps inherits the 1e-10 bar of the gradient through a mildly expanding
     map; 1e-8 relative to the scale of z and of the energies leaves two orders of margin (measured ~1e-12)."""
@@ -44,15 +44,22 @@ def test_hmc_matches_oracle_trajectory(torch, cache_bg):
     mass0 = np.ones(M)
     V = otree.vg(tree.parent, tree.branch, M, tau0)
     target = ohmc.hawkes_target(ev.x, ev.t, idx, beta, ev.params, V, s2, threads=THREADS)
-    ref = ohmc.run(target, z0, normals, uniforms, n_iter, L, eps, every, mass0, floor)
+    pp = otree.precision_diag(V, s2) if with_prior_prec else None
+    if with_prior_prec:
+        eps = 0.3          # the preconditioned dynamics take a far larger step
+    ref = ohmc.run(target, z0, normals, uniforms, n_iter, L, eps, every, mass0, floor, prior_prec=pp)
 
     ctx = hp.HawkesContext(ev.n, ev.dim, 0)
     tr = hp.HawkesTree(tree.parent, tree.branch, 0)
     z = dev(torch, z0.copy())
     mass = dev(torch, mass0.copy())
+    pp_d = tr.precision_diag(s2, tau0) if with_prior_prec else None
+    if with_prior_prec:
+        assert np.max(np.abs(pp_d.cpu().numpy() - pp) / pp) <= 1e-10
     trace = ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z, beta, ev.params, s2, tau0,
                         n_iter=n_iter, n_leapfrog=L, step=eps, precond_every=every, mass=mass, mass_floor=floor,
-                        normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=cache_bg)
+                        normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=cache_bg,
+                        prior_prec=pp_d)
     torch.cuda.synchronize()
     assert ctx.last_status() == 0
     trace = trace.cpu().numpy()

@@ -100,3 +100,20 @@ def test_h4_hawkes_target_is_ell_plus_prior():
         fd = (tgt(z + e, False)[0] - tgt(z - e, False)[0]) / 2e-5
         assert abs(fd - g[k]) <= 2e-7 * max(1.0, abs(g[k]))
     assert h.shape == (4,)
+
+
+def test_h5_prior_precision_adds_to_the_mass():
+    """With prior_prec = P the dynamics use M = A + P: one-dimensional Gaussian target re-traced by hand."""
+    a, P, eps, L = 1.7, 0.9, 0.2, 2
+    tgt = gaussian_target([a])
+    out = hmc.run(tgt, np.array([0.6]), np.array([[0.9]]), np.array([1e-300]), 1, L, eps, 1, np.array([1.0]), 0.5,
+                  prior_prec=np.array([P]))
+    m = a + P                                  # A = a after the first refresh
+    assert abs(out["mass"][0] - a) < 1e-15
+    A = np.array([[1 - eps * eps * a / (2 * m), eps / m],
+                  [-eps * a * (1 - eps * eps * a / (4 * m)), 1 - eps * eps * a / (2 * m)]])
+    p = math.sqrt(m) * 0.9
+    z1, p1 = np.linalg.matrix_power(A, L) @ np.array([0.6, p])
+    assert abs(out["z"][0] - z1) < 1e-14
+    assert abs(out["trace"][0, 1] - (0.5 * a * 0.36 + 0.5 * p * p / m)) < 1e-14
+    assert abs(out["trace"][0, 2] - (0.5 * a * z1 * z1 + 0.5 * p1 * p1 / m)) < 1e-14

@@ -62,6 +62,8 @@ def test_tree_prior_small_trees(torch, M, seed, tau0):
     lps, gs = prior_scales(V, z, s2)
     check("logp", lp, lp_o, lps)
     check("grad_z", g, g_o, gs)
+    tr = hp.HawkesTree(tree.parent, tree.branch, 0)
+    check("prior precision diagonal", tr.precision_diag(s2, tau0).cpu().numpy(), otree.precision_diag(V, s2))
 
 
 def test_tree_prior_config2_full_size_and_determinism(torch):
@@ -81,6 +83,8 @@ def test_tree_prior_config2_full_size_and_determinism(torch):
     assert float(lp2.item()) == lp and np.array_equal(g2.cpu().numpy(), g)      # bit-identical run to run
     lp3, none = tr.prior(dev(torch, z), synth.TREE_SIGMA2, synth.TREE_TAU0, grad=False)
     assert none is None and float(lp3.item()) == lp
+    pd = tr.precision_diag(synth.TREE_SIGMA2, synth.TREE_TAU0).cpu().numpy()
+    check("prior precision diagonal", pd, otree.precision_diag(V, synth.TREE_SIGMA2))
 
 
 @pytest.mark.parametrize("M", [500, 8000])

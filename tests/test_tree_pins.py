@@ -187,3 +187,29 @@ def test_t9_config_tree_generator_shape():
     assert np.allclose(ev.theta[ev.free_idx], np.exp(z)) and np.all(np.delete(ev.theta, ev.free_idx) == 1.0)
     V = otree.vg(tr.parent, tr.branch, M, 0.0)
     assert abs(np.mean(np.diag(V)) - 1.0) < 1e-12
+
+
+def test_t10_prior_precision_diagonal():
+    """diag(V_G^-1)/sigma^2 (the prior's own curvature, -d2 log p/dz_m^2): 2x2 closed form, the star tree by
+    Sherman-Morrison ((V^-1)_ii = 1/w_i - tau0 / (w_i^2 (1 + tau0 sum 1/w))), numpy's inverse on a random tree, and
+    central differences of the oracle's own gradient."""
+    tau0, s2, w1, w2 = 0.1, 0.25, 0.5, 0.7
+    V = otree.vg([2, 2, -1], [w1, w2, 0.0], 2, tau0)
+    det = (tau0 + w1) * (tau0 + w2) - tau0 * tau0
+    assert np.allclose(otree.precision_diag(V, s2), [(tau0 + w2) / det / s2, (tau0 + w1) / det / s2], rtol=1e-14)
+    w = np.array([0.5, 0.9, 0.3, 1.4, 0.7, 1.1])
+    parent = [6, 6, 7, 8, 9, 10, 7, 8, 9, 10, -1]
+    V = otree.vg(parent, list(w) + [0.0] * 5, 6, 0.2)
+    denom = 1 + 0.2 * np.sum(1 / w)
+    assert np.allclose(otree.precision_diag(V, 0.3), (1 / w - 0.2 / (w * w * denom)) / 0.3, rtol=1e-13)
+    M, seed = 35, 13
+    tr = synth.make_tree(np.sort(synth.uniforms(seed, 200, M) * 500.0), seed)
+    V = otree.vg(tr.parent, tr.branch, M, 0.1)
+    pd = otree.precision_diag(V, 0.25)
+    assert np.allclose(pd, np.diag(np.linalg.inv(V)) / 0.25, rtol=1e-8)
+    z = synth.normals(seed, 210, M) * 0.5
+    for k in (0, 7, 34):
+        e = np.zeros(M)
+        e[k] = 1e-4
+        fd = (otree.log_prior(V, z + e, 0.25)[1][k] - otree.log_prior(V, z - e, 0.25)[1][k]) / 2e-4
+        assert abs(-fd - pd[k]) <= 1e-7 * pd[k]
