@@ -209,6 +209,28 @@ def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
 
 
+# Multi-GPU = independent replicas: rank r evaluates the problem drawn with seed + r on its own
+# GPU, no data-path collective; the only exchange is the MAX over ranks of the timed totals.  These three helpers are
+# the whole N > 1 logic and are covered by world-size-2 gloo tests on CPU (tests/test_multiproc.py).
+def replica_seed(seed: int, rank: int) -> int:
+    return int(seed) + int(rank)
+
+
+def max_over_ranks(dist, values, device):
+    """all-reduce(MAX) of a list of floats; identity when dist is None (single process)."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    v = torch.tensor([float(a) for a in values], dtype=torch.float64, device=device)
+    dist.all_reduce(v, op=dist.ReduceOp.MAX)
+    return [float(a) for a in v]
+
+
+def whole_job_value(world: int, steps: int, total_ms_max: float) -> float:
+    """evaluations/s of the whole job: every rank did `steps` evaluations within the slowest rank's time."""
+    return world * steps / (total_ms_max * 1e-3)
+
+
 def ncu_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full
     summary (profiles/traffic.csv: kernel,dram_bytes_per_launch; profiles/traffic.md names the command), or None."""
@@ -289,10 +311,7 @@ def run_b200(args, ev, workload: str) -> dict:
     barrier()
     e_total = float(sum(e_ms))
     clocks = sampler.stop()
-    if dist is not None:
-        v = torch.tensor([total_ms, e_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(v, op=dist.ReduceOp.MAX)
-        total_ms, e_total = float(v[0]), float(v[1])
+    total_ms, e_total = max_over_ranks(dist, [total_ms, e_total], dev)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -302,8 +321,8 @@ def run_b200(args, ev, workload: str) -> dict:
     ll_dev = float(out.ll.item())
     ll_host = float(hout.ll.item())
     assert ll_dev == ll_host, "device-resident and host-buffer evaluations must be bit-identical"
-    value = world * K / (total_ms * 1e-3)
-    e_value = world * K / (e_total * 1e-3)
+    value = whole_job_value(world, K, total_ms)
+    e_value = whole_job_value(world, K, e_total)
     props = torch.cuda.get_device_properties(dev)
     sm_max = clocks.get("sm_max_mhz") or 1965
     peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
@@ -519,6 +538,9 @@ def run_hmc(args) -> dict:
 
 def workload_of(args):
     from paper_2103_03348_b200 import synth
+    rank, world, _ = dist_env()
+    if world > 1 and args.impl != "reference":
+        args = argparse.Namespace(**{**vars(args), "seed": replica_seed(args.seed, rank)})
     if args.n is not None:
         ev = synth.make_events(args.n, args.seed)
         return ev, f"BASELINE.json configs[4] generator at N={args.n} (seed {args.seed})"
