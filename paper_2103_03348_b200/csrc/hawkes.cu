@@ -83,25 +83,16 @@ enum { ST_UNSORTED = 1, ST_NONFINITE = 2, ST_ZERO_RATE = 4 };
 // `lane_base` = shared-space address of the table (64 KB aligned) | lane*8.
 constexpr int N_DEAD = -1023 * TAB_N;
 // KILL_MODE 0: no extra kill; 1: kill when kv == 0 (kv = r2, the coincident-location indicator);
-// 2: kill unless kv > 0 (kv = dt, the causal indicator; fp64 compare).
+// 2: kill unless kv > 0 (kv = dt, the causal indicator; fp64 compare); 4 / 5: as 1 / 2 and kill unless `live` != 0
+// (an index condition: the pair belongs to this block's share of the pair space).
 struct ExpC {       // loop-invariant operands of the exponential
     double d0, d1, d2, d3;   // monic polynomial: from the kernel parameters (uniform registers)
     double magic;            // MAGIC as a run-time value in a vector register (see pinned_consts)
 };
+// table part of the exponential: T = 2^(n>>8) T[n&255] (or +0.0 for a killed term), n = low word of t
 template <int KILL_MODE>
-__device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi, double kv, const ExpC& c,
-                                              unsigned lane_base) {
-    // operand discipline (DESIGN.md section 5): an FP64 instruction reading three distinct vector registers
-    // issues every 3 cycles, one reading two every 2.  negc and the polynomial constants therefore sit in
-    // uniform registers, MAGIC in a vector register, and the polynomial is monic so that each Horner step has
-    // one constant: q(f) = (((f + d3) f + d2) f + d1) f + d0 = 2^f / S.
-    const double t = fma(a, negc, c.magic);
-    const double nf = t - c.magic;
-    const double f = fma(a, negc, -nf);
-    double p = f + c.d3;
-    p = fma(p, f, c.d2);
-    p = fma(p, f, c.d1);
-    p = fma(p, f, c.d0);
+__device__ __forceinline__ double exp2_table(double a, double t, int lim_hi, double kv, unsigned lane_base,
+                                             int live = 1) {
     double T;
 #define HAWKES_EXP2_TAIL                                 \
         "selp.s32 ne, n, %4, p;\n\t"                     \
@@ -110,8 +101,30 @@ __device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi,
         "mad.lo.s32 hi, ne, 4096, hi;\n\t"               \
         "mov.b64 %0, {lo, hi};\n\t"                      \
         "}"                                              \
-        : "=d"(T) : "d"(a), "d"(t), "r"(lim_hi), "n"(N_DEAD), "r"(lane_base), "d"(kv)
-    if constexpr (KILL_MODE == 1) {
+        : "=d"(T) : "d"(a), "d"(t), "r"(lim_hi), "n"(N_DEAD), "r"(lane_base), "d"(kv), "r"(live)
+    if constexpr (KILL_MODE == 4) {
+        asm("{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 alo, ahi, n, thi, klo, khi, ne, ad, lo, hi;\n\t"
+            "mov.b64 {alo, ahi}, %1;\n\t"
+            "mov.b64 {n, thi}, %2;\n\t"
+            "mov.b64 {klo, khi}, %6;\n\t"
+            "or.b32 klo, klo, khi;\n\t"
+            "setp.ne.s32 p, klo, 0;\n\t"
+            "setp.ne.and.s32 p, %7, 0, p;\n\t"
+            "setp.lt.and.s32 p, ahi, %3, p;\n\t"
+            HAWKES_EXP2_TAIL);
+    } else if constexpr (KILL_MODE == 5) {
+        asm("{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 alo, ahi, n, thi, ne, ad, lo, hi;\n\t"
+            "mov.b64 {alo, ahi}, %1;\n\t"
+            "mov.b64 {n, thi}, %2;\n\t"
+            "setp.gt.f64 p, %6, 0d0000000000000000;\n\t"
+            "setp.ne.and.s32 p, %7, 0, p;\n\t"
+            "setp.lt.and.s32 p, ahi, %3, p;\n\t"
+            HAWKES_EXP2_TAIL);
+    } else if constexpr (KILL_MODE == 1) {
         asm("{\n\t"
             ".reg .pred p;\n\t"
             ".reg .b32 alo, ahi, n, thi, klo, khi, ne, ad, lo, hi;\n\t"
@@ -141,7 +154,24 @@ __device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi,
             HAWKES_EXP2_TAIL);
     }
 #undef HAWKES_EXP2_TAIL
-    return T * p;
+    return T;
+}
+
+template <int KILL_MODE>
+__device__ __forceinline__ double exp2_scaled(double a, double negc, int lim_hi, double kv, const ExpC& c,
+                                              unsigned lane_base, int live = 1) {
+    // operand discipline (DESIGN.md section 5): an FP64 instruction reading three distinct vector registers
+    // issues every 3 cycles, one reading two every 2.  negc and the polynomial constants therefore sit in
+    // uniform registers, MAGIC in a vector register, and the polynomial is monic so that each Horner step has
+    // one constant: q(f) = (((f + d3) f + d2) f + d1) f + d0 = 2^f / S.
+    const double t = fma(a, negc, c.magic);
+    const double nf = t - c.magic;
+    const double f = fma(a, negc, -nf);
+    double p = f + c.d3;
+    p = fma(p, f, c.d2);
+    p = fma(p, f, c.d1);
+    p = fma(p, f, c.d0);
+    return exp2_table<KILL_MODE>(a, t, lim_hi, kv, lane_base, live) * p;
 }
 
 // fill the table (entry j, replica r at byte j*256 + r*8) with the biased bit patterns
@@ -168,7 +198,8 @@ __device__ __forceinline__ SmemPlan smem_plan(unsigned base, unsigned buf_bytes)
 // dynamic shared memory to request.  gap = distance to the boundary (< 64 KB): buffers in the gap need
 // gap + 64 KB <= 128 KB; buffers after the table (gap < buf) need gap + 64 KB + buf < 64 KB + 2 buf.
 constexpr unsigned smem_request(unsigned buf_bytes) {
-    return 2u * buf_bytes > TAB_BYTES ? TAB_BYTES + 2u * buf_bytes : 2u * TAB_BYTES;
+    return buf_bytes >= TAB_BYTES ? 2u * TAB_BYTES + buf_bytes
+                                  : (2u * buf_bytes > TAB_BYTES ? TAB_BYTES + 2u * buf_bytes : 2u * TAB_BYTES);
 }
 constexpr unsigned SMEM_MAX = 227u * 1024u;
 template <bool DIM3> constexpr unsigned group_buf_bytes() { return 2u * TS * (DIM3 ? 6 : 4) * sizeof(double); }
@@ -476,6 +507,8 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_kernel(const double* __restri
     }
 }
 
+#include "pass1_sym.cuh"
+
 // ------------------------------------------------------------------------------------------------
 // block-wide fixed-order sum of NV values per thread; result valid in threads < NV of warp 0.
 template <int NV>
@@ -517,7 +550,8 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
                                                         double* __restrict__ trec, double* __restrict__ glam,
                                                         double* __restrict__ blockpart,
                                                         unsigned* __restrict__ status, double* __restrict__ bgcache,
-                                                        int bg_mode) {
+                                                        int bg_mode, const double* __restrict__ partc, int sym_tiles,
+                                                        int sym_tile) {
     constexpr int RS = DIM3 ? 6 : 4;
     constexpr int NB = Mom<LEVEL>::NB;
     const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
@@ -550,6 +584,26 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
             for (int k = 0; k < 2 * NB; ++k) v[k] = o[(int64_t)k * ld];
 #pragma unroll
             for (int k = 0; k < NB; ++k) { b[k] += v[k]; s[k] += v[NB + k]; }
+        }
+        // symmetric pass 1: add the column partials of this event (its background pairs with later targets), one per
+        // target tile from its own tile upwards, in tile order
+        if (partc != nullptr) {
+            const int n_slots_c = sym_tiles - (int)(i / sym_tile);
+            int sc = 0;
+            for (; sc + 4 <= n_slots_c; sc += 4) {
+                double v[4][NB];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int k = 0; k < NB; ++k) v[u][k] = partc[colpart_index(sym_tiles, sym_tile, NB, sc + u, k, i)];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int k = 0; k < NB; ++k) b[k] += v[u][k];
+            }
+            for (; sc < n_slots_c; ++sc)
+#pragma unroll
+                for (int k = 0; k < NB; ++k) b[k] += partc[colpart_index(sym_tiles, sym_tile, NB, sc, k, i)];
         }
         // background-sum cache (LEVEL 0 only; the sum does not depend on theta): 1 = store, 2 = use
         if (bg_mode == 1) bgcache[i] = b[0];
@@ -1086,6 +1140,9 @@ struct hawkes_ctx {
     double* d_out;        // staging for outputs: 1 + n + 6 + n + 36 + 6n
     double* d_post;       // hawkes_posterior_z scratch: theta, grad_theta, hess_theta_diag, prior grad (n_max each) + 8
     double* d_bgcache;    // n_max: cached background sums of pass 1 (LEVEL 0)
+    double* d_partc;      // column partials of the symmetric pass 1 (NULL: symmetric path disabled)
+    size_t partc_doubles;
+    int plan_sym;
     int bg_mode;          // 0 normal, 1 store the cache, 2 use it (set by hawkes_hmc_run only)
     int plan_bg;
     double* d_hmc;        // hawkes_hmc_run scratch: z_prop, p, grad_cur, grad_prop, hess_z (n_max each) + 16
@@ -1121,10 +1178,10 @@ constexpr int P1_R = HAWKES_P1_R;   // targets per thread in pass 1
 constexpr int P2_R = HAWKES_P2_R;   // sources per thread in pass 2
 // work groups (of NT threads) per CTA, one CTA per SM: bounded by 65536 registers / (NT x registers per thread)
 #ifndef HAWKES_P1_G0
-#define HAWKES_P1_G0 4
+#define HAWKES_P1_G0 3
 #endif
 #ifndef HAWKES_P1_G1
-#define HAWKES_P1_G1 4
+#define HAWKES_P1_G1 3
 #endif
 #ifndef HAWKES_P1_G2
 #define HAWKES_P1_G2 3
@@ -1215,13 +1272,17 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     const int level2 = (want & HAWKES_WANT_HESS_THETA) ? 1 : 0;
     const int bg_mode = level1 == 0 ? ctx->bg_mode : 0;   // the cache holds the LEVEL-0 sum only
     const int no_bg = bg_mode == 2 ? 1 : 0;
-    if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2 || ctx->plan_bg != no_bg) {
+    // symmetric pass 1 (background once per unordered pair) for levels 0 and 1 unless the cached-background path runs
+    const int sym = (ctx->d_partc != nullptr && level1 <= 1 && !no_bg) ? 1 : 0;
+    if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2 || ctx->plan_bg != no_bg ||
+        ctx->plan_sym != sym) {
         Plan& q = ctx->plan;
         q.ld = round_up(n, 256);
         q.nblk = (int)((n + RED_T - 1) / RED_T);
-        q.grid1 = plan_split(&q.sp1, n, NT * P1_R, no_bg ? 0 : W_ALL[level1], W_HEAD[level1], 0,
+        q.grid1 = plan_split(&q.sp1, n, NT * P1_R, (no_bg || sym) ? 0 : W_ALL[level1], W_HEAD[level1], 0,
                              ctx->sm_count * ctx->occ1[level1], q.ld, 12, ctx->part1_doubles);
         ctx->plan_bg = no_bg;
+        ctx->plan_sym = sym;
         q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, ctx->sm_count * ctx->occ2[level2], q.ld, 2,
                              ctx->part2_doubles);
         ctx->plan_n = n; ctx->plan_l1 = level1; ctx->plan_l2 = level2;
@@ -1237,22 +1298,27 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
-            if (no_bg)
+            if (sym)
+                pass1s_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * sym_group_bytes<DIM3>(1)), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, ctx->d_partc, pl.sp1);
+            else if (no_bg)
                 pass1_kernel<P1_R, 0, DIM3, P1_G[0], false><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             else
             pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
             break;
         case 1:
+            if (sym)
+                pass1s_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * sym_group_bytes<DIM3>(3)), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, ctx->d_partc, pl.sp1);
+            else
             pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
             break;
     }
     ctx->launches += 2;
@@ -1306,6 +1372,8 @@ int query_occupancy(hawkes_ctx* ctx) {
     int rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), &ctx->occ1[0]))) return rc;
     int dummy;
+    if ((rc = setup_kernel(pass1s_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * sym_group_bytes<DIM3>(1)), &dummy))) return rc;
+    if ((rc = setup_kernel(pass1s_kernel<P1_R, 1, DIM3, P1_G[1]>, P1_G[1], smem_request(P1_G[1] * sym_group_bytes<DIM3>(3)), &dummy))) return rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 0, DIM3, P1_G[0], false>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), &dummy))) return rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 1, DIM3, P1_G[1]>, P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), &ctx->occ1[1]))) return rc;
     if ((rc = setup_kernel(pass1_kernel<P1_R, 2, DIM3, P1_G[2]>, P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), &ctx->occ1[2]))) return rc;
@@ -1362,6 +1430,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->plan_l1 = c->plan_l2 = -1;
     c->bg_mode = 0;
     c->plan_bg = -1;
+    c->plan_sym = -1;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess ||
         (dim == 3 ? query_occupancy<true>(c) : query_occupancy<false>(c)) != HAWKES_OK) {
@@ -1382,7 +1451,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_part1, (void**)&c->d_part2,
                      (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
-                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_bgcache, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
+                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
     alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
@@ -1398,6 +1467,13 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_post, sizeof(double) * (size_t)(8 + 4 * n_max));
     alloc((void**)&c->d_hmc, sizeof(double) * (size_t)(16 + 5 * n_max));
     alloc((void**)&c->d_bgcache, sizeof(double) * (size_t)n_max);
+    {   // column partials of the symmetric pass 1 (levels 0 and 1: NB <= 3); HAWKES_DENSE_PASS1=1 disables that path
+        const int nt = (int)((n_max + NT * P1_R - 1) / (NT * P1_R));
+        c->partc_doubles = (size_t)colpart_doubles(nt, NT * P1_R, 3);
+        const char* dense = getenv("HAWKES_DENSE_PASS1");
+        if ((dense && dense[0] == '1') || c->partc_doubles * sizeof(double) > ((size_t)16 << 30)) c->partc_doubles = 0;
+        if (c->partc_doubles) alloc((void**)&c->d_partc, sizeof(double) * c->partc_doubles);
+    }
     alloc((void**)&c->d_status, sizeof(unsigned) * 2);
     alloc(&c->d_cub, c->cub_bytes);
     alloc((void**)&c->d_sort_keys, sizeof(double) * (size_t)n_max);
@@ -1417,7 +1493,7 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
-                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_bgcache, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
+                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     if (c->prof_ev) {
