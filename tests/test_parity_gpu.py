@@ -9,6 +9,8 @@ import pytest
 
 import oracle
 import paper_2103_03348_b200 as hp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 from paper_2103_03348_b200 import synth
 from parity import TOL, check, hess_hyper_scale, scales
 
@@ -266,3 +268,40 @@ def test_sort_events_helper(torch):
     assert np.array_equal(to.cpu().numpy(), ev.t[perm][order])
     assert np.array_equal(xo.cpu().numpy(), ev.x[:, perm][:, order])
     assert np.array_equal(tho.cpu().numpy(), ev.theta[perm][order])
+
+
+def test_dense_pass1_kernel_agrees_with_symmetric_pass1(torch):
+    """The default pass 1 evaluates the background once per unordered pair (csrc/pass1_sym.cuh); HAWKES_DENSE_PASS1=1
+    selects the dense ordered-pair kernel (also the fallback when the column-partial buffer is not allocated).  Both
+    must give the same sums up to summation order: compared here on configs[0] (ragged last tile, stream-K cuts) and
+    a problem with ties and duplicated locations, the dense run in a subprocess so that the switch is read at create."""
+    import json
+    import subprocess
+    import sys
+    import paper_2103_03348_b200 as hp
+    code = r'''
+import json, sys
+import numpy as np, torch
+sys.path.insert(0, %r)
+import paper_2103_03348_b200 as hp
+from paper_2103_03348_b200 import synth
+out = []
+for ev in (synth.config(0), synth.small_random(700, seed=21, ties=True, duplicates=True)):
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
+    r = ctx.grad(dev(ev.x), dev(ev.t), dev(ev.theta), ev.params)
+    out.append([r.ll.item(), r.grad_theta.cpu().tolist(), r.grad_hyper.cpu().tolist()])
+print(json.dumps(out))
+''' % ROOT
+    res = {}
+    for mode in ("0", "1"):
+        env = dict(os.environ, HAWKES_DENSE_PASS1=mode)
+        p = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        assert p.returncode == 0, p.stderr
+        res[mode] = json.loads(p.stdout.strip().splitlines()[-1])
+    for sym, dense in zip(res["0"], res["1"]):
+        assert abs(sym[0] - dense[0]) <= 1e-12 * abs(dense[0])
+        gs, gd = np.array(sym[1]), np.array(dense[1])
+        assert np.max(np.abs(gs - gd)) <= 1e-11 * np.max(np.abs(gd))
+        hs, hd = np.array(sym[2]), np.array(dense[2])
+        assert np.max(np.abs(hs - hd) / np.maximum(np.abs(hd), 1e-300)) <= 1e-9
