@@ -54,6 +54,23 @@ class RefResult:
     row_d1: np.ndarray | None = None
 
 
+def background_mode(mode: str):
+    """Context manager: "ST" (default model) or "S" (paper-literal space-only background)."""
+    import contextlib
+
+    @contextlib.contextmanager
+    def cm():
+        l = lib()
+        l.hawkes_ref_set_background_mode.restype = ctypes.c_int
+        l.hawkes_ref_set_background_mode.argtypes = [ctypes.c_int]
+        old = l.hawkes_ref_set_background_mode(1 if mode == "S" else 0)
+        try:
+            yield
+        finally:
+            l.hawkes_ref_set_background_mode(old)
+    return cm()
+
+
 def evaluate(x, t, theta, params, *, grad=True, hess=False, cross=False, dense=False,
              row_d1=False, threads: int = 1) -> RefResult:
     """x: [dim, n] SoA; t: [n] sorted; theta: [n]; params: 6 floats.  Always returns ll, the

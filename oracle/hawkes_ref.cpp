@@ -47,6 +47,14 @@ typedef long double ld;
 
 const double kPi = 3.14159265358979323846264338327950288;
 
+// Background mode.  0 = "ST" (default): Gaussian-space x Gaussian-time background, the model above (DESIGN R1).
+// 1 = "S": the paper's background exactly as printed -- space only,
+//   mu(x) = mu0 tau_x^-D sum_n phi_D((x - x_n)/tau_x) I[x != x_n]
+//   with the integral term printed beside it, Lambda_background = mu0 t_N     (DESIGN R2: the print
+//   does not integrate the printed mu(x) -- N unit-mass kernels give mu0 N t_N -- and is followed as printed).
+// tau_t is then unused: every derivative with respect to it is 0.
+int g_bg_mode = 0;
+
 struct P {
     double mu0, tau_x, tau_t, xi0, h, omega;
     double norm_b, norm_k;   // (2 pi)^-(D+1)/2 tau_x^-D tau_t^-1  and  (2 pi)^-D/2 h^-D
@@ -54,7 +62,8 @@ struct P {
 
 P make_params(const double* q, int dim) {
     P p = {q[0], q[1], q[2], q[3], q[4], q[5], 0.0, 0.0};
-    p.norm_b = std::pow(2.0 * kPi, -0.5 * (dim + 1)) * std::pow(p.tau_x, -dim) / p.tau_t;
+    p.norm_b = g_bg_mode == 1 ? std::pow(2.0 * kPi, -0.5 * dim) * std::pow(p.tau_x, -dim)
+                              : std::pow(2.0 * kPi, -0.5 * (dim + 1)) * std::pow(p.tau_x, -dim) / p.tau_t;
     p.norm_k = std::pow(2.0 * kPi, -0.5 * dim) * std::pow(p.h, -dim);
     return p;
 }
@@ -87,6 +96,7 @@ inline Pair make_pair(int dim, int64_t N, const double* x, const double* t, int6
 // Background term B_{nm} (without the indicator) and excitation kernel k_{nm} (theta-free, without
 // the causal indicator), exactly as the formulas above read.
 inline double background(const P& p, double r2, double dt) {
+    if (g_bg_mode == 1) return p.mu0 * p.norm_b * std::exp(-r2 / (2.0 * p.tau_x * p.tau_x));
     return p.mu0 * p.norm_b * std::exp(-r2 / (2.0 * p.tau_x * p.tau_x) - dt * dt / (2.0 * p.tau_t * p.tau_t));
 }
 inline double excitation(const P& p, double r2, double dt) {
@@ -101,6 +111,7 @@ inline void dlog_background(const P& p, int dim, double r2, double dt, double g[
     h[0] = -1.0 / (p.mu0 * p.mu0);
     h[1] = -3.0 * r2 / (p.tau_x * p.tau_x * p.tau_x * p.tau_x) + dim / (p.tau_x * p.tau_x);
     h[2] = -3.0 * dt * dt / (p.tau_t * p.tau_t * p.tau_t * p.tau_t) + 1.0 / (p.tau_t * p.tau_t);
+    if (g_bg_mode == 1) g[2] = h[2] = 0.0;   // space-only background: no tau_t
 }
 // same for k with (xi0, h, omega);  log k = log xi0 + log omega - D log h - omega dt - r2/(2h^2) + c.
 inline void dlog_excitation(const P& p, int dim, double r2, double dt, double g[3], double h[3]) {
@@ -158,6 +169,13 @@ void compute_row(const P& p, int dim, int64_t N, const double* x, const double* 
 }  // namespace
 
 extern "C" {
+
+// 0 = ST (default), 1 = S (paper-literal space-only background); returns the previous mode.  Process-global.
+int hawkes_ref_set_background_mode(int mode) {
+    const int old = g_bg_mode;
+    g_bg_mode = mode == 1 ? 1 : 0;
+    return old;
+}
 
 // Status: 0 ok; 1 some lambda_n == 0 (ell = -inf, entries dividing by it are NaN); <0 bad argument.
 // All pointers are HOST pointers; any output may be NULL (= not wanted).
@@ -222,6 +240,7 @@ int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const 
             sThTE += (ld)theta[i] * T * E;
             sThT2E += (ld)theta[i] * T * T * E;
         }
+        if (g_bg_mode == 1) { sPhi = (ld)tN; sAphi = 0; sAphi2 = 0; }   // Lambda_background = mu0 t_N
         Lam = (ld)p.mu0 * sPhi + (ld)p.xi0 * sTh;
         L1[0] = sPhi;
         L1[2] = -(ld)p.mu0 / p.tau_t * sAphi;

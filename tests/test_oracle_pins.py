@@ -345,3 +345,65 @@ def test_generator_is_reproducible_and_has_the_configured_shape():
     assert abs(u.mean() - 0.5) < 5e-3 and abs(u.var() - 1 / 12) < 2e-3
     z = synth.normals(0, 1, 200000)
     assert abs(z.mean()) < 1e-2 and abs(z.var() - 1) < 1e-2
+
+
+# ------------------------------------------------------------------ S mode: the paper's background as printed
+def test_s_mode_two_events_closed_form_and_printed_integral():
+    """Paper-literal background: mu(x) = mu0 tau_x^-D sum phi_D((x-x_n)/tau_x) I[x != x_n], no time
+    factor, with the integral printed at l.72, mu0 t_N (DESIGN R2).  N = 2 typed out; tau_t drops out."""
+    mu0, tx, tt, xi0, h, om = 0.4, 2.5, 3.0, 0.6, 1.3, 0.45
+    x = np.array([[0.3, 1.9], [-0.4, 0.8]])
+    t = np.array([1.2, 2.9])
+    th = np.array([1.7, 0.6])
+    r2, dt = 1.6 ** 2 + 1.2 ** 2, 1.7
+    B = mu0 / (2 * math.pi * tx * tx) * math.exp(-r2 / (2 * tx * tx))
+    k = xi0 * om / (2 * math.pi * h * h) * math.exp(-om * dt - r2 / (2 * h * h))
+    Lam = mu0 * t[1] + xi0 * th[0] * (1 - math.exp(-om * dt))
+    with oracle.background_mode("S"):
+        r = oracle.evaluate(x, t, th, (mu0, tx, tt, xi0, h, om), hess=True)
+        r_tt = oracle.evaluate(x, t, th, (mu0, tx, 7.7, xi0, h, om))
+    assert abs(r.lam[0] - B) < 1e-16 and abs(r.lam[1] - (B + th[0] * k)) < 1e-16
+    assert abs(r.integral - Lam) < 1e-15
+    assert abs(r.ll - (math.log(B) + math.log(B + th[0] * k) - Lam)) < 1e-14
+    assert r.ll == r_tt.ll                                   # tau_t is not in the model
+    assert r.grad_hyper[2] == 0.0 and np.all(r.hess_hyper[2, :] == 0.0) and np.all(r.hess_hyper[:, 2] == 0.0)
+    assert abs(r.grad_theta[0] - (k / (B + th[0] * k) - xi0 * (1 - math.exp(-om * dt)))) < 1e-14
+    # and the default mode is restored
+    assert abs(oracle.evaluate(x, t, th, (mu0, tx, tt, xi0, h, om)).ll - r.ll) > 1.0
+
+
+def test_s_mode_gradient_and_hessian_by_finite_differences():
+    ev = synth.small_random(18, seed=31, regime="mixed", ties=True, duplicates=True)
+    prm = np.array(ev.params)
+    with oracle.background_mode("S"):
+        r = oracle.evaluate(ev.x, ev.t, ev.theta, prm, hess=True)
+        for a in range(6):
+            e = np.zeros(6)
+            e[a] = 1e-6 * prm[a]
+            lp = oracle.evaluate(ev.x, ev.t, ev.theta, prm + e)
+            lm = oracle.evaluate(ev.x, ev.t, ev.theta, prm - e)
+            fd = (lp.ll - lm.ll) / (2 * e[a])
+            assert abs(fd - r.grad_hyper[a]) <= 1e-7 * max(1.0, abs(r.grad_hyper[a]))
+            fdh = (lp.grad_hyper - lm.grad_hyper) / (2 * e[a])
+            assert np.max(np.abs(fdh - r.hess_hyper[a]) / np.maximum(1.0, np.abs(r.hess_hyper[a]))) <= 2e-6
+        for m in (0, 5, 17):
+            e = np.zeros(ev.n)
+            e[m] = 1e-6
+            fd = (oracle.evaluate(ev.x, ev.t, ev.theta + e, prm).ll - oracle.evaluate(ev.x, ev.t, ev.theta - e, prm).ll) / 2e-6
+            assert abs(fd - r.grad_theta[m]) <= 1e-7 * max(1.0, abs(r.grad_theta[m]))
+
+
+def test_s_mode_background_is_the_leave_one_out_kde():
+    """With xi0 -> 0 every lambda_n is mu0 N' times the leave-one-out Gaussian KDE of the other locations
+    (scikit-learn's KernelDensity, an independent library routine)."""
+    from sklearn.neighbors import KernelDensity
+    ev = synth.small_random(40, seed=33, regime="background")
+    mu0, tx = 0.7, 0.9
+    with oracle.background_mode("S"):
+        r = oracle.evaluate(ev.x, ev.t, ev.theta, (mu0, tx, 1.0, 1e-300, 0.5, 1.0))
+    X = ev.x.T
+    for n in (0, 7, 39):
+        others = np.delete(X, n, axis=0)
+        kde = KernelDensity(kernel="gaussian", bandwidth=tx).fit(others)
+        dens = math.exp(kde.score_samples(X[n:n + 1])[0])      # mean of the kernels
+        assert abs(r.lam[n] - mu0 * len(others) * dens) <= 1e-10 * r.lam[n]
