@@ -139,6 +139,15 @@ int hawkes_sort_events(hawkes_ctx* ctx, int64_t n, int dim, const double* x_in, 
                        const double* theta_in, double* x_out, double* t_out, double* theta_out,
                        int64_t* perm, void* stream);
 
+/* Background model of the context (readings R1, R2).
+ *   HAWKES_BG_SPACE_TIME (default): Gaussian-space x Gaussian-time background, the model at the top of this file.
+ *   HAWKES_BG_SPACE_ONLY: the paper's background exactly as printed -- B_{nn'} = mu0 tau_x^-D phi_D((x_n-x_n')/tau_x)
+ *     I[x_n != x_n'] with the integral term printed beside it, mu0 t_N.  tau_t is then
+ *     unused (it must still be > 0) and every derivative with respect to it is exactly 0.
+ * Applies to every later evaluation of the context.  HAWKES_ERR_ARG for another value. */
+enum { HAWKES_BG_SPACE_TIME = 0, HAWKES_BG_SPACE_ONLY = 1 };
+int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
+
 /* After an evaluation queued on this context has been enqueued: copies of the per-event rates
  * lambda_n (n doubles) into a caller buffer, on `stream`.  For tests and diagnostics. */
 int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stream);

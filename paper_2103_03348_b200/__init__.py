@@ -16,6 +16,7 @@ WARN_ZERO_RATE = 1
 WANT_LL, WANT_GRAD_THETA, WANT_GRAD_HYPER, WANT_HESS_THETA, WANT_HESS_HYPER, WANT_HESS_CROSS = 1, 2, 4, 8, 16, 32
 WANT_GRAD = WANT_LL | WANT_GRAD_THETA | WANT_GRAD_HYPER
 WANT_ALL = 63
+BG_SPACE_TIME, BG_SPACE_ONLY = 0, 1
 
 
 class HawkesError(RuntimeError):
@@ -243,6 +244,12 @@ class HawkesContext:
         if rc != 0:
             raise HawkesError(rc, "hawkes_hmc_run")
         return trace
+
+    def set_background_mode(self, mode: int):
+        """hawkes_set_background_mode: BG_SPACE_TIME (default) or BG_SPACE_ONLY (the paper's background as printed)."""
+        rc = self._lib.hawkes_set_background_mode(self._h, int(mode))
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_set_background_mode")
 
     def get_lambda(self, n: int):
         lam = self._torch.empty(n, dtype=self._torch.float64, device=self._dev)

@@ -66,6 +66,7 @@ struct DevConsts {
     int lim_b_hi;   // hi word of the smallest argument whose background exponential is flushed to 0
     int lim_s_hi;
     int dim;
+    int s_mode;     // 1: paper-literal space-only background (no time factor, Lambda_background = mu0 t_N)
 };
 
 enum { ST_UNSORTED = 1, ST_NONFINITE = 2, ST_ZERO_RATE = 4 };
@@ -635,6 +636,7 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
             d1[3] = SS / c.xi0;
             d1[4] = SSr2 / (h * h * h) - D * SS / h;
             d1[5] = SS / om - SSd;
+            if (c.s_mode) d1[2] = 0.0;   // space-only background: lambda does not depend on tau_t
 #pragma unroll
             for (int p = 0; p < 6; ++p) v[1 + p] = d1[p] * iL;
             if (glam != nullptr) {
@@ -655,6 +657,7 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
                 d2[1][1] = SBr4 / (tx2 * tx2 * tx2) - (2.0 * D + 3.0) * SBr2 / (tx2 * tx2) + D * (D + 1.0) * SB / tx2;
                 d2[2][2] = SBd4 / (tt2 * tt2 * tt2) - 5.0 * SBd2 / (tt2 * tt2) + 2.0 * SB / tt2;
                 d2[1][2] = SBr2d2 / (tx2 * tx * tt2 * tt) - SBr2 / (tx2 * tx * tt) - D * SBd2 / (tx * tt2 * tt) + D * SB / (tx * tt);
+                if (c.s_mode) { d2[0][2] = 0.0; d2[1][2] = 0.0; d2[2][2] = 0.0; }
                 d2[3][4] = d1[4] / c.xi0;
                 d2[3][5] = d1[5] / c.xi0;
                 d2[4][4] = SSr4 / (h2 * h2 * h2) - (2.0 * D + 3.0) * SSr2 / (h2 * h2) + D * (D + 1.0) * SS / h2;
@@ -678,6 +681,11 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
         v[28] = norm_cdf(a) - norm_cdf(bb);
         v[29] = a * pa - bb * pb;
         v[30] = a * pa * (2.0 - a * a) - bb * pb * (2.0 - bb * bb);
+        if (c.s_mode) {   // Lambda_background = mu0 t_N as printed: the last event carries t_N, no tau_t terms
+            v[28] = (i == n - 1) ? tN : 0.0;
+            v[29] = 0.0;
+            v[30] = 0.0;
+        }
         const double E = exp(-c.omega * T);
         v[31] = e.w * (-expm1(-c.omega * T));
         v[32] = e.w * T * E;
@@ -1144,6 +1152,7 @@ struct hawkes_ctx {
     size_t partc_doubles;
     int plan_sym;
     int bg_mode;          // 0 normal, 1 store the cache, 2 use it (set by hawkes_hmc_run only)
+    int s_mode;           // hawkes_set_background_mode
     int plan_bg;
     double* d_hmc;        // hawkes_hmc_run scratch: z_prop, p, grad_cur, grad_prop, hess_z (n_max each) + 16
     unsigned* d_status;
@@ -1234,7 +1243,7 @@ size_t part_bound(int64_t n_max, int ctas_max, int tile, int n_mom) {
     return (size_t)n_mom * ((size_t)2 * ctas_max * tile + 4 * (size_t)round_up(n_max, 256));
 }
 
-int make_consts(const hawkes_params* p, int dim, DevConsts* c) {
+int make_consts(const hawkes_params* p, int dim, int s_mode, DevConsts* c) {
     const double v[6] = {p->mu0, p->tau_x, p->tau_t, p->xi0, p->h, p->omega};
     for (int i = 0; i < 6; ++i)
         if (!(v[i] > 0.0) || !std::isfinite(v[i])) return HAWKES_ERR_PARAM;
@@ -1247,6 +1256,11 @@ int make_consts(const hawkes_params* p, int dim, DevConsts* c) {
     c->negcs = (double)(-cs);
     c->rho_s = (double)(2.0L * p->h * p->h * p->omega);
     c->CB = (double)((long double)p->mu0 * powl(two_pi, -0.5L * (dim + 1)) * powl(p->tau_x, -dim) / p->tau_t);
+    c->s_mode = s_mode ? 1 : 0;
+    if (s_mode) {   // PAPER.md:60 as printed: mu0 tau_x^-D phi_D(.), no time factor
+        c->rho_b = 0.0;
+        c->CB = (double)((long double)p->mu0 * powl(two_pi, -0.5L * dim) * powl(p->tau_x, -dim));
+    }
     c->CS = (double)((long double)p->xi0 * p->omega * powl(two_pi, -0.5L * dim) * powl(p->h, -dim));
     c->mu0 = p->mu0; c->tau_x = p->tau_x; c->tau_t = p->tau_t; c->xi0 = p->xi0; c->h = p->h; c->omega = p->omega;
     c->CBS = (double)((long double)c->CB * (long double)HAWKES_EXP2_S);
@@ -1429,6 +1443,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->plan_n = -1;
     c->plan_l1 = c->plan_l2 = -1;
     c->bg_mode = 0;
+    c->s_mode = 0;
     c->plan_bg = -1;
     c->plan_sym = -1;
     cudaDeviceProp prop;
@@ -1525,7 +1540,7 @@ int hawkes_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, co
         ((want & HAWKES_WANT_HESS_HYPER) && !hess_hyper) || ((want & HAWKES_WANT_HESS_CROSS) && !hess_cross))
         return HAWKES_ERR_ARG;
     DevConsts c;
-    rc = make_consts(p, ctx->dim, &c);
+    rc = make_consts(p, ctx->dim, ctx->s_mode, &c);
     if (rc) return rc;
     CK(cudaSetDevice(ctx->device));
     if (ctx->dim == 3)
@@ -1601,7 +1616,7 @@ int hawkes_hessian_theta_dense(hawkes_ctx* ctx, int64_t n, const double* x, cons
     rc = hawkes_eval(ctx, n, x, t, theta, p, HAWKES_WANT_LL, ctx->d_scal + 4, nullptr, nullptr, nullptr, nullptr, nullptr, stream);
     if (rc) return rc;
     DevConsts c;
-    make_consts(p, ctx->dim, &c);
+    make_consts(p, ctx->dim, ctx->s_mode, &c);
     const dim3 blk(16, 16), grd((unsigned)((n + 15) / 16), (unsigned)((n + 15) / 16));
     if (ctx->dim == 3) dense_kernel<true><<<grd, blk, 0, (cudaStream_t)stream>>>(ctx->d_rec, ctx->d_trec, n, c, hess_theta);
     else dense_kernel<false><<<grd, blk, 0, (cudaStream_t)stream>>>(ctx->d_rec, ctx->d_trec, n, c, hess_theta);
@@ -1745,6 +1760,12 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         ctx->launches++;
     }
     CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+int hawkes_set_background_mode(hawkes_ctx* ctx, int mode) {
+    if (!ctx || (mode != HAWKES_BG_SPACE_TIME && mode != HAWKES_BG_SPACE_ONLY)) return HAWKES_ERR_ARG;
+    ctx->s_mode = mode == HAWKES_BG_SPACE_ONLY ? 1 : 0;
     return HAWKES_OK;
 }
 

@@ -305,3 +305,31 @@ print(json.dumps(out))
         assert np.max(np.abs(gs - gd)) <= 1e-11 * np.max(np.abs(gd))
         hs, hd = np.array(sym[2]), np.array(dense[2])
         assert np.max(np.abs(hs - hd) / np.maximum(np.abs(hd), 1e-300)) <= 1e-9
+
+
+@pytest.mark.parametrize("n,seed,dim", [(3, 41, 2), (300, 42, 2), (777, 43, 3), (1000, 44, 2)])
+def test_space_only_background_mode(torch, n, seed, dim):
+    """hawkes_set_background_mode(HAWKES_BG_SPACE_ONLY): the paper's background as printed against the
+    oracle in the same mode; every output, ties and duplicated locations included; d/dtau_t exactly 0; the default
+    mode comes back unchanged."""
+    ev = synth.small_random(n, seed, dim=dim, regime="mixed", ties=True, duplicates=True)
+    if n > 64:
+        ev.x *= math.sqrt(n / 16.0)
+        ev.t *= n / 40.0
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    r_st, st0, lam_st, _ = run_gpu(torch, ev, ctx=ctx)
+    ctx.set_background_mode(hp.BG_SPACE_ONLY)
+    with oracle.background_mode("S"):
+        ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev, ctx=ctx)
+    assert st == ref.status == 0
+    compare_all(ev, r, lam, ref)
+    assert r.grad_hyper.cpu().numpy()[2] == 0.0
+    H = r.hess_hyper.cpu().numpy()
+    assert np.all(H[2, :] == 0.0) and np.all(H[:, 2] == 0.0)
+    assert np.all(r.hess_cross.cpu().numpy()[:, 2] == 0.0)
+    ctx.set_background_mode(hp.BG_SPACE_TIME)
+    r_back, _, lam_back, _ = run_gpu(torch, ev, ctx=ctx)
+    assert np.array_equal(lam_back, lam_st) and r_back.ll.item() == r_st.ll.item()
+    with pytest.raises(hp.HawkesError):
+        ctx.set_background_mode(7)
