@@ -515,7 +515,7 @@ def run_hmc(args) -> dict:
     res_var = {}
     sampler = ClockSampler(0).start()
     launches = 0
-    for name, cache in (("recompute_all_pairs", False), ("cached_background", True)):
+    for name, cache in (("recompute_all_pairs", 0), ("cached_background", 1), ("cached_kernel_matrix", 2)):
         z, mass = to(z0.copy()), to(np.ones(M))
         nrm = to(synth.normals(args.seed, 500, (W + K) * M).reshape(W + K, M))
         uni = to(synth.uniforms(args.seed, 501, W + K))
@@ -537,7 +537,7 @@ def run_hmc(args) -> dict:
                          "log_posterior_last": float(tr_h[-1, 0]), "gpu_launches": int(launches),
                          "evals_per_s_implied": (K * L + K // every + 1) / (e1.elapsed_time(e2) * 1e-3)}
     clocks = sampler.stop()
-    best = res_var["cached_background"]
+    best = res_var["cached_background"]   # headline: exact, pair terms recomputed; the kernel-matrix variant is listed
     return {"metric": "hmc_seconds_per_iteration", "value": best["seconds_per_iteration"], "unit": "s/iteration",
             "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": best["seconds_per_iteration"] * 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",

@@ -258,8 +258,15 @@ typedef struct {
     int32_t n_refresh_done;  /* refreshes already averaged into `mass` (0 for a fresh chain) */
     double step;             /* eps > 0 */
     double mass_floor;       /* > 0 */
-    int32_t cache_background; /* 1: evaluate the theta-independent background sums of pass 1 once per call and reuse
-                                 them in every later evaluation (same values; pass 1 then visits causal pairs only) */
+    int32_t cache_background; /* 0: every evaluation recomputes every pair (the paper's method).
+                                 1: the theta-independent background sums of pass 1 are evaluated once per call and
+                                    reused (same values; pass 1 then visits causal pairs only).
+                                 2: cached kernel matrix: K[n][k] = k-term of (event n, sequenced event k) / (xi0-free
+                                    constant), N x M doubles built once per call (allocated by the context on first use
+                                    and kept: the one entry point that may allocate), plus lambda0 = everything that does
+                                    not involve a sequenced rate; an evaluation is then two passes over K (row sums ->
+                                    lambda, column sums -> d ell/d theta): HBM-bound instead of FP64-bound.  Same sums in
+                                    another order.  dim <= 2 only (HAWKES_ERR_UNSUPPORTED otherwise). */
     int32_t reserved;
 } hawkes_hmc_opts;
 

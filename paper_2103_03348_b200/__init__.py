@@ -226,7 +226,7 @@ class HawkesContext:
 
     def hmc_run(self, tree: "HawkesTree", x, t, idx, z, beta: float, params, sigma2: float, tau0: float, *, n_iter: int,
                 n_leapfrog: int, step: float, precond_every: int, mass, mass_floor: float, normals, uniforms,
-                n_refresh_done: int = 0, cache_background: bool = False, prior_prec=None, trace=None):
+                n_refresh_done: int = 0, cache_background: int = 0, prior_prec=None, trace=None):
         """hawkes_hmc_run: z [m] and mass [m] are updated in place (device tensors); normals [n_iter, m] and
         uniforms [n_iter] are device tensors; returns the trace [n_iter, 4] (device)."""
         torch = self._torch
@@ -236,7 +236,7 @@ class HawkesContext:
         if trace is None:
             trace = torch.empty(n_iter, 4, dtype=torch.float64, device=self._dev)
         o = HmcOpts(int(n_iter), int(n_leapfrog), int(precond_every), int(n_refresh_done), float(step),
-                    float(mass_floor), 1 if cache_background else 0, 0)
+                    float(mass_floor), int(cache_background), 0)
         p = _params(params)
         rc = self._lib.hawkes_hmc_run(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
                                       ctypes.byref(p), float(sigma2), float(tau0), ctypes.byref(o), _ptr(normals),

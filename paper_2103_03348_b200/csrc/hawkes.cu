@@ -591,14 +591,14 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
         if (partc != nullptr) {
             const int n_slots_c = sym_tiles - (int)(i / sym_tile);
             int sc = 0;
-            for (; sc + 4 <= n_slots_c; sc += 4) {
-                double v[4][NB];
+            for (; sc + 8 <= n_slots_c; sc += 8) {   // eight slots' loads in flight, adds in slot order
+                double v[8][NB];
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
+                for (int u = 0; u < 8; ++u)
 #pragma unroll
                     for (int k = 0; k < NB; ++k) v[u][k] = partc[colpart_index(sym_tiles, sym_tile, NB, sc + u, k, i)];
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
+                for (int u = 0; u < 8; ++u)
 #pragma unroll
                     for (int k = 0; k < NB; ++k) b[k] += v[u][k];
             }
@@ -1091,6 +1091,8 @@ __global__ void hmc_mass_kernel(int64_t m, const double* __restrict__ hess_z, do
     mass[i] = mi + (h - mi) * inv_k;
 }
 
+#include "hmc_kmat.cuh"
+
 // DFMA-chain microbenchmark: 8 independent chains per thread, `iters` x 8 x 8 FMAs.
 __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, double* out) {
     double a[8];
@@ -1154,6 +1156,10 @@ struct hawkes_ctx {
     int bg_mode;          // 0 normal, 1 store the cache, 2 use it (set by hawkes_hmc_run only)
     int s_mode;           // hawkes_set_background_mode
     int plan_bg;
+    double* d_kmat;       // cached kernel matrix of hawkes_hmc_run (allocated on first use, kept)
+    size_t kmat_doubles;
+    double* d_kmisc;      // its vectors and partials
+    size_t kmisc_doubles;
     double* d_hmc;        // hawkes_hmc_run scratch: z_prop, p, grad_cur, grad_prop, hess_z (n_max each) + 16
     unsigned* d_status;
     void* d_cub;          // temp storage for the sort
@@ -1444,6 +1450,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->plan_l1 = c->plan_l2 = -1;
     c->bg_mode = 0;
     c->s_mode = 0;
+    c->kmat_doubles = c->kmisc_doubles = 0;
     c->plan_bg = -1;
     c->plan_sym = -1;
     cudaDeviceProp prop;
@@ -1466,7 +1473,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_part1, (void**)&c->d_part2,
                      (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
-                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
+                     (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_kmat, (void**)&c->d_kmisc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
     alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
@@ -1508,7 +1515,7 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
-                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
+                    c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     if (c->prof_ev) {
@@ -1714,7 +1721,8 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
                    const double* prior_prec, double* trace, void* stream) {
     if (!ctx || !tree || !x || !t || !idx || !z || !p || !o || !normals || !uniforms || !mass) return HAWKES_ERR_ARG;
     if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
-    if (o->n_iter < 1 || o->n_leapfrog < 1 || o->precond_every < 0 || o->n_refresh_done < 0) return HAWKES_ERR_ARG;
+    if (o->n_iter < 1 || o->n_leapfrog < 1 || o->precond_every < 0 || o->n_refresh_done < 0 ||
+        o->cache_background < 0 || o->cache_background > 2) return HAWKES_ERR_ARG;
     if (!(o->step > 0.0) || !std::isfinite(o->step) || !(o->mass_floor > 0.0) || !std::isfinite(o->mass_floor))
         return HAWKES_ERR_PARAM;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1728,16 +1736,84 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     double* hz = gp + ctx->n_max;
     const double eps = o->step;
     const unsigned mb = (unsigned)((m + 255) / 256);
-    // the first evaluation fills the background cache, every later one (all at LEVEL 0) uses it
-    ctx->bg_mode = o->cache_background ? 1 : 0;
-    int rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, z, beta, p, sigma2, tau0, o3c, gc, nullptr, stream);
-    ctx->bg_mode = o->cache_background ? 2 : 0;
     struct Reset { hawkes_ctx* c; ~Reset() { c->bg_mode = 0; } } reset{ctx};
+    int rc;
+    // ---- cache_background == 2: cached kernel matrix (csrc/hmc_kmat.cuh) -------------------------------------
+    const bool kmat = o->cache_background == 2;
+    double *thM = nullptr, *kw = nullptr, *lam0 = nullptr, *logpart = nullptr, *cpart = nullptr, *intpart = nullptr,
+           *lam0_int = nullptr, *lp = nullptr, *pg = nullptr;
+    int nblk_r = 0, nblk_c = 0, nblk_f = 0, rows_per = 0;
+    DevConsts kc;
+    if (kmat) {
+        if (ctx->dim == 3) return HAWKES_ERR_UNSUPPORTED;
+        if ((size_t)m * sizeof(double) > 200 * 1024) return HAWKES_ERR_UNSUPPORTED;
+        rc = make_consts(p, ctx->dim, ctx->s_mode, &kc);
+        if (rc) return rc;
+        CK(cudaSetDevice(ctx->device));
+        nblk_r = (int)((n + KM_ROWS_T / 32 - 1) / (KM_ROWS_T / 32));
+        nblk_c = (int)(n < 4 * ctx->sm_count ? n : 4 * ctx->sm_count);
+        rows_per = (int)((n + nblk_c - 1) / nblk_c);
+        nblk_c = (int)((n + rows_per - 1) / rows_per);
+        nblk_f = (int)((m + 255) / 256);
+        const size_t need_k = (size_t)n * (size_t)m;
+        const size_t need_misc = (size_t)2 * m + 2 * (size_t)n + nblk_r + (size_t)2 * nblk_c * m + nblk_f + 8;
+        if (need_k > ctx->kmat_doubles) {          // first use (or a larger problem): the matrix is kept by the context
+            if (ctx->d_kmat) cudaFree(ctx->d_kmat);
+            ctx->d_kmat = nullptr; ctx->kmat_doubles = 0;
+            if (cudaMalloc((void**)&ctx->d_kmat, need_k * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+            ctx->kmat_doubles = need_k;
+        }
+        if (need_misc > ctx->kmisc_doubles) {
+            if (ctx->d_kmisc) cudaFree(ctx->d_kmisc);
+            ctx->d_kmisc = nullptr; ctx->kmisc_doubles = 0;
+            if (cudaMalloc((void**)&ctx->d_kmisc, need_misc * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+            ctx->kmisc_doubles = need_misc;
+        }
+        thM = ctx->d_kmisc; pg = thM + m; kw = pg + m; lam0 = kw + n; logpart = lam0 + n; cpart = logpart + nblk_r;
+        intpart = cpart + (size_t)2 * nblk_c * m; lam0_int = intpart + nblk_f; lp = lam0_int + 2;
+        CK(cudaFuncSetAttribute(kmat_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(m * sizeof(double))));
+        // lambda0 and Lambda0: one ordinary evaluation with the sequenced rates set to 0
+        double* th0 = ctx->d_post + 8;
+        fill_ones_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, th0);
+        kmat_zero_scatter_kernel<<<mb, 256, 0, st>>>(m, idx, th0);
+        ctx->launches += 2;
+        rc = hawkes_eval(ctx, n, x, t, th0, p, HAWKES_WANT_LL, ctx->d_post, nullptr, nullptr, nullptr, nullptr, nullptr, stream);
+        if (rc) return rc;
+        CK(cudaMemcpyAsync(lam0, ctx->d_lam, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemcpyAsync(lam0_int, ctx->d_scal + 1, sizeof(double), cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemsetAsync(ctx->d_status, 0, sizeof(unsigned), st));   // lambda0 = 0 is no zero rate of the model
+        const int64_t total = n * m;
+        kmat_build_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(ctx->d_rec, n, m, idx, kc.omega,
+                                                                          1.0 / (2.0 * kc.h * kc.h), ctx->d_kmat);
+        ctx->launches++;
+    }
+    auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess) -> int {
+        if (!kmat) return hawkes_posterior_z(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream);
+        kmat_theta_kernel<<<mb, 256, 0, st>>>(m, idx, zin, beta, t, thM);
+        kmat_rows_kernel<<<nblk_r, KM_ROWS_T, m * sizeof(double), st>>>(ctx->d_kmat, n, m, thM, lam0, kc.CS, kw, logpart,
+                                                                        ctx->d_status);
+        int r2 = hawkes_tree_prior(tree, zin, sigma2, tau0, lp, grad ? pg : nullptr, stream);
+        if (r2) return r2;
+        if (cudaSetDevice(ctx->device) != cudaSuccess) return HAWKES_ERR_CUDA;
+        kmat_cols_kernel<<<nblk_c, KM_COLS_T, 0, st>>>(ctx->d_kmat, n, m, kw, rows_per, hess ? 1 : 0, cpart);
+        kmat_finish_kernel<<<nblk_f, 256, 0, st>>>(m, nblk_c, cpart, hess ? 1 : 0, idx, t, n, thM, kc.CS, kc.xi0, kc.omega,
+                                                   grad ? pg : nullptr, grad, hess, intpart);
+        ctx->launches += 4;
+        if (out3) {
+            kmat_scalar_kernel<<<1, 32, 0, st>>>(nblk_r, logpart, nblk_f, intpart, lam0_int, kc.xi0, lp, out3);
+            ctx->launches++;
+        }
+        return HAWKES_OK;
+    };
+    // cache_background == 1: the first evaluation fills the background cache, every later one (all at LEVEL 0) uses it
+    ctx->bg_mode = o->cache_background == 1 ? 1 : 0;
+    rc = eval_post(z, o3c, gc, nullptr);
+    ctx->bg_mode = o->cache_background == 1 ? 2 : 0;
     if (rc) return rc;
     int n_refresh = o->n_refresh_done;
     for (int it = 0; it < o->n_iter; ++it) {
         if (o->precond_every > 0 && it % o->precond_every == 0) {
-            rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, z, beta, p, sigma2, tau0, nullptr, nullptr, hz, stream);
+            rc = eval_post(z, nullptr, nullptr, hz);
             if (rc) return rc;
             ++n_refresh;
             CK(cudaSetDevice(ctx->device));
@@ -1748,7 +1824,7 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, prior_prec, normals + (int64_t)it * m, eps, zp, pm, hs);
         ctx->launches++;
         for (int s = 0; s < o->n_leapfrog; ++s) {
-            rc = hawkes_posterior_z(ctx, tree, n, x, t, m, idx, zp, beta, p, sigma2, tau0, o3p, gp, nullptr, stream);
+            rc = eval_post(zp, o3p, gp, nullptr);
             if (rc) return rc;
             if (s + 1 < o->n_leapfrog) {
                 hmc_leap_kernel<<<mb, 256, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm);

@@ -24,7 +24,7 @@ def dev(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
 
 
-@pytest.mark.parametrize("cache_bg,with_prior_prec", [(False, False), (True, False), (True, True)])
+@pytest.mark.parametrize("cache_bg,with_prior_prec", [(0, False), (1, False), (1, True), (2, False), (2, True)])
 def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     """1,500 events, 90 sequenced; 6 iterations x 5 leapfrog steps, preconditioner refreshed every 3 iterations.
     Tolerance: the state after 30 leapfrog steps inherits the 1e-10 bar of the gradient through a mildly expanding
