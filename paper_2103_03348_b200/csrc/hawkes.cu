@@ -1159,6 +1159,9 @@ struct hawkes_ctx {
     double* d_kmat;       // cached kernel matrix of hawkes_hmc_run (allocated on first use, kept)
     size_t kmat_doubles;
     double* d_kmisc;      // its vectors and partials
+    cudaStream_t side;    // the tree prior runs here beside the passes over K (created on first use)
+    cudaEvent_t ev_fork, ev_join;
+    bool side_ready;
     size_t kmisc_doubles;
     double* d_hmc;        // hawkes_hmc_run scratch: z_prop, p, grad_cur, grad_prop, hess_z (n_max each) + 16
     unsigned* d_status;
@@ -1451,6 +1454,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->bg_mode = 0;
     c->s_mode = 0;
     c->kmat_doubles = c->kmisc_doubles = 0;
+    c->side_ready = false;
     c->plan_bg = -1;
     c->plan_sym = -1;
     cudaDeviceProp prop;
@@ -1518,6 +1522,11 @@ void hawkes_destroy(hawkes_ctx* c) {
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
+    if (c->side_ready) {
+        cudaEventDestroy(c->ev_fork);
+        cudaEventDestroy(c->ev_join);
+        cudaStreamDestroy(c->side);
+    }
     if (c->prof_ev) {
         for (int i = 0; i < PROF_RING * 6; ++i) cudaEventDestroy(c->prof_ev[i]);
         delete[] c->prof_ev;
@@ -1751,10 +1760,9 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         if (rc) return rc;
         CK(cudaSetDevice(ctx->device));
         nblk_r = (int)((n + KM_ROWS_T / 32 - 1) / (KM_ROWS_T / 32));
-        nblk_c = (int)(n < 4 * ctx->sm_count ? n : 4 * ctx->sm_count);
-        rows_per = (int)((n + nblk_c - 1) / nblk_c);
+        rows_per = 64;                                         // rows per CTA of the column pass
         nblk_c = (int)((n + rows_per - 1) / rows_per);
-        nblk_f = (int)((m + 255) / 256);
+        nblk_f = (int)((m + 7) / 8);                           // finish: one warp per column, 8 per CTA
         const size_t need_k = (size_t)n * (size_t)m;
         const size_t need_misc = (size_t)2 * m + 2 * (size_t)n + nblk_r + (size_t)2 * nblk_c * m + nblk_f + 8;
         if (need_k > ctx->kmat_doubles) {          // first use (or a larger problem): the matrix is kept by the context
@@ -1772,6 +1780,12 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         thM = ctx->d_kmisc; pg = thM + m; kw = pg + m; lam0 = kw + n; logpart = lam0 + n; cpart = logpart + nblk_r;
         intpart = cpart + (size_t)2 * nblk_c * m; lam0_int = intpart + nblk_f; lp = lam0_int + 2;
         CK(cudaFuncSetAttribute(kmat_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(m * sizeof(double))));
+        if (!ctx->side_ready) {
+            CK(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
+            CK(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
+            ctx->side_ready = true;
+        }
         // lambda0 and Lambda0: one ordinary evaluation with the sequenced rates set to 0
         double* th0 = ctx->d_post + 8;
         fill_ones_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, th0);
@@ -1789,13 +1803,19 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     }
     auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess) -> int {
         if (!kmat) return hawkes_posterior_z(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream);
+        // the O(M) tree prior (one latency-bound CTA) runs on a side stream beside the two passes over K
+        if (cudaEventRecord(ctx->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0) != cudaSuccess)
+            return HAWKES_ERR_CUDA;
+        int r2 = hawkes_tree_prior(tree, zin, sigma2, tau0, lp, grad ? pg : nullptr, (void*)ctx->side);
+        if (r2) return r2;
+        if (cudaSetDevice(ctx->device) != cudaSuccess || cudaEventRecord(ctx->ev_join, ctx->side) != cudaSuccess)
+            return HAWKES_ERR_CUDA;
         kmat_theta_kernel<<<mb, 256, 0, st>>>(m, idx, zin, beta, t, thM);
         kmat_rows_kernel<<<nblk_r, KM_ROWS_T, m * sizeof(double), st>>>(ctx->d_kmat, n, m, thM, lam0, kc.CS, kw, logpart,
                                                                         ctx->d_status);
-        int r2 = hawkes_tree_prior(tree, zin, sigma2, tau0, lp, grad ? pg : nullptr, stream);
-        if (r2) return r2;
-        if (cudaSetDevice(ctx->device) != cudaSuccess) return HAWKES_ERR_CUDA;
-        kmat_cols_kernel<<<nblk_c, KM_COLS_T, 0, st>>>(ctx->d_kmat, n, m, kw, rows_per, hess ? 1 : 0, cpart);
+        kmat_cols_kernel<<<dim3((unsigned)((m + KM_COL_TILE - 1) / KM_COL_TILE), (unsigned)nblk_c), KM_COL_TILE, 0, st>>>(
+            ctx->d_kmat, n, m, kw, rows_per, hess ? 1 : 0, cpart);
+        if (cudaStreamWaitEvent(st, ctx->ev_join, 0) != cudaSuccess) return HAWKES_ERR_CUDA;
         kmat_finish_kernel<<<nblk_f, 256, 0, st>>>(m, nblk_c, cpart, hess ? 1 : 0, idx, t, n, thM, kc.CS, kc.xi0, kc.omega,
                                                    grad ? pg : nullptr, grad, hess, intpart);
         ctx->launches += 4;

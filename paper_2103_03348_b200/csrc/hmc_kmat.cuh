@@ -12,7 +12,6 @@
 // reported as a separate variant.  All sums in fixed order.
 
 constexpr int KM_ROWS_T = 256;      // kmat_rows_kernel: 8 warps = 8 rows per CTA
-constexpr int KM_COLS_T = 1024;     // kmat_cols_kernel threads
 
 __global__ void kmat_build_kernel(const double* __restrict__ rec, int64_t n, int64_t m, const int64_t* __restrict__ idx,
                                   double omega, double inv_2h2, double* __restrict__ K) {
@@ -66,53 +65,71 @@ __global__ void __launch_bounds__(KM_ROWS_T) kmat_rows_kernel(const double* __re
     }
 }
 
-// columns: CTA b owns rows [b rows_per, (b+1) rows_per); thread owns columns t, t + 1024, ...: partial[b][k] (c) and
-// partial[nblk + b][k] (d, when want_d)
-__global__ void __launch_bounds__(KM_COLS_T) kmat_cols_kernel(const double* __restrict__ K, int64_t n, int64_t m,
-                                                              const double* __restrict__ w, int rows_per, int want_d,
-                                                              double* __restrict__ part) {
-    const int64_t r0 = (int64_t)blockIdx.x * rows_per, r1 = min(r0 + rows_per, n);
-    for (int64_t k = threadIdx.x; k < m; k += KM_COLS_T) {
-        double c = 0.0, d = 0.0;
-        for (int64_t i = r0; i < r1; ++i) {
-            const double q = K[i * m + k] * w[i];
-            c += q;
-            d = fma(q, q, d);
+// columns: CTA (bx, by) owns columns [256 bx, 256 bx + 256) and rows [by rows_per, (by+1) rows_per); one column per
+// thread, rows in order (eight loads in flight): partial[by][k] (c) and partial[nby + by][k] (d, when want_d)
+constexpr int KM_COL_TILE = 256;
+__global__ void __launch_bounds__(KM_COL_TILE) kmat_cols_kernel(const double* __restrict__ K, int64_t n, int64_t m,
+                                                                const double* __restrict__ w, int rows_per, int want_d,
+                                                                double* __restrict__ part) {
+    const int64_t k = (int64_t)blockIdx.x * KM_COL_TILE + threadIdx.x;
+    const int64_t r0 = (int64_t)blockIdx.y * rows_per, r1 = min(r0 + rows_per, n);
+    if (k >= m) return;
+    double c = 0.0, d = 0.0;
+    int64_t i = r0;
+    for (; i + 8 <= r1; i += 8) {
+        double q[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) q[u] = K[(i + u) * m + k];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const double v = q[u] * w[i + u];
+            c += v;
+            d = fma(v, v, d);
         }
-        part[(int64_t)blockIdx.x * m + k] = c;
-        if (want_d) part[((int64_t)gridDim.x + blockIdx.x) * m + k] = d;
     }
+    for (; i < r1; ++i) {
+        const double v = K[i * m + k] * w[i];
+        c += v;
+        d = fma(v, v, d);
+    }
+    part[(int64_t)blockIdx.y * m + k] = c;
+    if (want_d) part[((int64_t)gridDim.y + blockIdx.y) * m + k] = d;
 }
 
-// finish: c_k, d_k in CTA order; d ell/d theta_k = CS c_k - xi0 (1 - E_k); chain rule to z; log-likelihood and out3
-__global__ void kmat_finish_kernel(int64_t m, int nblk_c, const double* __restrict__ part, int want_d,
+// finish: one warp per column adds the row-block partials (lane l takes blocks l, l + 32, ... in order, then a fixed
+// shuffle tree); d ell/d theta_k = CS c_k - xi0 (1 - E_k); chain rule to z; CTA partial of sum_k theta_k (1 - E_k)
+__global__ void __launch_bounds__(256) kmat_finish_kernel(int64_t m, int nblk_c, const double* __restrict__ part, int want_d,
                                    const int64_t* __restrict__ idx, const double* __restrict__ t, int64_t n,
                                    const double* __restrict__ thM, double CS, double xi0, double omega,
                                    const double* __restrict__ prior_grad, double* __restrict__ grad_z,
                                    double* __restrict__ hess_z, double* __restrict__ intpart) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     __shared__ double sm[8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * 8 + wid;
     double ti = 0.0;
-    const double tN = t[n - 1];
     if (k < m) {
         double c = 0.0, d = 0.0;
-        for (int b = 0; b < nblk_c; ++b) c += part[(int64_t)b * m + k];
+        for (int b = lane; b < nblk_c; b += 32) c += part[(int64_t)b * m + k];
         if (want_d)
-            for (int b = 0; b < nblk_c; ++b) d += part[((int64_t)nblk_c + b) * m + k];
-        const double th = thM[k], one_minus_E = -expm1(-omega * (tN - t[idx[k]]));
-        const double g = th * (CS * c - xi0 * one_minus_E);
-        if (grad_z) grad_z[k] = prior_grad ? g + prior_grad[k] : g;
-        if (hess_z) hess_z[k] = fma(th * th, -(CS * CS) * d, g);
-        ti = th * one_minus_E;
-    }
-    // CTA partial of sum_k theta_k (1 - E_k) (256 threads)
+            for (int b = lane; b < nblk_c; b += 32) d += part[((int64_t)nblk_c + b) * m + k];
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) ti += __shfl_down_sync(0xffffffffu, ti, off);
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = ti;
+        for (int off = 16; off > 0; off >>= 1) {
+            c += __shfl_down_sync(0xffffffffu, c, off);
+            d += __shfl_down_sync(0xffffffffu, d, off);
+        }
+        if (lane == 0) {
+            const double th = thM[k], one_minus_E = -expm1(-omega * (t[n - 1] - t[idx[k]]));
+            const double g = th * (CS * c - xi0 * one_minus_E);
+            if (grad_z) grad_z[k] = prior_grad ? g + prior_grad[k] : g;
+            if (hess_z) hess_z[k] = fma(th * th, -(CS * CS) * d, g);
+            ti = th * one_minus_E;
+        }
+    }
+    if (lane == 0) sm[wid] = ti;
     __syncthreads();
     if (threadIdx.x == 0) {
         double a = 0.0;
-        for (int q = 0; q < (int)(blockDim.x >> 5); ++q) a += sm[q];
+        for (int q = 0; q < 8; ++q) a += sm[q];
         intpart[blockIdx.x] = a;
     }
 }
