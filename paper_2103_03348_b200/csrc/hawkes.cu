@@ -1159,7 +1159,7 @@ struct hawkes_ctx {
     double* d_kmat;       // cached kernel matrix of hawkes_hmc_run (allocated on first use, kept)
     size_t kmat_doubles;
     double* d_kmisc;      // its vectors and partials
-    cudaStream_t side;    // the tree prior runs here beside the passes over K (created on first use)
+    cudaStream_t side;    // small single-CTA kernels (scalars, tree prior) run here beside the big passes
     cudaEvent_t ev_fork, ev_join;
     bool side_ready;
     size_t kmisc_doubles;
@@ -1345,10 +1345,20 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             break;
     }
     ctx->launches += 2;
-    if (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) {
-        scalars_kernel<<<1, SCAL_T, 0, st>>>(ctx->d_blockpart, pl.nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
+    // the single-CTA scalar reduction runs on the side stream beside pass 2 when there is one (joined at the end)
+    const bool want_scal = (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) != 0;
+    const bool scal_aside = want_scal && (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) != 0;
+    if (want_scal) {
+        cudaStream_t ss = st;
+        if (scal_aside) {
+            CK(cudaEventRecord(ctx->ev_fork, st));
+            CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+            ss = ctx->side;
+        }
+        scalars_kernel<<<1, SCAL_T, 0, ss>>>(ctx->d_blockpart, pl.nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
                                          (want & HAWKES_WANT_GRAD_HYPER) ? grad_hyper : nullptr,
                                          (want & HAWKES_WANT_HESS_HYPER) ? hess_hyper : nullptr, ctx->d_scal);
+        if (scal_aside) CK(cudaEventRecord(ctx->ev_join, ctx->side));
         ctx->launches++;
     }
     if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
@@ -1371,6 +1381,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         cross_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, ctx->d_trec, ctx->d_glam, n, c, hess_cross);
         ctx->launches++;
     }
+    if (scal_aside) CK(cudaStreamWaitEvent(st, ctx->ev_join, 0));
     if (pe) {
         CK(cudaEventRecord(pe[5], st));
         ctx->prof_count++;
@@ -1511,6 +1522,14 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
         cudaGetLastError();
         return HAWKES_ERR_NOMEM;
     }
+    if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        hawkes_destroy(c);
+        cudaGetLastError();
+        return HAWKES_ERR_CUDA;
+    }
+    c->side_ready = true;
     *out = c;
     return HAWKES_OK;
 }
@@ -1780,12 +1799,7 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         thM = ctx->d_kmisc; pg = thM + m; kw = pg + m; lam0 = kw + n; logpart = lam0 + n; cpart = logpart + nblk_r;
         intpart = cpart + (size_t)2 * nblk_c * m; lam0_int = intpart + nblk_f; lp = lam0_int + 2;
         CK(cudaFuncSetAttribute(kmat_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(m * sizeof(double))));
-        if (!ctx->side_ready) {
-            CK(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
-            CK(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
-            CK(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
-            ctx->side_ready = true;
-        }
+
         // lambda0 and Lambda0: one ordinary evaluation with the sequenced rates set to 0
         double* th0 = ctx->d_post + 8;
         fill_ones_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, th0);
