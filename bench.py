@@ -184,11 +184,16 @@ def cpu_baseline(ev, budget_s: float = 15.0) -> dict:
     idx = sample_idx(ev.n, int(budget_s / max(per_row, 1e-9)))
     secs = oracle_sample_seconds(ev, idx, threads)
     evals_per_s = (len(idx) / ev.n) / secs
+    # the same oracle on ONE thread, on a smaller sample (about 3 s)
+    idx1 = sample_idx(ev.n, max(8, int(3.0 / max(per_row * threads, 1e-9))))
+    secs1 = oracle_sample_seconds(ev, idx1, 1)
     return {"value": evals_per_s, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": f"{len(idx)} of {ev.n} target rows (lambda_n + 6 hyper-derivatives) and the same {len(idx)} "
                       f"source columns (c_m), evenly strided, {secs:.1f} s on {threads} OpenMP threads; "
                       f"evals/s = (rows/N) / seconds",
-            "seconds_per_eval_extrapolated": 1.0 / evals_per_s}
+            "seconds_per_eval_extrapolated": 1.0 / evals_per_s,
+            "single_thread": {"seconds_per_eval_extrapolated": secs1 * ev.n / len(idx1), "cores": 1,
+                              "sample": f"{len(idx1)} of {ev.n} rows and columns, {secs1:.1f} s"}}
 
 
 def run_reference(args, ev, workload: str) -> dict:
@@ -394,8 +399,16 @@ def run_b200(args, ev, workload: str) -> dict:
         lstep = lambda: ctx.eval(x, t, th, ev.params, hp.WANT_LL | hp.WANT_GRAD_THETA, out=out)
         timed(lstep, 2)
         lms = timed(lstep, max(3, K // 4))
+        # same events at the paper's posterior scales (Table 2: tau_x = 194 km, h = 7.37 km, 1/omega = 29.8 d),
+        # where no exponential underflows: the kernels are dense, so the time must not depend on the regime
+        from paper_2103_03348_b200 import synth as _synth
+        t2step = lambda: ctx.grad(x, t, th, _synth.TABLE2_PARAMS, out=out)
+        timed(t2step, 2)
+        t2ms = timed(t2step, max(3, K // 4))
+        timed(step, 1)   # leave `out` holding the configs[1] result
         res["extras"] = {"hessian_ms": statistics.median(hms), "ll_grad_theta_only_ms": statistics.median(lms),
-                         "step_ms_min": min(ms), "step_ms_median": statistics.median(ms)}
+                         "step_ms_min": min(ms), "step_ms_median": statistics.median(ms),
+                         "table2_scales_step_ms": statistics.median(t2ms)}
     if world == 1 and not args.no_cpu_baseline:
         res["cpu_baseline"] = cpu_baseline(ev, args.cpu_budget)
     if dist is not None:
