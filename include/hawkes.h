@@ -139,6 +139,16 @@ int hawkes_sort_events(hawkes_ctx* ctx, int64_t n, int dim, const double* x_in, 
                        const double* theta_in, double* x_out, double* t_out, double* theta_out,
                        int64_t* perm, void* stream);
 
+/* Dense theta-theta Hessian block of the sequenced events: for the m events idx[0..m),
+ *   hess_block[k*m + k'] = d2 ell / d theta_idx[k] d theta_idx[k'] = - sum_n k_{n idx[k]} k_{n idx[k']} / lambda_n^2
+ * (Lambda is linear in theta; the diagonal is Eq. 5), row-major m x m doubles, symmetric, DEVICE.
+ * idx: DEVICE int64 [m].  Uses an n x m scratch matrix that the context allocates on first use and keeps (shared
+ * with hawkes_hmc_run's kernel matrix): this call may allocate.  dim <= 2 (HAWKES_ERR_UNSUPPORTED otherwise).  Not a
+ * hot-path call: a plain tiled fp64 contraction. */
+int hawkes_hessian_theta_block(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                               const hawkes_params* p /*HOST*/, int64_t m, const int64_t* idx, double* hess_block,
+                               void* stream);
+
 /* Background model of the context (readings R1, R2).
  *   HAWKES_BG_SPACE_TIME (default): Gaussian-space x Gaussian-time background, the model at the top of this file.
  *   HAWKES_BG_SPACE_ONLY: the paper's background exactly as printed -- B_{nn'} = mu0 tau_x^-D phi_D((x_n-x_n')/tau_x)

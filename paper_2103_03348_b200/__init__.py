@@ -172,6 +172,18 @@ class HawkesContext:
             raise HawkesError(rc, "hawkes_hessian_theta_dense")
         return H
 
+    def hessian_theta_block(self, x, t, theta, params, idx):
+        """hawkes_hessian_theta_block: the dense m x m Hessian of ell in the rates of the events idx (device tensor)."""
+        n = self._check_inputs(x, t, theta)
+        m = int(idx.shape[0])
+        H = self._torch.empty(m, m, dtype=self._torch.float64, device=self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_hessian_theta_block(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), m, _ptr(idx),
+                                                  _ptr(H), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_hessian_theta_block")
+        return H
+
     def sort_events(self, x, t, theta):
         """Stable sort by time on the device; returns (x_sorted, t_sorted, theta_sorted, perm)."""
         torch = self._torch

@@ -39,6 +39,7 @@ SYMBOLS = {
     "hawkes_sort_events": (cint, [vp, i64, cint, _dp, _dp, _dp, _dp, _dp, _dp, vp, vp]),
     "hawkes_get_lambda": (cint, [vp, i64, _dp, vp]),
     "hawkes_set_background_mode": (cint, [vp, cint]),
+    "hawkes_hessian_theta_block": (cint, [vp, i64, _dp, _dp, _dp, PP, i64, vp, _dp, vp]),
     "hawkes_launch_count": (i64, [vp]),
     "hawkes_profile_enable": (cint, [vp, cint]),
     "hawkes_profile_read": (cint, [vp, ctypes.POINTER(ctypes.c_double)]),

@@ -1873,6 +1873,38 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     return HAWKES_OK;
 }
 
+int hawkes_hessian_theta_block(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                               const hawkes_params* p, int64_t m, const int64_t* idx, double* hess_block, void* stream) {
+    int rc = check_common(ctx, n, x, t, theta, p);
+    if (rc) return rc;
+    if (!idx || !hess_block || m < 1 || m > n) return HAWKES_ERR_ARG;
+    if (ctx->dim == 3) return HAWKES_ERR_UNSUPPORTED;
+    DevConsts c;
+    rc = make_consts(p, ctx->dim, ctx->s_mode, &c);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t need = (size_t)n * (size_t)m;
+    if (need > ctx->kmat_doubles) {   // shares the kernel-matrix buffer of hawkes_hmc_run (allocated on first use, kept)
+        if (ctx->d_kmat) cudaFree(ctx->d_kmat);
+        ctx->d_kmat = nullptr; ctx->kmat_doubles = 0;
+        if (cudaMalloc((void**)&ctx->d_kmat, need * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+        ctx->kmat_doubles = need;
+    }
+    // lambda_n (and the packed records) from a log-likelihood-level evaluation
+    rc = hawkes_eval(ctx, n, x, t, theta, p, HAWKES_WANT_LL, ctx->d_scal + 4, nullptr, nullptr, nullptr, nullptr, nullptr, stream);
+    if (rc) return rc;
+    const int64_t total = n * m;
+    kmat_build_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(ctx->d_rec, n, m, idx, c.omega, 1.0 / (2.0 * c.h * c.h),
+                                                                      ctx->d_kmat);
+    kmat_scale_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(n, m, c.CS, ctx->d_lam, ctx->d_kmat);
+    const unsigned nt = (unsigned)((m + HB_TILE - 1) / HB_TILE);
+    hess_block_kernel<<<dim3(nt, nt), 256, 0, st>>>(ctx->d_kmat, n, m, hess_block);
+    ctx->launches += 3;
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
 int hawkes_set_background_mode(hawkes_ctx* ctx, int mode) {
     if (!ctx || (mode != HAWKES_BG_SPACE_TIME && mode != HAWKES_BG_SPACE_ONLY)) return HAWKES_ERR_ARG;
     ctx->s_mode = mode == HAWKES_BG_SPACE_ONLY ? 1 : 0;

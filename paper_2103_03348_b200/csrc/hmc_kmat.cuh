@@ -161,3 +161,59 @@ __global__ void kmat_zero_scatter_kernel(int64_t m, const int64_t* __restrict__ 
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k < m) theta[idx[k]] = 0.0;
 }
+
+// ------------------------------------------------------------------------------------------------
+// Dense Hessian block of the sequenced rates (hawkes_hessian_theta_block): A[n][k] = CS K[n][k] / lambda_n, then
+// H = -A^T A, M x M.  A contraction over n, written as a plain tiled fp64 kernel (64 x 64 output tile per CTA, 4 x 4
+// per thread, 16 rows of A per shared-memory stage); only tiles on or above the diagonal are computed, the mirror
+// image is written with them.  Not on the hot path; untuned.
+__global__ void kmat_scale_rows_kernel(int64_t n, int64_t m, double CS, const double* __restrict__ lam,
+                                       double* __restrict__ A) {
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n * m) return;
+    A[e] = CS * A[e] / lam[e / m];
+}
+
+constexpr int HB_TILE = 64, HB_ROWS = 16;
+__global__ void __launch_bounds__(256) hess_block_kernel(const double* __restrict__ A, int64_t n, int64_t m,
+                                                         double* __restrict__ H) {
+    if (blockIdx.x < blockIdx.y) return;                      // tiles on or above the diagonal only
+    __shared__ double sa[HB_ROWS][HB_TILE], sb[HB_ROWS][HB_TILE];
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    const int64_t k0 = (int64_t)blockIdx.y * HB_TILE, l0 = (int64_t)blockIdx.x * HB_TILE;
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    for (int64_t r0 = 0; r0 < n; r0 += HB_ROWS) {
+        for (int q = threadIdx.x; q < HB_ROWS * HB_TILE; q += 256) {
+            const int rr = q / HB_TILE, cc = q % HB_TILE;
+            const int64_t r = r0 + rr;
+            sa[rr][cc] = (r < n && k0 + cc < m) ? A[r * m + k0 + cc] : 0.0;
+            sb[rr][cc] = (r < n && l0 + cc < m) ? A[r * m + l0 + cc] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int rr = 0; rr < HB_ROWS; ++rr) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { a[i] = sa[rr][ty * 4 + i]; b[i] = sb[rr][tx * 4 + i]; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int64_t k = k0 + ty * 4 + i, l = l0 + tx * 4 + j;
+            if (k < m && l < m) {
+                H[k * m + l] = -acc[i][j];
+                H[l * m + k] = -acc[i][j];
+            }
+        }
+}

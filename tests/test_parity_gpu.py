@@ -333,3 +333,31 @@ def test_space_only_background_mode(torch, n, seed, dim):
     assert np.array_equal(lam_back, lam_st) and r_back.ll.item() == r_st.ll.item()
     with pytest.raises(hp.HawkesError):
         ctx.set_background_mode(7)
+
+
+def test_hessian_theta_block_of_sequenced_events(torch, cfg1_ref):
+    """hawkes_hessian_theta_block: the m x m block -sum_n k_nm k_nm' / lambda_n^2 against the oracle's dense N x N
+    Hessian restricted to idx (configs[0]), and at configs[1] size (N = 23,422, m = 1,610) its diagonal against
+    Eq. 5 as the pairwise kernels compute it, plus symmetry and negative semi-definiteness on a probe vector."""
+    ev = synth.config(0)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, dense=True, threads=THREADS)
+    idx = np.unique(np.concatenate([ev.free_idx, np.arange(0, ev.n, 37)])).astype(np.int64)
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    x, t, th = dev(torch, ev)
+    H = ctx.hessian_theta_block(x, t, th, ev.params, torch.from_numpy(idx).to("cuda")).cpu().numpy()
+    O = ref.hess_theta_dense[np.ix_(idx, idx)]
+    d = np.sqrt(np.abs(np.diag(O)))
+    check("hess_theta_block", H, O, np.outer(d, d), floor=1e-280)
+    assert np.array_equal(H, H.T)
+    ev1, ref1 = cfg1_ref
+    ctx1 = hp.HawkesContext(ev1.n, ev1.dim)
+    x1, t1, th1 = dev(torch, ev1)
+    idx1 = torch.from_numpy(ev1.free_idx).to("cuda")
+    H1 = ctx1.hessian_theta_block(x1, t1, th1, ev1.params, idx1)
+    r1 = ctx1.eval(x1, t1, th1, ev1.params, hp.WANT_HESS_THETA)
+    dg = torch.diagonal(H1).cpu().numpy()
+    check("diag(hess_theta_block)", dg, ref1.hess_theta_diag[ev1.free_idx], floor=1e-280)
+    check("diag vs pairwise", dg, r1.hess_theta_diag.cpu().numpy()[ev1.free_idx], floor=1e-280)
+    assert torch.equal(H1, H1.T)
+    v = torch.from_numpy(synth.normals(5, 900, H1.shape[0])).to("cuda")
+    assert float(v @ H1 @ v) <= 0.0
