@@ -361,3 +361,20 @@ def test_hessian_theta_block_of_sequenced_events(torch, cfg1_ref):
     assert torch.equal(H1, H1.T)
     v = torch.from_numpy(synth.normals(5, 900, H1.shape[0])).to("cuda")
     assert float(v @ H1 @ v) <= 0.0
+
+
+@pytest.mark.parametrize("n", [1, 31, 32, 33, 127, 128, 255, 256, 511, 512, 513, 769, 1024, 1281])
+def test_sizes_around_tile_and_block_boundaries(torch, n):
+    """Sizes on either side of the 32-event rotation block, the 128-event streamed tile and the 256-event target tile
+    (ragged blocks, ragged tiles, exactly-full tiles), with ties and duplicated locations: ll, gradient, Hessians."""
+    ev = synth.small_random(n, seed=100 + n, dim=2, regime="mixed", ties=n >= 4, duplicates=n >= 4)
+    if n > 64:
+        ev.x *= math.sqrt(n / 16.0)
+        ev.t *= n / 40.0
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev)
+    assert st == ref.status
+    if ref.status == 0:
+        compare_all(ev, r, lam, ref)
+    else:                                   # n = 1: the only event has no source, lambda = 0 (pin P1)
+        assert lam[0] == 0.0 and r.ll.item() == -math.inf
