@@ -350,10 +350,10 @@ def run_b200(args, ev, workload: str) -> dict:
     a1 = pass1_flops(n) / (p1_ms * 1e-3) / 1e12
     a2 = pass2_flops(n) / (p2_ms * 1e-3) / 1e12
     # FP64-pipe instructions as the kernels issue them (SASS count): symmetric pass 1 34 per unordered
-    # pair (background 21 incl. both sets of sums, excitation 13), pass 2 15 per causal pair
+    # pair (background 21 incl. both sets of sums, excitation 13), pass 2 13 per causal pair (factorised time decay)
     a1x = pass1_flops_executed(n) / (p1_ms * 1e-3) / 1e12
     p1_instr = 0.5 * n * (n - 1) * P1_SYM_INSTR
-    p2_instr = 0.5 * n * (n - 1) * 15
+    p2_instr = 0.5 * n * (n - 1) * 13
     instr_peak = props.multi_processor_count * FP64_LANES_PER_SM * sm_max * 1e6
     res = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,

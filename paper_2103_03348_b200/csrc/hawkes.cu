@@ -214,9 +214,15 @@ __device__ __forceinline__ void group_sync(int grp) {
 // (x0, x1, x2, t, theta, 0) for dim 3.
 __global__ void prep_kernel(int64_t n, int dim, const double* __restrict__ x, const double* __restrict__ t,
                             const double* __restrict__ theta, double* __restrict__ rec,
-                            unsigned* __restrict__ status) {
+                            unsigned* __restrict__ status, double omega) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    // status[1]: some streamed tile of TS events spans more than 600 / omega in time: pass 2 then keeps the unfactorised
+    // form of the excitation exponential (see pass2_kernel)
+    if (i % TS == 0) {
+        const int64_t last = min(i + TS - 1, n - 1);
+        if (!(omega * (t[last] - t[i]) <= 600.0)) atomicOr(status + 1, 1u);
+    }
     const double ti = t[i], th = theta[i];
     unsigned bad = 0;
     if (i > 0 && ti < t[i - 1]) bad |= ST_UNSORTED;
@@ -548,7 +554,8 @@ template <int LEVEL, bool DIM3>
 __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                         DevConsts c, const double* __restrict__ part,
                                                         Split sp, double* __restrict__ lam,
-                                                        double* __restrict__ trec, double* __restrict__ glam,
+                                                        double* __restrict__ trec, double* __restrict__ trec2,
+                                                        double* __restrict__ glam,
                                                         double* __restrict__ blockpart,
                                                         unsigned* __restrict__ status, double* __restrict__ bgcache,
                                                         int bg_mode, const double* __restrict__ partc, int sym_tiles,
@@ -624,6 +631,20 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
             o2[0] = make_double2(e.x, e.y);
             o2[1] = make_double2(e.z, e.t);
             o2[2] = make_double2(iL, 0.0);
+        }
+        // second target stream for the factorised pass 2: weight W_n = e^{-omega (t_n - t_ref)} / lambda_n, t_ref = time of
+        // the first event of the TS-aligned streamed tile that holds n
+        {
+            const double tref = rec[(i / TS) * TS * RS + (DIM3 ? 3 : 2)];
+            const double W = iL * exp(-c.omega * (e.t - tref));
+            if (!DIM3) {
+                reinterpret_cast<double4*>(trec2)[i] = make_double4(e.x, e.y, e.t, W);
+            } else {
+                double2* o2 = reinterpret_cast<double2*>(trec2) + 3 * i;
+                o2[0] = make_double2(e.x, e.y);
+                o2[1] = make_double2(e.z, e.t);
+                o2[2] = make_double2(W, 0.0);
+            }
         }
         v[0] = log(L);
         double d1[6] = {0, 0, 0, 0, 0, 0};
@@ -767,12 +788,42 @@ __device__ __forceinline__ void p2_tile(const double* __restrict__ sbuf, int cnt
     }
 }
 
+// Factorised form for pieces whose every pair is causal: e^{-omega (t_n - t_m)} = e^{-omega (t_n - t_ref)} e^{-omega (t_ref - t_m)},
+// t_ref = first time of the streamed tile.  The first factor sits in the streamed weight W_n (reduce1), the second
+// depends on the source only and multiplies the piece's sums once per piece: the per-pair work loses the time
+// difference and the exponent assembly (13 FP64 instructions instead of 15).  Both factors are <= 1 for such pieces,
+// so an underflow of G W_n can only hide a term that is itself below 1e-308.
+template <int R, int LEVEL, bool DIM3>
+__device__ __forceinline__ void p2_tile_fact(const double* __restrict__ sbuf, int cnt, const Ev<DIM3> (&g)[R],
+                                             double (&pc)[R], double (&pd)[R], const P1C& c, unsigned lane_base) {
+    constexpr int RS = DIM3 ? 6 : 4;
+#pragma unroll UNROLL_J
+    for (int j = 0; j < cnt; ++j) {
+        const Ev<DIM3> s = read_rec<DIM3>(sbuf + j * RS);   // a target; s.w = W_n
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const double dx = s.x - g[r].x, dy = s.y - g[r].y;
+            double u = fma(dy, dy, dx * dx);
+            if (DIM3) { const double dz = s.z - g[r].z; u = fma(dz, dz, u); }
+            const double e = exp2_scaled<0>(u, c.negcs, c.lim_s_hi, 0.0, c.e, lane_base);
+            if (LEVEL == 0) {
+                pc[r] = fma(e, s.w, pc[r]);
+            } else {
+                const double q = e * s.w;
+                pc[r] += q;
+                pd[r] = fma(q, q, pd[r]);
+            }
+        }
+    }
+}
+
 // a4: G work groups per CTA as in pass 1 (decomposition: see Split above, `tri` form -- the streamed
 // targets of source tile M are those with index >= the tile's first source).
 // part2[(slot*2 + k)*ld + m], k = 0 (c), 1 (d).
 template <int R, int LEVEL, bool DIM3, int G>
 __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
-                                                          int64_t n, int64_t ld, DevConsts c,
+                                                          const double* __restrict__ trec2,
+                                                          const unsigned* __restrict__ status, int64_t n, int64_t ld, DevConsts c,
                                                           const double* __restrict__ tab_g, double* __restrict__ part2,
                                                           Split sp) {
     constexpr int RS = DIM3 ? 6 : 4;
@@ -797,7 +848,8 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
     const int64_t lo = vcta * sp.chunk;
     if (lo >= total) return;
     const int64_t hi = min(lo + sp.chunk, total);
-    const P1C pc = pinned_consts(smagic, c);
+    const P1C pc_ = pinned_consts(smagic, c);
+    const bool fact = status[1] == 0;   // warp-uniform: set by prep_kernel for the whole evaluation
 
     for (int M = split_tile_of(sp, lo); M < sp.n_tiles; ++M) {
         const int64_t base = split_prefix(sp, M);
@@ -819,12 +871,15 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
         }
         const double t_last = rec[(m1 - 1) * RS + TOFF];   // latest own source time
 
+        // a piece is "plain" when every pair in it is causal (all targets after the tile, no tie across the boundary);
+        // plain pieces take the factorised form unless a streamed tile spans too much time (status[1], prep_kernel)
+        auto is_plain = [&](int64_t a_) { return a_ >= m1 && trec[a_ * RS + TOFF] > t_last; };
         RecIO<DIM3> io;
         int64_t a = jb;
         int64_t b = min(je, (a / TS + 1) * TS);
         group_sync(grp);
         if (a < je) {
-            io.load(trec, a, (int)(b - a), tid);
+            io.load((fact && is_plain(a)) ? trec2 : trec, a, (int)(b - a), tid);
             io.store(sbuf0, tid);
         }
         group_sync(grp);
@@ -832,12 +887,26 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
         while (a < je) {
             const int cnt = (int)(b - a);
             const int64_t a2 = b, b2 = min(je, b + TS);
-            if (a2 < je) io.load(trec, a2, (int)(b2 - a2), tid);
+            if (a2 < je) io.load((fact && is_plain(a2)) ? trec2 : trec, a2, (int)(b2 - a2), tid);
             const double* sb = cur ? sbuf1 : sbuf0;
-            if (a >= m1 && trec[a * RS + TOFF] > t_last) {
-                p2_tile<R, LEVEL, false, DIM3>(sb, cnt, g, cm, dm, pc, lane_base);
+            if (is_plain(a)) {
+                if (fact) {
+                    double pc[R], pd[R];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) { pc[r] = 0.0; pd[r] = 0.0; }
+                    p2_tile_fact<R, LEVEL, DIM3>(sb, cnt, g, pc, pd, pc_, lane_base);
+                    const double tref = trec[(a / TS) * TS * RS + TOFF];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double F = exp(-c.omega * (tref - g[r].t));
+                        cm[r] = fma(F, pc[r], cm[r]);
+                        if (LEVEL >= 1) dm[r] = fma(F * F, pd[r], dm[r]);
+                    }
+                } else {
+                    p2_tile<R, LEVEL, false, DIM3>(sb, cnt, g, cm, dm, pc_, lane_base);
+                }
             } else {
-                p2_tile<R, LEVEL, true, DIM3>(sb, cnt, g, cm, dm, pc, lane_base);
+                p2_tile<R, LEVEL, true, DIM3>(sb, cnt, g, cm, dm, pc_, lane_base);
             }
             if (a2 < je) io.store(cur ? sbuf0 : sbuf1, tid);
             group_sync(grp);
@@ -1133,6 +1202,7 @@ struct hawkes_ctx {
     double* d_tab;        // 128 doubles
     double* d_rec;        // n_max * RS
     double* d_trec;       // n_max * RS
+    double* d_trec2;      // n_max * RS: same records with the factorised pass-2 weight
     double* d_part1;      // pass-1 partials
     size_t part1_doubles;
     double* d_part2;      // pass-2 partials
@@ -1312,9 +1382,9 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     }
     const Plan& pl = ctx->plan;
     cudaEvent_t* pe = ctx->prof_on ? ctx->prof_ev + 6 * (ctx->prof_count % PROF_RING) : nullptr;
-    CK(cudaMemsetAsync(ctx->d_status, 0, sizeof(unsigned), st));
+    CK(cudaMemsetAsync(ctx->d_status, 0, 2 * sizeof(unsigned), st));
     if (pe) CK(cudaEventRecord(pe[0], st));
-    prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status);
+    prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status, c.omega);
     ctx->launches++;
     const unsigned g1 = (unsigned)((pl.grid1 + P1_G[level1] - 1) / P1_G[level1]);
     double* glam = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_glam : nullptr;
@@ -1328,7 +1398,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
             break;
         case 1:
             if (sym)
@@ -1336,12 +1406,12 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
             break;
     }
     ctx->launches += 2;
@@ -1365,9 +1435,9 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         const unsigned g2 = (unsigned)((pl.grid2 + P2_G[level2] - 1) / P2_G[level2]);
         if (pe) CK(cudaEventRecord(pe[3], st));
         if (want & HAWKES_WANT_HESS_THETA)
-            pass2_kernel<P2_R, 1, DIM3, P2_G[1]><<<g2, NT * P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
+            pass2_kernel<P2_R, 1, DIM3, P2_G[1]><<<g2, NT * P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, ctx->d_trec, ctx->d_trec2, ctx->d_status, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
         else
-            pass2_kernel<P2_R, 0, DIM3, P2_G[0]><<<g2, NT * P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, ctx->d_trec, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
+            pass2_kernel<P2_R, 0, DIM3, P2_G[0]><<<g2, NT * P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, ctx->d_trec, ctx->d_trec2, ctx->d_status, n, pl.ld, c, ctx->d_tab, ctx->d_part2, pl.sp2);
         if (pe) CK(cudaEventRecord(pe[4], st));
         theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.sp2,
                                                       (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
@@ -1486,13 +1556,14 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
                                     (const int64_t*)nullptr, (int64_t*)nullptr, (int)n_max);
     bool ok = true;
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
-    void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_part1, (void**)&c->d_part2,
+    void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_trec2, (void**)&c->d_part1, (void**)&c->d_part2,
                      (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
                      (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_kmat, (void**)&c->d_kmisc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
     alloc((void**)&c->d_rec, sizeof(double) * RS * (size_t)c->ld_max);
     alloc((void**)&c->d_trec, sizeof(double) * RS * (size_t)c->ld_max);
+    alloc((void**)&c->d_trec2, sizeof(double) * RS * (size_t)c->ld_max);
     alloc((void**)&c->d_part1, sizeof(double) * c->part1_doubles);
     alloc((void**)&c->d_part2, sizeof(double) * c->part2_doubles);
     alloc((void**)&c->d_lam, sizeof(double) * (size_t)c->ld_max);
@@ -1537,7 +1608,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
 void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
-    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
+    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);

@@ -378,3 +378,22 @@ def test_sizes_around_tile_and_block_boundaries(torch, n):
         compare_all(ev, r, lam, ref)
     else:                                   # n = 1: the only event has no source, lambda = 0 (pin P1)
         assert lam[0] == 0.0 and r.ll.item() == -math.inf
+
+
+@pytest.mark.parametrize("scale", [1.0, 60.0])
+def test_pass2_factorised_and_unfactorised_time_decay(torch, scale):
+    """Pass 2 splits e^{-omega dt} into a per-target and a per-source factor on pieces whose every pair is causal, unless
+    a streamed tile of 128 events spans more than 600/omega in time (then it keeps the unfactorised exponent).  Both
+    branches against the oracle: 1,500 events over a few decay times (factorised) and the same events with the time
+    axis stretched 60-fold (a 128-event tile then spans ~1,900 time units > 600/omega = 857: unfactorised), with a
+    background time bandwidth long enough to keep every rate positive."""
+    ev = synth.small_random(1500, seed=77, dim=2, regime="excite", ties=True, duplicates=True)
+    ev.x *= 6.0
+    ev.t *= 1500 / 40.0 * scale
+    if scale > 1.0:
+        mu0, tx, tt, xi0, h, om = ev.params
+        ev.params = (mu0, tx, 1.0e5, xi0, h, om)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev)
+    assert st == ref.status == 0
+    compare_all(ev, r, lam, ref)
