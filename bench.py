@@ -409,7 +409,39 @@ def run_b200(args, ev, workload: str) -> dict:
         res["extras"] = {"hessian_ms": statistics.median(hms), "ll_grad_theta_only_ms": statistics.median(lms),
                          "step_ms_min": min(ms), "step_ms_median": statistics.median(ms),
                          "table2_scales_step_ms": statistics.median(t2ms)}
+    # the O(N) kernels (prep, reduce1, theta) against the measured HBM copy peak: bytes they move per evaluation
+    # (records in and out, row-partial slots, column partials: about N^2 * 12 / tile of them), time from the ring
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            hbm_peak = float(json.load(fh)["hbm_gbs"])
+    except Exception:
+        hbm_peak = 6537.3   # SURVEY.md 8(d) fallback
+    tile, w1, w2 = 256, 3 * props.multi_processor_count, 4 * props.multi_processor_count
+    n_tiles = (n + tile - 1) // tile
+    on_bytes = (n * 64.0                                                      # prep: SoA in, records out
+                + (n + w1 * tile) * 6 * 8.0 + 0.5 * n * n_tiles * 3 * 8.0     # reduce1: row slots + column partials
+                + n * (32 + 32 + 8 + 34 * 8 / 64.0)                           #          two record streams, lambda, block sums
+                + (n + w2 * tile) * 8.0 + n * 16.0)                           # theta: pass-2 slots in, gradient out
+    on_ms = (prof["prep_ms"] + prof["mid_ms"] + prof["tail_ms"]) / max(prof["evals"], 1)
+    res["o_n_kernels"] = {"ms_with_launch_gaps": on_ms, "bytes_per_eval_estimate": on_bytes,
+                          "achieved_gb_s": on_bytes / (on_ms * 1e-3) / 1e9, "hbm_peak_gb_s": hbm_peak,
+                          "frac": on_bytes / (on_ms * 1e-3) / 1e9 / hbm_peak,
+                          "note": "launch-latency-bound by nature; the data they touch is L2-resident"}
     if world == 1 and not args.no_cpu_baseline:
+        # parity on a sample, in this very run: 256 rows of lambda_n and 256 columns of c_m against the oracle
+        import oracle
+        sidx = sample_idx(n, 256)
+        lam_gpu = ctx.get_lambda(n).cpu().numpy()
+        lam_ref, _ = oracle.rows(ev.x, ev.t, ev.theta, ev.params, sidx, derivs=False, threads=oracle.max_threads())
+        c_ref, _ = oracle.cols(ev.x, ev.t, ev.params, lam_gpu, sidx, threads=oracle.max_threads())
+        xi0, om = ev.params[3], ev.params[5]
+        integ = xi0 * (-np.expm1(-om * (ev.t[-1] - ev.t[sidx])))
+        g_gpu = out.grad_theta.cpu().numpy()[sidx]
+        res["parity_sample"] = {
+            "rows": int(len(sidx)),
+            "max_rel_err_lambda": float(np.max(np.abs(lam_gpu[sidx] - lam_ref) / lam_ref)),
+            "max_scaled_err_grad_theta": float(np.max(np.abs(g_gpu - (c_ref - integ)) / (np.abs(c_ref) + integ + 1e-300))),
+            "tolerance": 1e-10}
         res["cpu_baseline"] = cpu_baseline(ev, args.cpu_budget)
     if dist is not None:
         dist.destroy_process_group()
