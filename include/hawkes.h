@@ -158,6 +158,35 @@ int hawkes_hessian_theta_block(hawkes_ctx* ctx, int64_t n, const double* x, cons
 enum { HAWKES_BG_SPACE_TIME = 0, HAWKES_BG_SPACE_ONLY = 1 };
 int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
 
+/* ---- Exact-zero skipping: a separately reported variant of the evaluation ---------------------
+ * A term of Eq. 1 or Eq. 4 is exp(-z) with z = |dx|^2/(2 tau_x^2) + dt^2/(2 tau_t^2)
+ * (background) or z = |dx|^2/(2 h^2) + omega dt (self-excitation); in IEEE double arithmetic it is exactly +0.0 once
+ * z > 745.14.  hawkes_skip_plan orders the events along a space-time Morton curve, boxes every run of 128 of them and
+ * lists the (target tile, source run) pairs whose smallest possible z is below 746 (for the self-excitation: that
+ * also hold a causal pair); hawkes_eval_skip then runs the two pairwise passes over those lists only.  Nothing but
+ * exact zeros is left out, so each output differs from hawkes_eval's by summation order alone (same tolerance).
+ *
+ * hawkes_skip_plan: x (dim x n, coordinate-major) and t (n) are HOST or DEVICE pointers; the events may be in any
+ *   order (time-sorted input is not required by this variant).  Synchronous: copies the events to the host, builds
+ *   the plan there (O(n log n) + one box test per tile pair) and uploads it; the context owns it until the next
+ *   hawkes_skip_plan or hawkes_destroy.  The plan depends on the events, the hyperparameters and the background mode
+ *   -- not on theta -- so one plan serves every evaluation of an HMC trajectory.
+ *   Errors: HAWKES_ERR_ARG, HAWKES_ERR_PARAM, HAWKES_ERR_NONFINITE (events), HAWKES_ERR_NOMEM, HAWKES_ERR_CUDA,
+ *   HAWKES_ERR_UNSUPPORTED (work lists do not fit the context's partial buffers).
+ * hawkes_eval_skip: arguments, outputs (in the caller's event order), stream semantics and device status as
+ *   hawkes_eval, without the cross block (`want` bits 0..4).  HAWKES_ERR_ARG if there is no plan or it was built
+ *   for another n, other hyperparameters or another background mode; the caller guarantees x and t are the planned
+ *   events.  HAWKES_ERR_UNSORTED is never raised here.
+ * hawkes_skip_stats: out[0..6] = pass-1 items with a live background, with a live self-excitation, of the dense
+ *   pass; pass-2 items, of the dense pass; workers of pass 1, of pass 2 (item = 256 records x 128 records).
+ * hawkes_skip_perm: the curve order (record i is the caller's event perm[i]) into a HOST buffer of n int64. */
+int hawkes_skip_plan(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p);
+int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                     const hawkes_params* p, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
+                     double* hess_theta_diag, double* hess_hyper, void* stream);
+int hawkes_skip_stats(hawkes_ctx* ctx, int64_t* out);
+int hawkes_skip_perm(hawkes_ctx* ctx, int64_t n, int64_t* perm_host);
+
 /* After an evaluation queued on this context has been enqueued: copies of the per-event rates
  * lambda_n (n doubles) into a caller buffer, on `stream`.  For tests and diagnostics. */
 int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stream);

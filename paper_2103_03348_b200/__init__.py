@@ -117,6 +117,46 @@ class HawkesContext:
             raise HawkesError(rc, "hawkes_eval")
         return r
 
+    def skip_plan(self, x, t, params) -> dict:
+        """hawkes_skip_plan: curve order, boxes and work lists of the exact-zero-skipping variant for these events
+        and hyperparameters (synchronous, host work).  Returns the item counts of hawkes_skip_stats."""
+        if x.dim() != 2 or x.shape[0] != self.dim or t.shape[0] != x.shape[1]:
+            raise ValueError("x must be (dim, n) and t (n,)")
+        n = int(t.shape[0])
+        p = _params(params)
+        rc = self._lib.hawkes_skip_plan(self._h, n, _ptr(x), _ptr(t), ctypes.byref(p))
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_skip_plan")
+        st = (ctypes.c_int64 * 7)()
+        rc = self._lib.hawkes_skip_stats(self._h, st)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_skip_stats")
+        return {"items_background": st[0], "items_excitation": st[1], "items_dense_pass1": st[2],
+                "items_pass2": st[3], "items_dense_pass2": st[4], "workers_pass1": st[5], "workers_pass2": st[6]}
+
+    def skip_perm(self, n: int):
+        """The curve order of the current plan: record i is the caller's event perm[i] (host int64 tensor)."""
+        perm = self._torch.empty(n, dtype=self._torch.int64)
+        rc = self._lib.hawkes_skip_perm(self._h, n, perm.data_ptr())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_skip_perm")
+        return perm
+
+    def eval_skip(self, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None) -> EvalResult:
+        """hawkes_eval_skip: hawkes_eval over the work lists of skip_plan (same arguments, same outputs in the
+        caller's event order, no cross block); the events need not be sorted by time."""
+        n = self._check_inputs(x, t, theta)
+        if not x.is_cuda:
+            raise ValueError("eval_skip() takes CUDA tensors")
+        r = out if out is not None else self._outputs(n, want, self._dev)
+        p = _params(params)
+        rc = self._lib.hawkes_eval_skip(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want,
+                                        _ptr(r.ll), _ptr(r.grad_theta), _ptr(r.grad_hyper), _ptr(r.hess_theta_diag),
+                                        _ptr(r.hess_hyper), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_eval_skip")
+        return r
+
     def loglik(self, x, t, theta, params):
         n = self._check_inputs(x, t, theta)
         r = self._outputs(n, WANT_LL, self._dev)

@@ -38,6 +38,10 @@ SYMBOLS = {
     "hawkes_hessian_theta_dense": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, vp]),
     "hawkes_sort_events": (cint, [vp, i64, cint, _dp, _dp, _dp, _dp, _dp, _dp, vp, vp]),
     "hawkes_get_lambda": (cint, [vp, i64, _dp, vp]),
+    "hawkes_skip_plan": (cint, [vp, i64, _dp, _dp, PP]),
+    "hawkes_eval_skip": (cint, [vp, i64, _dp, _dp, _dp, PP, u32, _dp, _dp, _dp, _dp, _dp, vp]),
+    "hawkes_skip_stats": (cint, [vp, vp]),
+    "hawkes_skip_perm": (cint, [vp, i64, vp]),
     "hawkes_set_background_mode": (cint, [vp, cint]),
     "hawkes_hessian_theta_block": (cint, [vp, i64, _dp, _dp, _dp, PP, i64, vp, _dp, vp]),
     "hawkes_launch_count": (i64, [vp]),

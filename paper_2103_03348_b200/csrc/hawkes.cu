@@ -386,6 +386,7 @@ struct Split {
     int w_all;       // cost of a streamed event every owned event pairs with       (pass 1: background)
     int w_head;      // extra cost of the streamed events with index < tile end     (pass 1: excitation)
     int tri;         // 1: only streamed events with index >= tile begin are visited (pass 2)
+    const int* slot_tab;   // device table of slots per tile (list-driven passes of skip.cuh); NULL: closed form
 };
 
 __host__ __device__ inline int64_t split_prefix(const Split& s, int64_t I) {   // cost of tiles [0, I)
@@ -413,6 +414,7 @@ __host__ __device__ inline int64_t split_pos(const Split& s, int64_t I, int64_t 
 }
 // first CTA and number of CTAs (= partial slots) that hold a segment of tile I
 __host__ __device__ inline void split_slots(const Split& s, int64_t I, int* first, int* count) {
+    if (s.slot_tab != nullptr) { *first = 0; *count = s.slot_tab[I]; return; }
     const int64_t a = split_prefix(s, I) / s.chunk, b = (split_prefix(s, I + 1) - 1) / s.chunk;
     *first = (int)a;
     *count = (int)(b - a + 1);
@@ -559,7 +561,7 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
                                                         double* __restrict__ blockpart,
                                                         unsigned* __restrict__ status, double* __restrict__ bgcache,
                                                         int bg_mode, const double* __restrict__ partc, int sym_tiles,
-                                                        int sym_tile) {
+                                                        int sym_tile, const double* __restrict__ tn_ptr) {
     constexpr int RS = DIM3 ? 6 : 4;
     constexpr int NB = Mom<LEVEL>::NB;
     const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
@@ -695,7 +697,8 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
             }
         }
         // integral terms (a3)
-        const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
+        // t_N: the last record in time order, or the value the caller of an unordered layout supplies
+        const double tN = tn_ptr ? *tn_ptr : rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
         const double T = tN - e.t;
         const double a = T / c.tau_t, bb = -e.t / c.tau_t;
         const double pa = norm_pdf(a), pb = norm_pdf(bb);
@@ -931,10 +934,13 @@ template <bool DIM3>
 __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                       DevConsts c, const double* __restrict__ part2, Split sp,
                                                       double* __restrict__ grad_theta,
-                                                      double* __restrict__ hess_theta_diag) {
+                                                      double* __restrict__ hess_theta_diag,
+                                                      const double* __restrict__ tn_ptr,
+                                                      const int64_t* __restrict__ perm) {
     constexpr int RS = DIM3 ? 6 : 4;
     const int64_t i = (int64_t)blockIdx.x * RED_T + threadIdx.x;
     if (i >= n) return;
+    const int64_t o = perm ? perm[i] : i;   // record i is the caller's event perm[i]
     double cs = 0.0, ds = 0.0;
     int slot0, n_slots;
     split_slots(sp, i / sp.tile, &slot0, &n_slots);
@@ -954,11 +960,11 @@ __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__
         if (hess_theta_diag) ds += part2[(int64_t)(s * 2 + 1) * ld + i];
     }
     if (grad_theta) {
-        const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
+        const double tN = tn_ptr ? *tn_ptr : rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
         const double ti = rec[i * RS + (DIM3 ? 3 : 2)];
-        grad_theta[i] = c.CSS * cs - c.xi0 * (-expm1(-c.omega * (tN - ti)));
+        grad_theta[o] = c.CSS * cs - c.xi0 * (-expm1(-c.omega * (tN - ti)));
     }
-    if (hess_theta_diag) hess_theta_diag[i] = -(c.CSS * c.CSS) * ds;
+    if (hess_theta_diag) hess_theta_diag[o] = -(c.CSS * c.CSS) * ds;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1244,6 +1250,7 @@ struct hawkes_ctx {
     bool prof_on;
     int64_t prof_count;           // evaluations recorded since the last read
     cudaEvent_t* prof_ev;         // [PROF_RING * 6] or NULL
+    struct SkipPlan* skip;        // hawkes_skip_plan (skip.cuh) or NULL
 };
 
 namespace {
@@ -1298,6 +1305,7 @@ int plan_split(Split* sp, int64_t n, int tile, int w_all, int w_head, int tri, i
     sp->w_all = w_all;
     sp->w_head = w_head;
     sp->tri = tri;
+    sp->slot_tab = nullptr;
     const int64_t total = split_prefix(*sp, sp->n_tiles);
     const int64_t min_chunk = (int64_t)(tri ? 1 : w_all + w_head) * 32;   // >= ~32 streamed events per CTA
     int64_t chunk = (total + ctas - 1) / ctas;
@@ -1398,7 +1406,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
         case 1:
             if (sym)
@@ -1406,12 +1414,12 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
     }
     ctx->launches += 2;
@@ -1441,7 +1449,8 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         if (pe) CK(cudaEventRecord(pe[4], st));
         theta_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part2, pl.sp2,
                                                       (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
-                                                      (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr);
+                                                      (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr,
+                                                      nullptr, nullptr);
         ctx->launches += 2;
     } else if (pe) {
         CK(cudaEventRecord(pe[3], st));
@@ -1495,6 +1504,8 @@ int check_common(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
 
 }  // namespace
 
+#include "skip.cuh"
+
 extern "C" {
 
 const char* hawkes_strerror(int status) {
@@ -1528,6 +1539,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->prof_on = false;
     c->prof_count = 0;
     c->prof_ev = nullptr;
+    c->skip = nullptr;
     const int RS = dim == 3 ? 6 : 4;
     const int nblk = (int)((n_max + RED_T - 1) / RED_T);
     c->plan_n = -1;
@@ -1608,6 +1620,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
 void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
+    skip_plan_free(c);
     void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)

@@ -1,0 +1,568 @@
+// Exact-zero skipping: a variant of the pairwise passes that visits only those tile
+// pairs which can hold a non-zero term of Eq. 1 / Eq. 4, reported separately from the
+// dense path (the paper's method visits every pair).
+//
+// A term exp(-z) of either kernel is exactly +0.0 in IEEE double arithmetic once z > 1075 ln 2 = 745.14.  The
+// events are re-ordered along a space-time Morton curve whose cell sizes are a quarter of the cut-off radii
+// (so consecutive events are neighbours on the scale that matters), every run of TS records gets a bounding
+// box in space and time, and a (target tile, source chunk) pair is dropped when the smallest exponent any of
+// its pairs can have exceeds SKIP_Z0 = 746 -- or, for the excitation term, when no pair of it is causal.  Only
+// exact zeros are dropped: every sum changes by its summation order alone.  In the curve order time is no
+// longer sorted, so every excitation pair takes the per-pair test dt > 0 (MODE 2 / MASKED of the dense tiles).
+//
+// The plan (order, boxes, work lists, their cut into workers) is built on the host by hawkes_skip_plan: it
+// depends on the events and the hyperparameters, not on theta, so one plan serves every evaluation of an HMC
+// trajectory.  Included by hawkes.cu after its kernels and the context struct.
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+constexpr double SKIP_Z0 = 746.0;      // exp(-z) == +0.0 for z >= 745.14
+constexpr int SK_B = 1, SK_S = 2;      // item kinds: background live, excitation live (3 = both)
+static_assert(P1_G[0] == P1_G[1] && P1_G[1] == P1_G[2] && P2_G[0] == P2_G[1], "one worker count per pass");
+
+// a0': pack the caller's event perm[i] into record i; times need not be sorted here.
+__global__ void skip_gather_kernel(int64_t n, int dim, const int64_t* __restrict__ perm, const double* __restrict__ x,
+                                   const double* __restrict__ t, const double* __restrict__ theta,
+                                   double* __restrict__ rec, unsigned* __restrict__ status) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int64_t o = perm[i];
+    const double ti = t[o], th = theta[o];
+    unsigned bad = 0;
+    if (!isfinite(ti) || !isfinite(th) || th < 0.0) bad |= ST_NONFINITE;
+    double xv[3] = {0.0, 0.0, 0.0};
+    for (int d = 0; d < dim; ++d) {
+        xv[d] = x[(int64_t)d * n + o];
+        if (!isfinite(xv[d])) bad |= ST_NONFINITE;
+    }
+    if (dim <= 2) {
+        reinterpret_cast<double4*>(rec)[i] = make_double4(xv[0], xv[1], ti, th);
+    } else {
+        double2* r2 = reinterpret_cast<double2*>(rec) + 3 * i;
+        r2[0] = make_double2(xv[0], xv[1]);
+        r2[1] = make_double2(xv[2], ti);
+        r2[2] = make_double2(th, 0.0);
+    }
+    if (bad) atomicOr(status, bad);
+}
+
+// a1 over a work list.  items[k] = (target tile I of NT*R records, source chunk J of TS records * 4 + kind), sorted
+// by I then J; worker w (one group of NT threads) takes items [wstart[w], wstart[w+1]) and writes, for every tile
+// it touches, partial slot (w - wfirst[I]) in the layout of pass1_kernel.
+template <int R, int LEVEL, bool DIM3, int G>
+__global__ void __launch_bounds__(NT * G, 1) pass1_list_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
+                                                               DevConsts c, const double* __restrict__ tab_g,
+                                                               double* __restrict__ part, const int2* __restrict__ items,
+                                                               const int* __restrict__ wstart,
+                                                               const int* __restrict__ wfirst, int n_workers) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    constexpr int NB = Mom<LEVEL>::NB;
+    constexpr unsigned BUF = group_buf_bytes<DIM3>();
+    static_assert(smem_request(G * BUF) <= SMEM_MAX, "table + streaming buffers must fit shared memory");
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double smagic;
+    const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem);
+    const SmemPlan plan = smem_plan(smem_base, G * BUF);
+    fill_table(reinterpret_cast<double*>(smem + plan.tab_off), tab_g);
+    stash_consts(smagic);
+    __syncthreads();
+
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
+    const int w = blockIdx.x * G + grp;
+    if (w >= n_workers) return;
+    const int k0 = wstart[w], k1 = wstart[w + 1];
+    if (k0 >= k1) return;
+    double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
+    double* const sbuf1 = sbuf0 + TS * RS;
+    const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
+    const P1C pc = pinned_consts(smagic, c);
+
+    auto chunk_cnt = [&](int J) { return (int)min((int64_t)TS, n - (int64_t)J * TS); };
+    Ev<DIM3> g[R];
+    Mom<LEVEL> m[R];
+    auto flush = [&](int I) {
+        const int slot = w - wfirst[I];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = (int64_t)I * (NT * R) + r * NT + tid;
+            if (i < n) {
+                double* o = part + (int64_t)slot * (2 * NB) * ld + i;
+#pragma unroll
+                for (int k = 0; k < NB; ++k) {
+                    o[(int64_t)k * ld] = m[r].b[k];
+                    o[(int64_t)(NB + k) * ld] = m[r].s[k];
+                }
+            }
+        }
+    };
+
+    RecIO<DIM3> io;
+    int2 it = items[k0];
+    io.load(rec, (int64_t)(it.y >> 2) * TS, chunk_cnt(it.y >> 2), tid);
+    io.store(sbuf0, tid);
+    group_sync(grp);
+    int cur = 0, I = -1;
+    for (int k = k0; k < k1; ++k) {
+        if (it.x != I) {
+            if (I >= 0) flush(I);
+            I = it.x;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int64_t i = min((int64_t)I * (NT * R) + r * NT + tid, n - 1);
+                g[r] = read_rec<DIM3>(rec + i * RS);
+#pragma unroll
+                for (int q = 0; q < NB; ++q) { m[r].b[q] = 0.0; m[r].s[q] = 0.0; }
+            }
+        }
+        int2 nx = it;
+        if (k + 1 < k1) {
+            nx = items[k + 1];
+            io.load(rec, (int64_t)(nx.y >> 2) * TS, chunk_cnt(nx.y >> 2), tid);
+        }
+        const double* sb = cur ? sbuf1 : sbuf0;
+        const int cnt = chunk_cnt(it.y >> 2);
+        const int kind = it.y & 3;
+        if (kind == SK_B) p1_tile<R, LEVEL, 0, DIM3, true>(sb, cnt, g, m, pc, lane_base);
+        else if (kind == SK_S) p1_tile<R, LEVEL, 2, DIM3, false>(sb, cnt, g, m, pc, lane_base);
+        else p1_tile<R, LEVEL, 2, DIM3, true>(sb, cnt, g, m, pc, lane_base);
+        if (k + 1 < k1) io.store(cur ? sbuf0 : sbuf1, tid);
+        group_sync(grp);
+        cur ^= 1;
+        it = nx;
+    }
+    flush(I);
+}
+
+// a4 over a work list: items[k] = (source tile M of NT*R records, target chunk J * 4 + SK_S); the targets
+// (x, t, 1/lambda) stream from trec and every pair takes the test t_n > t_m.
+template <int R, int LEVEL, bool DIM3, int G>
+__global__ void __launch_bounds__(NT * G, 1) pass2_list_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
+                                                               int64_t n, int64_t ld, DevConsts c,
+                                                               const double* __restrict__ tab_g, double* __restrict__ part2,
+                                                               const int2* __restrict__ items, const int* __restrict__ wstart,
+                                                               const int* __restrict__ wfirst, int n_workers) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    constexpr unsigned BUF = group_buf_bytes<DIM3>();
+    static_assert(smem_request(G * BUF) <= SMEM_MAX, "table + streaming buffers must fit shared memory");
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double smagic;
+    const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem);
+    const SmemPlan plan = smem_plan(smem_base, G * BUF);
+    fill_table(reinterpret_cast<double*>(smem + plan.tab_off), tab_g);
+    stash_consts(smagic);
+    __syncthreads();
+
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
+    const int w = blockIdx.x * G + grp;
+    if (w >= n_workers) return;
+    const int k0 = wstart[w], k1 = wstart[w + 1];
+    if (k0 >= k1) return;
+    double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
+    double* const sbuf1 = sbuf0 + TS * RS;
+    const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
+    const P1C pc = pinned_consts(smagic, c);
+
+    auto chunk_cnt = [&](int J) { return (int)min((int64_t)TS, n - (int64_t)J * TS); };
+    Ev<DIM3> g[R];
+    double cm[R], dm[R];
+    auto flush = [&](int M) {
+        const int slot = w - wfirst[M];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = (int64_t)M * (NT * R) + r * NT + tid;
+            if (i < n) {
+                part2[(int64_t)(slot * 2 + 0) * ld + i] = cm[r];
+                if (LEVEL >= 1) part2[(int64_t)(slot * 2 + 1) * ld + i] = dm[r];
+            }
+        }
+    };
+
+    RecIO<DIM3> io;
+    int2 it = items[k0];
+    io.load(trec, (int64_t)(it.y >> 2) * TS, chunk_cnt(it.y >> 2), tid);
+    io.store(sbuf0, tid);
+    group_sync(grp);
+    int cur = 0, M = -1;
+    for (int k = k0; k < k1; ++k) {
+        if (it.x != M) {
+            if (M >= 0) flush(M);
+            M = it.x;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int64_t i = min((int64_t)M * (NT * R) + r * NT + tid, n - 1);
+                g[r] = read_rec<DIM3>(rec + i * RS);
+                cm[r] = 0.0;
+                dm[r] = 0.0;
+            }
+        }
+        int2 nx = it;
+        if (k + 1 < k1) {
+            nx = items[k + 1];
+            io.load(trec, (int64_t)(nx.y >> 2) * TS, chunk_cnt(nx.y >> 2), tid);
+        }
+        p2_tile<R, LEVEL, true, DIM3>(cur ? sbuf1 : sbuf0, chunk_cnt(it.y >> 2), g, cm, dm, pc, lane_base);
+        if (k + 1 < k1) io.store(cur ? sbuf0 : sbuf1, tid);
+        group_sync(grp);
+        cur ^= 1;
+        it = nx;
+    }
+    flush(M);
+}
+
+}  // namespace
+
+// -------------------------------------------------------------------------------------------------
+// host side: the plan
+struct SkipPlan {
+    int64_t n;
+    hawkes_params p;
+    int s_mode;
+    int64_t* d_perm;       // record i of the curve order is the caller's event perm[i]
+    double* d_tn;          // t_N = max t
+    int2* d_items1;        // pass-1 work list and its cut
+    int* d_w1start;
+    int* d_w1first;
+    int* d_slots1;
+    int workers1;
+    int2* d_items2;        // pass-2 work list and its cut
+    int* d_w2start;
+    int* d_w2first;
+    int* d_slots2;
+    int workers2;
+    // what the lists hold, for hawkes_skip_stats
+    int64_t items_b, items_s, items_p2, items_dense1, items_dense2;
+};
+
+namespace {
+
+void skip_plan_free(hawkes_ctx* c) {
+    SkipPlan* s = c->skip;
+    if (!s) return;
+    void* ptrs[] = {s->d_perm, s->d_tn, s->d_items1, s->d_w1start, s->d_w1first, s->d_slots1,
+                    s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
+    for (void* q : ptrs)
+        if (q) cudaFree(q);
+    delete s;
+    c->skip = nullptr;
+}
+
+struct SkipBox {           // bounding box of a run of records: up to 3 coordinates, then time
+    double lo[4], hi[4];
+};
+
+inline uint64_t skip_spread(uint64_t v) {   // 16 bits -> every 4th bit
+    v &= 0xffffull;
+    v = (v | (v << 24)) & 0x000000ff000000ffull;
+    v = (v | (v << 12)) & 0x000f000f000f000full;
+    v = (v | (v << 6)) & 0x0303030303030303ull;
+    v = (v | (v << 3)) & 0x1111111111111111ull;
+    return v;
+}
+
+// Cut a list (sorted by tile) into at most `workers` non-empty consecutive ranges of about equal cost; fills
+// wstart (workers + 1 entries), wfirst and slots (per tile).  Returns the number of workers used.
+int skip_cut(const std::vector<int2>& items, const std::vector<int>& cost, int n_tiles, int workers,
+             std::vector<int>* wstart, std::vector<int>* wfirst, std::vector<int>* slots) {
+    int64_t total = 0;
+    for (int v : cost) total += v;
+    const int64_t chunk = (total + workers - 1) / workers;
+    wstart->assign(1, 0);
+    wfirst->assign(n_tiles, 0);
+    slots->assign(n_tiles, 0);
+    std::vector<int> wlast(n_tiles, -1);
+    int64_t acc = 0;
+    int w = 0;
+    for (size_t k = 0; k < items.size(); ++k) {
+        const int I = items[k].x;
+        if (wlast[I] < 0) (*wfirst)[I] = w;
+        wlast[I] = w;
+        acc += cost[k];
+        if (acc >= (int64_t)(w + 1) * chunk && k + 1 < items.size()) {
+            ++w;
+            wstart->push_back((int)k + 1);
+        }
+    }
+    wstart->push_back((int)items.size());
+    for (int I = 0; I < n_tiles; ++I) (*slots)[I] = wlast[I] < 0 ? 0 : wlast[I] - (*wfirst)[I] + 1;
+    return (int)wstart->size() - 1;
+}
+
+template <typename T>
+int skip_upload(T** dst, const std::vector<T>& v) {
+    *dst = nullptr;
+    if (cudaMalloc((void**)dst, sizeof(T) * (v.size() ? v.size() : 1)) != cudaSuccess) return HAWKES_ERR_NOMEM;
+    if (v.size() && cudaMemcpy(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice) != cudaSuccess)
+        return HAWKES_ERR_CUDA;
+    return HAWKES_OK;
+}
+
+int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p) {
+    const int dim = ctx->dim, nd = dim + 1;   // axes: coordinates, then time
+    std::vector<double> hx((size_t)dim * n), ht((size_t)n);
+    CK(cudaMemcpy(hx.data(), x, sizeof(double) * dim * n, cudaMemcpyDefault));
+    CK(cudaMemcpy(ht.data(), t, sizeof(double) * n, cudaMemcpyDefault));
+    for (int64_t i = 0; i < n; ++i)
+        if (!std::isfinite(ht[i])) return HAWKES_ERR_NONFINITE;
+    for (size_t i = 0; i < hx.size(); ++i)
+        if (!std::isfinite(hx[i])) return HAWKES_ERR_NONFINITE;
+    auto val = [&](int a, int64_t i) { return a < dim ? hx[(size_t)a * n + i] : ht[i]; };
+
+    // cut-off radii: a term is an exact zero beyond them whatever the other coordinates are
+    const double inf = INFINITY;
+    const double rs = p->h * std::sqrt(2.0 * SKIP_Z0), rb = p->tau_x * std::sqrt(2.0 * SKIP_Z0);
+    const double ts_ = SKIP_Z0 / p->omega, tb = ctx->s_mode ? inf : p->tau_t * std::sqrt(2.0 * SKIP_Z0);
+    // curve order: cells of a quarter of the smaller radius per axis, 16 bits per axis
+    std::vector<uint64_t> key((size_t)n, 0);
+    for (int a = 0; a < nd; ++a) {
+        double lo = inf, hi = -inf;
+        for (int64_t i = 0; i < n; ++i) { lo = std::min(lo, val(a, i)); hi = std::max(hi, val(a, i)); }
+        double cell = 0.25 * (a < dim ? std::min(rs, rb) : std::min(ts_, tb));
+        if (!(cell > 0.0) || !std::isfinite(cell)) cell = inf;
+        if ((hi - lo) / cell > 65535.0) cell = (hi - lo) / 65535.0;
+        for (int64_t i = 0; i < n; ++i) {
+            const double q = std::isfinite(cell) ? std::floor((val(a, i) - lo) / cell) : 0.0;
+            const uint64_t cq = q < 0.0 ? 0 : (q > 65535.0 ? 65535 : (uint64_t)q);
+            key[i] |= skip_spread(cq) << a;
+        }
+    }
+    std::vector<int64_t> perm((size_t)n);
+    for (int64_t i = 0; i < n; ++i) perm[i] = i;
+    std::stable_sort(perm.begin(), perm.end(), [&](int64_t a, int64_t b) { return key[a] < key[b]; });
+
+    // boxes of the TS-record chunks and of the NT*R-record tiles
+    auto boxes = [&](int run) {
+        const int64_t nb = (n + run - 1) / run;
+        std::vector<SkipBox> bx((size_t)nb);
+        for (int64_t b = 0; b < nb; ++b) {
+            for (int a = 0; a < 4; ++a) { bx[b].lo[a] = inf; bx[b].hi[a] = -inf; }
+            for (int64_t i = b * run; i < std::min(n, (b + 1) * run); ++i)
+                for (int a = 0; a < nd; ++a) {
+                    const double v = val(a, perm[i]);
+                    bx[b].lo[a] = std::min(bx[b].lo[a], v);
+                    bx[b].hi[a] = std::max(bx[b].hi[a], v);
+                }
+        }
+        return bx;
+    };
+    const std::vector<SkipBox> chunk = boxes(TS), tile1 = boxes(NT * P1_R), tile2 = boxes(NT * P2_R);
+    auto gap2 = [&](const SkipBox& A, const SkipBox& B) {   // squared distance between the spatial boxes
+        double s = 0.0;
+        for (int a = 0; a < dim; ++a) {
+            const double g = std::max(0.0, std::max(A.lo[a] - B.hi[a], B.lo[a] - A.hi[a]));
+            s += g * g;
+        }
+        return s;
+    };
+    // background of (targets T, sources S): min exponent r^2/2tau_x^2 + dt^2/2tau_t^2
+    auto live_b = [&](const SkipBox& T, const SkipBox& S) {
+        double z = gap2(T, S) / (2.0 * p->tau_x * p->tau_x);
+        if (!ctx->s_mode) {
+            const double g = std::max(0.0, std::max(T.lo[dim] - S.hi[dim], S.lo[dim] - T.hi[dim]));
+            z += g * g / (2.0 * p->tau_t * p->tau_t);
+        }
+        return !(z >= SKIP_Z0);
+    };
+    // excitation of targets T by sources S: some pair must be causal (t_n > t_m), min exponent r^2/2h^2 + omega dt
+    auto live_s = [&](const SkipBox& T, const SkipBox& S) {
+        if (!(T.hi[dim] > S.lo[dim])) return false;
+        const double z = gap2(T, S) / (2.0 * p->h * p->h) + p->omega * std::max(0.0, T.lo[dim] - S.hi[dim]);
+        return !(z >= SKIP_Z0);
+    };
+
+    SkipPlan* sp = new (std::nothrow) SkipPlan();
+    if (!sp) return HAWKES_ERR_NOMEM;
+    std::memset(sp, 0, sizeof(*sp));
+    ctx->skip = sp;
+    sp->n = n;
+    sp->p = *p;
+    sp->s_mode = ctx->s_mode;
+    const int nc = (int)chunk.size(), nt1 = (int)tile1.size(), nt2 = (int)tile2.size();
+    std::vector<int2> items1, items2;
+    std::vector<int> cost1, cost2;
+    for (int I = 0; I < nt1; ++I)
+        for (int J = 0; J < nc; ++J) {
+            const int kind = (live_b(tile1[I], chunk[J]) ? SK_B : 0) | (live_s(tile1[I], chunk[J]) ? SK_S : 0);
+            if (!kind) continue;
+            items1.push_back(make_int2(I, J * 4 + kind));
+            cost1.push_back(((kind & SK_B) ? W_ALL[1] : 0) + ((kind & SK_S) ? W_HEAD[1] + 4 : 0));
+            sp->items_b += (kind & SK_B) ? 1 : 0;
+            sp->items_s += (kind & SK_S) ? 1 : 0;
+        }
+    for (int M = 0; M < nt2; ++M)
+        for (int J = 0; J < nc; ++J)
+            if (live_s(chunk[J], tile2[M])) {
+                items2.push_back(make_int2(M, J * 4 + SK_S));
+                cost2.push_back(1);
+            }
+    sp->items_p2 = (int64_t)items2.size();
+    sp->items_dense1 = (int64_t)nt1 * nc;
+    sp->items_dense2 = (int64_t)nt2 * nc;
+
+    // cut into workers; halve the worker count while the fullest tile's slots do not fit the partial buffers
+    const int64_t ld = round_up(n, 256);
+    std::vector<int> ws, wf, sl;
+    auto cut = [&](const std::vector<int2>& items, const std::vector<int>& cost, int n_tiles, int workers, int n_mom,
+                   size_t cap, int* used) {
+        for (;; workers = (workers + 1) / 2) {
+            *used = skip_cut(items, cost, n_tiles, workers, &ws, &wf, &sl);
+            int worst = 0;
+            for (int v : sl) worst = std::max(worst, v);
+            if ((size_t)worst * n_mom * (size_t)ld <= cap) return HAWKES_OK;
+            if (workers == 1) return HAWKES_ERR_UNSUPPORTED;
+        }
+    };
+    int rc;
+    if ((rc = cut(items1, cost1, nt1, ctx->sm_count * P1_G[0], 12, ctx->part1_doubles, &sp->workers1))) return rc;
+    if ((rc = skip_upload(&sp->d_items1, items1)) || (rc = skip_upload(&sp->d_w1start, ws)) ||
+        (rc = skip_upload(&sp->d_w1first, wf)) || (rc = skip_upload(&sp->d_slots1, sl))) return rc;
+    if ((rc = cut(items2, cost2, nt2, ctx->sm_count * P2_G[0], 2, ctx->part2_doubles, &sp->workers2))) return rc;
+    if ((rc = skip_upload(&sp->d_items2, items2)) || (rc = skip_upload(&sp->d_w2start, ws)) ||
+        (rc = skip_upload(&sp->d_w2first, wf)) || (rc = skip_upload(&sp->d_slots2, sl))) return rc;
+    if ((rc = skip_upload(&sp->d_perm, perm))) return rc;
+    double tn = -inf;
+    for (int64_t i = 0; i < n; ++i) tn = std::max(tn, ht[i]);
+    std::vector<double> tnv(1, tn);
+    if ((rc = skip_upload(&sp->d_tn, tnv))) return rc;
+    return HAWKES_OK;
+}
+
+template <bool DIM3>
+int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                      const DevConsts& c, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
+                      double* hess_theta_diag, double* hess_hyper, cudaStream_t st) {
+    const SkipPlan& sp = *ctx->skip;
+    const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2 : ((want & HAWKES_WANT_GRAD_HYPER) ? 1 : 0);
+    const int64_t ld = round_up(n, 256);
+    const int nblk = (int)((n + RED_T - 1) / RED_T);
+    CK(cudaMemsetAsync(ctx->d_status, 0, 2 * sizeof(unsigned), st));
+    skip_gather_kernel<<<nblk, RED_T, 0, st>>>(n, ctx->dim, sp.d_perm, x, t, theta, ctx->d_rec, ctx->d_status);
+    Split s1{};
+    s1.n = n;
+    s1.tile = NT * P1_R;
+    s1.n_tiles = (int)((n + s1.tile - 1) / s1.tile);
+    s1.chunk = 1;
+    s1.slot_tab = sp.d_slots1;
+    constexpr int G1 = P1_G[0];
+    constexpr unsigned SM1 = smem_request(G1 * group_buf_bytes<DIM3>());
+    const unsigned g1 = (unsigned)((sp.workers1 + G1 - 1) / G1);
+#define SKIP_PASS1(L)                                                                                                     \
+    pass1_list_kernel<P1_R, L, DIM3, G1><<<g1, NT * G1, SM1, st>>>(ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_part1,       \
+                                                                   sp.d_items1, sp.d_w1start, sp.d_w1first, sp.workers1); \
+    reduce1_kernel<L, DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, ctx->d_part1, s1, ctx->d_lam, ctx->d_trec,      \
+                                                    ctx->d_trec2, nullptr, ctx->d_blockpart, ctx->d_status,               \
+                                                    ctx->d_bgcache, 0, nullptr, 0, NT * P1_R, sp.d_tn)
+    if (level1 == 0) { SKIP_PASS1(0); }
+    else if (level1 == 1) { SKIP_PASS1(1); }
+    else { SKIP_PASS1(2); }
+#undef SKIP_PASS1
+    ctx->launches += 3;
+    if (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) {
+        scalars_kernel<<<1, SCAL_T, 0, st>>>(ctx->d_blockpart, nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
+                                             (want & HAWKES_WANT_GRAD_HYPER) ? grad_hyper : nullptr,
+                                             (want & HAWKES_WANT_HESS_HYPER) ? hess_hyper : nullptr, ctx->d_scal);
+        ctx->launches++;
+    }
+    if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
+        Split s2{};
+        s2.n = n;
+        s2.tile = NT * P2_R;
+        s2.n_tiles = (int)((n + s2.tile - 1) / s2.tile);
+        s2.chunk = 1;
+        s2.slot_tab = sp.d_slots2;
+        constexpr int G2 = P2_G[0];
+        constexpr unsigned SM2 = smem_request(G2 * group_buf_bytes<DIM3>());
+        const unsigned g2 = (unsigned)((sp.workers2 + G2 - 1) / G2);
+        if (sp.items_p2 > 0) {
+            if (want & HAWKES_WANT_HESS_THETA)
+                pass2_list_kernel<P2_R, 1, DIM3, G2><<<g2, NT * G2, SM2, st>>>(ctx->d_rec, ctx->d_trec, n, ld, c, ctx->d_tab, ctx->d_part2, sp.d_items2, sp.d_w2start, sp.d_w2first, sp.workers2);
+            else
+                pass2_list_kernel<P2_R, 0, DIM3, G2><<<g2, NT * G2, SM2, st>>>(ctx->d_rec, ctx->d_trec, n, ld, c, ctx->d_tab, ctx->d_part2, sp.d_items2, sp.d_w2start, sp.d_w2first, sp.workers2);
+            ctx->launches++;
+        }
+        theta_kernel<DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, ctx->d_part2, s2,
+                                                   (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr,
+                                                   (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr, sp.d_tn,
+                                                   sp.d_perm);
+        ctx->launches++;
+    }
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+template <bool DIM3>
+int skip_setup_kernels() {
+    int dummy;
+    int rc;
+    constexpr unsigned SM1 = smem_request(P1_G[0] * group_buf_bytes<DIM3>());
+    constexpr unsigned SM2 = smem_request(P2_G[0] * group_buf_bytes<DIM3>());
+    if ((rc = setup_kernel(pass1_list_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], SM1, &dummy))) return rc;
+    if ((rc = setup_kernel(pass1_list_kernel<P1_R, 1, DIM3, P1_G[0]>, P1_G[0], SM1, &dummy))) return rc;
+    if ((rc = setup_kernel(pass1_list_kernel<P1_R, 2, DIM3, P1_G[0]>, P1_G[0], SM1, &dummy))) return rc;
+    if ((rc = setup_kernel(pass2_list_kernel<P2_R, 0, DIM3, P2_G[0]>, P2_G[0], SM2, &dummy))) return rc;
+    if ((rc = setup_kernel(pass2_list_kernel<P2_R, 1, DIM3, P2_G[0]>, P2_G[0], SM2, &dummy))) return rc;
+    return HAWKES_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hawkes_skip_plan(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p) {
+    if (!ctx || !x || !t || !p) return HAWKES_ERR_ARG;
+    if (n < 1 || n > ctx->n_max) return HAWKES_ERR_ARG;
+    DevConsts c;
+    int rc = make_consts(p, ctx->dim, ctx->s_mode, &c);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaDeviceSynchronize());   // evaluations in flight may still read the old plan
+    skip_plan_free(ctx);
+    if ((rc = (ctx->dim == 3 ? skip_setup_kernels<true>() : skip_setup_kernels<false>()))) return rc;
+    rc = skip_build(ctx, n, x, t, p);
+    if (rc) skip_plan_free(ctx);
+    return rc;
+}
+
+int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                     const hawkes_params* p, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,
+                     double* hess_theta_diag, double* hess_hyper, void* stream) {
+    int rc = check_common(ctx, n, x, t, theta, p);
+    if (rc) return rc;
+    if (want == 0 || (want & ~31u)) return HAWKES_ERR_ARG;   // no cross block in this variant
+    if (((want & HAWKES_WANT_LL) && !ll) || ((want & HAWKES_WANT_GRAD_THETA) && !grad_theta) ||
+        ((want & HAWKES_WANT_GRAD_HYPER) && !grad_hyper) || ((want & HAWKES_WANT_HESS_THETA) && !hess_theta_diag) ||
+        ((want & HAWKES_WANT_HESS_HYPER) && !hess_hyper))
+        return HAWKES_ERR_ARG;
+    const SkipPlan* sp = ctx->skip;
+    if (!sp || sp->n != n || sp->s_mode != ctx->s_mode || sp->p.mu0 != p->mu0 || sp->p.tau_x != p->tau_x ||
+        sp->p.tau_t != p->tau_t || sp->p.xi0 != p->xi0 || sp->p.h != p->h || sp->p.omega != p->omega)
+        return HAWKES_ERR_ARG;     // no plan, or one built for other events / hyperparameters
+    DevConsts c;
+    rc = make_consts(p, ctx->dim, ctx->s_mode, &c);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    if (ctx->dim == 3)
+        return enqueue_eval_skip<true>(ctx, n, x, t, theta, c, want, ll, grad_theta, grad_hyper, hess_theta_diag, hess_hyper, (cudaStream_t)stream);
+    return enqueue_eval_skip<false>(ctx, n, x, t, theta, c, want, ll, grad_theta, grad_hyper, hess_theta_diag, hess_hyper, (cudaStream_t)stream);
+}
+
+// out[0..5]: pass-1 items with a live background / with a live excitation / dense count; pass-2 items / dense count;
+// out[5] = workers of pass 1, out[6] = workers of pass 2 (an item = NT*R records x TS records)
+int hawkes_skip_stats(hawkes_ctx* ctx, int64_t* out) {
+    if (!ctx || !out || !ctx->skip) return HAWKES_ERR_ARG;
+    const SkipPlan* sp = ctx->skip;
+    out[0] = sp->items_b; out[1] = sp->items_s; out[2] = sp->items_dense1;
+    out[3] = sp->items_p2; out[4] = sp->items_dense2;
+    out[5] = sp->workers1; out[6] = sp->workers2;
+    return HAWKES_OK;
+}
+
+int hawkes_skip_perm(hawkes_ctx* ctx, int64_t n, int64_t* perm_host) {
+    if (!ctx || !perm_host || !ctx->skip || ctx->skip->n != n) return HAWKES_ERR_ARG;
+    CK(cudaMemcpy(perm_host, ctx->skip->d_perm, sizeof(int64_t) * n, cudaMemcpyDeviceToHost));
+    return HAWKES_OK;
+}
+
+}  // extern "C"
