@@ -161,7 +161,7 @@ int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
 /* ---- Exact-zero skipping: a separately reported variant of the evaluation ---------------------
  * A term of Eq. 1 or Eq. 4 is exp(-z) with z = |dx|^2/(2 tau_x^2) + dt^2/(2 tau_t^2)
  * (background) or z = |dx|^2/(2 h^2) + omega dt (self-excitation); in IEEE double arithmetic it is exactly +0.0 once
- * z > 745.14.  hawkes_skip_plan orders the events along a space-time Morton curve, boxes every run of 128 of them and
+ * z > 745.14.  hawkes_skip_plan orders the events as the leaves of a space-time k-d tree, boxes every run of 128 of them and
  * lists the (target tile, source run) pairs whose smallest possible z is below 746 (for the self-excitation: that
  * also hold a causal pair); hawkes_eval_skip then runs the two pairwise passes over those lists only.  Nothing but
  * exact zeros is left out, so each output differs from hawkes_eval's by summation order alone (same tolerance).
@@ -179,7 +179,7 @@ int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
  *   events.  HAWKES_ERR_UNSORTED is never raised here.
  * hawkes_skip_stats: out[0..6] = pass-1 items with a live background, with a live self-excitation, of the dense
  *   pass; pass-2 items, of the dense pass; workers of pass 1, of pass 2 (item = 256 records x 128 records).
- * hawkes_skip_perm: the curve order (record i is the caller's event perm[i]) into a HOST buffer of n int64. */
+ * hawkes_skip_perm: the tree order (record i is the caller's event perm[i]) into a HOST buffer of n int64. */
 int hawkes_skip_plan(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p);
 int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
                      const hawkes_params* p, uint32_t want, double* ll, double* grad_theta, double* grad_hyper,

@@ -118,7 +118,7 @@ class HawkesContext:
         return r
 
     def skip_plan(self, x, t, params) -> dict:
-        """hawkes_skip_plan: curve order, boxes and work lists of the exact-zero-skipping variant for these events
+        """hawkes_skip_plan: k-d order, boxes and work lists of the exact-zero-skipping variant for these events
         and hyperparameters (synchronous, host work).  Returns the item counts of hawkes_skip_stats."""
         if x.dim() != 2 or x.shape[0] != self.dim or t.shape[0] != x.shape[1]:
             raise ValueError("x must be (dim, n) and t (n,)")
@@ -135,7 +135,7 @@ class HawkesContext:
                 "items_pass2": st[3], "items_dense_pass2": st[4], "workers_pass1": st[5], "workers_pass2": st[6]}
 
     def skip_perm(self, n: int):
-        """The curve order of the current plan: record i is the caller's event perm[i] (host int64 tensor)."""
+        """The k-d order of the current plan: record i is the caller's event perm[i] (host int64 tensor)."""
         perm = self._torch.empty(n, dtype=self._torch.int64)
         rc = self._lib.hawkes_skip_perm(self._h, n, perm.data_ptr())
         if rc != 0:

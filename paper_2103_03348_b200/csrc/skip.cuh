@@ -3,11 +3,11 @@
 // dense path (the paper's method visits every pair).
 //
 // A term exp(-z) of either kernel is exactly +0.0 in IEEE double arithmetic once z > 1075 ln 2 = 745.14.  The
-// events are re-ordered along a space-time Morton curve whose cell sizes are a quarter of the cut-off radii
-// (so consecutive events are neighbours on the scale that matters), every run of TS records gets a bounding
+// events are re-ordered as the leaves of a space-time k-d tree (median splits along the axis of furthest reach in
+// units of the cut-off radius; leaves = the runs of TS records the kernels stream), every run gets a bounding
 // box in space and time, and a (target tile, source chunk) pair is dropped when the smallest exponent any of
 // its pairs can have exceeds SKIP_Z0 = 746 -- or, for the excitation term, when no pair of it is causal.  Only
-// exact zeros are dropped: every sum changes by its summation order alone.  In the curve order time is no
+// exact zeros are dropped: every sum changes by its summation order alone.  In the tree order time is no
 // longer sorted, so every excitation pair takes the per-pair test dt > 0 (MODE 2 / MASKED of the dense tiles).
 //
 // The plan (order, boxes, work lists, their cut into workers) is built on the host by hawkes_skip_plan: it
@@ -220,7 +220,7 @@ struct SkipPlan {
     int64_t n;
     hawkes_params p;
     int s_mode;
-    int64_t* d_perm;       // record i of the curve order is the caller's event perm[i]
+    int64_t* d_perm;       // record i of the tree order is the caller's event perm[i]
     double* d_tn;          // t_N = max t
     int2* d_items1;        // pass-1 work list and its cut
     int* d_w1start;
@@ -252,15 +252,6 @@ void skip_plan_free(hawkes_ctx* c) {
 struct SkipBox {           // bounding box of a run of records: up to 3 coordinates, then time
     double lo[4], hi[4];
 };
-
-inline uint64_t skip_spread(uint64_t v) {   // 16 bits -> every 4th bit
-    v &= 0xffffull;
-    v = (v | (v << 24)) & 0x000000ff000000ffull;
-    v = (v | (v << 12)) & 0x000f000f000f000full;
-    v = (v | (v << 6)) & 0x0303030303030303ull;
-    v = (v | (v << 3)) & 0x1111111111111111ull;
-    return v;
-}
 
 // Cut a list (sorted by tile) into at most `workers` non-empty consecutive ranges of about equal cost; fills
 // wstart (workers + 1 entries), wfirst and slots (per tile).  Returns the number of workers used.
@@ -314,23 +305,40 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     const double inf = INFINITY;
     const double rs = p->h * std::sqrt(2.0 * SKIP_Z0), rb = p->tau_x * std::sqrt(2.0 * SKIP_Z0);
     const double ts_ = SKIP_Z0 / p->omega, tb = ctx->s_mode ? inf : p->tau_t * std::sqrt(2.0 * SKIP_Z0);
-    // curve order: cells of a quarter of the smaller radius per axis, 16 bits per axis
-    std::vector<uint64_t> key((size_t)n, 0);
-    for (int a = 0; a < nd; ++a) {
-        double lo = inf, hi = -inf;
-        for (int64_t i = 0; i < n; ++i) { lo = std::min(lo, val(a, i)); hi = std::max(hi, val(a, i)); }
-        double cell = 0.25 * (a < dim ? std::min(rs, rb) : std::min(ts_, tb));
-        if (!(cell > 0.0) || !std::isfinite(cell)) cell = inf;
-        if ((hi - lo) / cell > 65535.0) cell = (hi - lo) / 65535.0;
-        for (int64_t i = 0; i < n; ++i) {
-            const double q = std::isfinite(cell) ? std::floor((val(a, i) - lo) / cell) : 0.0;
-            const uint64_t cq = q < 0.0 ? 0 : (q > 65535.0 ? 65535 : (uint64_t)q);
-            key[i] |= skip_spread(cq) << a;
-        }
-    }
+    // k-d order: split the events at a median of the axis along which they reach furthest in units of the cut-off
+    // radius, the left part a whole number of tiles (of chunks, inside a tile), until every part is one chunk.
+    // Tiles and chunks are then the leaves of the tree: compact boxes that end where the runs end.
+    double cutoff[4];
+    for (int a = 0; a < nd; ++a) cutoff[a] = a < dim ? std::min(rs, rb) : std::min(ts_, tb);
     std::vector<int64_t> perm((size_t)n);
     for (int64_t i = 0; i < n; ++i) perm[i] = i;
-    std::stable_sort(perm.begin(), perm.end(), [&](int64_t a, int64_t b) { return key[a] < key[b]; });
+    {
+        const int64_t tile = NT * P1_R;
+        static_assert(NT * P1_R == NT * P2_R && (NT * P1_R) % TS == 0, "tiles of both passes are whole chunks");
+        std::vector<std::pair<int64_t, int64_t>> stack(1, {0, n});
+        while (!stack.empty()) {
+            const int64_t b0 = stack.back().first, b1 = stack.back().second, len = b1 - b0;
+            stack.pop_back();
+            if (len <= TS) continue;
+            int axis = 0;
+            double best = -1.0;
+            for (int a = 0; a < nd; ++a) {
+                double lo = inf, hi = -inf;
+                for (int64_t i = b0; i < b1; ++i) { lo = std::min(lo, val(a, perm[i])); hi = std::max(hi, val(a, perm[i])); }
+                const double e = (hi - lo) / cutoff[a];
+                if (e > best) { best = e; axis = a; }
+            }
+            const int64_t unit = len > tile ? tile : TS;
+            int64_t nl = ((len + unit - 1) / unit / 2) * unit;
+            if (nl <= 0) nl = unit;
+            std::nth_element(perm.begin() + b0, perm.begin() + b0 + nl, perm.begin() + b1, [&](int64_t u, int64_t w) {
+                const double vu = val(axis, u), vw = val(axis, w);
+                return vu < vw || (vu == vw && u < w);
+            });
+            stack.push_back({b0, b0 + nl});
+            stack.push_back({b0 + nl, b1});
+        }
+    }
 
     // boxes of the TS-record chunks and of the NT*R-record tiles
     auto boxes = [&](int run) {

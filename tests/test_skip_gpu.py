@@ -35,7 +35,7 @@ def run_skip(torch, ev, want=WANT, order=None, ctx=None):
     stats = ctx.skip_plan(x, t, ev.params)
     r = ctx.eval_skip(x, t, th, ev.params, want)
     st = ctx.last_status()
-    lam_rec = ctx.get_lambda(ev.n).cpu().numpy()          # in record (curve) order
+    lam_rec = ctx.get_lambda(ev.n).cpu().numpy()          # in record (k-d tree) order
     perm = ctx.skip_perm(ev.n).numpy()
     assert np.array_equal(np.sort(perm), np.arange(ev.n))
     lam = np.empty(ev.n)
