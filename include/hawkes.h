@@ -271,6 +271,13 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
                        const int64_t* idx, const double* z, double beta, const hawkes_params* p /*HOST*/,
                        double sigma2, double tau0, double* out3, double* grad_z, double* hess_z, void* stream);
 
+/* hawkes_posterior_z with the likelihood evaluated by hawkes_eval_skip (the caller has called hawkes_skip_plan for
+ * these events and hyperparameters; HAWKES_ERR_ARG otherwise).  Same outputs up to summation order. */
+int hawkes_posterior_z_skip(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t,
+                            int64_t m, const int64_t* idx, const double* z, double beta,
+                            const hawkes_params* p /*HOST*/, double sigma2, double tau0, double* out3, double* grad_z,
+                            double* hess_z, void* stream);
+
 /* ------------------------------------------------------------------------------------------------------
  * Preconditioned HMC update of the log-rates z with all likelihood work on the GPU (
  * BASELINE.json configs[3]).  Target: log pi(z) = ell(theta(z)) + log p(z | V_G, sigma2, tau0).
@@ -305,7 +312,10 @@ typedef struct {
                                     and kept: the one entry point that may allocate), plus lambda0 = everything that does
                                     not involve a sequenced rate; an evaluation is then two passes over K (row sums ->
                                     lambda, column sums -> d ell/d theta): HBM-bound instead of FP64-bound.  Same sums in
-                                    another order.  dim <= 2 only (HAWKES_ERR_UNSUPPORTED otherwise). */
+                                    another order.  dim <= 2 only (HAWKES_ERR_UNSUPPORTED otherwise).
+                                 3, 4: variants 0 and 1 with every evaluation over the work lists of hawkes_skip_plan
+                                    (exact zeros left out; the caller has planned these events and hyperparameters,
+                                    HAWKES_ERR_ARG otherwise).  Same sums in another order. */
     int32_t reserved;
 } hawkes_hmc_opts;
 

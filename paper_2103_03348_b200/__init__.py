@@ -260,16 +260,17 @@ class HawkesContext:
         return gz, hz, gb
 
     def posterior_z(self, tree: "HawkesTree", x, t, idx, z, beta: float, params, sigma2: float, tau0: float,
-                    hess: bool = False, out=None):
+                    hess: bool = False, out=None, skip: bool = False):
         """hawkes_posterior_z: returns (out3 [ell, log prior, sum], grad_z [m], hess_z [m] or None), device tensors;
-        `out` = a previous return value to reuse its buffers."""
+        `out` = a previous return value to reuse its buffers; skip=True: hawkes_posterior_z_skip (after skip_plan)."""
         torch = self._torch
         n, m = int(t.shape[0]), int(idx.shape[0])
         if out is None:
             mk = lambda k: torch.empty(k, dtype=torch.float64, device=self._dev)
             out = (mk(3), mk(m), mk(m) if hess else None)
         p = _params(params)
-        rc = self._lib.hawkes_posterior_z(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
+        fn = self._lib.hawkes_posterior_z_skip if skip else self._lib.hawkes_posterior_z
+        rc = fn(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
                                           ctypes.byref(p), float(sigma2), float(tau0), _ptr(out[0]), _ptr(out[1]),
                                           _ptr(out[2]), self._stream())
         if rc != 0:

@@ -57,6 +57,8 @@ SYMBOLS = {
     "hawkes_z_chain": (cint, [vp, i64, i64, vp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, vp]),
     "hawkes_posterior_z": (cint, [vp, vp, i64, _dp, _dp, i64, vp, _dp, ctypes.c_double, PP, ctypes.c_double,
                                   ctypes.c_double, _dp, _dp, _dp, vp]),
+    "hawkes_posterior_z_skip": (cint, [vp, vp, i64, _dp, _dp, i64, vp, _dp, ctypes.c_double, PP, ctypes.c_double,
+                                  ctypes.c_double, _dp, _dp, _dp, vp]),
     "hawkes_hmc_run": (cint, [vp, vp, i64, _dp, _dp, i64, vp, _dp, ctypes.c_double, PP, ctypes.c_double,
                               ctypes.c_double, ctypes.POINTER(HmcOpts), _dp, _dp, _dp, _dp, _dp, vp]),
     "hawkes_tree_precision_diag": (cint, [vp, ctypes.c_double, ctypes.c_double, _dp, vp]),

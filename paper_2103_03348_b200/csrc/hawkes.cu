@@ -1799,9 +1799,9 @@ int hawkes_z_chain(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, co
     return HAWKES_OK;
 }
 
-int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
-                       const int64_t* idx, const double* z, double beta, const hawkes_params* p, double sigma2,
-                       double tau0, double* out3, double* grad_z, double* hess_z, void* stream) {
+static int posterior_z_impl(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                            const int64_t* idx, const double* z, double beta, const hawkes_params* p, double sigma2,
+                            double tau0, double* out3, double* grad_z, double* hess_z, void* stream, bool skip) {
     if (!ctx || !tree || !x || !t || !idx || !z || !p) return HAWKES_ERR_ARG;
     if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
     if (!out3 && !grad_z && !hess_z) return HAWKES_ERR_ARG;
@@ -1814,8 +1814,12 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
     if (rc) return rc;
     const uint32_t want = HAWKES_WANT_LL | ((grad_z || hess_z) ? HAWKES_WANT_GRAD_THETA : 0u) |
                           (hess_z ? HAWKES_WANT_HESS_THETA : 0u);
-    rc = hawkes_eval(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr, hess_z ? ht : nullptr,
-                     nullptr, nullptr, stream);
+    if (skip)
+        rc = hawkes_eval_skip(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr,
+                              hess_z ? ht : nullptr, nullptr, stream);
+    else
+        rc = hawkes_eval(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr, hess_z ? ht : nullptr,
+                         nullptr, nullptr, stream);
     if (rc) return rc;
     rc = hawkes_tree_prior(tree, z, sigma2, tau0, sc + 1, grad_z ? pg : nullptr, stream);
     if (rc) return rc;
@@ -1827,6 +1831,18 @@ int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const doub
     return HAWKES_OK;
 }
 
+int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                       const int64_t* idx, const double* z, double beta, const hawkes_params* p, double sigma2,
+                       double tau0, double* out3, double* grad_z, double* hess_z, void* stream) {
+    return posterior_z_impl(ctx, tree, n, x, t, m, idx, z, beta, p, sigma2, tau0, out3, grad_z, hess_z, stream, false);
+}
+
+int hawkes_posterior_z_skip(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
+                            const int64_t* idx, const double* z, double beta, const hawkes_params* p, double sigma2,
+                            double tau0, double* out3, double* grad_z, double* hess_z, void* stream) {
+    return posterior_z_impl(ctx, tree, n, x, t, m, idx, z, beta, p, sigma2, tau0, out3, grad_z, hess_z, stream, true);
+}
+
 int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
                    const int64_t* idx, double* z, double beta, const hawkes_params* p, double sigma2, double tau0,
                    const hawkes_hmc_opts* o, const double* normals, const double* uniforms, double* mass,
@@ -1834,7 +1850,11 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     if (!ctx || !tree || !x || !t || !idx || !z || !p || !o || !normals || !uniforms || !mass) return HAWKES_ERR_ARG;
     if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
     if (o->n_iter < 1 || o->n_leapfrog < 1 || o->precond_every < 0 || o->n_refresh_done < 0 ||
-        o->cache_background < 0 || o->cache_background > 2) return HAWKES_ERR_ARG;
+        o->cache_background < 0 || o->cache_background > 4) return HAWKES_ERR_ARG;
+    // 3 / 4: variants 0 / 1 over the work lists of hawkes_skip_plan (exact zeros left out, csrc/skip.cuh)
+    const bool use_skip = o->cache_background >= 3;
+    const bool cache_bg = o->cache_background == 1 || o->cache_background == 4;
+    if (use_skip && !ctx->skip) return HAWKES_ERR_ARG;
     if (!(o->step > 0.0) || !std::isfinite(o->step) || !(o->mass_floor > 0.0) || !std::isfinite(o->mass_floor))
         return HAWKES_ERR_PARAM;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1900,7 +1920,7 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         ctx->launches++;
     }
     auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess) -> int {
-        if (!kmat) return hawkes_posterior_z(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream);
+        if (!kmat) return posterior_z_impl(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream, use_skip);
         // the O(M) tree prior (one latency-bound CTA) runs on a side stream beside the two passes over K
         if (cudaEventRecord(ctx->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0) != cudaSuccess)
             return HAWKES_ERR_CUDA;
@@ -1924,9 +1944,9 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         return HAWKES_OK;
     };
     // cache_background == 1: the first evaluation fills the background cache, every later one (all at LEVEL 0) uses it
-    ctx->bg_mode = o->cache_background == 1 ? 1 : 0;
+    ctx->bg_mode = cache_bg ? 1 : 0;
     rc = eval_post(z, o3c, gc, nullptr);
-    ctx->bg_mode = o->cache_background == 1 ? 2 : 0;
+    ctx->bg_mode = cache_bg ? 2 : 0;
     if (rc) return rc;
     int n_refresh = o->n_refresh_done;
     for (int it = 0; it < o->n_iter; ++it) {

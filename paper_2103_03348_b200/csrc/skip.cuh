@@ -227,6 +227,11 @@ struct SkipPlan {
     int* d_w1first;
     int* d_slots1;
     int workers1;
+    int2* d_items1s;       // pass 1 without the background term (cached sums, hawkes_hmc_run): the S items alone
+    int* d_w1sstart;
+    int* d_w1sfirst;
+    int* d_slots1s;
+    int workers1s;
     int2* d_items2;        // pass-2 work list and its cut
     int* d_w2start;
     int* d_w2first;
@@ -242,7 +247,7 @@ void skip_plan_free(hawkes_ctx* c) {
     SkipPlan* s = c->skip;
     if (!s) return;
     void* ptrs[] = {s->d_perm, s->d_tn, s->d_items1, s->d_w1start, s->d_w1first, s->d_slots1,
-                    s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
+                    s->d_items1s, s->d_w1sstart, s->d_w1sfirst, s->d_slots1s, s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     delete s;
@@ -388,8 +393,8 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     sp->p = *p;
     sp->s_mode = ctx->s_mode;
     const int nc = (int)chunk.size(), nt1 = (int)tile1.size(), nt2 = (int)tile2.size();
-    std::vector<int2> items1, items2;
-    std::vector<int> cost1, cost2;
+    std::vector<int2> items1, items1s, items2;
+    std::vector<int> cost1, cost1s, cost2;
     for (int I = 0; I < nt1; ++I)
         for (int J = 0; J < nc; ++J) {
             const int kind = (live_b(tile1[I], chunk[J]) ? SK_B : 0) | (live_s(tile1[I], chunk[J]) ? SK_S : 0);
@@ -398,6 +403,10 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
             cost1.push_back(((kind & SK_B) ? W_ALL[1] : 0) + ((kind & SK_S) ? W_HEAD[1] + 4 : 0));
             sp->items_b += (kind & SK_B) ? 1 : 0;
             sp->items_s += (kind & SK_S) ? 1 : 0;
+            if (kind & SK_S) {
+                items1s.push_back(make_int2(I, J * 4 + SK_S));
+                cost1s.push_back(1);
+            }
         }
     for (int M = 0; M < nt2; ++M)
         for (int J = 0; J < nc; ++J)
@@ -426,6 +435,9 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     if ((rc = cut(items1, cost1, nt1, ctx->sm_count * P1_G[0], 12, ctx->part1_doubles, &sp->workers1))) return rc;
     if ((rc = skip_upload(&sp->d_items1, items1)) || (rc = skip_upload(&sp->d_w1start, ws)) ||
         (rc = skip_upload(&sp->d_w1first, wf)) || (rc = skip_upload(&sp->d_slots1, sl))) return rc;
+    if ((rc = cut(items1s, cost1s, nt1, ctx->sm_count * P1_G[0], 12, ctx->part1_doubles, &sp->workers1s))) return rc;
+    if ((rc = skip_upload(&sp->d_items1s, items1s)) || (rc = skip_upload(&sp->d_w1sstart, ws)) ||
+        (rc = skip_upload(&sp->d_w1sfirst, wf)) || (rc = skip_upload(&sp->d_slots1s, sl))) return rc;
     if ((rc = cut(items2, cost2, nt2, ctx->sm_count * P2_G[0], 2, ctx->part2_doubles, &sp->workers2))) return rc;
     if ((rc = skip_upload(&sp->d_items2, items2)) || (rc = skip_upload(&sp->d_w2start, ws)) ||
         (rc = skip_upload(&sp->d_w2first, wf)) || (rc = skip_upload(&sp->d_slots2, sl))) return rc;
@@ -443,6 +455,10 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
                       double* hess_theta_diag, double* hess_hyper, cudaStream_t st) {
     const SkipPlan& sp = *ctx->skip;
     const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2 : ((want & HAWKES_WANT_GRAD_HYPER) ? 1 : 0);
+    // background-sum cache of hawkes_hmc_run (LEVEL 0 only, record order of this plan): 1 = store, 2 = use; with the
+    // cached sums pass 1 walks the list of the self-excitation items alone
+    const int bg_mode = level1 == 0 ? ctx->bg_mode : 0;
+    const bool s_only = bg_mode == 2;
     const int64_t ld = round_up(n, 256);
     const int nblk = (int)((n + RED_T - 1) / RED_T);
     CK(cudaMemsetAsync(ctx->d_status, 0, 2 * sizeof(unsigned), st));
@@ -452,25 +468,39 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
     s1.tile = NT * P1_R;
     s1.n_tiles = (int)((n + s1.tile - 1) / s1.tile);
     s1.chunk = 1;
-    s1.slot_tab = sp.d_slots1;
+    s1.slot_tab = s_only ? sp.d_slots1s : sp.d_slots1;
+    const int2* items1 = s_only ? sp.d_items1s : sp.d_items1;
+    const int* w1start = s_only ? sp.d_w1sstart : sp.d_w1start;
+    const int* w1first = s_only ? sp.d_w1sfirst : sp.d_w1first;
+    const int workers1 = s_only ? sp.workers1s : sp.workers1;
     constexpr int G1 = P1_G[0];
     constexpr unsigned SM1 = smem_request(G1 * group_buf_bytes<DIM3>());
-    const unsigned g1 = (unsigned)((sp.workers1 + G1 - 1) / G1);
+    const unsigned g1 = (unsigned)((workers1 + G1 - 1) / G1);
 #define SKIP_PASS1(L)                                                                                                     \
     pass1_list_kernel<P1_R, L, DIM3, G1><<<g1, NT * G1, SM1, st>>>(ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_part1,       \
-                                                                   sp.d_items1, sp.d_w1start, sp.d_w1first, sp.workers1); \
+                                                                   items1, w1start, w1first, workers1);                   \
     reduce1_kernel<L, DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, ctx->d_part1, s1, ctx->d_lam, ctx->d_trec,      \
                                                     ctx->d_trec2, nullptr, ctx->d_blockpart, ctx->d_status,               \
-                                                    ctx->d_bgcache, 0, nullptr, 0, NT * P1_R, sp.d_tn)
+                                                    ctx->d_bgcache, bg_mode, nullptr, 0, NT * P1_R, sp.d_tn)
     if (level1 == 0) { SKIP_PASS1(0); }
     else if (level1 == 1) { SKIP_PASS1(1); }
     else { SKIP_PASS1(2); }
 #undef SKIP_PASS1
     ctx->launches += 3;
-    if (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) {
-        scalars_kernel<<<1, SCAL_T, 0, st>>>(ctx->d_blockpart, nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
+    // as in the dense path: the single-CTA scalar reduction runs on the side stream beside pass 2 when there is one
+    const bool want_scal = (want & (HAWKES_WANT_LL | HAWKES_WANT_GRAD_HYPER | HAWKES_WANT_HESS_HYPER)) != 0;
+    const bool scal_aside = want_scal && (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) != 0;
+    if (want_scal) {
+        cudaStream_t ss = st;
+        if (scal_aside) {
+            CK(cudaEventRecord(ctx->ev_fork, st));
+            CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+            ss = ctx->side;
+        }
+        scalars_kernel<<<1, SCAL_T, 0, ss>>>(ctx->d_blockpart, nblk, c, (want & HAWKES_WANT_LL) ? ll : nullptr,
                                              (want & HAWKES_WANT_GRAD_HYPER) ? grad_hyper : nullptr,
                                              (want & HAWKES_WANT_HESS_HYPER) ? hess_hyper : nullptr, ctx->d_scal);
+        if (scal_aside) CK(cudaEventRecord(ctx->ev_join, ctx->side));
         ctx->launches++;
     }
     if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
@@ -496,6 +526,7 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
                                                    sp.d_perm);
         ctx->launches++;
     }
+    if (scal_aside) CK(cudaStreamWaitEvent(st, ctx->ev_join, 0));
     CK(cudaGetLastError());
     return HAWKES_OK;
 }

@@ -24,7 +24,8 @@ def dev(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
 
 
-@pytest.mark.parametrize("cache_bg,with_prior_prec", [(0, False), (1, False), (1, True), (2, False), (2, True)])
+@pytest.mark.parametrize("cache_bg,with_prior_prec", [(0, False), (1, False), (1, True), (2, False), (2, True),
+                                                      (3, False), (4, False), (4, True)])
 def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     """1,500 events, 90 sequenced; 6 iterations x 5 leapfrog steps, preconditioner refreshed every 3 iterations.
     Tolerance: the state after 30 leapfrog steps inherits the 1e-10 bar of the gradient through a mildly expanding
@@ -56,6 +57,13 @@ def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     pp_d = tr.precision_diag(s2, tau0) if with_prior_prec else None
     if with_prior_prec:
         assert np.max(np.abs(pp_d.cpu().numpy() - pp) / pp) <= 1e-10
+    if cache_bg >= 3:     # variants 0 / 1 over the work lists of hawkes_skip_plan (exact zeros left out)
+        with pytest.raises(hp.HawkesError):
+            ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z.clone(), beta, ev.params, s2, tau0,
+                        n_iter=1, n_leapfrog=1, step=eps, precond_every=0, mass=mass.clone(), mass_floor=floor,
+                        normals=dev(torch, normals[:1]), uniforms=dev(torch, uniforms[:1]), cache_background=cache_bg)
+        stats = ctx.skip_plan(dev(torch, ev.x), dev(torch, ev.t), ev.params)
+        assert stats["items_excitation"] < stats["items_dense_pass1"]
     trace = ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z, beta, ev.params, s2, tau0,
                         n_iter=n_iter, n_leapfrog=L, step=eps, precond_every=every, mass=mass, mass_floor=floor,
                         normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=cache_bg,

@@ -197,6 +197,19 @@ def posterior_case(torch, ev, tree, z, s2, tau0, beta=0.0):
     out_b = ctx.posterior_z(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), dev(torch, z), beta, ev.params, s2,
                             tau0, hess=True)
     assert all(np.array_equal(a.cpu().numpy(), b) for a, b in zip(out_b, (out3, gz, hz)))
+    # hawkes_posterior_z_skip: the same posterior over the work lists of hawkes_skip_plan, against the same oracle values
+    with pytest.raises(hp.HawkesError):
+        ctx.posterior_z(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), dev(torch, z), beta, ev.params, s2, tau0,
+                        hess=True, skip=True)
+    ctx.skip_plan(dev(torch, ev.x), dev(torch, ev.t), ev.params)
+    out_s = ctx.posterior_z(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), dev(torch, z), beta, ev.params, s2,
+                            tau0, hess=True, skip=True)
+    assert ctx.last_status() == 0
+    o3s, gzs, hzs = (o.cpu().numpy() for o in out_s)
+    check("ell (skip)", o3s[0], ref.ll, ll_scale)
+    check("log posterior (skip)", o3s[2], ref.ll + lp_o, ll_scale + lps)
+    check("grad_z (skip)", gzs, gz_o + pg_o, gscale + pgs)
+    check("hess_z (skip)", hzs, hz_o, th_o[idx] ** 2 * np.abs(ref.hess_theta_diag[idx]) + gscale)
 
 
 def test_posterior_z_small_problem(torch):
