@@ -461,7 +461,8 @@ def run_b200(args, ev, workload: str) -> dict:
             "speedup_over_dense": total_ms / float(sum(sms)), "plan_ms_host_once": plan_ms,
             "tile_pairs_visited": {"pass1_background": stats["items_background"] / stats["items_dense_pass1"],
                                    "pass1_excitation": stats["items_excitation"] / stats["items_dense_pass1"],
-                                   "pass2": stats["items_pass2"] / stats["items_dense_pass2"]},
+                                   "pass2": stats["items_pass2"] / stats["items_dense_pass2"],
+                                   "pass1_background_unordered_items": stats["items_background_unordered"]},
             "max_rel_diff_vs_dense": {"ll": abs(sout.ll.item() - ll_dev) / abs(ll_dev),
                                       "grad_theta": float((g_s - g_d).abs().max() / g_d.abs().max()),
                                       "grad_hyper": float((sout.grad_hyper - out.grad_hyper).abs().max()

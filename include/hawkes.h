@@ -177,8 +177,9 @@ int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
  *   hawkes_eval, without the cross block (`want` bits 0..4).  HAWKES_ERR_ARG if there is no plan or it was built
  *   for another n, other hyperparameters or another background mode; the caller guarantees x and t are the planned
  *   events.  HAWKES_ERR_UNSORTED is never raised here.
- * hawkes_skip_stats: out[0..6] = pass-1 items with a live background, with a live self-excitation, of the dense
- *   pass; pass-2 items, of the dense pass; workers of pass 1, of pass 2 (item = 256 records x 128 records).
+ * hawkes_skip_stats: out[0..7] = pass-1 items with a live background, with a live self-excitation, of the dense
+ *   pass; pass-2 items, of the dense pass; workers of pass 1, of pass 2 (item = 256 records x 128 records); items of
+ *   the background evaluated once per unordered pair (levels 0 and 1; 0 if that form is not in use).
  * hawkes_skip_perm: the tree order (record i is the caller's event perm[i]) into a HOST buffer of n int64. */
 int hawkes_skip_plan(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p);
 int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,

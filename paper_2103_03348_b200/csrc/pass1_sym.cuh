@@ -57,14 +57,15 @@ struct SoaIO {
 // MASKED: the pair (target gi[r], streamed event of global index jg0 + k) is evaluated iff k < nvalid and
 // jg0 + k < gi[r] (index order: each unordered pair once, no self pair) -- plus, always, the paper's indicators
 // (r2 != 0 for the background, dt > 0 for the excitation) and the underflow flush.
-template <int R, int LEVEL, bool MASKED, bool DIM3>
+// S_ON = false: background only (the list-driven pass of skip.cuh, where the excitation term has its own items).
+template <int R, int LEVEL, bool MASKED, bool DIM3, bool S_ON = true>
 __device__ __forceinline__ void p1s_block(const double* __restrict__ sb, int j0, int nvalid, int64_t jg0,
                                           const Ev<DIM3> (&g)[R], const int64_t (&gi)[R], Mom<LEVEL> (&m)[R],
                                           double* __restrict__ colout /* this warp's [TS][NB] */, const P1C& c,
                                           unsigned lane_base, int lane) {
     constexpr int NB = Mom<LEVEL>::NB;
     constexpr int TO = DIM3 ? 3 : 2;        // array index of t
-    constexpr int K = 2 * R;                // exponentials per step: background of the R pairs, then excitation
+    constexpr int K = S_ON ? 2 * R : R;     // exponentials per step: background of the R pairs, then excitation
     double cc[NB];
 #pragma unroll
     for (int k = 0; k < NB; ++k) cc[k] = 0.0;
@@ -79,7 +80,7 @@ __device__ __forceinline__ void p1s_block(const double* __restrict__ sb, int j0,
         // in vector registers: a Horner step would read three of them.  The K exponentials of a step are therefore
         // evaluated in lockstep, stage by stage, so that consecutive FP64 instructions share the constant (and negc)
         // in the same operand slot and hit the operand-reuse cache (2 fresh registers each: DESIGN.md section 5).
-        double u[R], w[R], dt[R], a[K], t[K], f[K], q[K];
+        double u[R], w[R], dt[R], a[2 * R], t[2 * R], f[2 * R], q[2 * R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const double dx = g[r].x - e.x, dy = g[r].y - e.y;
@@ -90,8 +91,10 @@ __device__ __forceinline__ void p1s_block(const double* __restrict__ sb, int j0,
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) a[r] = fma(c.rho_b, w[r], u[r]);
+        if (S_ON) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) a[R + r] = fma(c.rho_s, dt[r], u[r]);
+            for (int r = 0; r < R; ++r) a[R + r] = fma(c.rho_s, dt[r], u[r]);
+        }
 #pragma unroll
         for (int i = 0; i < K; ++i) t[i] = fma(a[i], i < R ? c.negcb : c.negcs, c.e.magic);
 #pragma unroll
@@ -108,26 +111,28 @@ __device__ __forceinline__ void p1s_block(const double* __restrict__ sb, int j0,
         for (int i = 0; i < K; ++i) q[i] = fma(q[i], f[i], c.e.d0);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            double eB, eS;
+            double eB, eS = 0.0;
             if (MASKED) {
                 const int live = (idx < nvalid && jg0 + idx < gi[r]) ? 1 : 0;
                 eB = exp2_table<4>(a[r], t[r], c.lim_b_hi, u[r], lane_base, live) * q[r];
-                eS = exp2_table<5>(a[R + r], t[R + r], c.lim_s_hi, dt[r], lane_base, live) * q[R + r];
+                if (S_ON) eS = exp2_table<5>(a[R + r], t[R + r], c.lim_s_hi, dt[r], lane_base, live) * q[R + r];
             } else {
                 eB = exp2_table<1>(a[r], t[r], c.lim_b_hi, u[r], lane_base) * q[r];
-                eS = exp2_table<0>(a[R + r], t[R + r], c.lim_s_hi, dt[r], lane_base) * q[R + r];
+                if (S_ON) eS = exp2_table<0>(a[R + r], t[R + r], c.lim_s_hi, dt[r], lane_base) * q[R + r];
             }
-            eS *= e.w;
+            if (S_ON) eS *= e.w;
             m[r].b[0] += eB;
             cc[0] += eB;
-            m[r].s[0] += eS;
+            if (S_ON) m[r].s[0] += eS;
             if (LEVEL == 1) {
                 m[r].b[1] = fma(eB, u[r], m[r].b[1]);
                 cc[1 % NB] = fma(eB, u[r], cc[1 % NB]);
                 m[r].b[2] = fma(eB, w[r], m[r].b[2]);
                 cc[2 % NB] = fma(eB, w[r], cc[2 % NB]);
-                m[r].s[1] = fma(eS, u[r], m[r].s[1]);
-                m[r].s[2] = fma(eS, dt[r], m[r].s[2]);
+                if (S_ON) {
+                    m[r].s[1] = fma(eS, u[r], m[r].s[1]);
+                    m[r].s[2] = fma(eS, dt[r], m[r].s[2]);
+                }
             }
         }
 #pragma unroll

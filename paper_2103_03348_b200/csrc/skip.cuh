@@ -73,14 +73,22 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_list_kernel(const double* __r
     const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
     const int w = blockIdx.x * G + grp;
     if (w >= n_workers) return;
-    const int k0 = wstart[w], k1 = wstart[w + 1];
-    if (k0 >= k1) return;
+    const int q0 = wstart[w], q1 = wstart[w + 1];   // in 32-record blocks, 4 per item
+    if (q0 >= q1) return;
+    const int k0 = q0 / 4, k1 = (q1 - 1) / 4 + 1;
     double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
     double* const sbuf1 = sbuf0 + TS * RS;
     const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
     const P1C pc = pinned_consts(smagic, c);
 
-    auto chunk_cnt = [&](int J) { return (int)min((int64_t)TS, n - (int64_t)J * TS); };
+    // the piece of item k this worker holds: streamed records [a, a + cnt)
+    auto piece = [&](int k, int y, int64_t* a, int* cnt) {
+        const int jb = k == q0 / 4 ? q0 % 4 : 0;
+        const int je = k == (q1 - 1) / 4 ? (q1 - 1) % 4 + 1 : 4;
+        const int64_t c0 = (int64_t)(y >> 2) * TS;
+        *a = c0 + jb * 32;
+        *cnt = (int)max(min(c0 + je * 32, n) - *a, (int64_t)0);
+    };
     Ev<DIM3> g[R];
     Mom<LEVEL> m[R];
     auto flush = [&](int I) {
@@ -101,7 +109,10 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_list_kernel(const double* __r
 
     RecIO<DIM3> io;
     int2 it = items[k0];
-    io.load(rec, (int64_t)(it.y >> 2) * TS, chunk_cnt(it.y >> 2), tid);
+    int64_t a, a2 = 0;
+    int cnt, cnt2 = 0;
+    piece(k0, it.y, &a, &cnt);
+    io.load(rec, a, cnt, tid);
     io.store(sbuf0, tid);
     group_sync(grp);
     int cur = 0, I = -1;
@@ -120,10 +131,10 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_list_kernel(const double* __r
         int2 nx = it;
         if (k + 1 < k1) {
             nx = items[k + 1];
-            io.load(rec, (int64_t)(nx.y >> 2) * TS, chunk_cnt(nx.y >> 2), tid);
+            piece(k + 1, nx.y, &a2, &cnt2);
+            io.load(rec, a2, cnt2, tid);
         }
         const double* sb = cur ? sbuf1 : sbuf0;
-        const int cnt = chunk_cnt(it.y >> 2);
         const int kind = it.y & 3;
         if (kind == SK_B) p1_tile<R, LEVEL, 0, DIM3, true>(sb, cnt, g, m, pc, lane_base);
         else if (kind == SK_S) p1_tile<R, LEVEL, 2, DIM3, false>(sb, cnt, g, m, pc, lane_base);
@@ -132,6 +143,8 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_list_kernel(const double* __r
         group_sync(grp);
         cur ^= 1;
         it = nx;
+        a = a2;
+        cnt = cnt2;
     }
     flush(I);
 }
@@ -158,14 +171,21 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_list_kernel(const double* __r
     const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
     const int w = blockIdx.x * G + grp;
     if (w >= n_workers) return;
-    const int k0 = wstart[w], k1 = wstart[w + 1];
-    if (k0 >= k1) return;
+    const int q0 = wstart[w], q1 = wstart[w + 1];   // in 32-record blocks, 4 per item
+    if (q0 >= q1) return;
+    const int k0 = q0 / 4, k1 = (q1 - 1) / 4 + 1;
     double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
     double* const sbuf1 = sbuf0 + TS * RS;
     const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
     const P1C pc = pinned_consts(smagic, c);
 
-    auto chunk_cnt = [&](int J) { return (int)min((int64_t)TS, n - (int64_t)J * TS); };
+    auto piece = [&](int k, int y, int64_t* a, int* cnt) {
+        const int jb = k == q0 / 4 ? q0 % 4 : 0;
+        const int je = k == (q1 - 1) / 4 ? (q1 - 1) % 4 + 1 : 4;
+        const int64_t c0 = (int64_t)(y >> 2) * TS;
+        *a = c0 + jb * 32;
+        *cnt = (int)max(min(c0 + je * 32, n) - *a, (int64_t)0);
+    };
     Ev<DIM3> g[R];
     double cm[R], dm[R];
     auto flush = [&](int M) {
@@ -182,7 +202,10 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_list_kernel(const double* __r
 
     RecIO<DIM3> io;
     int2 it = items[k0];
-    io.load(trec, (int64_t)(it.y >> 2) * TS, chunk_cnt(it.y >> 2), tid);
+    int64_t a, a2 = 0;
+    int cnt, cnt2 = 0;
+    piece(k0, it.y, &a, &cnt);
+    io.load(trec, a, cnt, tid);
     io.store(sbuf0, tid);
     group_sync(grp);
     int cur = 0, M = -1;
@@ -201,15 +224,153 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_list_kernel(const double* __r
         int2 nx = it;
         if (k + 1 < k1) {
             nx = items[k + 1];
-            io.load(trec, (int64_t)(nx.y >> 2) * TS, chunk_cnt(nx.y >> 2), tid);
+            piece(k + 1, nx.y, &a2, &cnt2);
+            io.load(trec, a2, cnt2, tid);
         }
-        p2_tile<R, LEVEL, true, DIM3>(cur ? sbuf1 : sbuf0, chunk_cnt(it.y >> 2), g, cm, dm, pc, lane_base);
+        p2_tile<R, LEVEL, true, DIM3>(cur ? sbuf1 : sbuf0, cnt, g, cm, dm, pc, lane_base);
         if (k + 1 < k1) io.store(cur ? sbuf0 : sbuf1, tid);
         group_sync(grp);
         cur ^= 1;
         it = nx;
+        a = a2;
+        cnt = cnt2;
     }
     flush(M);
+}
+
+
+// a1, background term over a list, once per UNORDERED pair (pass1_sym.cuh: row sums in registers, column sums in an
+// accumulator that rotates through the warp).  items[k] = (target tile I, source chunk J) with J <= the last chunk of
+// tile I: the pairs (target i of I, source j of J, j < i).  Work is cut in units of 32-source blocks (4 per item):
+// worker w takes the blocks [wstart[w], wstart[w+1]) of the flattened (item, block) sequence; a column partial
+// (tile I, source j) is written by the one worker that holds j's block, a row partial slot per worker as elsewhere.
+// The excitation sums of the slot are written as zeros (the S items have their own slots, after these).
+template <int R, int LEVEL, bool DIM3, int G>
+__global__ void __launch_bounds__(NT * G, 1) pass1_symb_list_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
+                                                                    DevConsts c, const double* __restrict__ tab_g,
+                                                                    double* __restrict__ part, double* __restrict__ partc,
+                                                                    int n_tiles, const int2* __restrict__ items,
+                                                                    const int* __restrict__ wstart,
+                                                                    const int* __restrict__ wfirst, int n_workers) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    constexpr int NB = Mom<LEVEL>::NB;
+    constexpr int NA = SoaIO<DIM3>::NA;
+    constexpr unsigned GB = sym_group_bytes<DIM3>(NB);
+    static_assert(smem_request(G * GB) <= SMEM_MAX, "table + group buffers must fit shared memory");
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ P1C spc;
+    const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem);
+    const SmemPlan plan = smem_plan(smem_base, G * GB);
+    fill_table(reinterpret_cast<double*>(smem + plan.tab_off), tab_g);
+    if (threadIdx.x == 0)
+        spc = P1C{c.negcb, c.negcs, c.rho_b, c.rho_s, c.lim_b_hi, c.lim_s_hi, {c.d0, c.d1, c.d2, c.d3, MAGIC}};
+    __syncthreads();
+
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT, lane = threadIdx.x & 31, wrp = tid >> 5;
+    const int w = blockIdx.x * G + grp;
+    if (w >= n_workers) return;
+    const int q0 = wstart[w], q1 = wstart[w + 1];
+    if (q0 >= q1) return;
+    double* const gbuf = reinterpret_cast<double*>(smem + plan.buf_off + grp * GB);
+    double* const sbuf0 = gbuf;
+    double* const sbuf1 = gbuf + NA * TS;
+    double* const colacc = gbuf + 2 * NA * TS;            // [NT/32][TS][NB]
+    double* const mycol = colacc + wrp * TS * NB;
+    const unsigned lane_base = (smem_base + plan.tab_off) | (8u * lane);
+    P1C pc;
+    {
+        const volatile P1C& v = spc;
+        pc.negcb = v.negcb; pc.negcs = v.negcs; pc.rho_b = v.rho_b; pc.rho_s = v.rho_s;
+        pc.lim_b_hi = v.lim_b_hi; pc.lim_s_hi = v.lim_s_hi;
+        pc.e.d0 = v.e.d0; pc.e.d1 = v.e.d1; pc.e.d2 = v.e.d2; pc.e.d3 = v.e.d3; pc.e.magic = v.e.magic;
+    }
+
+    Ev<DIM3> g[R];
+    int64_t gi[R];
+    Mom<LEVEL> m[R];
+    auto flush = [&](int I) {
+        const int slot = w - wfirst[I];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = (int64_t)I * (NT * R) + r * NT + tid;
+            if (i < n) {
+                double* o = part + (int64_t)slot * (2 * NB) * ld + i;
+#pragma unroll
+                for (int k = 0; k < NB; ++k) {
+                    o[(int64_t)k * ld] = m[r].b[k];
+                    o[(int64_t)(NB + k) * ld] = 0.0;
+                }
+            }
+        }
+    };
+    // the piece of item k this worker holds: source records [a, a + cnt)
+    auto piece = [&](int k, int64_t* a, int* cnt) {
+        const int jb = k == q0 / 4 ? q0 % 4 : 0;
+        const int je = k == (q1 - 1) / 4 ? (q1 - 1) % 4 + 1 : 4;
+        const int64_t c0 = (int64_t)items[k].y * TS;
+        *a = c0 + jb * 32;
+        const int64_t e = min(c0 + je * 32, n);
+        *cnt = (int)max(e - *a, (int64_t)0);
+    };
+
+    SoaIO<DIM3> io;
+    const int k_first = q0 / 4, k_last = (q1 - 1) / 4;
+    int64_t a, a2 = 0;
+    int cnt, cnt2 = 0;
+    piece(k_first, &a, &cnt);
+    io.load(rec, a, cnt, tid);
+    io.store(sbuf0, tid);
+    group_sync(grp);
+    int cur = 0, I = -1;
+    bool ragged_tile = false;
+    for (int k = k_first; k <= k_last; ++k) {
+        const int It = items[k].x;
+        if (It != I) {
+            if (I >= 0) flush(I);
+            I = It;
+            const int64_t i0 = (int64_t)I * (NT * R);
+            ragged_tile = n - i0 < NT * R;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int64_t i = i0 + r * NT + tid;
+                gi[r] = i < n ? i : -1;
+                g[r] = read_rec<DIM3>(rec + min(i, n - 1) * RS);
+#pragma unroll
+                for (int q = 0; q < NB; ++q) { m[r].b[q] = 0.0; m[r].s[q] = 0.0; }
+            }
+        }
+        if (k < k_last) {
+            piece(k + 1, &a2, &cnt2);
+            io.load(rec, a2, cnt2, tid);
+        }
+        const double* sb = cur ? sbuf1 : sbuf0;
+        const bool plain = !ragged_tile && a + cnt <= (int64_t)I * (NT * R);   // every source index below every target's
+        for (int j0 = 0; j0 < cnt; j0 += 32) {
+            const int nvalid = min(32, cnt - j0);
+            if (plain && nvalid == 32)
+                p1s_block<R, LEVEL, false, DIM3, false>(sb, j0, nvalid, a + j0, g, gi, m, mycol, pc, lane_base, lane);
+            else
+                p1s_block<R, LEVEL, true, DIM3, false>(sb, j0, nvalid, a + j0, g, gi, m, mycol, pc, lane_base, lane);
+        }
+        if (k < k_last) io.store(cur ? sbuf0 : sbuf1, tid);
+        group_sync(grp);
+        if (tid < cnt) {   // column sums of this piece: the four warps' shares in warp order, one source per thread
+            const int64_t j = a + tid;
+            const int sl = I - (int)(j / (NT * R));
+#pragma unroll
+            for (int q = 0; q < NB; ++q) {
+                double v = 0.0;
+#pragma unroll
+                for (int ww = 0; ww < NT / 32; ++ww) v += colacc[(ww * TS + tid) * NB + q];
+                partc[colpart_index(n_tiles, NT * R, NB, sl, q, j)] = v;
+            }
+        }
+        group_sync(grp);
+        cur ^= 1;
+        a = a2;
+        cnt = cnt2;
+    }
+    flush(I);
 }
 
 }  // namespace
@@ -232,6 +393,20 @@ struct SkipPlan {
     int* d_w1sfirst;
     int* d_slots1s;
     int workers1s;
+    // symmetric background (levels 0 and 1): unordered (tile, chunk) items cut in 32-source blocks, the S items after
+    // them in every tile's slots, and the plan's own column partials (zero wherever no item writes)
+    int2* d_itemsb;
+    int* d_wbstart;
+    int* d_wbfirst;
+    int* d_w1sfirst_sym;
+    int* d_slots_sym;
+    int workersb;
+    double* d_partc;
+    size_t partc_doubles;
+    double* d_part_sym;    // row partials of that form: the late tiles of the unordered enumeration take more slots
+                           // than the context's buffer is sized for
+    int partc_level;       // NB layout the buffer currently holds (-1: freshly zeroed)
+    int64_t items_bsym;
     int2* d_items2;        // pass-2 work list and its cut
     int* d_w2start;
     int* d_w2first;
@@ -247,7 +422,8 @@ void skip_plan_free(hawkes_ctx* c) {
     SkipPlan* s = c->skip;
     if (!s) return;
     void* ptrs[] = {s->d_perm, s->d_tn, s->d_items1, s->d_w1start, s->d_w1first, s->d_slots1,
-                    s->d_items1s, s->d_w1sstart, s->d_w1sfirst, s->d_slots1s, s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
+                    s->d_items1s, s->d_w1sstart, s->d_w1sfirst, s->d_slots1s, s->d_itemsb, s->d_wbstart, s->d_wbfirst,
+                    s->d_w1sfirst_sym, s->d_slots_sym, s->d_partc, s->d_part_sym, s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     delete s;
@@ -258,12 +434,14 @@ struct SkipBox {           // bounding box of a run of records: up to 3 coordina
     double lo[4], hi[4];
 };
 
-// Cut a list (sorted by tile) into at most `workers` non-empty consecutive ranges of about equal cost; fills
-// wstart (workers + 1 entries), wfirst and slots (per tile).  Returns the number of workers used.
+// Cut a list (sorted by tile) into at most `workers` non-empty consecutive ranges of about equal cost.  The unit
+// of the cut is a block of 32 streamed records, 4 per item (cost[k] is the cost of one block of item k): wstart
+// (workers + 1 entries) is in blocks of the flattened (item, block) sequence; wfirst and slots are per tile.
+// Returns the number of workers used.
 int skip_cut(const std::vector<int2>& items, const std::vector<int>& cost, int n_tiles, int workers,
              std::vector<int>* wstart, std::vector<int>* wfirst, std::vector<int>* slots) {
     int64_t total = 0;
-    for (int v : cost) total += v;
+    for (int v : cost) total += 4 * (int64_t)v;
     const int64_t chunk = (total + workers - 1) / workers;
     wstart->assign(1, 0);
     wfirst->assign(n_tiles, 0);
@@ -271,17 +449,18 @@ int skip_cut(const std::vector<int2>& items, const std::vector<int>& cost, int n
     std::vector<int> wlast(n_tiles, -1);
     int64_t acc = 0;
     int w = 0;
-    for (size_t k = 0; k < items.size(); ++k) {
-        const int I = items[k].x;
+    const size_t nblocks = 4 * items.size();
+    for (size_t q = 0; q < nblocks; ++q) {
+        const int I = items[q / 4].x;
         if (wlast[I] < 0) (*wfirst)[I] = w;
         wlast[I] = w;
-        acc += cost[k];
-        if (acc >= (int64_t)(w + 1) * chunk && k + 1 < items.size()) {
+        acc += cost[q / 4];
+        if (acc >= (int64_t)(w + 1) * chunk && q + 1 < nblocks) {
             ++w;
-            wstart->push_back((int)k + 1);
+            wstart->push_back((int)q + 1);
         }
     }
-    wstart->push_back((int)items.size());
+    wstart->push_back((int)nblocks);
     for (int I = 0; I < n_tiles; ++I) (*slots)[I] = wlast[I] < 0 ? 0 : wlast[I] - (*wfirst)[I] + 1;
     return (int)wstart->size() - 1;
 }
@@ -438,6 +617,50 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     if ((rc = cut(items1s, cost1s, nt1, ctx->sm_count * P1_G[0], 12, ctx->part1_doubles, &sp->workers1s))) return rc;
     if ((rc = skip_upload(&sp->d_items1s, items1s)) || (rc = skip_upload(&sp->d_w1sstart, ws)) ||
         (rc = skip_upload(&sp->d_w1sfirst, wf)) || (rc = skip_upload(&sp->d_slots1s, sl))) return rc;
+    {   // symmetric background: off unless it fits (HAWKES_DENSE_PASS1=1 switches it off as in the dense path)
+        const std::vector<int> wf_s = wf, sl_s = sl;          // cut of the S items, just made
+        std::vector<int2> itemsb;
+        for (int I = 0; I < nt1; ++I)
+            for (int J = 0; J < nc && (int64_t)J * TS < std::min(n, (int64_t)(I + 1) * NT * P1_R); ++J)
+                if (live_b(tile1[I], chunk[J])) itemsb.push_back(make_int2(I, J));
+        sp->items_bsym = (int64_t)itemsb.size();
+        const int64_t Q = 4 * (int64_t)itemsb.size();
+        const int W = (int)std::min<int64_t>(ctx->sm_count * P1_G[0], Q);
+        std::vector<int> wb(W + 1), wbf(nt1, 0), slb(nt1, 0), wbl(nt1, -1);
+        for (int w = 0; w <= W; ++w) wb[w] = (int)(Q * w / W);
+        for (int w = 0; w < W; ++w)
+            for (int k = wb[w] / 4; k <= (wb[w + 1] - 1) / 4 && wb[w] < wb[w + 1]; ++k) {
+                const int I = itemsb[k].x;
+                if (wbl[I] < 0) wbf[I] = w;
+                wbl[I] = w;
+            }
+        int worst = 0;
+        std::vector<int> wfs_sym(nt1), sl_sym(nt1);
+        for (int I = 0; I < nt1; ++I) {
+            slb[I] = wbl[I] < 0 ? 0 : wbl[I] - wbf[I] + 1;
+            wfs_sym[I] = wf_s[I] - slb[I];
+            sl_sym[I] = slb[I] + sl_s[I];
+            worst = std::max(worst, sl_sym[I]);
+        }
+        const char* dense = getenv("HAWKES_DENSE_PASS1");
+        const size_t pcd = (size_t)colpart_doubles(nt1, NT * P1_R, 3);
+        const size_t prd = (size_t)worst * 12 * (size_t)ld;
+        if (!(dense && dense[0] == '1') && Q > 0 && Q < ((int64_t)1 << 31) && prd * sizeof(double) <= ((size_t)8 << 30) &&
+            pcd * sizeof(double) <= ((size_t)16 << 30) && cudaMalloc((void**)&sp->d_partc, pcd * sizeof(double)) == cudaSuccess &&
+            cudaMalloc((void**)&sp->d_part_sym, prd * sizeof(double)) == cudaSuccess) {
+            sp->partc_doubles = pcd;
+            sp->partc_level = -1;
+            sp->workersb = W;
+            CK(cudaMemset(sp->d_partc, 0, pcd * sizeof(double)));
+            if ((rc = skip_upload(&sp->d_itemsb, itemsb)) || (rc = skip_upload(&sp->d_wbstart, wb)) ||
+                (rc = skip_upload(&sp->d_wbfirst, wbf)) || (rc = skip_upload(&sp->d_w1sfirst_sym, wfs_sym)) ||
+                (rc = skip_upload(&sp->d_slots_sym, sl_sym))) return rc;
+        } else {
+            cudaGetLastError();
+            if (sp->d_partc) cudaFree(sp->d_partc);
+            sp->d_partc = nullptr;
+        }
+    }
     if ((rc = cut(items2, cost2, nt2, ctx->sm_count * P2_G[0], 2, ctx->part2_doubles, &sp->workers2))) return rc;
     if ((rc = skip_upload(&sp->d_items2, items2)) || (rc = skip_upload(&sp->d_w2start, ws)) ||
         (rc = skip_upload(&sp->d_w2first, wf)) || (rc = skip_upload(&sp->d_slots2, sl))) return rc;
@@ -459,6 +682,7 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
     // cached sums pass 1 walks the list of the self-excitation items alone
     const int bg_mode = level1 == 0 ? ctx->bg_mode : 0;
     const bool s_only = bg_mode == 2;
+    const bool sym = !s_only && level1 <= 1 && sp.d_partc != nullptr;   // background once per unordered pair
     const int64_t ld = round_up(n, 256);
     const int nblk = (int)((n + RED_T - 1) / RED_T);
     CK(cudaMemsetAsync(ctx->d_status, 0, 2 * sizeof(unsigned), st));
@@ -468,20 +692,35 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
     s1.tile = NT * P1_R;
     s1.n_tiles = (int)((n + s1.tile - 1) / s1.tile);
     s1.chunk = 1;
-    s1.slot_tab = s_only ? sp.d_slots1s : sp.d_slots1;
-    const int2* items1 = s_only ? sp.d_items1s : sp.d_items1;
-    const int* w1start = s_only ? sp.d_w1sstart : sp.d_w1start;
-    const int* w1first = s_only ? sp.d_w1sfirst : sp.d_w1first;
-    const int workers1 = s_only ? sp.workers1s : sp.workers1;
+    s1.slot_tab = sym ? sp.d_slots_sym : (s_only ? sp.d_slots1s : sp.d_slots1);
+    const int2* items1 = (s_only || sym) ? sp.d_items1s : sp.d_items1;
+    const int* w1start = (s_only || sym) ? sp.d_w1sstart : sp.d_w1start;
+    const int* w1first = sym ? sp.d_w1sfirst_sym : (s_only ? sp.d_w1sfirst : sp.d_w1first);
+    const int workers1 = (s_only || sym) ? sp.workers1s : sp.workers1;
+    const int nb1 = level1 == 0 ? 1 : 3;
+    if (sym && ctx->skip->partc_level != nb1) {   // another moment layout: entries no item writes must read as zero
+        if (ctx->skip->partc_level != -1) CK(cudaMemsetAsync(sp.d_partc, 0, sp.partc_doubles * sizeof(double), st));
+        ctx->skip->partc_level = nb1;
+    }
+    const unsigned gb = (unsigned)((sp.workersb + P1_G[0] - 1) / P1_G[0]);
+    double* const part1 = sym ? sp.d_part_sym : ctx->d_part1;
     constexpr int G1 = P1_G[0];
     constexpr unsigned SM1 = smem_request(G1 * group_buf_bytes<DIM3>());
     const unsigned g1 = (unsigned)((workers1 + G1 - 1) / G1);
 #define SKIP_PASS1(L)                                                                                                     \
-    pass1_list_kernel<P1_R, L, DIM3, G1><<<g1, NT * G1, SM1, st>>>(ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_part1,       \
+    if (sym) {                                                                                                            \
+        pass1_symb_list_kernel<P1_R, (L) <= 1 ? (L) : 1, DIM3, G1>                                                        \
+            <<<gb, NT * G1, smem_request(G1 * sym_group_bytes<DIM3>((L) == 0 ? 1 : 3)), st>>>(                            \
+                ctx->d_rec, n, ld, c, ctx->d_tab, part1, sp.d_partc, s1.n_tiles, sp.d_itemsb, sp.d_wbstart,               \
+                sp.d_wbfirst, sp.workersb);                                                                               \
+        ctx->launches++;                                                                                                  \
+    }                                                                                                                     \
+    pass1_list_kernel<P1_R, L, DIM3, G1><<<g1, NT * G1, SM1, st>>>(ctx->d_rec, n, ld, c, ctx->d_tab, part1,              \
                                                                    items1, w1start, w1first, workers1);                   \
-    reduce1_kernel<L, DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, ctx->d_part1, s1, ctx->d_lam, ctx->d_trec,      \
+    reduce1_kernel<L, DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, part1, s1, ctx->d_lam, ctx->d_trec,             \
                                                     ctx->d_trec2, nullptr, ctx->d_blockpart, ctx->d_status,               \
-                                                    ctx->d_bgcache, bg_mode, nullptr, 0, NT * P1_R, sp.d_tn)
+                                                    ctx->d_bgcache, bg_mode, sym ? sp.d_partc : nullptr, s1.n_tiles,      \
+                                                    NT * P1_R, sp.d_tn)
     if (level1 == 0) { SKIP_PASS1(0); }
     else if (level1 == 1) { SKIP_PASS1(1); }
     else { SKIP_PASS1(2); }
@@ -540,6 +779,8 @@ int skip_setup_kernels() {
     if ((rc = setup_kernel(pass1_list_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], SM1, &dummy))) return rc;
     if ((rc = setup_kernel(pass1_list_kernel<P1_R, 1, DIM3, P1_G[0]>, P1_G[0], SM1, &dummy))) return rc;
     if ((rc = setup_kernel(pass1_list_kernel<P1_R, 2, DIM3, P1_G[0]>, P1_G[0], SM1, &dummy))) return rc;
+    if ((rc = setup_kernel(pass1_symb_list_kernel<P1_R, 0, DIM3, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * sym_group_bytes<DIM3>(1)), &dummy))) return rc;
+    if ((rc = setup_kernel(pass1_symb_list_kernel<P1_R, 1, DIM3, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * sym_group_bytes<DIM3>(3)), &dummy))) return rc;
     if ((rc = setup_kernel(pass2_list_kernel<P2_R, 0, DIM3, P2_G[0]>, P2_G[0], SM2, &dummy))) return rc;
     if ((rc = setup_kernel(pass2_list_kernel<P2_R, 1, DIM3, P2_G[0]>, P2_G[0], SM2, &dummy))) return rc;
     return HAWKES_OK;
@@ -587,14 +828,16 @@ int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* 
     return enqueue_eval_skip<false>(ctx, n, x, t, theta, c, want, ll, grad_theta, grad_hyper, hess_theta_diag, hess_hyper, (cudaStream_t)stream);
 }
 
-// out[0..5]: pass-1 items with a live background / with a live excitation / dense count; pass-2 items / dense count;
-// out[5] = workers of pass 1, out[6] = workers of pass 2 (an item = NT*R records x TS records)
+// out[0..4]: pass-1 items with a live background / with a live excitation / dense count; pass-2 items / dense count;
+// out[5] = workers of pass 1, out[6] = workers of pass 2 (an item = NT*R records x TS records); out[7] = unordered
+// background items of the symmetric form (0: not in use)
 int hawkes_skip_stats(hawkes_ctx* ctx, int64_t* out) {
     if (!ctx || !out || !ctx->skip) return HAWKES_ERR_ARG;
     const SkipPlan* sp = ctx->skip;
     out[0] = sp->items_b; out[1] = sp->items_s; out[2] = sp->items_dense1;
     out[3] = sp->items_p2; out[4] = sp->items_dense2;
     out[5] = sp->workers1; out[6] = sp->workers2;
+    out[7] = sp->d_partc ? sp->items_bsym : 0;
     return HAWKES_OK;
 }
 
