@@ -170,16 +170,19 @@ int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
  *   order (time-sorted input is not required by this variant).  Synchronous: copies the events to the host, builds
  *   the plan there (O(n log n) + one box test per tile pair) and uploads it; the context owns it until the next
  *   hawkes_skip_plan or hawkes_destroy.  The plan depends on the events, the hyperparameters and the background mode
- *   -- not on theta -- so one plan serves every evaluation of an HMC trajectory.
+ *   -- not on theta -- so one plan serves every evaluation of an HMC trajectory.  Planning the same events again for
+ *   other hyperparameters (what an MCMC sweep does between HMC updates) keeps the order and the boxes as long as
+ *   every cut-off radius stays within a factor 2 of the one the order was built for, and rebuilds only the lists.
  *   Errors: HAWKES_ERR_ARG, HAWKES_ERR_PARAM, HAWKES_ERR_NONFINITE (events), HAWKES_ERR_NOMEM, HAWKES_ERR_CUDA,
  *   HAWKES_ERR_UNSUPPORTED (work lists do not fit the context's partial buffers).
  * hawkes_eval_skip: arguments, outputs (in the caller's event order), stream semantics and device status as
  *   hawkes_eval, without the cross block (`want` bits 0..4).  HAWKES_ERR_ARG if there is no plan or it was built
  *   for another n, other hyperparameters or another background mode; the caller guarantees x and t are the planned
  *   events.  HAWKES_ERR_UNSORTED is never raised here.
- * hawkes_skip_stats: out[0..7] = pass-1 items with a live background, with a live self-excitation, of the dense
+ * hawkes_skip_stats: out[0..8] = pass-1 items with a live background, with a live self-excitation, of the dense
  *   pass; pass-2 items, of the dense pass; workers of pass 1, of pass 2 (item = 256 records x 128 records); items of
- *   the background evaluated once per unordered pair (levels 0 and 1; 0 if that form is not in use).
+ *   the background evaluated once per unordered pair (levels 0 and 1; 0 if that form is not in use); 1 if this plan
+ *   kept the previous plan's order and boxes (9 entries in all).
  * hawkes_skip_perm: the tree order (record i is the caller's event perm[i]) into a HOST buffer of n int64. */
 int hawkes_skip_plan(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p);
 int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,

@@ -127,13 +127,13 @@ class HawkesContext:
         rc = self._lib.hawkes_skip_plan(self._h, n, _ptr(x), _ptr(t), ctypes.byref(p))
         if rc != 0:
             raise HawkesError(rc, "hawkes_skip_plan")
-        st = (ctypes.c_int64 * 8)()
+        st = (ctypes.c_int64 * 9)()
         rc = self._lib.hawkes_skip_stats(self._h, st)
         if rc != 0:
             raise HawkesError(rc, "hawkes_skip_stats")
         return {"items_background": st[0], "items_excitation": st[1], "items_dense_pass1": st[2],
                 "items_pass2": st[3], "items_dense_pass2": st[4], "workers_pass1": st[5], "workers_pass2": st[6],
-                "items_background_unordered": st[7]}
+                "items_background_unordered": st[7], "order_reused": st[8]}
 
     def skip_perm(self, n: int):
         """The k-d order of the current plan: record i is the caller's event perm[i] (host int64 tensor)."""

@@ -403,6 +403,7 @@ struct SkipPlan {
     int workersb;
     double* d_partc;
     size_t partc_doubles;
+    size_t part_sym_doubles;
     double* d_part_sym;    // row partials of that form: the late tiles of the unordered enumeration take more slots
                            // than the context's buffer is sized for
     int partc_level;       // NB layout the buffer currently holds (-1: freshly zeroed)
@@ -414,6 +415,11 @@ struct SkipPlan {
     int workers2;
     // what the lists hold, for hawkes_skip_stats
     int64_t items_b, items_s, items_p2, items_dense1, items_dense2;
+    // host copy of the planned events, their order and boxes: a re-plan for other hyperparameters of the same events
+    // (an MCMC sweep changes them between HMC updates) keeps the order while the cut-off radii stay within a factor 2
+    // of those it was built for -- any order is valid, the boxes are exact for it -- and only rebuilds the lists
+    struct SkipHost* host;
+    int order_reused;
 };
 
 namespace {
@@ -426,6 +432,7 @@ void skip_plan_free(hawkes_ctx* c) {
                     s->d_w1sfirst_sym, s->d_slots_sym, s->d_partc, s->d_part_sym, s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
     for (void* q : ptrs)
         if (q) cudaFree(q);
+    delete s->host;
     delete s;
     c->skip = nullptr;
 }
@@ -433,6 +440,14 @@ void skip_plan_free(hawkes_ctx* c) {
 struct SkipBox {           // bounding box of a run of records: up to 3 coordinates, then time
     double lo[4], hi[4];
 };
+}  // namespace
+struct SkipHost {
+    std::vector<double> hx, ht;
+    std::vector<int64_t> perm;
+    std::vector<SkipBox> chunk, tile;
+    double cutoff[4];
+};
+namespace {
 
 // Cut a list (sorted by tile) into at most `workers` non-empty consecutive ranges of about equal cost.  The unit
 // of the cut is a block of 32 streamed records, 4 per item (cost[k] is the cost of one block of item k): wstart
@@ -474,9 +489,14 @@ int skip_upload(T** dst, const std::vector<T>& v) {
     return HAWKES_OK;
 }
 
-int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p) {
+int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const hawkes_params* p, SkipPlan* old) {
     const int dim = ctx->dim, nd = dim + 1;   // axes: coordinates, then time
-    std::vector<double> hx((size_t)dim * n), ht((size_t)n);
+    SkipHost* hs = new (std::nothrow) SkipHost();
+    if (!hs) return HAWKES_ERR_NOMEM;
+    struct Guard { SkipHost*& h; ~Guard() { delete h; } } guard{hs};   // owned here until the plan takes it
+    std::vector<double>&hx = hs->hx, &ht = hs->ht;
+    hx.resize((size_t)dim * n);
+    ht.resize((size_t)n);
     CK(cudaMemcpy(hx.data(), x, sizeof(double) * dim * n, cudaMemcpyDefault));
     CK(cudaMemcpy(ht.data(), t, sizeof(double) * n, cudaMemcpyDefault));
     for (int64_t i = 0; i < n; ++i)
@@ -492,11 +512,25 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     // k-d order: split the events at a median of the axis along which they reach furthest in units of the cut-off
     // radius, the left part a whole number of tiles (of chunks, inside a tile), until every part is one chunk.
     // Tiles and chunks are then the leaves of the tree: compact boxes that end where the runs end.
-    double cutoff[4];
+    double cutoff[4] = {0, 0, 0, 0};
     for (int a = 0; a < nd; ++a) cutoff[a] = a < dim ? std::min(rs, rb) : std::min(ts_, tb);
-    std::vector<int64_t> perm((size_t)n);
-    for (int64_t i = 0; i < n; ++i) perm[i] = i;
-    {
+    bool reuse = old && old->host && old->n == n && old->host->hx.size() == hx.size() &&
+                 std::memcmp(old->host->hx.data(), hx.data(), hx.size() * sizeof(double)) == 0 &&
+                 std::memcmp(old->host->ht.data(), ht.data(), ht.size() * sizeof(double)) == 0;
+    for (int a = 0; a < nd && reuse; ++a) {
+        const double r = cutoff[a] / old->host->cutoff[a];
+        if (!(r >= 0.5 && r <= 2.0) && !(std::isinf(cutoff[a]) && std::isinf(old->host->cutoff[a]))) reuse = false;
+    }
+    std::vector<int64_t>& perm = hs->perm;
+    if (reuse) {
+        perm.swap(old->host->perm);
+        hs->chunk.swap(old->host->chunk);
+        hs->tile.swap(old->host->tile);
+        for (int a = 0; a < 4; ++a) hs->cutoff[a] = old->host->cutoff[a];
+    } else {
+        for (int a = 0; a < 4; ++a) hs->cutoff[a] = cutoff[a];
+        perm.resize((size_t)n);
+        for (int64_t i = 0; i < n; ++i) perm[i] = i;
         const int64_t tile = NT * P1_R;
         static_assert(NT * P1_R == NT * P2_R && (NT * P1_R) % TS == 0, "tiles of both passes are whole chunks");
         std::vector<std::pair<int64_t, int64_t>> stack(1, {0, n});
@@ -539,7 +573,11 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
         }
         return bx;
     };
-    const std::vector<SkipBox> chunk = boxes(TS), tile1 = boxes(NT * P1_R), tile2 = boxes(NT * P2_R);
+    if (!reuse) {
+        hs->chunk = boxes(TS);
+        hs->tile = boxes(NT * P1_R);
+    }
+    const std::vector<SkipBox>&chunk = hs->chunk, &tile1 = hs->tile, &tile2 = hs->tile;
     auto gap2 = [&](const SkipBox& A, const SkipBox& B) {   // squared distance between the spatial boxes
         double s = 0.0;
         for (int a = 0; a < dim; ++a) {
@@ -568,6 +606,9 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     if (!sp) return HAWKES_ERR_NOMEM;
     std::memset(sp, 0, sizeof(*sp));
     ctx->skip = sp;
+    sp->host = hs;
+    hs = nullptr;          // the plan owns it now (freed by skip_plan_free)
+    sp->order_reused = reuse ? 1 : 0;
     sp->n = n;
     sp->p = *p;
     sp->s_mode = ctx->s_mode;
@@ -645,13 +686,24 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
         const char* dense = getenv("HAWKES_DENSE_PASS1");
         const size_t pcd = (size_t)colpart_doubles(nt1, NT * P1_R, 3);
         const size_t prd = (size_t)worst * 12 * (size_t)ld;
+        // the two large buffers of the previous plan are taken over when they are large enough
+        if (old && old->d_partc && old->partc_doubles >= pcd) {
+            sp->d_partc = old->d_partc; sp->partc_doubles = old->partc_doubles;
+            old->d_partc = nullptr;
+        }
+        if (old && old->d_part_sym && old->part_sym_doubles >= prd) {
+            sp->d_part_sym = old->d_part_sym; sp->part_sym_doubles = old->part_sym_doubles;
+            old->d_part_sym = nullptr;
+        }
         if (!(dense && dense[0] == '1') && Q > 0 && Q < ((int64_t)1 << 31) && prd * sizeof(double) <= ((size_t)8 << 30) &&
-            pcd * sizeof(double) <= ((size_t)16 << 30) && cudaMalloc((void**)&sp->d_partc, pcd * sizeof(double)) == cudaSuccess &&
-            cudaMalloc((void**)&sp->d_part_sym, prd * sizeof(double)) == cudaSuccess) {
-            sp->partc_doubles = pcd;
+            pcd * sizeof(double) <= ((size_t)16 << 30) &&
+            (sp->d_partc || cudaMalloc((void**)&sp->d_partc, pcd * sizeof(double)) == cudaSuccess) &&
+            (sp->d_part_sym || cudaMalloc((void**)&sp->d_part_sym, prd * sizeof(double)) == cudaSuccess)) {
+            if (!sp->partc_doubles) sp->partc_doubles = pcd;
+            if (!sp->part_sym_doubles) sp->part_sym_doubles = prd;
             sp->partc_level = -1;
             sp->workersb = W;
-            CK(cudaMemset(sp->d_partc, 0, pcd * sizeof(double)));
+            CK(cudaMemset(sp->d_partc, 0, sp->partc_doubles * sizeof(double)));
             if ((rc = skip_upload(&sp->d_itemsb, itemsb)) || (rc = skip_upload(&sp->d_wbstart, wb)) ||
                 (rc = skip_upload(&sp->d_wbfirst, wbf)) || (rc = skip_upload(&sp->d_w1sfirst_sym, wfs_sym)) ||
                 (rc = skip_upload(&sp->d_slots_sym, sl_sym))) return rc;
@@ -798,10 +850,15 @@ int hawkes_skip_plan(hawkes_ctx* ctx, int64_t n, const double* x, const double* 
     if (rc) return rc;
     CK(cudaSetDevice(ctx->device));
     CK(cudaDeviceSynchronize());   // evaluations in flight may still read the old plan
-    skip_plan_free(ctx);
-    if ((rc = (ctx->dim == 3 ? skip_setup_kernels<true>() : skip_setup_kernels<false>()))) return rc;
-    rc = skip_build(ctx, n, x, t, p);
+    SkipPlan* old = ctx->skip;     // detached: the new plan may take over its order, boxes and large buffers
+    ctx->skip = nullptr;
+    if (!old && (rc = (ctx->dim == 3 ? skip_setup_kernels<true>() : skip_setup_kernels<false>()))) return rc;
+    rc = skip_build(ctx, n, x, t, p, old);
     if (rc) skip_plan_free(ctx);
+    SkipPlan* fresh = ctx->skip;
+    ctx->skip = old;
+    skip_plan_free(ctx);           // what is left of the old plan
+    ctx->skip = fresh;
     return rc;
 }
 
@@ -830,7 +887,7 @@ int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* 
 
 // out[0..4]: pass-1 items with a live background / with a live excitation / dense count; pass-2 items / dense count;
 // out[5] = workers of pass 1, out[6] = workers of pass 2 (an item = NT*R records x TS records); out[7] = unordered
-// background items of the symmetric form (0: not in use)
+// background items of the symmetric form (0: not in use); out[8] = 1 if the order of the previous plan was kept
 int hawkes_skip_stats(hawkes_ctx* ctx, int64_t* out) {
     if (!ctx || !out || !ctx->skip) return HAWKES_ERR_ARG;
     const SkipPlan* sp = ctx->skip;
@@ -838,6 +895,7 @@ int hawkes_skip_stats(hawkes_ctx* ctx, int64_t* out) {
     out[3] = sp->items_p2; out[4] = sp->items_dense2;
     out[5] = sp->workers1; out[6] = sp->workers2;
     out[7] = sp->d_partc ? sp->items_bsym : 0;
+    out[8] = sp->order_reused;
     return HAWKES_OK;
 }
 

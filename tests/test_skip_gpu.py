@@ -203,3 +203,32 @@ def test_skip_plan_is_checked(torch):
     ctx.skip_plan(x, t, other)               # re-planning replaces the plan
     ctx.eval_skip(x, t, th, other)
     assert ctx.last_status() == 0
+
+
+def test_skip_replan_keeps_order_for_nearby_hyperparameters(torch):
+    """An MCMC sweep re-plans the same events for new hyperparameters: the order and boxes are kept while the cut-off
+    radii stay within a factor 2, rebuilt otherwise or for other events; results match the oracle either way."""
+    ev = synth.config(0)
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda")
+    x, t, th = f(ev.x), f(ev.t), f(ev.theta)
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    assert ctx.skip_plan(x, t, ev.params)["order_reused"] == 0
+    perm0 = ctx.skip_perm(ev.n).numpy().copy()
+    near = (0.35, 12.0, 11.0, 0.6, 1.3, 0.4)
+    far = (0.35, 2.0, 11.0, 0.6, 0.2, 0.4)
+    for params, reused in ((near, 1), (far, 0), (far, 1)):
+        st = ctx.skip_plan(x, t, params)
+        assert st["order_reused"] == reused
+        if params is near:
+            assert np.array_equal(ctx.skip_perm(ev.n).numpy(), perm0)
+        ev.params = params
+        ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+        r = ctx.eval_skip(x, t, th, params, WANT)
+        assert ctx.last_status() == ref.status
+        if ref.status == 0:
+            lam = np.empty(ev.n)
+            lam[ctx.skip_perm(ev.n).numpy()] = ctx.get_lambda(ev.n).cpu().numpy()
+            compare(ev, ref, r, lam, r.grad_theta.cpu().numpy(), r.hess_theta_diag.cpu().numpy())
+    x2 = x.clone()
+    x2[0, 0] += 1.0
+    assert ctx.skip_plan(x2, t, far)["order_reused"] == 0        # other events: a fresh order
