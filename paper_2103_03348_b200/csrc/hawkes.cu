@@ -1229,6 +1229,8 @@ struct hawkes_ctx {
     double* d_partc;      // column partials of the symmetric pass 1 (NULL: symmetric path disabled)
     size_t partc_doubles;
     int plan_sym;
+    int reserve_sm;       // SMs the pairwise passes leave free (hawkes_posterior_z: the tree prior runs beside them)
+    int plan_reserve;
     int bg_mode;          // 0 normal, 1 store the cache, 2 use it (set by hawkes_hmc_run only)
     int s_mode;           // hawkes_set_background_mode
     int plan_bg;
@@ -1237,6 +1239,7 @@ struct hawkes_ctx {
     double* d_kmisc;      // its vectors and partials
     cudaStream_t side;    // small single-CTA kernels (scalars, tree prior) run here beside the big passes
     cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_fork2, ev_tree;   // hawkes_posterior_z_skip: tree prior on the side stream
     bool side_ready;
     size_t kmisc_doubles;
     double* d_hmc;        // hawkes_hmc_run scratch: z_prop, p, grad_cur, grad_prop, hess_z (n_max each) + 16
@@ -1376,15 +1379,17 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     // symmetric pass 1 (background once per unordered pair) for levels 0 and 1 unless the cached-background path runs
     const int sym = (ctx->d_partc != nullptr && level1 <= 1 && !no_bg) ? 1 : 0;
     if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2 || ctx->plan_bg != no_bg ||
-        ctx->plan_sym != sym) {
+        ctx->plan_sym != sym || ctx->plan_reserve != ctx->reserve_sm) {
+        const int sms = ctx->sm_count > ctx->reserve_sm ? ctx->sm_count - ctx->reserve_sm : 1;
+        ctx->plan_reserve = ctx->reserve_sm;
         Plan& q = ctx->plan;
         q.ld = round_up(n, 256);
         q.nblk = (int)((n + RED_T - 1) / RED_T);
         q.grid1 = plan_split(&q.sp1, n, NT * P1_R, (no_bg || sym) ? 0 : W_ALL[level1], W_HEAD[level1], 0,
-                             ctx->sm_count * ctx->occ1[level1], q.ld, 12, ctx->part1_doubles);
+                             sms * ctx->occ1[level1], q.ld, 12, ctx->part1_doubles);
         ctx->plan_bg = no_bg;
         ctx->plan_sym = sym;
-        q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, ctx->sm_count * ctx->occ2[level2], q.ld, 2,
+        q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, sms * ctx->occ2[level2], q.ld, 2,
                              ctx->part2_doubles);
         ctx->plan_n = n; ctx->plan_l1 = level1; ctx->plan_l2 = level2;
     }
@@ -1550,6 +1555,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->side_ready = false;
     c->plan_bg = -1;
     c->plan_sym = -1;
+    c->reserve_sm = 0;
+    c->plan_reserve = -1;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess ||
         (dim == 3 ? query_occupancy<true>(c) : query_occupancy<false>(c)) != HAWKES_OK) {
@@ -1607,7 +1614,9 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     }
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork2, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_tree, cudaEventDisableTiming) != cudaSuccess) {
         hawkes_destroy(c);
         cudaGetLastError();
         return HAWKES_ERR_CUDA;
@@ -1628,6 +1637,8 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (c->side_ready) {
         cudaEventDestroy(c->ev_fork);
         cudaEventDestroy(c->ev_join);
+        cudaEventDestroy(c->ev_fork2);
+        cudaEventDestroy(c->ev_tree);
         cudaStreamDestroy(c->side);
     }
     if (c->prof_ev) {
@@ -1814,16 +1825,26 @@ static int posterior_z_impl(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const
     if (rc) return rc;
     const uint32_t want = HAWKES_WANT_LL | ((grad_z || hess_z) ? HAWKES_WANT_GRAD_THETA : 0u) |
                           (hess_z ? HAWKES_WANT_HESS_THETA : 0u);
-    if (skip)
-        rc = hawkes_eval_skip(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr,
-                              hess_z ? ht : nullptr, nullptr, stream);
-    else
-        rc = hawkes_eval(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr, hess_z ? ht : nullptr,
-                         nullptr, nullptr, stream);
-    if (rc) return rc;
-    rc = hawkes_tree_prior(tree, z, sigma2, tau0, sc + 1, grad_z ? pg : nullptr, stream);
+    // the O(M) tree prior (one latency-bound CTA) runs on the side stream beside the pairwise passes, which leave it
+    // an SM: a CTA of theirs that had to wait for that SM would hold up the whole pass
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaEventRecord(ctx->ev_fork2, (cudaStream_t)stream));
+    CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork2, 0));
+    rc = hawkes_tree_prior(tree, z, sigma2, tau0, sc + 1, grad_z ? pg : nullptr, (void*)ctx->side);
     if (rc) return rc;
     CK(cudaSetDevice(ctx->device));
+    CK(cudaEventRecord(ctx->ev_tree, ctx->side));
+    if (skip) {
+        rc = hawkes_eval_skip(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr,
+                              hess_z ? ht : nullptr, nullptr, stream);
+    } else {
+        ctx->reserve_sm = 1;
+        rc = hawkes_eval(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr, hess_z ? ht : nullptr,
+                         nullptr, nullptr, stream);
+        ctx->reserve_sm = 0;
+    }
+    if (rc) return rc;
+    CK(cudaStreamWaitEvent((cudaStream_t)stream, ctx->ev_tree, 0));
     z_chain_kernel<<<(unsigned)((m + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
         m, idx, th, gt, hess_z ? ht : nullptr, grad_z ? pg : nullptr, grad_z, hess_z, sc, out3);
     ctx->launches++;

@@ -437,6 +437,10 @@ void skip_plan_free(hawkes_ctx* c) {
     c->skip = nullptr;
 }
 
+// One SM is left free: hawkes_posterior_z_skip runs the single-CTA tree prior on the side stream beside the list
+// kernels, and a CTA of theirs that had to wait for that SM would hold up the whole pass.
+inline int skip_sms(const hawkes_ctx* ctx) { return ctx->sm_count > 1 ? ctx->sm_count - 1 : 1; }
+
 struct SkipBox {           // bounding box of a run of records: up to 3 coordinates, then time
     double lo[4], hi[4];
 };
@@ -652,10 +656,10 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
         }
     };
     int rc;
-    if ((rc = cut(items1, cost1, nt1, ctx->sm_count * P1_G[0], 12, ctx->part1_doubles, &sp->workers1))) return rc;
+    if ((rc = cut(items1, cost1, nt1, skip_sms(ctx) * P1_G[0], 12, ctx->part1_doubles, &sp->workers1))) return rc;
     if ((rc = skip_upload(&sp->d_items1, items1)) || (rc = skip_upload(&sp->d_w1start, ws)) ||
         (rc = skip_upload(&sp->d_w1first, wf)) || (rc = skip_upload(&sp->d_slots1, sl))) return rc;
-    if ((rc = cut(items1s, cost1s, nt1, ctx->sm_count * P1_G[0], 12, ctx->part1_doubles, &sp->workers1s))) return rc;
+    if ((rc = cut(items1s, cost1s, nt1, skip_sms(ctx) * P1_G[0], 12, ctx->part1_doubles, &sp->workers1s))) return rc;
     if ((rc = skip_upload(&sp->d_items1s, items1s)) || (rc = skip_upload(&sp->d_w1sstart, ws)) ||
         (rc = skip_upload(&sp->d_w1sfirst, wf)) || (rc = skip_upload(&sp->d_slots1s, sl))) return rc;
     {   // symmetric background: off unless it fits (HAWKES_DENSE_PASS1=1 switches it off as in the dense path)
@@ -666,7 +670,7 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
                 if (live_b(tile1[I], chunk[J])) itemsb.push_back(make_int2(I, J));
         sp->items_bsym = (int64_t)itemsb.size();
         const int64_t Q = 4 * (int64_t)itemsb.size();
-        const int W = (int)std::min<int64_t>(ctx->sm_count * P1_G[0], Q);
+        const int W = (int)std::min<int64_t>(skip_sms(ctx) * P1_G[0], Q);
         std::vector<int> wb(W + 1), wbf(nt1, 0), slb(nt1, 0), wbl(nt1, -1);
         for (int w = 0; w <= W; ++w) wb[w] = (int)(Q * w / W);
         for (int w = 0; w < W; ++w)
@@ -713,7 +717,7 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
             sp->d_partc = nullptr;
         }
     }
-    if ((rc = cut(items2, cost2, nt2, ctx->sm_count * P2_G[0], 2, ctx->part2_doubles, &sp->workers2))) return rc;
+    if ((rc = cut(items2, cost2, nt2, skip_sms(ctx) * P2_G[0], 2, ctx->part2_doubles, &sp->workers2))) return rc;
     if ((rc = skip_upload(&sp->d_items2, items2)) || (rc = skip_upload(&sp->d_w2start, ws)) ||
         (rc = skip_upload(&sp->d_w2first, wf)) || (rc = skip_upload(&sp->d_slots2, sl))) return rc;
     if ((rc = skip_upload(&sp->d_perm, perm))) return rc;
