@@ -232,3 +232,29 @@ def test_skip_replan_keeps_order_for_nearby_hyperparameters(torch):
     x2 = x.clone()
     x2[0, 0] += 1.0
     assert ctx.skip_plan(x2, t, far)["order_reused"] == 0        # other events: a fresh order
+
+
+def test_skip_rejects_bad_data(torch):
+    """Non-finite events are refused when planning (host check); a negative or non-finite theta is a device status
+    of the evaluation, as in the dense path."""
+    ev = synth.config(0)
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda")
+    x, t, th = f(ev.x), f(ev.t), f(ev.theta)
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    xb = x.clone()
+    xb[1, 17] = float("nan")
+    with pytest.raises(hp.HawkesError):
+        ctx.skip_plan(xb, t, ev.params)
+    tb = t.clone()
+    tb[3] = float("inf")
+    with pytest.raises(hp.HawkesError):
+        ctx.skip_plan(x, tb, ev.params)
+    with pytest.raises(hp.HawkesError):
+        ctx.skip_plan(x, t, ev.params[:4] + (-1.0,) + ev.params[5:])
+    ctx.skip_plan(x, t, ev.params)
+    thb = th.clone()
+    thb[5] = -0.5
+    ctx.eval_skip(x, t, thb, ev.params)
+    assert ctx.last_status() == hp.ERR_NONFINITE
+    ctx.eval_skip(x, t, th, ev.params)
+    assert ctx.last_status() == 0
