@@ -619,9 +619,15 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     const int nc = (int)chunk.size(), nt1 = (int)tile1.size(), nt2 = (int)tile2.size();
     std::vector<int2> items1, items1s, items2;
     std::vector<int> cost1, cost1s, cost2;
+    // a chunk's box lies inside its tile's: a pair of tiles that is dead leaves nothing to test below it
+    constexpr int CPT = (NT * P1_R) / TS;   // chunks per tile
     for (int I = 0; I < nt1; ++I)
-        for (int J = 0; J < nc; ++J) {
-            const int kind = (live_b(tile1[I], chunk[J]) ? SK_B : 0) | (live_s(tile1[I], chunk[J]) ? SK_S : 0);
+        for (int Jt = 0; Jt < nt1; ++Jt) {
+            const bool tb_live = live_b(tile1[I], tile1[Jt]), ts_live = live_s(tile1[I], tile1[Jt]);
+            if (!tb_live && !ts_live) continue;
+            for (int J = Jt * CPT; J < std::min(nc, (Jt + 1) * CPT); ++J) {
+            const int kind = ((tb_live && live_b(tile1[I], chunk[J])) ? SK_B : 0) |
+                             ((ts_live && live_s(tile1[I], chunk[J])) ? SK_S : 0);
             if (!kind) continue;
             items1.push_back(make_int2(I, J * 4 + kind));
             cost1.push_back(((kind & SK_B) ? W_ALL[1] : 0) + ((kind & SK_S) ? W_HEAD[1] + 4 : 0));
@@ -631,13 +637,17 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
                 items1s.push_back(make_int2(I, J * 4 + SK_S));
                 cost1s.push_back(1);
             }
+            }
         }
     for (int M = 0; M < nt2; ++M)
-        for (int J = 0; J < nc; ++J)
-            if (live_s(chunk[J], tile2[M])) {
-                items2.push_back(make_int2(M, J * 4 + SK_S));
-                cost2.push_back(1);
-            }
+        for (int Jt = 0; Jt < nt2; ++Jt) {
+            if (!live_s(tile2[Jt], tile2[M])) continue;
+            for (int J = Jt * CPT; J < std::min(nc, (Jt + 1) * CPT); ++J)
+                if (live_s(chunk[J], tile2[M])) {
+                    items2.push_back(make_int2(M, J * 4 + SK_S));
+                    cost2.push_back(1);
+                }
+        }
     sp->items_p2 = (int64_t)items2.size();
     sp->items_dense1 = (int64_t)nt1 * nc;
     sp->items_dense2 = (int64_t)nt2 * nc;
@@ -666,8 +676,11 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
         const std::vector<int> wf_s = wf, sl_s = sl;          // cut of the S items, just made
         std::vector<int2> itemsb;
         for (int I = 0; I < nt1; ++I)
-            for (int J = 0; J < nc && (int64_t)J * TS < std::min(n, (int64_t)(I + 1) * NT * P1_R); ++J)
-                if (live_b(tile1[I], chunk[J])) itemsb.push_back(make_int2(I, J));
+            for (int Jt = 0; Jt <= I; ++Jt) {
+                if (!live_b(tile1[I], tile1[Jt])) continue;
+                for (int J = Jt * CPT; J < std::min(nc, (Jt + 1) * CPT); ++J)
+                    if (live_b(tile1[I], chunk[J])) itemsb.push_back(make_int2(I, J));
+            }
         sp->items_bsym = (int64_t)itemsb.size();
         const int64_t Q = 4 * (int64_t)itemsb.size();
         const int W = (int)std::min<int64_t>(skip_sms(ctx) * P1_G[0], Q);
