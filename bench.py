@@ -586,7 +586,8 @@ def run_hmc(args) -> dict:
     sampler = ClockSampler(0).start()
     launches = 0
     for name, cache in (("recompute_all_pairs", 0), ("cached_background", 1), ("cached_kernel_matrix", 2),
-                        ("skip_lists_recompute", 3), ("skip_lists_cached_background", 4)):
+                        ("skip_lists_recompute", 3), ("skip_lists_cached_background", 4),
+                        ("sparse_kernel_matrix", 5)):
         if cache == 3:   # the exact-zero-skipping variants need the plan of these events and hyperparameters
             ctx.skip_plan(x, t, ev.params)
         z, mass = to(z0.copy()), to(np.ones(M))

@@ -319,7 +319,12 @@ typedef struct {
                                     another order.  dim <= 2 only (HAWKES_ERR_UNSUPPORTED otherwise).
                                  3, 4: variants 0 and 1 with every evaluation over the work lists of hawkes_skip_plan
                                     (exact zeros left out; the caller has planned these events and hyperparameters,
-                                    HAWKES_ERR_ARG otherwise).  Same sums in another order. */
+                                    HAWKES_ERR_ARG otherwise).  Same sums in another order.
+                                 5: variant 2 with the exact zeros of K left out: after the dense build its non-zeros
+                                    (acausal pairs and pairs beyond the kernel's fp64 reach are exactly +0.0) are
+                                    compressed by row and by column, in index order, and an evaluation reads those
+                                    lists only.  Synchronises `stream` once per call, during this set-up (the number
+                                    of non-zeros sizes the arrays, allocated on first use and kept); dim <= 2. */
     int32_t reserved;
 } hawkes_hmc_opts;
 

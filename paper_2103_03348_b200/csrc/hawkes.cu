@@ -25,6 +25,7 @@
 
 #include <cuda_runtime.h>
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 
 #include <cmath>
 #include <cstdio>
@@ -1167,6 +1168,7 @@ __global__ void hmc_mass_kernel(int64_t m, const double* __restrict__ hess_z, do
 }
 
 #include "hmc_kmat.cuh"
+#include "hmc_ksparse.cuh"
 
 // DFMA-chain microbenchmark: 8 independent chains per thread, `iters` x 8 x 8 FMAs.
 __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, double* out) {
@@ -1237,6 +1239,10 @@ struct hawkes_ctx {
     double* d_kmat;       // cached kernel matrix of hawkes_hmc_run (allocated on first use, kept)
     size_t kmat_doubles;
     double* d_kmisc;      // its vectors and partials
+    void* d_ksp_a;        // sparse form of the kernel matrix (hmc_ksparse.cuh): pointers and counts ...
+    size_t ksp_a_bytes;
+    void* d_ksp_b;        // ... and the non-zeros by row and by column (allocated on first use, kept)
+    size_t ksp_b_bytes;
     cudaStream_t side;    // small single-CTA kernels (scalars, tree prior) run here beside the big passes
     cudaEvent_t ev_fork, ev_join;
     cudaEvent_t ev_fork2, ev_tree;   // hawkes_posterior_z_skip: tree prior on the side stream
@@ -1552,6 +1558,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->bg_mode = 0;
     c->s_mode = 0;
     c->kmat_doubles = c->kmisc_doubles = 0;
+    c->d_ksp_a = c->d_ksp_b = nullptr;
+    c->ksp_a_bytes = c->ksp_b_bytes = 0;
     c->side_ready = false;
     c->plan_bg = -1;
     c->plan_sym = -1;
@@ -1573,6 +1581,11 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->cub_bytes = 0;
     cub::DeviceRadixSort::SortPairs(nullptr, c->cub_bytes, (const double*)nullptr, (double*)nullptr,
                                     (const int64_t*)nullptr, (int64_t*)nullptr, (int)n_max);
+    {   // the same scratch serves the exclusive scan of hmc_ksparse.cuh (n_max + 1 counts)
+        size_t scan_bytes = 0;
+        cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, (const int64_t*)nullptr, (int64_t*)nullptr, (int)(n_max + 1));
+        if (scan_bytes > c->cub_bytes) c->cub_bytes = scan_bytes;
+    }
     bool ok = true;
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_trec2, (void**)&c->d_part1, (void**)&c->d_part2,
@@ -1634,6 +1647,8 @@ void hawkes_destroy(hawkes_ctx* c) {
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
+    if (c->d_ksp_a) cudaFree(c->d_ksp_a);
+    if (c->d_ksp_b) cudaFree(c->d_ksp_b);
     if (c->side_ready) {
         cudaEventDestroy(c->ev_fork);
         cudaEventDestroy(c->ev_join);
@@ -1871,9 +1886,9 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     if (!ctx || !tree || !x || !t || !idx || !z || !p || !o || !normals || !uniforms || !mass) return HAWKES_ERR_ARG;
     if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
     if (o->n_iter < 1 || o->n_leapfrog < 1 || o->precond_every < 0 || o->n_refresh_done < 0 ||
-        o->cache_background < 0 || o->cache_background > 4) return HAWKES_ERR_ARG;
+        o->cache_background < 0 || o->cache_background > 5) return HAWKES_ERR_ARG;
     // 3 / 4: variants 0 / 1 over the work lists of hawkes_skip_plan (exact zeros left out, csrc/skip.cuh)
-    const bool use_skip = o->cache_background >= 3;
+    const bool use_skip = o->cache_background == 3 || o->cache_background == 4;
     const bool cache_bg = o->cache_background == 1 || o->cache_background == 4;
     if (use_skip && !ctx->skip) return HAWKES_ERR_ARG;
     if (!(o->step > 0.0) || !std::isfinite(o->step) || !(o->mass_floor > 0.0) || !std::isfinite(o->mass_floor))
@@ -1892,7 +1907,11 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     struct Reset { hawkes_ctx* c; ~Reset() { c->bg_mode = 0; } } reset{ctx};
     int rc;
     // ---- cache_background == 2: cached kernel matrix (csrc/hmc_kmat.cuh) -------------------------------------
-    const bool kmat = o->cache_background == 2;
+    const bool kmat = o->cache_background == 2 || o->cache_background == 5;
+    const bool ksp = o->cache_background == 5;      // the same matrix with its exact zeros left out (hmc_ksparse.cuh)
+    int64_t *sp_rowptr = nullptr, *sp_colptr = nullptr;
+    int *sp_col = nullptr, *sp_rowi = nullptr;
+    double *sp_val = nullptr, *sp_valc = nullptr;
     double *thM = nullptr, *kw = nullptr, *lam0 = nullptr, *logpart = nullptr, *cpart = nullptr, *intpart = nullptr,
            *lam0_int = nullptr, *lp = nullptr, *pg = nullptr;
     int nblk_r = 0, nblk_c = 0, nblk_f = 0, rows_per = 0;
@@ -1939,6 +1958,53 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         kmat_build_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(ctx->d_rec, n, m, idx, kc.omega,
                                                                           1.0 / (2.0 * kc.h * kc.h), ctx->d_kmat);
         ctx->launches++;
+        if (ksp) {
+            // compress the non-zeros by row and by column, each in index order (the one place this call synchronises:
+            // the number of non-zeros sizes the arrays)
+            const int nrb = (int)((n + KS_ROWS_PER - 1) / KS_ROWS_PER);
+            const size_t a_bytes = sizeof(int64_t) * (2 * (size_t)(n + 1) + (size_t)(m + 1) + (size_t)nrb * m) +
+                                   sizeof(int) * (size_t)nrb * m;
+            if (a_bytes > ctx->ksp_a_bytes) {
+                if (ctx->d_ksp_a) cudaFree(ctx->d_ksp_a);
+                ctx->d_ksp_a = nullptr; ctx->ksp_a_bytes = 0;
+                if (cudaMalloc(&ctx->d_ksp_a, a_bytes) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+                ctx->ksp_a_bytes = a_bytes;
+            }
+            int64_t* cnt = (int64_t*)ctx->d_ksp_a;
+            sp_rowptr = cnt + (n + 1);
+            sp_colptr = sp_rowptr + (n + 1);
+            int64_t* offc = sp_colptr + (m + 1);
+            int* cntc = (int*)(offc + (size_t)nrb * m);
+            const unsigned rowblocks = (unsigned)((n + 1 + 7) / 8);
+            ksp_row_count_kernel<<<rowblocks, 256, 0, st>>>(ctx->d_kmat, n, m, cnt);
+            size_t scan_bytes = 0;
+            cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, cnt, sp_rowptr, (int)(n + 1), st);
+            if (scan_bytes > ctx->cub_bytes) return HAWKES_ERR_UNSUPPORTED;
+            scan_bytes = ctx->cub_bytes;
+            CK(cub::DeviceScan::ExclusiveSum(ctx->d_cub, scan_bytes, cnt, sp_rowptr, (int)(n + 1), st));
+            int64_t nnz = 0;
+            CK(cudaMemcpyAsync(&nnz, sp_rowptr + n, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            const size_t b_bytes = (size_t)(nnz > 0 ? nnz : 1) * (2 * sizeof(double) + 2 * sizeof(int));
+            if (b_bytes > ctx->ksp_b_bytes) {
+                if (ctx->d_ksp_b) cudaFree(ctx->d_ksp_b);
+                ctx->d_ksp_b = nullptr; ctx->ksp_b_bytes = 0;
+                if (cudaMalloc(&ctx->d_ksp_b, b_bytes) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+                ctx->ksp_b_bytes = b_bytes;
+            }
+            const size_t nz = (size_t)(nnz > 0 ? nnz : 1);
+            sp_val = (double*)ctx->d_ksp_b;
+            sp_valc = sp_val + nz;
+            sp_col = (int*)(sp_valc + nz);
+            sp_rowi = sp_col + nz;
+            ksp_row_fill_kernel<<<(unsigned)((n + 7) / 8), 256, 0, st>>>(ctx->d_kmat, n, m, sp_rowptr, sp_col, sp_val);
+            const dim3 cg((unsigned)((m + 255) / 256), (unsigned)nrb);
+            ksp_col_count_kernel<<<cg, 256, 0, st>>>(ctx->d_kmat, n, m, cntc);
+            ksp_col_offsets_kernel<<<1, 1024, 0, st>>>(nrb, m, cntc, sp_colptr, offc);
+            ksp_col_fill_kernel<<<cg, 256, 0, st>>>(ctx->d_kmat, n, m, offc, sp_rowi, sp_valc);
+            ctx->launches += 6;
+            nblk_c = 1;                                        // one partial per column (kmat_finish_kernel)
+        }
     }
     auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess) -> int {
         if (!kmat) return posterior_z_impl(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream, use_skip);
@@ -1950,10 +2016,16 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         if (cudaSetDevice(ctx->device) != cudaSuccess || cudaEventRecord(ctx->ev_join, ctx->side) != cudaSuccess)
             return HAWKES_ERR_CUDA;
         kmat_theta_kernel<<<mb, 256, 0, st>>>(m, idx, zin, beta, t, thM);
+        if (ksp) {
+            ksp_rows_kernel<<<nblk_r, KM_ROWS_T, 0, st>>>(sp_rowptr, sp_col, sp_val, n, thM, lam0, kc.CS, kw, logpart,
+                                                          ctx->d_status);
+            ksp_cols_kernel<<<(unsigned)((m + 7) / 8), 256, 0, st>>>(sp_colptr, sp_rowi, sp_valc, m, kw, hess ? 1 : 0, cpart);
+        } else {
         kmat_rows_kernel<<<nblk_r, KM_ROWS_T, m * sizeof(double), st>>>(ctx->d_kmat, n, m, thM, lam0, kc.CS, kw, logpart,
                                                                         ctx->d_status);
         kmat_cols_kernel<<<dim3((unsigned)((m + KM_COL_TILE - 1) / KM_COL_TILE), (unsigned)nblk_c), KM_COL_TILE, 0, st>>>(
             ctx->d_kmat, n, m, kw, rows_per, hess ? 1 : 0, cpart);
+        }
         if (cudaStreamWaitEvent(st, ctx->ev_join, 0) != cudaSuccess) return HAWKES_ERR_CUDA;
         kmat_finish_kernel<<<nblk_f, 256, 0, st>>>(m, nblk_c, cpart, hess ? 1 : 0, idx, t, n, thM, kc.CS, kc.xi0, kc.omega,
                                                    grad ? pg : nullptr, grad, hess, intpart);

@@ -25,7 +25,7 @@ def dev(torch, a):
 
 
 @pytest.mark.parametrize("cache_bg,with_prior_prec", [(0, False), (1, False), (1, True), (2, False), (2, True),
-                                                      (3, False), (4, False), (4, True)])
+                                                      (3, False), (4, False), (4, True), (5, False), (5, True)])
 def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     """1,500 events, 90 sequenced; 6 iterations x 5 leapfrog steps, preconditioner refreshed every 3 iterations.
     Tolerance: the state after 30 leapfrog steps inherits the 1e-10 bar of the gradient through a mildly expanding
@@ -57,7 +57,7 @@ def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     pp_d = tr.precision_diag(s2, tau0) if with_prior_prec else None
     if with_prior_prec:
         assert np.max(np.abs(pp_d.cpu().numpy() - pp) / pp) <= 1e-10
-    if cache_bg >= 3:     # variants 0 / 1 over the work lists of hawkes_skip_plan (exact zeros left out)
+    if cache_bg in (3, 4):     # variants 0 / 1 over the work lists of hawkes_skip_plan (exact zeros left out)
         with pytest.raises(hp.HawkesError):
             ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z.clone(), beta, ev.params, s2, tau0,
                         n_iter=1, n_leapfrog=1, step=eps, precond_every=0, mass=mass.clone(), mass_floor=floor,
