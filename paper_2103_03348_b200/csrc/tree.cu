@@ -53,16 +53,20 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double* red /*[
     }
 }
 
+// The message variances, hence s_u, alpha_u and sum log s_u, depend on the branch lengths alone: hawkes_tree_create
+// computes them once on the host (alpha[q], inv[q] = 1 / s_u by level-order position q, the sum of log s_u and the
+// root's message variance), and a call walks the means only -- no division and no logarithm on the per-level
+// critical path.
 // node storage: nm[v], nv[v] (v = node id).  Life of the slots of the children a, b of an internal node u:
-//   up sweep, before u:   nm = message mean, nv = message variance
-//   up sweep, after u:    nm[a] = alpha_u, nm[b] = c_u / (sigma^2 s_u), nv[a] = s_u   (the messages of a, b are dead)
-//   down sweep:           nv[a], nv[b] = adjoints mbar_a, mbar_b (s_u has been consumed by the log pass)
+//   up sweep, before u:   nm = message mean
+//   up sweep, after u:    nm[b] = c_u / (sigma^2 s_u)   (the messages of a, b are dead)
+//   down sweep:           nv[a], nv[b] = adjoints mbar_a, mbar_b
 template <bool SMEM>
 __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_levels, int narrow_from,
                                                             const int* __restrict__ g_level_start,
                                                             const int* __restrict__ g_order, const int* __restrict__ g_child_a,
                                                             const int* __restrict__ g_child_b, const double* __restrict__ g_wa,
-                                                            const double* __restrict__ g_wb,
+                                                            const double* __restrict__ g_wb, double logs_tree, double v_root,
                                                             int root, const double* __restrict__ z, double sigma2,
                                                             double tau0, double* __restrict__ scratch,
                                                             double* __restrict__ logp, double* __restrict__ grad_z) {
@@ -88,7 +92,7 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
         for (int l = threadIdx.x; l <= n_levels; l += TREE_T) s_ls[l] = g_level_start[l];
         order = s_order; child_a = s_a; child_b = s_b; wa = s_wa; wb = s_wb; level_start = s_ls;
     }
-    for (int i = threadIdx.x; i < n_tips; i += TREE_T) { nm[i] = z[i]; nv[i] = 0.0; }
+    for (int i = threadIdx.x; i < n_tips; i += TREE_T) nm[i] = z[i];
     __syncthreads();
     const double inv_s2 = 1.0 / sigma2;
     double quad = 0.0;
@@ -97,16 +101,11 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
     // level has at most 32 nodes and warp 0 walks them alone, one warp barrier per level.
     auto up_node = [&](int q) {
         const int u = order[q], a = child_a[q], b = child_b[q];
-        const double va = nv[a] + wa[q], vb = nv[b] + wb[q];
         const double ma = nm[a], mb = nm[b];
-        const double c = ma - mb, s = va + vb, inv = 1.0 / s;
-        const double alpha = vb * inv;
+        const double c = ma - mb, alpha = wa[q], inv = wb[q];   // wa / wb hold alpha_u and 1 / s_u
         nm[u] = fma(alpha, c, mb);          // alpha ma + (1 - alpha) mb
-        nv[u] = va * vb * inv;
         quad = fma(c * c, inv, quad);
-        nm[a] = alpha;
         nm[b] = c * inv * inv_s2;
-        nv[a] = s;
     };
     for (int l = 0; l < narrow_from; ++l) {
         for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) up_node(q);
@@ -120,14 +119,13 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
         }
     }
     __syncthreads();
-    // log pass: sum of log s over the internal nodes (s sits in nv[child_a])
+    // sum of log s over the internal nodes: a constant of the tree; the root term holds tau0
     double logs = 0.0;
-    for (int q = threadIdx.x; q < n_int; q += TREE_T) logs += log(nv[child_a[q]]);
     double mbar_root = 0.0;
     if (threadIdx.x == 0) {
-        const double s = nv[root] + tau0, c = nm[root];
+        const double s = v_root + tau0, c = nm[root];
         quad = fma(c * c, 1.0 / s, quad);
-        logs += log(s);
+        logs = logs_tree + log(s);
         mbar_root = -c / (sigma2 * s);
     }
     __syncthreads();
@@ -139,7 +137,7 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
     // down sweep (narrow levels first, by warp 0)
     auto down_node = [&](int q) {
         const int u = order[q], a = child_a[q], b = child_b[q];
-        const double mbar = nv[u], alpha = nm[a], k = nm[b];
+        const double mbar = nv[u], alpha = wa[q], k = nm[b];
         nv[a] = fma(alpha, mbar, -k);
         nv[b] = fma(1.0 - alpha, mbar, k);
     };
@@ -201,7 +199,8 @@ struct hawkes_tree {
     int n_tips, n_levels, narrow_from, root;
     int *d_level_start, *d_order, *d_child_a, *d_child_b;   // child_a/b: by node id (precision kernel)
     int *d_qa, *d_qb;                                       // children by level-order position (prior kernel)
-    double *d_qwa, *d_qwb;                                  // their branch lengths, same order
+    double *d_qwa, *d_qwb;                                  // alpha_u and 1 / s_u of the up sweep, same order
+    double logs_tree, v_root;                               // sum log s_u over the internal nodes; the root's message variance
     double *d_branch, *d_scratch;
     bool smem;
     size_t smem_bytes;
@@ -274,11 +273,21 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
                     (size_t)(n_levels + 1) * sizeof(int) + 16;
     std::vector<int> qa(M > 1 ? M - 1 : 1, 0), qb(M > 1 ? M - 1 : 1, 0);
     std::vector<double> qwa(M > 1 ? M - 1 : 1, 0.0), qwb(M > 1 ? M - 1 : 1, 0.0);
+    // variance half of the independent-contrasts recursion: it involves the branch lengths only
+    std::vector<double> hv(nn, 0.0);
+    double logs_tree = 0.0;
     for (int q = 0; q < M - 1; ++q) {
         const int u = order[q];
         qa[q] = ca[u]; qb[q] = cb[u];
-        qwa[q] = branch[ca[u]]; qwb[q] = branch[cb[u]];
+        const double va = hv[ca[u]] + branch[ca[u]], vb = hv[cb[u]] + branch[cb[u]];
+        const double sm_ = va + vb, inv = 1.0 / sm_;
+        qwa[q] = vb * inv;       // alpha_u
+        qwb[q] = inv;            // 1 / s_u
+        hv[u] = va * vb * inv;
+        logs_tree += std::log(sm_);
     }
+    t->logs_tree = logs_tree;
+    t->v_root = hv[root];
     t->smem = t->smem_bytes <= TREE_SMEM_MAX;
     t->d_level_start = t->d_order = t->d_child_a = t->d_child_b = t->d_qa = t->d_qb = nullptr;
     t->d_qwa = t->d_qwb = nullptr;
@@ -329,12 +338,12 @@ int hawkes_tree_prior(hawkes_tree* t, const double* z, double sigma2, double tau
     cudaStream_t st = (cudaStream_t)stream;
     if (t->smem)
         tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_order,
-                                                                 t->d_qa, t->d_qb, t->d_qwa, t->d_qwb, t->root, z,
-                                                                 sigma2, tau0, t->d_scratch, logp, grad_z);
+                                                                 t->d_qa, t->d_qb, t->d_qwa, t->d_qwb, t->logs_tree, t->v_root,
+                                                                 t->root, z, sigma2, tau0, t->d_scratch, logp, grad_z);
     else
         tree_prior_kernel<false><<<1, TREE_T, 0, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_order, t->d_qa,
-                                                       t->d_qb, t->d_qwa, t->d_qwb, t->root, z, sigma2, tau0, t->d_scratch,
-                                                       logp, grad_z);
+                                                       t->d_qb, t->d_qwa, t->d_qwb, t->logs_tree, t->v_root, t->root, z, sigma2,
+                                                       tau0, t->d_scratch, logp, grad_z);
     t->launches++;
     CKT(cudaGetLastError());
     return HAWKES_OK;
