@@ -1838,7 +1838,7 @@ static int posterior_z_impl(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const
     double* sc = ctx->d_post;   // sc[0] = ell, sc[1] = log prior
     int rc = hawkes_theta_from_z(ctx, n, m, idx, z, beta, t, th, stream);
     if (rc) return rc;
-    const uint32_t want = HAWKES_WANT_LL | ((grad_z || hess_z) ? HAWKES_WANT_GRAD_THETA : 0u) |
+    const uint32_t want = (out3 ? HAWKES_WANT_LL : 0u) | ((grad_z || hess_z) ? HAWKES_WANT_GRAD_THETA : 0u) |
                           (hess_z ? HAWKES_WANT_HESS_THETA : 0u);
     // the O(M) tree prior (one latency-bound CTA) runs on the side stream beside the pairwise passes, which leave it
     // an SM: a CTA of theirs that had to wait for that SM would hold up the whole pass
@@ -2055,7 +2055,8 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, prior_prec, normals + (int64_t)it * m, eps, zp, pm, hs);
         ctx->launches++;
         for (int s = 0; s < o->n_leapfrog; ++s) {
-            rc = eval_post(zp, o3p, gp, nullptr);
+            // the energies are needed at the end of the trajectory only
+            rc = eval_post(zp, s + 1 == o->n_leapfrog ? o3p : nullptr, gp, nullptr);
             if (rc) return rc;
             if (s + 1 < o->n_leapfrog) {
                 hmc_leap_kernel<<<mb, 256, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm);
