@@ -36,6 +36,12 @@ constexpr size_t TREE_SMEM_MAX = 200 * 1024;
         if ((call) != cudaSuccess) return HAWKES_ERR_CUDA; \
     } while (0)
 
+// an internal node in level order: its id, its children, alpha_u and 1 / s_u of the up sweep
+struct __align__(16) TreeQ {
+    int u, a, b, pad;
+    double alpha, inv;
+};
+
 // fixed-order block sum of two values; result in thread 0
 __device__ __forceinline__ void block_sum2(double& a, double& b, double* red /*[2 * TREE_T / 32]*/) {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -64,9 +70,7 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double* red /*[
 template <bool SMEM>
 __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_levels, int narrow_from,
                                                             const int* __restrict__ g_level_start,
-                                                            const int* __restrict__ g_order, const int* __restrict__ g_child_a,
-                                                            const int* __restrict__ g_child_b, const double* __restrict__ g_wa,
-                                                            const double* __restrict__ g_wb, double logs_tree, double v_root,
+                                                            const TreeQ* __restrict__ g_tq, double logs_tree, double v_root,
                                                             int root, const double* __restrict__ z, double sigma2,
                                                             double tau0, double* __restrict__ scratch,
                                                             double* __restrict__ logp, double* __restrict__ grad_z) {
@@ -77,20 +81,14 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
     double* nv = nm + n_nodes;
     // topology in level order (position q = 0 .. M-2): node id, children, the children's branch lengths.  With SMEM
     // it is copied next to the messages so that a level costs shared-memory latency only.
-    const int *order = g_order, *child_a = g_child_a, *child_b = g_child_b, *level_start = g_level_start;
-    const double *wa = g_wa, *wb = g_wb;
+    const TreeQ* tq = g_tq;
+    const int* level_start = g_level_start;
     if (SMEM) {
-        double* s_wa = nv + n_nodes;
-        double* s_wb = s_wa + n_int;
-        int* s_order = reinterpret_cast<int*>(s_wb + n_int);
-        int* s_a = s_order + n_int;
-        int* s_b = s_a + n_int;
-        int* s_ls = s_b + n_int;
-        for (int q = threadIdx.x; q < n_int; q += TREE_T) {
-            s_wa[q] = g_wa[q]; s_wb[q] = g_wb[q]; s_order[q] = g_order[q]; s_a[q] = g_child_a[q]; s_b[q] = g_child_b[q];
-        }
+        TreeQ* s_tq = reinterpret_cast<TreeQ*>(nv + n_nodes);   // 32-byte records: two 16-byte loads per node
+        int* s_ls = reinterpret_cast<int*>(s_tq + n_int);
+        for (int q = threadIdx.x; q < n_int; q += TREE_T) s_tq[q] = g_tq[q];
         for (int l = threadIdx.x; l <= n_levels; l += TREE_T) s_ls[l] = g_level_start[l];
-        order = s_order; child_a = s_a; child_b = s_b; wa = s_wa; wb = s_wb; level_start = s_ls;
+        tq = s_tq; level_start = s_ls;
     }
     for (int i = threadIdx.x; i < n_tips; i += TREE_T) nm[i] = z[i];
     __syncthreads();
@@ -100,12 +98,12 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
     // Levels below `narrow_from` are walked by the whole CTA with a block barrier each; from `narrow_from` on every
     // level has at most 32 nodes and warp 0 walks them alone, one warp barrier per level.
     auto up_node = [&](int q) {
-        const int u = order[q], a = child_a[q], b = child_b[q];
-        const double ma = nm[a], mb = nm[b];
-        const double c = ma - mb, alpha = wa[q], inv = wb[q];   // wa / wb hold alpha_u and 1 / s_u
-        nm[u] = fma(alpha, c, mb);          // alpha ma + (1 - alpha) mb
-        quad = fma(c * c, inv, quad);
-        nm[b] = c * inv * inv_s2;
+        const TreeQ r = tq[q];
+        const double ma = nm[r.a], mb = nm[r.b];
+        const double c = ma - mb;
+        nm[r.u] = fma(r.alpha, c, mb);      // alpha ma + (1 - alpha) mb
+        quad = fma(c * c, r.inv, quad);
+        nm[r.b] = c * r.inv * inv_s2;
     };
     for (int l = 0; l < narrow_from; ++l) {
         for (int q = level_start[l] + threadIdx.x; q < level_start[l + 1]; q += TREE_T) up_node(q);
@@ -136,10 +134,10 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
     if (grad_z == nullptr) return;
     // down sweep (narrow levels first, by warp 0)
     auto down_node = [&](int q) {
-        const int u = order[q], a = child_a[q], b = child_b[q];
-        const double mbar = nv[u], alpha = wa[q], k = nm[b];
-        nv[a] = fma(alpha, mbar, -k);
-        nv[b] = fma(1.0 - alpha, mbar, k);
+        const TreeQ r = tq[q];
+        const double mbar = nv[r.u], k = nm[r.b];
+        nv[r.a] = fma(r.alpha, mbar, -k);
+        nv[r.b] = fma(1.0 - r.alpha, mbar, k);
     };
     if (threadIdx.x < 32) {
         for (int l = n_levels - 1; l >= narrow_from; --l) {
@@ -198,8 +196,7 @@ struct hawkes_tree {
     int device;
     int n_tips, n_levels, narrow_from, root;
     int *d_level_start, *d_order, *d_child_a, *d_child_b;   // child_a/b: by node id (precision kernel)
-    int *d_qa, *d_qb;                                       // children by level-order position (prior kernel)
-    double *d_qwa, *d_qwb;                                  // alpha_u and 1 / s_u of the up sweep, same order
+    TreeQ* d_tq;                                            // prior kernel: one record per internal node, level order
     double logs_tree, v_root;                               // sum log s_u over the internal nodes; the root's message variance
     double *d_branch, *d_scratch;
     bool smem;
@@ -269,7 +266,7 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
     t->narrow_from = n_levels;
     while (t->narrow_from > 0 && level_start[t->narrow_from] - level_start[t->narrow_from - 1] <= 32) t->narrow_from--;
     // shared memory of the prior kernel: 2 message doubles per node + per internal node 2 doubles and 3 ints + the level offsets
-    t->smem_bytes = sizeof(double) * 2 * (size_t)nn + (size_t)(M - 1) * (2 * sizeof(double) + 3 * sizeof(int)) +
+    t->smem_bytes = sizeof(double) * 2 * (size_t)nn + (size_t)(M - 1) * sizeof(TreeQ) +
                     (size_t)(n_levels + 1) * sizeof(int) + 16;
     std::vector<int> qa(M > 1 ? M - 1 : 1, 0), qb(M > 1 ? M - 1 : 1, 0);
     std::vector<double> qwa(M > 1 ? M - 1 : 1, 0.0), qwb(M > 1 ? M - 1 : 1, 0.0);
@@ -288,9 +285,11 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
     }
     t->logs_tree = logs_tree;
     t->v_root = hv[root];
+    std::vector<TreeQ> tqv(M > 1 ? M - 1 : 1);
+    for (int q = 0; q < M - 1; ++q) tqv[q] = TreeQ{order[q], qa[q], qb[q], 0, qwa[q], qwb[q]};
     t->smem = t->smem_bytes <= TREE_SMEM_MAX;
-    t->d_level_start = t->d_order = t->d_child_a = t->d_child_b = t->d_qa = t->d_qb = nullptr;
-    t->d_qwa = t->d_qwb = nullptr;
+    t->d_level_start = t->d_order = t->d_child_a = t->d_child_b = nullptr;
+    t->d_tq = nullptr;
     t->d_branch = t->d_scratch = nullptr;
     bool ok = true;
     auto up = [&](void** d, const void* h, size_t bytes) {
@@ -303,10 +302,7 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
     up((void**)&t->d_child_a, ca.data(), sizeof(int) * nn);
     up((void**)&t->d_child_b, cb.data(), sizeof(int) * nn);
     up((void**)&t->d_branch, branch, sizeof(double) * nn);
-    up((void**)&t->d_qa, qa.data(), sizeof(int) * qa.size());
-    up((void**)&t->d_qb, qb.data(), sizeof(int) * qb.size());
-    up((void**)&t->d_qwa, qwa.data(), sizeof(double) * qwa.size());
-    up((void**)&t->d_qwb, qwb.data(), sizeof(double) * qwb.size());
+    up((void**)&t->d_tq, tqv.data(), sizeof(TreeQ) * tqv.size());
     up((void**)&t->d_scratch, nullptr, sizeof(double) * 2 * (size_t)nn);
     if (ok && t->smem &&
         cudaFuncSetAttribute(tree_prior_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem_bytes) != cudaSuccess)
@@ -324,7 +320,7 @@ void hawkes_tree_destroy(hawkes_tree* t) {
     if (!t) return;
     cudaSetDevice(t->device);
     void* ptrs[] = {t->d_level_start, t->d_order, t->d_child_a, t->d_child_b, t->d_branch, t->d_scratch,
-                    t->d_qa, t->d_qb, t->d_qwa, t->d_qwb};
+                    t->d_tq};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     delete t;
@@ -337,12 +333,12 @@ int hawkes_tree_prior(hawkes_tree* t, const double* z, double sigma2, double tau
     CKT(cudaSetDevice(t->device));
     cudaStream_t st = (cudaStream_t)stream;
     if (t->smem)
-        tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_order,
-                                                                 t->d_qa, t->d_qb, t->d_qwa, t->d_qwb, t->logs_tree, t->v_root,
+        tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start,
+                                                                 t->d_tq, t->logs_tree, t->v_root,
                                                                  t->root, z, sigma2, tau0, t->d_scratch, logp, grad_z);
     else
-        tree_prior_kernel<false><<<1, TREE_T, 0, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_order, t->d_qa,
-                                                       t->d_qb, t->d_qwa, t->d_qwb, t->logs_tree, t->v_root, t->root, z, sigma2,
+        tree_prior_kernel<false><<<1, TREE_T, 0, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start,
+                                                       t->d_tq, t->logs_tree, t->v_root, t->root, z, sigma2,
                                                        tau0, t->d_scratch, logp, grad_z);
     t->launches++;
     CKT(cudaGetLastError());
