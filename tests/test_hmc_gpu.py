@@ -97,3 +97,35 @@ def test_hmc_rejects_bad_options(torch):
     with pytest.raises(hp.HawkesError) as e:
         ctx.hmc_run(*args, **{**kw, "n_leapfrog": 0})
     assert e.value.status == hp.ERR_ARG
+
+
+def test_hmc_sparse_kernel_matrix_edge_cases(torch):
+    """Variant 5 against variant 2 (the dense cached kernel matrix, itself checked against the oracle above) where
+    the compression is degenerate: a self-excitation reach so short that K has no non-zero at all, and a second call
+    on the same context (buffers kept from the first)."""
+    import paper_2103_03348_b200 as hp
+    ev = synth.make_events(1200, seed=21, n_centres=5, n_free=64)
+    idx = ev.free_idx
+    M = len(idx)
+    tree = synth.make_tree(ev.t[idx], 21)
+    s2, tau0 = 0.25, 0.1
+    z0 = synth.draw_z(tree, s2, tau0, 21)
+    n_iter, L = 3, 4
+    normals = synth.normals(21, 400, n_iter * M).reshape(n_iter, M)
+    uniforms = synth.uniforms(21, 401, n_iter)
+    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
+    tr = hp.HawkesTree(tree.parent, tree.branch, 0)
+    pp = tr.precision_diag(s2, tau0)
+    for params in (ev.params[:4] + (1e-4,) + ev.params[5:], ev.params):
+        out = {}
+        for variant in (2, 5):
+            z, mass = dev(torch, z0.copy()), dev(torch, np.ones(M))
+            trace = ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z, 0.0, params, s2, tau0,
+                                n_iter=n_iter, n_leapfrog=L, step=0.2, precond_every=2, mass=mass, mass_floor=0.5,
+                                normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=variant,
+                                prior_prec=pp)
+            torch.cuda.synchronize()
+            out[variant] = (ctx.last_status(), trace.cpu().numpy(), z.cpu().numpy(), mass.cpu().numpy())
+        assert out[2][0] == out[5][0] == 0
+        for a, b in zip(out[2][1:], out[5][1:]):
+            assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(a)), 1.0)
