@@ -258,3 +258,34 @@ def test_skip_rejects_bad_data(torch):
     assert ctx.last_status() == hp.ERR_NONFINITE
     ctx.eval_skip(x, t, th, ev.params)
     assert ctx.last_status() == 0
+
+
+@pytest.mark.parametrize("n", [50000, 250000])
+def test_skip_scaling_sweep_sampled_rows_and_columns(torch, n):
+    """BASELINE.json configs[4] sizes through the lists: 1,024 sampled target rows (lambda_n) and, with the GPU's
+    lambda, 1,024 source columns (c_m, d_m) against the oracle; properties that hold at any size."""
+    ev = synth.config(4, n=n)
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda")
+    x, t, th = f(ev.x), f(ev.t), f(ev.theta)
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    stats = ctx.skip_plan(x, t, ev.params)
+    assert stats["items_background"] < 0.6 * stats["items_dense_pass1"]
+    assert stats["items_pass2"] < 0.1 * stats["items_dense_pass2"]
+    r = ctx.eval_skip(x, t, th, ev.params, hp.WANT_GRAD | hp.WANT_HESS_THETA)
+    assert ctx.last_status() == 0
+    lam = np.empty(ev.n)
+    lam[ctx.skip_perm(ev.n).numpy()] = ctx.get_lambda(ev.n).cpu().numpy()
+    k = 1024
+    idx = np.sort((synth.uniforms(123, 7, k) * n).astype(np.int64))
+    idx[0], idx[-1] = 0, n - 1
+    lam_o, _ = oracle.rows(ev.x, ev.t, ev.theta, ev.params, idx, derivs=False, threads=THREADS)
+    check("lambda rows", lam[idx], lam_o)
+    c_o, d_o = oracle.cols(ev.x, ev.t, ev.params, lam, idx, threads=THREADS)
+    xi0, om = ev.params[3], ev.params[5]
+    integ = xi0 * (-np.expm1(-om * (ev.t[-1] - ev.t[idx])))
+    gt = r.grad_theta.cpu().numpy()
+    hd = r.hess_theta_diag.cpu().numpy()
+    check("grad_theta cols", gt[idx], c_o - integ, np.abs(c_o) + integ)
+    check("hess_theta cols", hd[idx], -d_o, floor=1e-280)
+    assert gt[-1] == 0.0 and np.all(np.isfinite(gt)) and np.all(hd <= 0)
+    assert np.all(lam > 0) and math.isfinite(r.ll.item())
