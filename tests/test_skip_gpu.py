@@ -87,10 +87,21 @@ def test_skip_small_problems_shuffled_input(torch, n, seed, dim, regime, ties, d
         ev.t *= n / 40.0
     ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
     order = np.argsort(synth.uniforms(seed, 77, n), kind="stable")
-    r, st, lam, g, hd, stats, _ = run_skip(torch, ev, order=order)
+    r, st, lam, g, hd, stats, ctx = run_skip(torch, ev, order=order)
     assert st == ref.status
     if ref.status == 0:
         compare(ev, ref, r, lam, g, hd)
+        # the gradient level and the likelihood level take the background once per unordered pair (another kernel):
+        # same oracle values
+        s = scales(ev, ref)
+        for want in (hp.WANT_GRAD, hp.WANT_LL | hp.WANT_GRAD_THETA):
+            r1, st1, lam1, g1, _, stats1, _ = run_skip(torch, ev, want=want, order=order, ctx=ctx)
+            assert st1 == 0 and stats1["items_background_unordered"] > 0 and stats1["order_reused"] == 1
+            check("lambda", lam1, ref.lam)
+            check("ll", r1.ll.cpu().numpy()[0], ref.ll, s["ll"])
+            check("grad_theta", g1, ref.grad_theta, s["grad_theta"])
+            if want & hp.WANT_GRAD_HYPER:
+                check("grad_hyper", r1.grad_hyper.cpu().numpy(), ref.grad_hyper, s["grad_hyper"])
     else:   # (last case) some lambda_n is exactly zero in the oracle as well: ll = -inf on both sides
         assert r.ll.item() == ref.ll == -math.inf
         zero_rates_agree(lam, ref.lam)
