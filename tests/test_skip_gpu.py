@@ -160,6 +160,13 @@ def test_skip_space_only_background(torch):
     r, st, lam, g, hd, stats, _ = run_skip(torch, ev, ctx=ctx)
     assert st == ref.status == 0
     compare(ev, ref, r, lam, g, hd)
+    r1, st1, lam1, g1, _, stats1, _ = run_skip(torch, ev, want=hp.WANT_GRAD, ctx=ctx)   # symmetric background lists
+    assert st1 == 0 and stats1["items_background_unordered"] > 0
+    s = scales(ev, ref)
+    check("lambda", lam1, ref.lam)
+    check("ll", r1.ll.cpu().numpy()[0], ref.ll, s["ll"])
+    check("grad_theta", g1, ref.grad_theta, s["grad_theta"])
+    check("grad_hyper", r1.grad_hyper.cpu().numpy(), ref.grad_hyper, s["grad_hyper"])
 
 
 def test_skip_full_size_against_dense_gpu_and_sampled_oracle(torch):
