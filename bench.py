@@ -405,10 +405,20 @@ def run_b200(args, ev, workload: str) -> dict:
         t2step = lambda: ctx.grad(x, t, th, _synth.TABLE2_PARAMS, out=out)
         timed(t2step, 2)
         t2ms = timed(t2step, max(3, K // 4))
+        # ... and the exact-zero-skipping variant at those scales: the background reaches the whole domain there,
+        # only the self-excitation lists shrink (the gain of that variant is data-dependent)
+        t2stats = ctx.skip_plan(x, t, _synth.TABLE2_PARAMS)
+        t2skip = lambda: ctx.eval_skip(x, t, th, _synth.TABLE2_PARAMS, hp.WANT_GRAD, out=out)
+        timed(t2skip, 2)
+        t2sms = timed(t2skip, max(3, K // 4))
         timed(step, 1)   # leave `out` holding the configs[1] result
         res["extras"] = {"hessian_ms": statistics.median(hms), "ll_grad_theta_only_ms": statistics.median(lms),
                          "step_ms_min": min(ms), "step_ms_median": statistics.median(ms),
-                         "table2_scales_step_ms": statistics.median(t2ms)}
+                         "table2_scales_step_ms": statistics.median(t2ms),
+                         "table2_scales_skip_step_ms": statistics.median(t2sms),
+                         "table2_scales_skip_tile_pairs": {
+                             "pass1_background": t2stats["items_background"] / t2stats["items_dense_pass1"],
+                             "pass1_excitation": t2stats["items_excitation"] / t2stats["items_dense_pass1"]}}
     # the O(N) kernels (prep, reduce1, theta) against the measured HBM copy peak: bytes they move per evaluation
     # (records in and out, row-partial slots, column partials: about N^2 * 12 / tile of them), time from the ring
     try:
