@@ -191,9 +191,38 @@ int hawkes_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double* 
 int hawkes_skip_stats(hawkes_ctx* ctx, int64_t* out);
 int hawkes_skip_perm(hawkes_ctx* ctx, int64_t n, int64_t* perm_host);
 
+/* Pass-1 form of the context.  Eq. 1's double sum holds the background term of
+ * every ORDERED pair, and B_{nn'} = B_{n'n}:
+ *   HAWKES_PASS1_AUTO (default): log-likelihood- and gradient-level evaluations compute each background exponential
+ *     once per UNORDERED pair and add it to both events' sums (when the context holds the column-partial buffer:
+ *     problems of up to ~290,000 events);
+ *   HAWKES_PASS1_DENSE: every evaluation uses the ordered-pair kernel.
+ * Same sums in another order.  Applies to every later evaluation and to later hawkes_skip_plan calls.
+ * hawkes_pass1_is_symmetric: 1 if an evaluation whose pass 1 runs at `level` (0: ll / theta-gradient, 1: + hyper-
+ * gradient, 2: + hyper-Hessian) would take the once-per-unordered-pair form, else 0 (benchmarks label their lines
+ * with it). */
+enum { HAWKES_PASS1_AUTO = 0, HAWKES_PASS1_DENSE = 1 };
+int hawkes_set_pass1_mode(hawkes_ctx* ctx, int mode);
+int hawkes_pass1_is_symmetric(const hawkes_ctx* ctx, int level);
+
 /* After an evaluation queued on this context has been enqueued: copies of the per-event rates
  * lambda_n (n doubles) into a caller buffer, on `stream`.  For tests and diagnostics. */
 int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stream);
+
+/* Diagnostics, as hawkes_get_lambda: the per-event derivatives of lambda_n (Eq. 1) that the O(N) reduction
+ * formed from the pass-1 moment sums in the most recent evaluation,
+ *   d1_out[i*6 + p]  = d lambda_i / dp,            p over (mu0, tau_x, tau_t, xi0, h, omega)     (evaluations that
+ *                      asked for grad_hyper, hess_hyper or hess_cross)
+ *   d2_out[i*21 + k] = d2 lambda_i / dp dq, k over the upper triangle p <= q row-major            (evaluations that
+ *                      asked for hess_hyper, after hawkes_row_moments_enable(ctx, 1))
+ * in the record order of that evaluation (the caller's time order for hawkes_eval; the plan's order for
+ * hawkes_eval_skip).  Either pointer may be NULL.  DEVICE buffers; copies on `stream`.  The second derivatives
+ * take 168 bytes per event of extra scratch, which hawkes_row_moments_enable allocates (1) or frees (0):
+ * that call may allocate and, when freeing, synchronises the device.  HAWKES_ERR_ARG if d2_out is wanted
+ * but not enabled.  They let a test check ell, grad_hyper and hess_hyper at sizes where the O(N^2) oracle can only
+ * afford a sample of rows. */
+int hawkes_row_moments_enable(hawkes_ctx* ctx, int enable);
+int hawkes_get_row_moments(hawkes_ctx* ctx, int64_t n, double* d1_out, double* d2_out, void* stream);
 
 /* Launch bookkeeping for benchmarks: number of kernels this context has launched since creation. */
 int64_t hawkes_launch_count(const hawkes_ctx* ctx);

@@ -20,10 +20,12 @@ def lib():
     if _lib is None:
         _lib = ctypes.CDLL(_build.build())
         _lib.hawkes_ref_eval.restype = ctypes.c_int
-        _lib.hawkes_ref_eval.argtypes = [ctypes.c_int64, ctypes.c_int] + [_dp] * 14 + [ctypes.c_int]
+        _lib.hawkes_ref_eval.argtypes = [ctypes.c_int64, ctypes.c_int] + [_dp] * 14 + [ctypes.c_int, ctypes.c_int]
         _lib.hawkes_ref_rows.restype = ctypes.c_int
         _lib.hawkes_ref_rows.argtypes = [ctypes.c_int64, ctypes.c_int, _dp, _dp, _dp, _dp,
-                                         ctypes.c_int64, _ip, _dp, _dp, ctypes.c_int]
+                                         ctypes.c_int64, _ip, _dp, _dp, _dp, ctypes.c_int, ctypes.c_int]
+        _lib.hawkes_ref_integral.restype = ctypes.c_int
+        _lib.hawkes_ref_integral.argtypes = [ctypes.c_int64, ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp, ctypes.c_int]
         _lib.hawkes_ref_cols.restype = ctypes.c_int
         _lib.hawkes_ref_cols.argtypes = [ctypes.c_int64, ctypes.c_int, _dp, _dp, _dp, _dp,
                                          ctypes.c_int64, _ip, _dp, _dp, ctypes.c_int]
@@ -54,27 +56,17 @@ class RefResult:
     row_d1: np.ndarray | None = None
 
 
-def background_mode(mode: str):
-    """Context manager: "ST" (default model) or "S" (paper-literal space-only background)."""
-    import contextlib
-
-    @contextlib.contextmanager
-    def cm():
-        l = lib()
-        l.hawkes_ref_set_background_mode.restype = ctypes.c_int
-        l.hawkes_ref_set_background_mode.argtypes = [ctypes.c_int]
-        old = l.hawkes_ref_set_background_mode(1 if mode == "S" else 0)
-        try:
-            yield
-        finally:
-            l.hawkes_ref_set_background_mode(old)
-    return cm()
+def _bg(bg: str) -> int:
+    """"ST" (default model) or "S" (paper-literal space-only background) -> the C argument."""
+    if bg not in ("ST", "S"):
+        raise ValueError("bg must be 'ST' or 'S'")
+    return 1 if bg == "S" else 0
 
 
 def evaluate(x, t, theta, params, *, grad=True, hess=False, cross=False, dense=False,
-             row_d1=False, threads: int = 1) -> RefResult:
+             row_d1=False, threads: int = 1, bg: str = "ST") -> RefResult:
     """x: [dim, n] SoA; t: [n] sorted; theta: [n]; params: 6 floats.  Always returns ll, the
-    integral Lambda(t_N) and lambda[n]; gradient / Hessian pieces on request."""
+    integral Lambda(t_N) and lambda[n]; gradient / Hessian pieces on request.  bg: background model, "ST" or "S"."""
     x = np.ascontiguousarray(x, dtype=np.float64)
     t = np.ascontiguousarray(t, dtype=np.float64)
     theta = np.ascontiguousarray(theta, dtype=np.float64)
@@ -91,7 +83,7 @@ def evaluate(x, t, theta, params, *, grad=True, hess=False, cross=False, dense=F
     hde = np.zeros(n * n) if dense else None
     rd1 = np.zeros(n * 6) if row_d1 else None
     st = lib().hawkes_ref_eval(n, dim, _p(x), _p(t), _p(theta), _p(prm), _p(ll), _p(integ), _p(lam),
-                               _p(gth), _p(ghy), _p(hth), _p(hhy), _p(hcr), _p(hde), _p(rd1), threads)
+                               _p(gth), _p(ghy), _p(hth), _p(hhy), _p(hcr), _p(hde), _p(rd1), threads, _bg(bg))
     if st < 0:
         raise ValueError(f"hawkes_ref_eval: bad argument (status {st})")
     return RefResult(status=st, ll=float(ll[0]), integral=float(integ[0]), lam=lam, grad_theta=gth,
@@ -102,8 +94,9 @@ def evaluate(x, t, theta, params, *, grad=True, hess=False, cross=False, dense=F
                      row_d1=None if rd1 is None else rd1.reshape(n, 6))
 
 
-def rows(x, t, theta, params, idx, *, derivs=True, threads: int = 1):
-    """lambda_n and d lambda_n / dp for the listed target rows."""
+def rows(x, t, theta, params, idx, *, derivs=True, second=False, threads: int = 1, bg: str = "ST"):
+    """lambda_n and d lambda_n / dp for the listed target rows; with second=True a third value, d2 lambda_n / dp dq
+    as [rows, 6, 6]."""
     x = np.ascontiguousarray(x, dtype=np.float64)
     t = np.ascontiguousarray(t, dtype=np.float64)
     theta = np.ascontiguousarray(theta, dtype=np.float64)
@@ -112,11 +105,26 @@ def rows(x, t, theta, params, idx, *, derivs=True, threads: int = 1):
     dim, n = x.shape
     lam = np.zeros(len(idx))
     d1 = np.zeros(len(idx) * 6) if derivs else None
+    d2 = np.zeros(len(idx) * 36) if second else None
     st = lib().hawkes_ref_rows(n, dim, _p(x), _p(t), _p(theta), _p(prm), len(idx),
-                               idx.ctypes.data_as(_ip), _p(lam), _p(d1), threads)
+                               idx.ctypes.data_as(_ip), _p(lam), _p(d1), _p(d2), threads, _bg(bg))
     if st != 0:
         raise ValueError(f"hawkes_ref_rows: status {st}")
+    if second:
+        return lam, (None if d1 is None else d1.reshape(-1, 6)), d2.reshape(-1, 6, 6)
     return lam, (None if d1 is None else d1.reshape(-1, 6))
+
+
+def integral(t, theta, params, dim: int, *, bg: str = "ST"):
+    """Lambda(t_N) and its first [6] and second [6, 6] derivatives in the hyperparameters (O(N))."""
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    theta = np.ascontiguousarray(theta, dtype=np.float64)
+    prm = np.asarray(params, dtype=np.float64)
+    lam, d1, d2 = np.zeros(1), np.zeros(6), np.zeros(36)
+    st = lib().hawkes_ref_integral(len(t), dim, _p(t), _p(theta), _p(prm), _p(lam), _p(d1), _p(d2), _bg(bg))
+    if st != 0:
+        raise ValueError(f"hawkes_ref_integral: status {st}")
+    return float(lam[0]), d1, d2.reshape(6, 6)
 
 
 def cols(x, t, params, lam, idx, *, threads: int = 1):

@@ -10,14 +10,30 @@ SOURCES = [SRC, os.path.join(HERE, "tree_ref.cpp")]
 LIB = os.path.join(HERE, "libhawkes_ref.so")
 
 
+STAMP = LIB + ".srchash"   # sha256 of the sources the library was built from (mtimes do not survive a copy)
+
+
+def _source_hash() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for f in SOURCES:
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(f) for f in SOURCES)):
-        return LIB
+    if not force and os.path.exists(LIB) and os.path.exists(STAMP):
+        with open(STAMP) as fh:
+            if fh.read().strip() == _source_hash():
+                return LIB
     tmp = LIB + f".tmp{os.getpid()}"
     cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra",
            "-o", tmp] + SOURCES
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
+    with open(STAMP, "w") as fh:
+        fh.write(_source_hash() + "\n")
     return LIB
 
 

@@ -53,16 +53,16 @@ const double kPi = 3.14159265358979323846264338327950288;
 //   with the integral term printed beside it, Lambda_background = mu0 t_N     (DESIGN R2: the print
 //   does not integrate the printed mu(x) -- N unit-mass kernels give mu0 N t_N -- and is followed as printed).
 // tau_t is then unused: every derivative with respect to it is 0.
-int g_bg_mode = 0;
-
+// The mode is an argument of every entry point (`bg_mode`), carried in P: no process-global state.
 struct P {
     double mu0, tau_x, tau_t, xi0, h, omega;
     double norm_b, norm_k;   // (2 pi)^-(D+1)/2 tau_x^-D tau_t^-1  and  (2 pi)^-D/2 h^-D
+    int bg_mode;
 };
 
-P make_params(const double* q, int dim) {
-    P p = {q[0], q[1], q[2], q[3], q[4], q[5], 0.0, 0.0};
-    p.norm_b = g_bg_mode == 1 ? std::pow(2.0 * kPi, -0.5 * dim) * std::pow(p.tau_x, -dim)
+P make_params(const double* q, int dim, int bg_mode) {
+    P p = {q[0], q[1], q[2], q[3], q[4], q[5], 0.0, 0.0, bg_mode == 1 ? 1 : 0};
+    p.norm_b = p.bg_mode == 1 ? std::pow(2.0 * kPi, -0.5 * dim) * std::pow(p.tau_x, -dim)
                               : std::pow(2.0 * kPi, -0.5 * (dim + 1)) * std::pow(p.tau_x, -dim) / p.tau_t;
     p.norm_k = std::pow(2.0 * kPi, -0.5 * dim) * std::pow(p.h, -dim);
     return p;
@@ -96,7 +96,7 @@ inline Pair make_pair(int dim, int64_t N, const double* x, const double* t, int6
 // Background term B_{nm} (without the indicator) and excitation kernel k_{nm} (theta-free, without
 // the causal indicator), exactly as the formulas above read.
 inline double background(const P& p, double r2, double dt) {
-    if (g_bg_mode == 1) return p.mu0 * p.norm_b * std::exp(-r2 / (2.0 * p.tau_x * p.tau_x));
+    if (p.bg_mode == 1) return p.mu0 * p.norm_b * std::exp(-r2 / (2.0 * p.tau_x * p.tau_x));
     return p.mu0 * p.norm_b * std::exp(-r2 / (2.0 * p.tau_x * p.tau_x) - dt * dt / (2.0 * p.tau_t * p.tau_t));
 }
 inline double excitation(const P& p, double r2, double dt) {
@@ -111,7 +111,7 @@ inline void dlog_background(const P& p, int dim, double r2, double dt, double g[
     h[0] = -1.0 / (p.mu0 * p.mu0);
     h[1] = -3.0 * r2 / (p.tau_x * p.tau_x * p.tau_x * p.tau_x) + dim / (p.tau_x * p.tau_x);
     h[2] = -3.0 * dt * dt / (p.tau_t * p.tau_t * p.tau_t * p.tau_t) + 1.0 / (p.tau_t * p.tau_t);
-    if (g_bg_mode == 1) g[2] = h[2] = 0.0;   // space-only background: no tau_t
+    if (p.bg_mode == 1) g[2] = h[2] = 0.0;   // space-only background: no tau_t
 }
 // same for k with (xi0, h, omega);  log k = log xi0 + log omega - D log h - omega dt - r2/(2h^2) + c.
 inline void dlog_excitation(const P& p, int dim, double r2, double dt, double g[3], double h[3]) {
@@ -166,16 +166,43 @@ void compute_row(const P& p, int dim, int64_t N, const double* x, const double* 
     *out = r;
 }
 
+// Integral term Lambda(t_N) (Eq. 7, l.253; background part per DESIGN R1/R2) and its first and second
+// derivatives in the six hyperparameters: an O(N) sum, written once and used by hawkes_ref_eval and hawkes_ref_integral.
+void integral_terms(const P& p, int64_t N, const double* t, const double* theta, ld* Lam_out, ld L1[6], ld L2[6][6]) {
+    const double tN = t[N - 1];
+    ld Lam = 0;
+    for (int a = 0; a < 6; ++a) L1[a] = 0;
+    std::memset(L2, 0, sizeof(ld) * 36);
+    {
+        ld sPhi = 0, sAphi = 0, sAphi2 = 0, sTh = 0, sThTE = 0, sThT2E = 0;
+        for (int64_t i = 0; i < N; ++i) {
+            const double a = (tN - t[i]) / p.tau_t, b = -t[i] / p.tau_t;
+            sPhi += (ld)std_normal_cdf(a) - (ld)std_normal_cdf(b);
+            sAphi += (ld)a * std_normal_pdf(a) - (ld)b * std_normal_pdf(b);
+            sAphi2 += (ld)a * std_normal_pdf(a) * (2.0 - a * a) - (ld)b * std_normal_pdf(b) * (2.0 - b * b);
+            const double T = tN - t[i];
+            const double E = std::exp(-p.omega * T);
+            sTh += (ld)theta[i] * (-std::expm1(-p.omega * T));
+            sThTE += (ld)theta[i] * T * E;
+            sThT2E += (ld)theta[i] * T * T * E;
+        }
+        if (p.bg_mode == 1) { sPhi = (ld)tN; sAphi = 0; sAphi2 = 0; }   // Lambda_background = mu0 t_N
+        Lam = (ld)p.mu0 * sPhi + (ld)p.xi0 * sTh;
+        L1[0] = sPhi;
+        L1[2] = -(ld)p.mu0 / p.tau_t * sAphi;
+        L1[3] = sTh;
+        L1[5] = (ld)p.xi0 * sThTE;
+        L2[0][2] = L2[2][0] = -sAphi / p.tau_t;
+        L2[2][2] = (ld)p.mu0 / (p.tau_t * p.tau_t) * sAphi2;
+        L2[3][5] = L2[5][3] = sThTE;
+        L2[5][5] = -(ld)p.xi0 * sThT2E;
+    }
+    *Lam_out = Lam;
+}
+
 }  // namespace
 
 extern "C" {
-
-// 0 = ST (default), 1 = S (paper-literal space-only background); returns the previous mode.  Process-global.
-int hawkes_ref_set_background_mode(int mode) {
-    const int old = g_bg_mode;
-    g_bg_mode = mode == 1 ? 1 : 0;
-    return old;
-}
 
 // Status: 0 ok; 1 some lambda_n == 0 (ell = -inf, entries dividing by it are NaN); <0 bad argument.
 // All pointers are HOST pointers; any output may be NULL (= not wanted).
@@ -184,17 +211,18 @@ int hawkes_ref_set_background_mode(int mode) {
 //   hess_theta_diag[n], hess_hyper[36] row-major, hess_cross[n*6] row-major (m, p),
 //   hess_theta_dense[n*n] row-major (small n only; O(n^3)),
 //   row_d1[n*6] row-major: d lambda_n / dp (intermediate, for error scales in the parity tests).
+//   bg_mode: 0 = ST (default model), 1 = S (paper-literal space-only background), see above.
 int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const double* theta,
                     const double* params, double* ll, double* integral, double* lambda,
                     double* grad_theta, double* grad_hyper, double* hess_theta_diag,
                     double* hess_hyper, double* hess_cross, double* hess_theta_dense, double* row_d1,
-                    int threads) {
+                    int threads, int bg_mode) {
     if (n < 1 || dim < 1 || dim > 3 || !x || !t || !theta || !params) return -1;
     for (int i = 0; i < 6; ++i)
         if (!(params[i] > 0.0) || !std::isfinite(params[i])) return -2;
     for (int64_t i = 1; i < n; ++i)
         if (t[i] < t[i - 1]) return -3;
-    const P p = make_params(params, dim);
+    const P p = make_params(params, dim, bg_mode);
     const int64_t N = n;
     const bool want_hyper = grad_hyper || hess_hyper || hess_cross || row_d1;
     const bool want_cols = grad_theta || hess_theta_diag || hess_cross || hess_theta_dense;
@@ -225,32 +253,8 @@ int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const 
 
     // ---- integral Lambda(t_N) and its derivatives ----
     const double tN = t[N - 1];
-    ld Lam = 0, L1[6] = {0, 0, 0, 0, 0, 0}, L2[6][6];
-    std::memset(L2, 0, sizeof(L2));
-    {
-        ld sPhi = 0, sAphi = 0, sAphi2 = 0, sTh = 0, sThTE = 0, sThT2E = 0;
-        for (int64_t i = 0; i < N; ++i) {
-            const double a = (tN - t[i]) / p.tau_t, b = -t[i] / p.tau_t;
-            sPhi += (ld)std_normal_cdf(a) - (ld)std_normal_cdf(b);
-            sAphi += (ld)a * std_normal_pdf(a) - (ld)b * std_normal_pdf(b);
-            sAphi2 += (ld)a * std_normal_pdf(a) * (2.0 - a * a) - (ld)b * std_normal_pdf(b) * (2.0 - b * b);
-            const double T = tN - t[i];
-            const double E = std::exp(-p.omega * T);
-            sTh += (ld)theta[i] * (-std::expm1(-p.omega * T));
-            sThTE += (ld)theta[i] * T * E;
-            sThT2E += (ld)theta[i] * T * T * E;
-        }
-        if (g_bg_mode == 1) { sPhi = (ld)tN; sAphi = 0; sAphi2 = 0; }   // Lambda_background = mu0 t_N
-        Lam = (ld)p.mu0 * sPhi + (ld)p.xi0 * sTh;
-        L1[0] = sPhi;
-        L1[2] = -(ld)p.mu0 / p.tau_t * sAphi;
-        L1[3] = sTh;
-        L1[5] = (ld)p.xi0 * sThTE;
-        L2[0][2] = L2[2][0] = -sAphi / p.tau_t;
-        L2[2][2] = (ld)p.mu0 / (p.tau_t * p.tau_t) * sAphi2;
-        L2[3][5] = L2[5][3] = sThTE;
-        L2[5][5] = -(ld)p.xi0 * sThT2E;
-    }
+    ld Lam = 0, L1[6], L2[6][6];
+    integral_terms(p, N, t, theta, &Lam, L1, L2);
     if (integral) *integral = (double)Lam;
 
     // ---- log-likelihood (Eq. 1) ----
@@ -333,13 +337,13 @@ int hawkes_ref_eval(int64_t n, int dim, const double* x, const double* t, const 
 }
 
 // Sampled evaluation for parity at sizes where the full oracle is too slow: the listed rows'
-// lambda_n and d lambda_n/dp (row_d1[k*6+p]), and the listed columns' c_m = sum_{t_m<t_n} k_nm/lambda_n
+// lambda_n, d lambda_n/dp (row_d1[k*6+p]) and d2 lambda_n/dp dq (row_d2[k*36+p*6+q]), and the listed columns' c_m = sum_{t_m<t_n} k_nm/lambda_n
 // and d_m = sum (k_nm/lambda_n)^2 given a full lambda vector supplied by the caller.
 int hawkes_ref_rows(int64_t n, int dim, const double* x, const double* t, const double* theta,
                     const double* params, int64_t n_rows, const int64_t* rows_idx, double* row_lambda,
-                    double* row_d1, int threads) {
+                    double* row_d1, double* row_d2, int threads, int bg_mode) {
     if (n < 1 || dim < 1 || dim > 3) return -1;
-    const P p = make_params(params, dim);
+    const P p = make_params(params, dim, bg_mode);
     (void)threads;
 #ifdef _OPENMP
     const int nthreads = threads > 0 ? threads : 1;
@@ -347,10 +351,13 @@ int hawkes_ref_rows(int64_t n, int dim, const double* x, const double* t, const 
 #endif
     for (int64_t k = 0; k < n_rows; ++k) {
         Row r;
-        compute_row(p, dim, n, x, t, theta, rows_idx[k], row_d1 != nullptr, &r);
+        compute_row(p, dim, n, x, t, theta, rows_idx[k], row_d1 != nullptr || row_d2 != nullptr, &r);
         row_lambda[k] = (double)r.lam;
         if (row_d1)
             for (int a = 0; a < 6; ++a) row_d1[k * 6 + a] = (double)r.d1[a];
+        if (row_d2)
+            for (int a = 0; a < 6; ++a)
+                for (int c = 0; c < 6; ++c) row_d2[k * 36 + a * 6 + c] = (double)r.d2[a][c];
     }
     return 0;
 }
@@ -359,7 +366,7 @@ int hawkes_ref_cols(int64_t n, int dim, const double* x, const double* t, const 
                     const double* lambda, int64_t n_cols, const int64_t* cols_idx, double* col_c,
                     double* col_d, int threads) {
     if (n < 1 || dim < 1 || dim > 3) return -1;
-    const P p = make_params(params, dim);
+    const P p = make_params(params, dim, 0);   // the excitation kernel does not depend on the background mode
     (void)threads;
 #ifdef _OPENMP
     const int nthreads = threads > 0 ? threads : 1;
@@ -377,6 +384,22 @@ int hawkes_ref_cols(int64_t n, int dim, const double* x, const double* t, const 
         }
         col_c[k] = (double)c;
         col_d[k] = (double)d;
+    }
+    return 0;
+}
+
+// Lambda(t_N) and its hyperparameter derivatives alone (O(N)): integral[1], d1[6], d2[36] row-major.
+int hawkes_ref_integral(int64_t n, int dim, const double* t, const double* theta, const double* params,
+                        double* integral, double* d1, double* d2, int bg_mode) {
+    if (n < 1 || dim < 1 || dim > 3 || !t || !theta || !params) return -1;
+    const P p = make_params(params, dim, bg_mode);
+    ld Lam, L1[6], L2[6][6];
+    integral_terms(p, n, t, theta, &Lam, L1, L2);
+    if (integral) *integral = (double)Lam;
+    for (int a = 0; a < 6; ++a) {
+        if (d1) d1[a] = (double)L1[a];
+        for (int c = 0; c < 6; ++c)
+            if (d2) d2[a * 6 + c] = (double)L2[a][c];
     }
     return 0;
 }

@@ -17,6 +17,7 @@ WANT_LL, WANT_GRAD_THETA, WANT_GRAD_HYPER, WANT_HESS_THETA, WANT_HESS_HYPER, WAN
 WANT_GRAD = WANT_LL | WANT_GRAD_THETA | WANT_GRAD_HYPER
 WANT_ALL = 63
 BG_SPACE_TIME, BG_SPACE_ONLY = 0, 1
+PASS1_AUTO, PASS1_DENSE = 0, 1
 
 
 class HawkesError(RuntimeError):
@@ -77,15 +78,41 @@ class HawkesContext:
     def _stream(self):
         return ctypes.c_void_p(self._torch.cuda.current_stream(self._dev).cuda_stream)
 
-    def _check_inputs(self, x, t, theta):
+    def _check_dev(self, a, name, shape=None, dtype=None, optional=False):
+        """Every pointer handed to a device-pointer entry point: a contiguous tensor of the expected dtype (float64
+        unless given) and shape on this context's device.  A host tensor or an int32 index would otherwise reach
+        the kernels as a wild address."""
+        torch = self._torch
+        if a is None:
+            if optional:
+                return
+            raise ValueError(f"{name} is required")
+        dtype = torch.float64 if dtype is None else dtype
+        if not a.is_cuda or a.device.index != self.device:
+            raise ValueError(f"{name} must be a CUDA tensor on device {self.device}")
+        if a.dtype != dtype or not a.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous {dtype} tensor")
+        if shape is not None and tuple(a.shape) != tuple(shape):
+            raise ValueError(f"{name} must have shape {tuple(shape)}, got {tuple(a.shape)}")
+
+    def _check_inputs(self, x, t, theta, host=False):
         torch = self._torch
         for a in (x, t, theta):
             if a.dtype != torch.float64 or not a.is_contiguous():
                 raise ValueError("x, t, theta must be contiguous float64 tensors")
+            if host and a.is_cuda:
+                raise ValueError("eval_host() takes host tensors")
+            if not host and (not a.is_cuda or a.device.index != self.device):
+                raise ValueError(f"x, t, theta must be CUDA tensors on device {self.device}; use eval_host() for host buffers")
         n = t.shape[0]
         if x.shape != (self.dim, n) or theta.shape != (n,):
             raise ValueError("expected x [dim, n] (SoA), t [n], theta [n]")
         return n
+
+    def _check_out(self, r, n):
+        for name, shape in (("ll", (1,)), ("grad_theta", (n,)), ("grad_hyper", (6,)), ("hess_theta_diag", (n,)),
+                            ("hess_hyper", (6, 6)), ("hess_cross", (n, 6))):
+            self._check_dev(getattr(r, name), "out." + name, shape, optional=True)
 
     def _outputs(self, n, want, device, pinned=False):
         torch = self._torch
@@ -106,9 +133,8 @@ class HawkesContext:
     def eval(self, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None) -> EvalResult:
         """hawkes_eval: device tensors in, device tensors out, asynchronous on the current stream."""
         n = self._check_inputs(x, t, theta)
-        if not x.is_cuda:
-            raise ValueError("eval() takes CUDA tensors; use eval_host() for host buffers")
         r = out if out is not None else self._outputs(n, want, self._dev)
+        self._check_out(r, n)
         p = _params(params)
         rc = self._lib.hawkes_eval(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want,
                                    _ptr(r.ll), _ptr(r.grad_theta), _ptr(r.grad_hyper), _ptr(r.hess_theta_diag),
@@ -122,6 +148,9 @@ class HawkesContext:
         and hyperparameters (synchronous, host work).  Returns the item counts of hawkes_skip_stats."""
         if x.dim() != 2 or x.shape[0] != self.dim or t.shape[0] != x.shape[1]:
             raise ValueError("x must be (dim, n) and t (n,)")
+        for a in (x, t):
+            if a.dtype != self._torch.float64 or not a.is_contiguous():
+                raise ValueError("x and t must be contiguous float64 tensors (host or device)")
         n = int(t.shape[0])
         p = _params(params)
         rc = self._lib.hawkes_skip_plan(self._h, n, _ptr(x), _ptr(t), ctypes.byref(p))
@@ -147,9 +176,8 @@ class HawkesContext:
         """hawkes_eval_skip: hawkes_eval over the work lists of skip_plan (same arguments, same outputs in the
         caller's event order, no cross block); the events need not be sorted by time."""
         n = self._check_inputs(x, t, theta)
-        if not x.is_cuda:
-            raise ValueError("eval_skip() takes CUDA tensors")
         r = out if out is not None else self._outputs(n, want, self._dev)
+        self._check_out(r, n)
         p = _params(params)
         rc = self._lib.hawkes_eval_skip(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want,
                                         _ptr(r.ll), _ptr(r.grad_theta), _ptr(r.grad_hyper), _ptr(r.hess_theta_diag),
@@ -170,6 +198,7 @@ class HawkesContext:
     def grad(self, x, t, theta, params, out: EvalResult | None = None) -> EvalResult:
         n = self._check_inputs(x, t, theta)
         r = out if out is not None else self._outputs(n, WANT_GRAD, self._dev)
+        self._check_out(r, n)
         p = _params(params)
         rc = self._lib.hawkes_grad(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), _ptr(r.ll),
                                    _ptr(r.grad_theta), _ptr(r.grad_hyper), self._stream())
@@ -181,6 +210,7 @@ class HawkesContext:
         n = self._check_inputs(x, t, theta)
         want = WANT_HESS_THETA | WANT_HESS_HYPER | (WANT_HESS_CROSS if cross else 0)
         r = out if out is not None else self._outputs(n, want, self._dev)
+        self._check_out(r, n)
         p = _params(params)
         rc = self._lib.hawkes_hessian(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p),
                                       _ptr(r.hess_theta_diag), _ptr(r.hess_hyper), _ptr(r.hess_cross), self._stream())
@@ -191,10 +221,12 @@ class HawkesContext:
     def eval_host(self, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None) -> EvalResult:
         """hawkes_eval_host: HOST tensors (pinned or pageable) in and out; copies run inside the call,
         which synchronises the stream and returns the evaluation's device status in `.status`."""
-        n = self._check_inputs(x, t, theta)
-        if x.is_cuda:
-            raise ValueError("eval_host() takes host tensors")
+        n = self._check_inputs(x, t, theta, host=True)
         r = out if out is not None else self._outputs(n, want, "cpu")
+        for name in ("ll", "grad_theta", "grad_hyper", "hess_theta_diag", "hess_hyper", "hess_cross"):
+            o = getattr(r, name)
+            if o is not None and (o.is_cuda or o.dtype != self._torch.float64 or not o.is_contiguous()):
+                raise ValueError(f"out.{name} must be a contiguous float64 host tensor")
         p = _params(params)
         rc = self._lib.hawkes_eval_host(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want,
                                         _ptr(r.ll), _ptr(r.grad_theta), _ptr(r.grad_hyper), _ptr(r.hess_theta_diag),
@@ -217,6 +249,7 @@ class HawkesContext:
         """hawkes_hessian_theta_block: the dense m x m Hessian of ell in the rates of the events idx (device tensor)."""
         n = self._check_inputs(x, t, theta)
         m = int(idx.shape[0])
+        self._check_dev(idx, "idx", (m,), self._torch.int64)
         H = self._torch.empty(m, m, dtype=self._torch.float64, device=self._dev)
         p = _params(params)
         rc = self._lib.hawkes_hessian_theta_block(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), m, _ptr(idx),
@@ -241,6 +274,11 @@ class HawkesContext:
     def theta_from_z(self, n: int, idx, z, beta: float, t, out=None):
         """hawkes_theta_from_z: idx int64 [m], z [m], t [n] device tensors -> theta [n]."""
         theta = out if out is not None else self._torch.empty(n, dtype=self._torch.float64, device=self._dev)
+        m = int(idx.shape[0])
+        self._check_dev(idx, "idx", (m,), self._torch.int64)
+        self._check_dev(z, "z", (m,))
+        self._check_dev(t, "t", (n,))
+        self._check_dev(theta, "theta", (n,))
         rc = self._lib.hawkes_theta_from_z(self._h, n, int(idx.shape[0]), _ptr(idx), _ptr(z), float(beta), _ptr(t),
                                            _ptr(theta), self._stream())
         if rc != 0:
@@ -251,6 +289,12 @@ class HawkesContext:
         """hawkes_z_chain: returns (grad_z [m], hess_z [m] or None, grad_beta [1] or None)."""
         torch = self._torch
         n, m = int(theta.shape[0]), int(idx.shape[0])
+        self._check_dev(idx, "idx", (m,), torch.int64)
+        self._check_dev(theta, "theta", (n,))
+        self._check_dev(t, "t", (n,), optional=not want_beta)
+        self._check_dev(grad_theta, "grad_theta", (n,))
+        self._check_dev(hess_theta_diag, "hess_theta_diag", (n,), optional=True)
+        self._check_dev(prior_grad_z, "prior_grad_z", (m,), optional=True)
         gz = torch.empty(m, dtype=torch.float64, device=self._dev)
         hz = torch.empty(m, dtype=torch.float64, device=self._dev) if hess_theta_diag is not None else None
         gb = torch.empty(1, dtype=torch.float64, device=self._dev) if want_beta else None
@@ -266,9 +310,16 @@ class HawkesContext:
         `out` = a previous return value to reuse its buffers; skip=True: hawkes_posterior_z_skip (after skip_plan)."""
         torch = self._torch
         n, m = int(t.shape[0]), int(idx.shape[0])
+        self._check_dev(x, "x", (self.dim, n))
+        self._check_dev(t, "t", (n,))
+        self._check_dev(idx, "idx", (m,), torch.int64)
+        self._check_dev(z, "z", (m,))
         if out is None:
             mk = lambda k: torch.empty(k, dtype=torch.float64, device=self._dev)
             out = (mk(3), mk(m), mk(m) if hess else None)
+        self._check_dev(out[0], "out[0]", (3,), optional=True)
+        self._check_dev(out[1], "out[1]", (m,), optional=True)
+        self._check_dev(out[2], "out[2]", (m,), optional=True)
         p = _params(params)
         fn = self._lib.hawkes_posterior_z_skip if skip else self._lib.hawkes_posterior_z
         rc = fn(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
@@ -289,6 +340,15 @@ class HawkesContext:
             raise ValueError("normals must be [n_iter, m] contiguous and uniforms [n_iter]")
         if trace is None:
             trace = torch.empty(n_iter, 4, dtype=torch.float64, device=self._dev)
+        self._check_dev(x, "x", (self.dim, n))
+        self._check_dev(t, "t", (n,))
+        self._check_dev(idx, "idx", (m,), torch.int64)
+        self._check_dev(z, "z", (m,))
+        self._check_dev(mass, "mass", (m,))
+        self._check_dev(normals, "normals", (n_iter, m))
+        self._check_dev(uniforms, "uniforms", (n_iter,))
+        self._check_dev(prior_prec, "prior_prec", (m,), optional=True)
+        self._check_dev(trace, "trace", (n_iter, 4))
         o = HmcOpts(int(n_iter), int(n_leapfrog), int(precond_every), int(n_refresh_done), float(step),
                     float(mass_floor), int(cache_background), 0)
         p = _params(params)
@@ -304,6 +364,31 @@ class HawkesContext:
         rc = self._lib.hawkes_set_background_mode(self._h, int(mode))
         if rc != 0:
             raise HawkesError(rc, "hawkes_set_background_mode")
+
+    def set_pass1_mode(self, mode: int):
+        """hawkes_set_pass1_mode: PASS1_AUTO (background once per unordered pair where it applies) or PASS1_DENSE."""
+        rc = self._lib.hawkes_set_pass1_mode(self._h, int(mode))
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_set_pass1_mode")
+
+    def pass1_is_symmetric(self, level: int) -> bool:
+        return bool(self._lib.hawkes_pass1_is_symmetric(self._h, int(level)))
+
+    def row_moments_enable(self, enable: bool = True):
+        rc = self._lib.hawkes_row_moments_enable(self._h, 1 if enable else 0)
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_row_moments_enable")
+
+    def get_row_moments(self, n: int, second: bool = False):
+        """hawkes_get_row_moments: d lambda_n/dp [n, 6] (and d2 lambda_n/dp dq [n, 21], upper triangle) of the last
+        evaluation; device tensors."""
+        torch = self._torch
+        d1 = torch.empty(n, 6, dtype=torch.float64, device=self._dev)
+        d2 = torch.empty(n, 21, dtype=torch.float64, device=self._dev) if second else None
+        rc = self._lib.hawkes_get_row_moments(self._h, n, _ptr(d1), _ptr(d2), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_get_row_moments")
+        return (d1, d2) if second else d1
 
     def get_lambda(self, n: int):
         lam = self._torch.empty(n, dtype=self._torch.float64, device=self._dev)
@@ -379,6 +464,9 @@ class HawkesTree:
         torch = self._torch
         lp = torch.empty(1, dtype=torch.float64, device=self._dev)
         g = torch.empty(self.n_tips, dtype=torch.float64, device=self._dev) if grad else None
+        if (not z.is_cuda or z.device.index != self.device or z.dtype != torch.float64 or not z.is_contiguous()
+                or tuple(z.shape) != (self.n_tips,)):
+            raise ValueError(f"z must be a contiguous float64 CUDA tensor of {self.n_tips} entries on device {self.device}")
         st = ctypes.c_void_p(torch.cuda.current_stream(self._dev).cuda_stream)
         rc = self._lib.hawkes_tree_prior(self._h, _ptr(z), float(sigma2), float(tau0), _ptr(lp), _ptr(g), st)
         if rc != 0:

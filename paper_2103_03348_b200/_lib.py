@@ -38,6 +38,10 @@ SYMBOLS = {
     "hawkes_hessian_theta_dense": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, vp]),
     "hawkes_sort_events": (cint, [vp, i64, cint, _dp, _dp, _dp, _dp, _dp, _dp, vp, vp]),
     "hawkes_get_lambda": (cint, [vp, i64, _dp, vp]),
+    "hawkes_set_pass1_mode": (cint, [vp, cint]),
+    "hawkes_pass1_is_symmetric": (cint, [vp, cint]),
+    "hawkes_row_moments_enable": (cint, [vp, cint]),
+    "hawkes_get_row_moments": (cint, [vp, i64, _dp, _dp, vp]),
     "hawkes_skip_plan": (cint, [vp, i64, _dp, _dp, PP]),
     "hawkes_eval_skip": (cint, [vp, i64, _dp, _dp, _dp, PP, u32, _dp, _dp, _dp, _dp, _dp, vp]),
     "hawkes_skip_stats": (cint, [vp, vp]),
@@ -78,11 +82,11 @@ def load():
     if not _build.up_to_date():
         try:
             _build.build()
-        except Exception as exc:   # no nvcc on this machine, or compile error
-            if not os.path.exists(path):
-                raise ImportError(
-                    f"paper_2103_03348_b200: CUDA library {path} is missing and could not be built "
-                    f"({exc}); run `python -m paper_2103_03348_b200.build` on a machine with nvcc") from exc
+        except Exception as exc:   # no nvcc on this machine, or compile error: never run a stale library silently
+            what = "is older than its sources" if os.path.exists(path) else "is missing"
+            raise ImportError(
+                f"paper_2103_03348_b200: CUDA library {path} {what} and could not be rebuilt "
+                f"({exc}); run `python -m paper_2103_03348_b200.build` on a machine with nvcc") from exc
     lib = ctypes.CDLL(path)
     for name, (res, args) in SYMBOLS.items():
         fn = getattr(lib, name)   # AttributeError if the symbol is not exported

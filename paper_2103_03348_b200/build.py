@@ -22,8 +22,25 @@ def nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+STAMP = LIB + ".srchash"   # sha256 of the sources the library was built from (mtimes do not survive a copy of the tree)
+
+
+def source_hash() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for d in DEPS:
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as fh:
+            h.update(fh.read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()
+
+
 def up_to_date() -> bool:
-    return os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)
+    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
+        return False
+    with open(STAMP) as fh:
+        return fh.read().strip() == source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -39,6 +56,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with open(os.path.join(HERE, "ptxas_info.log"), "w") as fh:
         fh.write(res.stderr)
     os.replace(tmp, LIB)
+    with open(STAMP, "w") as fh:
+        fh.write(source_hash() + "\n")
     return LIB
 
 

@@ -552,13 +552,14 @@ __device__ __forceinline__ double norm_cdf(double z) { return 0.5 * erfc(-z * 0.
 //   k = 7..27    sum [lambda_pq/lambda - lambda_p lambda_q/lambda^2], upper triangle row-major
 //   k = 28..30   sum [Phi(a)-Phi(b)],  sum [a phi(a) - b phi(b)],  sum [a phi(a)(2-a^2) - b phi(b)(2-b^2)]
 //   k = 31..33   sum theta (1-E),  sum theta T E,  sum theta T^2 E        (T = t_N - t_n, E = e^{-omega T})
-// glam[n*6 + p] = lambda_{n,p} / lambda_n^2 (only when `glam` != NULL; feeds the cross block).
+// rowd1[n*6 + p] = d lambda_n / dp (LEVEL >= 1, when `rowd1` != NULL: feeds the cross block and hawkes_get_row_moments);
+// rowd2[n*21 + k] = d2 lambda_n / dp dq, upper triangle row-major (LEVEL 2, when `rowd2` != NULL: diagnostics only).
 template <int LEVEL, bool DIM3>
 __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                         DevConsts c, const double* __restrict__ part,
                                                         Split sp, double* __restrict__ lam,
                                                         double* __restrict__ trec, double* __restrict__ trec2,
-                                                        double* __restrict__ glam,
+                                                        double* __restrict__ rowd1, double* __restrict__ rowd2,
                                                         double* __restrict__ blockpart,
                                                         unsigned* __restrict__ status, double* __restrict__ bgcache,
                                                         int bg_mode, const double* __restrict__ partc, int sym_tiles,
@@ -640,6 +641,10 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
         {
             const double tref = rec[(i / TS) * TS * RS + (DIM3 ? 3 : 2)];
             const double W = iL * exp(-c.omega * (e.t - tref));
+            // status[1] bit 1: some weight is so large (lambda_n below ~1e-150, or zero) that the square of a factorised
+            // term G W_n could overflow although the term itself, (F G W_n)^2, is representable: the d_m sums of pass 2
+            // then keep the unfactorised form
+            if (!(W <= 0x1p500)) atomicOr(status + 1, 2u);
             if (!DIM3) {
                 reinterpret_cast<double4*>(trec2)[i] = make_double4(e.x, e.y, e.t, W);
             } else {
@@ -663,9 +668,9 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
             if (c.s_mode) d1[2] = 0.0;   // space-only background: lambda does not depend on tau_t
 #pragma unroll
             for (int p = 0; p < 6; ++p) v[1 + p] = d1[p] * iL;
-            if (glam != nullptr) {
+            if (rowd1 != nullptr) {
 #pragma unroll
-                for (int p = 0; p < 6; ++p) glam[i * 6 + p] = d1[p] * iL * iL;
+                for (int p = 0; p < 6; ++p) rowd1[i * 6 + p] = d1[p];
             }
             if (LEVEL >= 2) {
                 const double SBr4 = c.CBS * b[3], SBr2d2 = c.CBS * b[4], SBd4 = c.CBS * b[5];
@@ -693,6 +698,7 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
 #pragma unroll
                     for (int q = p; q < 6; ++q) {
                         v[k] = d2[p][q] * iL - (d1[p] * iL) * (d1[q] * iL);
+                        if (rowd2 != nullptr) rowd2[i * 21 + (k - 7)] = d2[p][q];
                         ++k;
                     }
             }
@@ -853,7 +859,9 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
     if (lo >= total) return;
     const int64_t hi = min(lo + sp.chunk, total);
     const P1C pc_ = pinned_consts(smagic, c);
-    const bool fact = status[1] == 0;   // warp-uniform: set by prep_kernel for the whole evaluation
+    // warp-uniform, fixed for the whole evaluation: bit 0 (prep_kernel) a streamed tile spans too much time, bit 1
+    // (reduce1_kernel) a weight too large for the squares of the d_m sums
+    const bool fact = (status[1] & (LEVEL >= 1 ? 3u : 1u)) == 0;
 
     for (int M = split_tile_of(sp, lo); M < sp.n_tiles; ++M) {
         const int64_t base = split_prefix(sp, M);
@@ -904,7 +912,7 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
                     for (int r = 0; r < R; ++r) {
                         const double F = exp(-c.omega * (tref - g[r].t));
                         cm[r] = fma(F, pc[r], cm[r]);
-                        if (LEVEL >= 1) dm[r] = fma(F * F, pd[r], dm[r]);
+                        if (LEVEL >= 1) dm[r] = fma(F, F * pd[r], dm[r]);   // F (F pd): F F alone underflows before the term does
                     }
                 } else {
                     p2_tile<R, LEVEL, false, DIM3>(sb, cnt, g, cm, dm, pc_, lane_base);
@@ -973,7 +981,7 @@ __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__
 //   cross[m][p] = sum_n k_nm [ (dlog k_nm/dp) / lambda_n - lambda_{n,p} / lambda_n^2 ] - dLambda/(dtheta_m dp)
 template <bool DIM3>
 __global__ void __launch_bounds__(RED_T) cross_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
-                                                      const double* __restrict__ glam, int64_t n, DevConsts c,
+                                                      const double* __restrict__ rowd1, int64_t n, DevConsts c,
                                                       double* __restrict__ cross) {
     constexpr int RS = DIM3 ? 6 : 4;
     const int64_t m = (int64_t)blockIdx.x * RED_T + threadIdx.x;
@@ -991,7 +999,7 @@ __global__ void __launch_bounds__(RED_T) cross_kernel(const double* __restrict__
         const double a = k * s.w;
         const double gl[3] = {1.0 / c.xi0, u / (c.h * c.h * c.h) - D / c.h, 1.0 / c.omega - dt};
 #pragma unroll
-        for (int p = 0; p < 6; ++p) acc[p] += a * (p >= 3 ? gl[p - 3] : 0.0) - k * glam[i * 6 + p];
+        for (int p = 0; p < 6; ++p) acc[p] += a * (p >= 3 ? gl[p - 3] : 0.0) - a * (rowd1[i * 6 + p] * s.w);
     }
     const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
     const double T = tN - g.t;
@@ -1221,7 +1229,9 @@ struct hawkes_ctx {
     int64_t plan_n;
     int plan_l1, plan_l2;
     double* d_lam;        // n_max
-    double* d_glam;       // n_max * 6
+    double* d_rowd1;      // n_max * 6: d lambda_n / dp of the last evaluation at LEVEL >= 1
+    double* d_rowd2;      // n_max * 21 or NULL: d2 lambda_n / dp dq (hawkes_row_moments_enable)
+    int force_dense;      // hawkes_set_pass1_mode: 1 = dense ordered-pair pass 1 even where the symmetric form applies
     double* d_blockpart;  // nblk_max * NRED
     double* d_scal;       // 2 (sum log lambda, Lambda) + peak scratch
     double* d_in;         // staging for hawkes_eval_host: x[dim*n_max], t, theta
@@ -1383,7 +1393,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     const int bg_mode = level1 == 0 ? ctx->bg_mode : 0;   // the cache holds the LEVEL-0 sum only
     const int no_bg = bg_mode == 2 ? 1 : 0;
     // symmetric pass 1 (background once per unordered pair) for levels 0 and 1 unless the cached-background path runs
-    const int sym = (ctx->d_partc != nullptr && level1 <= 1 && !no_bg) ? 1 : 0;
+    const int sym = (ctx->d_partc != nullptr && level1 <= 1 && !no_bg && !ctx->force_dense) ? 1 : 0;
     if (ctx->plan_n != n || ctx->plan_l1 != level1 || ctx->plan_l2 != level2 || ctx->plan_bg != no_bg ||
         ctx->plan_sym != sym || ctx->plan_reserve != ctx->reserve_sm) {
         const int sms = ctx->sm_count > ctx->reserve_sm ? ctx->sm_count - ctx->reserve_sm : 1;
@@ -1406,7 +1416,8 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     prep_kernel<<<pl.nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status, c.omega);
     ctx->launches++;
     const unsigned g1 = (unsigned)((pl.grid1 + P1_G[level1] - 1) / P1_G[level1]);
-    double* glam = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_glam : nullptr;
+    double* const rowd1 = level1 >= 1 ? ctx->d_rowd1 : nullptr;
+    double* const rowd2 = level1 >= 2 ? ctx->d_rowd2 : nullptr;
     if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
@@ -1417,7 +1428,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
         case 1:
             if (sym)
@@ -1425,12 +1436,12 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, glam, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
     }
     ctx->launches += 2;
@@ -1468,7 +1479,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         CK(cudaEventRecord(pe[4], st));
     }
     if (want & HAWKES_WANT_HESS_CROSS) {
-        cross_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, ctx->d_trec, ctx->d_glam, n, c, hess_cross);
+        cross_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, ctx->d_trec, ctx->d_rowd1, n, c, hess_cross);
         ctx->launches++;
     }
     if (scal_aside) CK(cudaStreamWaitEvent(st, ctx->ev_join, 0));
@@ -1557,6 +1568,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->plan_l1 = c->plan_l2 = -1;
     c->bg_mode = 0;
     c->s_mode = 0;
+    c->force_dense = 0;
     c->kmat_doubles = c->kmisc_doubles = 0;
     c->d_ksp_a = c->d_ksp_b = nullptr;
     c->ksp_a_bytes = c->ksp_b_bytes = 0;
@@ -1589,7 +1601,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     bool ok = true;
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_trec2, (void**)&c->d_part1, (void**)&c->d_part2,
-                     (void**)&c->d_lam, (void**)&c->d_glam, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
+                     (void**)&c->d_lam, (void**)&c->d_rowd1, (void**)&c->d_rowd2, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
                      (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_kmat, (void**)&c->d_kmisc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
@@ -1599,7 +1611,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_part1, sizeof(double) * c->part1_doubles);
     alloc((void**)&c->d_part2, sizeof(double) * c->part2_doubles);
     alloc((void**)&c->d_lam, sizeof(double) * (size_t)c->ld_max);
-    alloc((void**)&c->d_glam, sizeof(double) * 6 * (size_t)c->ld_max);
+    alloc((void**)&c->d_rowd1, sizeof(double) * 6 * (size_t)c->ld_max);
     alloc((void**)&c->d_blockpart, sizeof(double) * NRED * (size_t)nblk);
     alloc((void**)&c->d_scal, sizeof(double) * 8);
     alloc((void**)&c->d_in, sizeof(double) * (size_t)(dim + 2) * (size_t)n_max);
@@ -1607,11 +1619,10 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_post, sizeof(double) * (size_t)(8 + 4 * n_max));
     alloc((void**)&c->d_hmc, sizeof(double) * (size_t)(16 + 5 * n_max));
     alloc((void**)&c->d_bgcache, sizeof(double) * (size_t)n_max);
-    {   // column partials of the symmetric pass 1 (levels 0 and 1: NB <= 3); HAWKES_DENSE_PASS1=1 disables that path
+    {   // column partials of the symmetric pass 1 (levels 0 and 1: NB <= 3); above 16 GB the dense kernel runs instead
         const int nt = (int)((n_max + NT * P1_R - 1) / (NT * P1_R));
         c->partc_doubles = (size_t)colpart_doubles(nt, NT * P1_R, 3);
-        const char* dense = getenv("HAWKES_DENSE_PASS1");
-        if ((dense && dense[0] == '1') || c->partc_doubles * sizeof(double) > ((size_t)16 << 30)) c->partc_doubles = 0;
+        if (c->partc_doubles * sizeof(double) > ((size_t)16 << 30)) c->partc_doubles = 0;
         if (c->partc_doubles) alloc((void**)&c->d_partc, sizeof(double) * c->partc_doubles);
     }
     alloc((void**)&c->d_status, sizeof(unsigned) * 2);
@@ -1643,7 +1654,7 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     skip_plan_free(c);
-    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_glam, c->d_blockpart,
+    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_rowd1, c->d_rowd2, c->d_blockpart,
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -2106,6 +2117,43 @@ int hawkes_hessian_theta_block(hawkes_ctx* ctx, int64_t n, const double* x, cons
 int hawkes_set_background_mode(hawkes_ctx* ctx, int mode) {
     if (!ctx || (mode != HAWKES_BG_SPACE_TIME && mode != HAWKES_BG_SPACE_ONLY)) return HAWKES_ERR_ARG;
     ctx->s_mode = mode == HAWKES_BG_SPACE_ONLY ? 1 : 0;
+    return HAWKES_OK;
+}
+
+int hawkes_set_pass1_mode(hawkes_ctx* ctx, int mode) {
+    if (!ctx || (mode != HAWKES_PASS1_AUTO && mode != HAWKES_PASS1_DENSE)) return HAWKES_ERR_ARG;
+    ctx->force_dense = mode == HAWKES_PASS1_DENSE ? 1 : 0;
+    return HAWKES_OK;
+}
+
+int hawkes_pass1_is_symmetric(const hawkes_ctx* ctx, int level) {
+    if (!ctx || level < 0 || level > 2) return 0;
+    return (ctx->d_partc != nullptr && level <= 1 && !ctx->force_dense) ? 1 : 0;
+}
+
+int hawkes_row_moments_enable(hawkes_ctx* ctx, int enable) {
+    if (!ctx) return HAWKES_ERR_ARG;
+    CK(cudaSetDevice(ctx->device));
+    if (enable && !ctx->d_rowd2) {
+        if (cudaMalloc((void**)&ctx->d_rowd2, sizeof(double) * 21 * (size_t)ctx->ld_max) != cudaSuccess) {
+            cudaGetLastError();
+            ctx->d_rowd2 = nullptr;
+            return HAWKES_ERR_NOMEM;
+        }
+    } else if (!enable && ctx->d_rowd2) {
+        CK(cudaDeviceSynchronize());   // an evaluation in flight may still write it
+        cudaFree(ctx->d_rowd2);
+        ctx->d_rowd2 = nullptr;
+    }
+    return HAWKES_OK;
+}
+
+int hawkes_get_row_moments(hawkes_ctx* ctx, int64_t n, double* d1_out, double* d2_out, void* stream) {
+    if (!ctx || (!d1_out && !d2_out) || n < 1 || n > ctx->n_max) return HAWKES_ERR_ARG;
+    if (d2_out && !ctx->d_rowd2) return HAWKES_ERR_ARG;
+    CK(cudaSetDevice(ctx->device));
+    if (d1_out) CK(cudaMemcpyAsync(d1_out, ctx->d_rowd1, sizeof(double) * 6 * n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    if (d2_out) CK(cudaMemcpyAsync(d2_out, ctx->d_rowd2, sizeof(double) * 21 * n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return HAWKES_OK;
 }
 

@@ -250,11 +250,7 @@ __global__ void HAWKES_SYM_BOUNDS pass1s_kernel(const double* __restrict__ rec, 
             const bool plain = !ragged_tile && b <= i0 && rec[(b - 1) * RS + TOFF] < t_first;
             for (int j0 = 0; j0 < cnt; j0 += 32) {
                 const int nvalid = min(32, cnt - j0);
-#ifdef HAWKES_EXPERIMENT_UNIFORM
-                if (sp.n_tiles > 0)
-#else
                 if (plain && nvalid == 32)
-#endif
                     p1s_block<R, LEVEL, false, DIM3>(sb, j0, nvalid, a + j0, g, gi, m, mycol, pc, lane_base, lane);
                 else
                     p1s_block<R, LEVEL, true, DIM3>(sb, j0, nvalid, a + j0, g, gi, m, mycol, pc, lane_base, lane);

@@ -672,7 +672,7 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     if ((rc = cut(items1s, cost1s, nt1, skip_sms(ctx) * P1_G[0], 12, ctx->part1_doubles, &sp->workers1s))) return rc;
     if ((rc = skip_upload(&sp->d_items1s, items1s)) || (rc = skip_upload(&sp->d_w1sstart, ws)) ||
         (rc = skip_upload(&sp->d_w1sfirst, wf)) || (rc = skip_upload(&sp->d_slots1s, sl))) return rc;
-    {   // symmetric background: off unless it fits (HAWKES_DENSE_PASS1=1 switches it off as in the dense path)
+    {   // symmetric background: off unless it fits (hawkes_set_pass1_mode(DENSE) switches it off as in the dense path)
         const std::vector<int> wf_s = wf, sl_s = sl;          // cut of the S items, just made
         std::vector<int2> itemsb;
         for (int I = 0; I < nt1; ++I)
@@ -700,7 +700,6 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
             sl_sym[I] = slb[I] + sl_s[I];
             worst = std::max(worst, sl_sym[I]);
         }
-        const char* dense = getenv("HAWKES_DENSE_PASS1");
         const size_t pcd = (size_t)colpart_doubles(nt1, NT * P1_R, 3);
         const size_t prd = (size_t)worst * 12 * (size_t)ld;
         // the two large buffers of the previous plan are taken over when they are large enough
@@ -712,7 +711,7 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
             sp->d_part_sym = old->d_part_sym; sp->part_sym_doubles = old->part_sym_doubles;
             old->d_part_sym = nullptr;
         }
-        if (!(dense && dense[0] == '1') && Q > 0 && Q < ((int64_t)1 << 31) && prd * sizeof(double) <= ((size_t)8 << 30) &&
+        if (!ctx->force_dense && Q > 0 && Q < ((int64_t)1 << 31) && prd * sizeof(double) <= ((size_t)8 << 30) &&
             pcd * sizeof(double) <= ((size_t)16 << 30) &&
             (sp->d_partc || cudaMalloc((void**)&sp->d_partc, pcd * sizeof(double)) == cudaSuccess) &&
             (sp->d_part_sym || cudaMalloc((void**)&sp->d_part_sym, prd * sizeof(double)) == cudaSuccess)) {
@@ -787,7 +786,7 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
     pass1_list_kernel<P1_R, L, DIM3, G1><<<g1, NT * G1, SM1, st>>>(ctx->d_rec, n, ld, c, ctx->d_tab, part1,              \
                                                                    items1, w1start, w1first, workers1);                   \
     reduce1_kernel<L, DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, part1, s1, ctx->d_lam, ctx->d_trec,             \
-                                                    ctx->d_trec2, nullptr, ctx->d_blockpart, ctx->d_status,               \
+                                                    ctx->d_trec2, (L) >= 1 ? ctx->d_rowd1 : nullptr, (L) >= 2 ? ctx->d_rowd2 : nullptr, ctx->d_blockpart, ctx->d_status,               \
                                                     ctx->d_bgcache, bg_mode, sym ? sp.d_partc : nullptr, s1.n_tiles,      \
                                                     NT * P1_R, sp.d_tn)
     if (level1 == 0) { SKIP_PASS1(0); }

@@ -54,3 +54,32 @@ def scales(ev, ref):
 def hess_hyper_scale(H):
     d = np.sqrt(np.abs(np.diag(H)))
     return np.outer(d, d)
+
+
+TRIU = [(p, q) for p in range(6) for q in range(p, 6)]
+
+
+def scalars_from_rows(lam, d1, d2_triu, Lam, L1, L2):
+    """ell, the hyper-gradient and the 6x6 Hessian as the plain O(N) sums of SURVEY.md 8(c) A2 / A6 / A7 over
+    per-event values (long-double accumulation):
+        ell = sum log lambda_n - Lambda,   g_p = sum lambda_{n,p}/lambda_n - Lambda_p,
+        H_pq = sum [lambda_{n,pq}/lambda_n - lambda_{n,p} lambda_{n,q}/lambda_n^2] - Lambda_pq,
+    with the error scales (sums of the magnitudes of the terms) beside them.  Used at sizes where the oracle can
+    afford only a sample of rows: the per-event values are the GPU's own, validated on that sample; Lambda and its
+    derivatives are the oracle's (oracle.integral)."""
+    ld = np.longdouble
+    lam = lam.astype(ld)
+    ll = float(np.sum(np.log(lam)) - ld(Lam))
+    s_ll = float(np.sum(np.abs(np.log(lam)))) + abs(Lam)
+    out = {"ll": ll, "s_ll": s_ll}
+    if d1 is not None:
+        r = d1.astype(ld) / lam[:, None]
+        out["grad_hyper"] = np.array(r.sum(0) - L1.astype(ld), dtype=float)
+        out["s_grad_hyper"] = np.array(np.abs(r).sum(0), dtype=float) + np.abs(L1)
+        if d2_triu is not None:
+            H = np.zeros((6, 6))
+            for k, (p, q) in enumerate(TRIU):
+                v = float(np.sum(d2_triu[:, k].astype(ld) / lam - r[:, p] * r[:, q]) - ld(L2[p, q]))
+                H[p, q] = H[q, p] = v
+            out["hess_hyper"] = H
+    return out

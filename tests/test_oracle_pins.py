@@ -322,6 +322,21 @@ def test_threads_do_not_change_results_and_sampled_rows_cols_agree():
     # row derivative sums reproduce the hyper-gradient's data part: sum_n d1/lambda - dLambda/dp
     lam_all, d1_all = oracle.rows(ev.x, ev.t, ev.theta, ev.params, np.arange(ev.n))
     assert np.allclose((d1_all / lam_all[:, None]).sum(0)[[1, 4]], a.grad_hyper[[1, 4]], rtol=1e-12)
+    # rows(second=True) and integral(): together they rebuild the pinned evaluate()'s ell, hyper-gradient and 6x6
+    # Hessian (sum_n [lambda_pq/lambda - lambda_p lambda_q/lambda^2] - Lambda_pq), in both background modes
+    for bg in ("ST", "S"):
+        e = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, bg=bg)
+        lam_r, d1_r, d2_r = oracle.rows(ev.x, ev.t, ev.theta, ev.params, np.arange(ev.n), second=True, bg=bg)
+        Lam, L1, L2 = oracle.integral(ev.t, ev.theta, ev.params, ev.dim, bg=bg)
+        assert np.array_equal(lam_r, e.lam) and Lam == e.integral
+        assert abs(np.sum(np.log(lam_r)) - Lam - e.ll) <= 1e-13 * abs(e.ll)
+        g = (d1_r / lam_r[:, None]).sum(0) - L1
+        assert np.allclose(g, e.grad_hyper, rtol=1e-11, atol=1e-11 * np.abs(d1_r / lam_r[:, None]).sum(0).max())
+        r = d1_r / lam_r[:, None]
+        H = (d2_r / lam_r[:, None, None] - r[:, :, None] * r[:, None, :]).sum(0) - L2
+        sc = np.sqrt(np.abs(np.diag(e.hess_hyper)))
+        assert np.all(np.abs(H - e.hess_hyper) <= 1e-11 * np.maximum(np.outer(sc, sc), np.abs(e.hess_hyper)) + 1e-300)
+        assert np.array_equal(d2_r, np.transpose(d2_r, (0, 2, 1)))
 
 
 def test_bad_arguments_are_rejected():
@@ -359,38 +374,37 @@ def test_s_mode_two_events_closed_form_and_printed_integral():
     B = mu0 / (2 * math.pi * tx * tx) * math.exp(-r2 / (2 * tx * tx))
     k = xi0 * om / (2 * math.pi * h * h) * math.exp(-om * dt - r2 / (2 * h * h))
     Lam = mu0 * t[1] + xi0 * th[0] * (1 - math.exp(-om * dt))
-    with oracle.background_mode("S"):
-        r = oracle.evaluate(x, t, th, (mu0, tx, tt, xi0, h, om), hess=True)
-        r_tt = oracle.evaluate(x, t, th, (mu0, tx, 7.7, xi0, h, om))
+    r = oracle.evaluate(x, t, th, (mu0, tx, tt, xi0, h, om), hess=True, bg="S")
+    r_tt = oracle.evaluate(x, t, th, (mu0, tx, 7.7, xi0, h, om), bg="S")
     assert abs(r.lam[0] - B) < 1e-16 and abs(r.lam[1] - (B + th[0] * k)) < 1e-16
     assert abs(r.integral - Lam) < 1e-15
     assert abs(r.ll - (math.log(B) + math.log(B + th[0] * k) - Lam)) < 1e-14
     assert r.ll == r_tt.ll                                   # tau_t is not in the model
     assert r.grad_hyper[2] == 0.0 and np.all(r.hess_hyper[2, :] == 0.0) and np.all(r.hess_hyper[:, 2] == 0.0)
     assert abs(r.grad_theta[0] - (k / (B + th[0] * k) - xi0 * (1 - math.exp(-om * dt)))) < 1e-14
-    # and the default mode is restored
+    # the mode is an argument, not a state: the default model is another likelihood
     assert abs(oracle.evaluate(x, t, th, (mu0, tx, tt, xi0, h, om)).ll - r.ll) > 1.0
 
 
 def test_s_mode_gradient_and_hessian_by_finite_differences():
     ev = synth.small_random(18, seed=31, regime="mixed", ties=True, duplicates=True)
     prm = np.array(ev.params)
-    with oracle.background_mode("S"):
-        r = oracle.evaluate(ev.x, ev.t, ev.theta, prm, hess=True)
-        for a in range(6):
-            e = np.zeros(6)
-            e[a] = 1e-6 * prm[a]
-            lp = oracle.evaluate(ev.x, ev.t, ev.theta, prm + e)
-            lm = oracle.evaluate(ev.x, ev.t, ev.theta, prm - e)
-            fd = (lp.ll - lm.ll) / (2 * e[a])
-            assert abs(fd - r.grad_hyper[a]) <= 1e-7 * max(1.0, abs(r.grad_hyper[a]))
-            fdh = (lp.grad_hyper - lm.grad_hyper) / (2 * e[a])
-            assert np.max(np.abs(fdh - r.hess_hyper[a]) / np.maximum(1.0, np.abs(r.hess_hyper[a]))) <= 2e-6
-        for m in (0, 5, 17):
-            e = np.zeros(ev.n)
-            e[m] = 1e-6
-            fd = (oracle.evaluate(ev.x, ev.t, ev.theta + e, prm).ll - oracle.evaluate(ev.x, ev.t, ev.theta - e, prm).ll) / 2e-6
-            assert abs(fd - r.grad_theta[m]) <= 1e-7 * max(1.0, abs(r.grad_theta[m]))
+    S = dict(bg="S")
+    r = oracle.evaluate(ev.x, ev.t, ev.theta, prm, hess=True, **S)
+    for a in range(6):
+        e = np.zeros(6)
+        e[a] = 1e-6 * prm[a]
+        lp = oracle.evaluate(ev.x, ev.t, ev.theta, prm + e, **S)
+        lm = oracle.evaluate(ev.x, ev.t, ev.theta, prm - e, **S)
+        fd = (lp.ll - lm.ll) / (2 * e[a])
+        assert abs(fd - r.grad_hyper[a]) <= 1e-7 * max(1.0, abs(r.grad_hyper[a]))
+        fdh = (lp.grad_hyper - lm.grad_hyper) / (2 * e[a])
+        assert np.max(np.abs(fdh - r.hess_hyper[a]) / np.maximum(1.0, np.abs(r.hess_hyper[a]))) <= 2e-6
+    for m in (0, 5, 17):
+        e = np.zeros(ev.n)
+        e[m] = 1e-6
+        fd = (oracle.evaluate(ev.x, ev.t, ev.theta + e, prm, **S).ll - oracle.evaluate(ev.x, ev.t, ev.theta - e, prm, **S).ll) / 2e-6
+        assert abs(fd - r.grad_theta[m]) <= 1e-7 * max(1.0, abs(r.grad_theta[m]))
 
 
 def test_s_mode_background_is_the_leave_one_out_kde():
@@ -399,8 +413,7 @@ def test_s_mode_background_is_the_leave_one_out_kde():
     from sklearn.neighbors import KernelDensity
     ev = synth.small_random(40, seed=33, regime="background")
     mu0, tx = 0.7, 0.9
-    with oracle.background_mode("S"):
-        r = oracle.evaluate(ev.x, ev.t, ev.theta, (mu0, tx, 1.0, 1e-300, 0.5, 1.0))
+    r = oracle.evaluate(ev.x, ev.t, ev.theta, (mu0, tx, 1.0, 1e-300, 0.5, 1.0), bg="S")
     X = ev.x.T
     for n in (0, 7, 39):
         others = np.delete(X, n, axis=0)

@@ -12,7 +12,7 @@ import paper_2103_03348_b200 as hp
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 from paper_2103_03348_b200 import synth
-from parity import TOL, check, hess_hyper_scale, scales
+from parity import TOL, TRIU, check, hess_hyper_scale, scalars_from_rows, scales
 
 pytestmark = pytest.mark.gpu
 THREADS = max(1, min(os.cpu_count() or 1, 64))
@@ -62,7 +62,10 @@ def compare_all(ev, r, lam, ref, cross=True):
         T = ev.t[-1] - ev.t
         c_m = np.abs(ref.grad_theta + xi0 * (-np.expm1(-om * T)))
         rr = np.max(np.abs(ref.row_d1 / ref.lam[:, None]), axis=0)
-        colB = rr + np.array([0, 0, 0, 1 / xi0, 40 / h, 1 / om + (ev.t[-1] - ev.t[0])])
+        # |d log k / dh| = |r^2/h^3 - D/h| on the pairs that are not exact zeros: exp(-r^2/2h^2) > 0 needs
+        # r^2/2h^2 < 1075 ln 2 = 745.2, so r^2/h^3 < 1490.3 / h
+        D = ev.dim
+        colB = rr + np.array([0, 0, 0, 1 / xi0, max(D, 1490.3 - D) / h, 1 / om + (ev.t[-1] - ev.t[0])])
         out["hess_cross"] = check("hess_cross", C, O, c_m[:, None] * colB[None, :] + np.array([0, 0, 0, 1, 0, xi0 * np.max(T)])[None, :], floor=1e-280)
         for p in range(6):
             assert np.max(np.abs(C[:, p] - O[:, p])) <= TOL * max(np.max(np.abs(O[:, p])), 1e-280)
@@ -180,29 +183,103 @@ def test_entry_points_agree_and_are_deterministic(torch, cfg1_ref):
     assert torch.equal(h.ll, a.ll.cpu()) and torch.equal(h.grad_theta, a.grad_theta.cpu()) and torch.equal(h.grad_hyper, a.grad_hyper.cpu())
 
 
-@pytest.mark.parametrize("n", [50000, 250000])
-def test_scaling_sweep_sampled_rows_and_columns(torch, n):
-    """BASELINE.json configs[4] sizes: the oracle evaluates a seeded sample of 1,024 target rows
-    (lambda_n and d lambda_n/dp) and, once those validate the GPU's lambda, 1,024 source columns
-    (c_m, d_m) with that lambda."""
+def _sweep_case(torch, n):
+    """One size of BASELINE.json configs[4]: both launch configurations -- hawkes_grad as bench.py times it (pass 1 at
+    the gradient level: background once per unordered pair) and the Hessian-level evaluation -- with the per-event
+    derivatives of lambda_n kept (hawkes_get_row_moments)."""
     ev = synth.config(4, n=n)
     ctx = hp.HawkesContext(ev.n, ev.dim)
-    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD | hp.WANT_HESS_THETA, ctx)
+    ctx.row_moments_enable(True)
+    rg, st, lam_g, _ = run_gpu(torch, ev, hp.WANT_GRAD, ctx)
+    assert st == 0 and ctx.pass1_is_symmetric(1)
+    d1_g = ctx.get_row_moments(n).cpu().numpy()
+    rh, st, lam_h, _ = run_gpu(torch, ev, hp.WANT_ALL & ~hp.WANT_HESS_CROSS, ctx)
     assert st == 0
+    d1_h, d2_h = (a.cpu().numpy() for a in ctx.get_row_moments(n, second=True))
+    return ev, ctx, (rg, lam_g, d1_g), (rh, lam_h, d1_h, d2_h)
+
+
+def _check_scalars_from_rows(ev, r, lam, d1, d2):
+    """ell, grad_hyper (and hess_hyper) of the GPU against the plain O(N) sums over its own per-event values and the
+    oracle's integral terms."""
+    Lam, L1, L2 = oracle.integral(ev.t, ev.theta, ev.params, ev.dim)
+    e = scalars_from_rows(lam, d1, d2, Lam, L1, L2)
+    out = {"ll": check("ll", r.ll.item(), e["ll"], e["s_ll"]),
+           "grad_hyper": check("grad_hyper", r.grad_hyper.cpu().numpy(), e["grad_hyper"], e["s_grad_hyper"])}
+    if d2 is not None:
+        H = r.hess_hyper.cpu().numpy()
+        assert np.array_equal(H, H.T)
+        out["hess_hyper"] = check("hess_hyper", H, e["hess_hyper"], hess_hyper_scale(e["hess_hyper"]))
+    return out
+
+
+@pytest.mark.parametrize("n", [50000, 100000, 250000])
+def test_scaling_sweep_every_output(torch, n):
+    """BASELINE.json configs[4] sizes (north_star: "log-lik, gradient and Hessian at N=23,422 and N=250,000"), every
+    output.  The O(N^2) oracle evaluates a seeded sample of 1,024 target rows -- lambda_n, d lambda_n/dp and
+    d2 lambda_n/dp dq, against the per-event values of both launch configurations -- and, once those validate the
+    GPU's lambda, 1,024 source columns (c_m, d_m) with that lambda.  ell, the six hyperparameter derivatives and the
+    6x6 Hessian are O(N) sums of those per-event values and of the integral terms: they are checked against the
+    plain sums over ALL N per-event values (tests/parity.py) with the oracle's Lambda, dLambda, d2Lambda."""
+    ev, ctx, (rg, lam_g, d1_g), (rh, lam_h, d1_h, d2_h) = _sweep_case(torch, n)
     k = 1024
     idx = np.sort((synth.uniforms(123, 7, k) * n).astype(np.int64))
     idx[0], idx[-1] = 0, n - 1
-    lam_o, _ = oracle.rows(ev.x, ev.t, ev.theta, ev.params, idx, derivs=False, threads=THREADS)
-    check("lambda rows", lam[idx], lam_o)
-    c_o, d_o = oracle.cols(ev.x, ev.t, ev.params, lam, idx, threads=THREADS)
+    lam_o, d1_o, d2_o = oracle.rows(ev.x, ev.t, ev.theta, ev.params, idx, second=True, threads=THREADS)
+    d2_o = np.stack([d2_o[:, p, q] for p, q in TRIU], axis=1)
+    # Error scales of a row's derivatives: the GPU forms them as linear combinations of positive moment sums (SURVEY 8(c)
+    # A6 / A7), e.g. d lambda/d tau_x = sum B r^2 / tau_x^3 - D sum B / tau_x, which may cancel.  With c_p the largest
+    # constant part of |d log term / dp| (1/mu0, D/tau_x, 1/tau_t, 1/xi0, D/h, 1/omega) each term of the first
+    # derivative is at most a_p = |d1_p| + c_p lambda_n, and each term of d2_pq beside its leading moment at most
+    # 3.5 (c_p a_q + c_q a_p) (the largest coefficient ratio in A7 is (2D+3)/D = 3.5 at D = 2, 7 for tau_t tau_t ... all
+    # below 8): scales from oracle values only.
+    D = ev.dim
     mu0, tx, tt, xi0, h, om = ev.params
+    cp = np.array([1 / mu0, D / tx, 1 / tt, 1 / xi0, D / h, 1 / om])
+    a1 = np.abs(d1_o) + cp[None, :] * lam_o[:, None]
+    s1 = a1
+    s2 = np.stack([np.abs(d2_o[:, k]) + 8.0 * (cp[p] * a1[:, q] + cp[q] * a1[:, p]) for k, (p, q) in enumerate(TRIU)], axis=1)
+    for name, lam, d1 in (("grad level", lam_g, d1_g), ("hessian level", lam_h, d1_h)):
+        check("lambda rows, " + name, lam[idx], lam_o)
+        check("d lambda/dp rows, " + name, d1[idx], d1_o, s1)
+    check("d2 lambda/dp dq rows", d2_h[idx], d2_o, s2)
+    assert np.allclose(lam_g, lam_h, rtol=1e-12, atol=0)
+    c_o, d_o = oracle.cols(ev.x, ev.t, ev.params, lam_g, idx, threads=THREADS)
     integ = xi0 * (-np.expm1(-om * (ev.t[-1] - ev.t[idx])))
-    check("grad_theta cols", r.grad_theta.cpu().numpy()[idx], c_o - integ, np.abs(c_o) + integ)
-    check("hess_theta cols", r.hess_theta_diag.cpu().numpy()[idx], -d_o, floor=1e-280)
+    for r in (rg, rh):
+        check("grad_theta cols", r.grad_theta.cpu().numpy()[idx], c_o - integ, np.abs(c_o) + integ)
+    check("hess_theta cols", rh.hess_theta_diag.cpu().numpy()[idx], -d_o, floor=1e-280)
+    res = {"grad level": _check_scalars_from_rows(ev, rg, lam_g, d1_g, None),
+           "hessian level": _check_scalars_from_rows(ev, rh, lam_h, d1_h, d2_h)}
     # properties that hold at any size
-    gt = r.grad_theta.cpu().numpy()
-    assert gt[-1] == 0.0 and np.all(np.isfinite(gt)) and np.all(r.hess_theta_diag.cpu().numpy() <= 0)
-    assert np.all(lam > 0) and math.isfinite(r.ll.item())
+    gt = rg.grad_theta.cpu().numpy()
+    assert gt[-1] == 0.0 and np.all(np.isfinite(gt)) and np.all(rh.hess_theta_diag.cpu().numpy() <= 0)
+    assert np.all(lam_g > 0) and math.isfinite(rg.ll.item())
+    print(f"N={n}: max scaled errors", res)
+
+
+def _full_oracle_case(torch, n):
+    ev, ctx, (rg, lam_g, d1_g), (rh, lam_h, d1_h, d2_h) = _sweep_case(torch, n)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+    assert ref.status == 0
+    res = {"grad level": compare_all(ev, rg, lam_g, ref, cross=False),
+           "hessian level": compare_all(ev, rh, lam_h, ref, cross=False)}
+    print(f"N={n}, full oracle: max scaled errors", res)
+
+
+def test_scaling_sweep_full_oracle_n50000(torch):
+    """The whole oracle (every row and column, all outputs but the cross block) at the first size of configs[4]."""
+    _full_oracle_case(torch, 50000)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n", [100000, 250000])
+def test_scaling_sweep_full_oracle_slow(torch, n):
+    """The same at N = 100,000 and N = 250,000: minutes of 16-thread oracle time each (250,000: 6.25e10 pairs), so
+    these run only with HAWKES_SLOW_TESTS=1; the log of the run that was made is profiles/r02_full_oracle_250k.txt."""
+    if os.environ.get("HAWKES_SLOW_TESTS") != "1":
+        pytest.skip("set HAWKES_SLOW_TESTS=1 (several minutes of oracle time)")
+    _full_oracle_case(torch, n)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -271,40 +348,37 @@ def test_sort_events_helper(torch):
 
 
 def test_dense_pass1_kernel_agrees_with_symmetric_pass1(torch):
-    """The default pass 1 evaluates the background once per unordered pair (csrc/pass1_sym.cuh); HAWKES_DENSE_PASS1=1
-    selects the dense ordered-pair kernel (also the fallback when the column-partial buffer is not allocated).  Both
-    must give the same sums up to summation order: compared here on configs[0] (ragged last tile, stream-K cuts) and
-    a problem with ties and duplicated locations, the dense run in a subprocess so that the switch is read at create."""
-    import json
-    import subprocess
-    import sys
-    import paper_2103_03348_b200 as hp
-    code = r'''
-import json, sys
-import numpy as np, torch
-sys.path.insert(0, %r)
-import paper_2103_03348_b200 as hp
-from paper_2103_03348_b200 import synth
-out = []
-for ev in (synth.config(0), synth.small_random(700, seed=21, ties=True, duplicates=True)):
-    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
-    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
-    r = ctx.grad(dev(ev.x), dev(ev.t), dev(ev.theta), ev.params)
-    out.append([r.ll.item(), r.grad_theta.cpu().tolist(), r.grad_hyper.cpu().tolist()])
-print(json.dumps(out))
-''' % ROOT
-    res = {}
-    for mode in ("0", "1"):
-        env = dict(os.environ, HAWKES_DENSE_PASS1=mode)
-        p = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
-        assert p.returncode == 0, p.stderr
-        res[mode] = json.loads(p.stdout.strip().splitlines()[-1])
-    for sym, dense in zip(res["0"], res["1"]):
-        assert abs(sym[0] - dense[0]) <= 1e-12 * abs(dense[0])
-        gs, gd = np.array(sym[1]), np.array(dense[1])
-        assert np.max(np.abs(gs - gd)) <= 1e-11 * np.max(np.abs(gd))
-        hs, hd = np.array(sym[2]), np.array(dense[2])
-        assert np.max(np.abs(hs - hd) / np.maximum(np.abs(hd), 1e-300)) <= 1e-9
+    """The default pass 1 evaluates the background once per unordered pair (csrc/pass1_sym.cuh);
+    hawkes_set_pass1_mode(HAWKES_PASS1_DENSE) selects the dense ordered-pair kernel (also the fallback when the
+    column-partial buffer is not allocated).  Both must give the same sums up to summation order: compared here on
+    configs[0] (ragged last tile, stream-K cuts) and a problem with ties and duplicated locations, at the
+    log-likelihood level and the gradient level, through the dense path and through the work lists."""
+    for ev in (synth.config(0), synth.small_random(700, seed=21, ties=True, duplicates=True)):
+        x, t, th = dev(torch, ev)
+        ctx = hp.HawkesContext(ev.n, ev.dim)
+        assert ctx.pass1_is_symmetric(0) and ctx.pass1_is_symmetric(1) and not ctx.pass1_is_symmetric(2)
+        sym = [ctx.eval(x, t, th, ev.params, w) for w in (hp.WANT_LL | hp.WANT_GRAD_THETA, hp.WANT_GRAD)]
+        ctx.skip_plan(x, t, ev.params)
+        sym.append(ctx.eval_skip(x, t, th, ev.params, hp.WANT_GRAD))
+        ctx.set_pass1_mode(hp.PASS1_DENSE)
+        assert not ctx.pass1_is_symmetric(0) and not ctx.pass1_is_symmetric(1)
+        dense = [ctx.eval(x, t, th, ev.params, w) for w in (hp.WANT_LL | hp.WANT_GRAD_THETA, hp.WANT_GRAD)]
+        stats = ctx.skip_plan(x, t, ev.params)
+        assert stats["items_background_unordered"] == 0
+        dense.append(ctx.eval_skip(x, t, th, ev.params, hp.WANT_GRAD))
+        ctx.set_pass1_mode(hp.PASS1_AUTO)
+        back = ctx.eval(x, t, th, ev.params, hp.WANT_GRAD)
+        torch.cuda.synchronize()
+        assert torch.equal(back.ll, sym[1].ll) and torch.equal(back.grad_theta, sym[1].grad_theta)
+        for a_, b_ in zip(sym, dense):
+            assert abs(a_.ll.item() - b_.ll.item()) <= 1e-12 * abs(b_.ll.item())
+            gs, gd = a_.grad_theta.cpu().numpy(), b_.grad_theta.cpu().numpy()
+            assert np.max(np.abs(gs - gd)) <= 1e-11 * np.max(np.abs(gd))
+            if a_.grad_hyper is not None:
+                hs, hd = a_.grad_hyper.cpu().numpy(), b_.grad_hyper.cpu().numpy()
+                assert np.max(np.abs(hs - hd) / np.maximum(np.abs(hd), 1e-300)) <= 1e-9
+    with pytest.raises(hp.HawkesError):
+        ctx.set_pass1_mode(5)
 
 
 @pytest.mark.parametrize("n,seed,dim", [(3, 41, 2), (300, 42, 2), (777, 43, 3), (1000, 44, 2)])
@@ -319,8 +393,7 @@ def test_space_only_background_mode(torch, n, seed, dim):
     ctx = hp.HawkesContext(ev.n, ev.dim)
     r_st, st0, lam_st, _ = run_gpu(torch, ev, ctx=ctx)
     ctx.set_background_mode(hp.BG_SPACE_ONLY)
-    with oracle.background_mode("S"):
-        ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS, bg="S")
     r, st, lam, _ = run_gpu(torch, ev, ctx=ctx)
     assert st == ref.status == 0
     compare_all(ev, r, lam, ref)
@@ -397,3 +470,33 @@ def test_pass2_factorised_and_unfactorised_time_decay(torch, scale):
     r, st, lam, _ = run_gpu(torch, ev)
     assert st == ref.status == 0
     compare_all(ev, r, lam, ref)
+
+
+@pytest.mark.parametrize("decay,zb", [(300.0, 330.0), (400.0, 460.0)])
+def test_pass2_far_in_time_sources_with_tiny_rates(torch, decay, zb):
+    """Column sums whose only terms are far in time: 512 sites far apart (background ~ e^-zb between neighbours, no
+    excitation across sites), at each one source event near t = 0 and one target event `decay`/omega later.  The
+    target's rate is its source's excitation alone, lambda ~ xi0 omega e^-decay / (2 pi h^2) (1e-129 / 1e-173), so
+    k/lambda = 1/theta_m: c_m and d_m are O(1) although every factor of the factorised pass 2
+    (F = e^{-omega (t_ref - t_m)}, W_n = e^{-omega (t_n - t_ref)} / lambda_n) is far from 1.  decay = 300: factorised
+    form with F ~ 1e-130, W up to 1e+145; decay = 400: (G W_n)^2 would overflow -- reduce1 must switch pass 2 to the
+    unfactorised form for the d_m sums.  Every output against the oracle."""
+    m = 512
+    mu0, tx, tt, xi0, h, om = 0.3, 1.0, 1.0e4, 0.7, 0.05, 0.5
+    s = tx * math.sqrt(2.0 * zb)                               # neighbour spacing: r^2 / 2 tau_x^2 = zb
+    gx, gy = np.meshgrid(np.arange(32) * s, np.arange(16) * s)
+    sites = np.stack([gx.ravel(), gy.ravel()])                 # [2, 512]
+    u = synth.uniforms(9, 31, 2 * m)
+    t = np.concatenate([np.sort(u[:m]), decay / om + np.sort(u[m:])])
+    perm = np.argsort(synth.uniforms(9, 32, m), kind="stable")  # targets visit the sites in another order
+    x = np.concatenate([sites, sites[:, perm]], axis=1)
+    theta = np.exp(0.5 * synth.normals(9, 33, 2 * m))
+    ev = synth.Events(x=np.ascontiguousarray(x), t=t, theta=theta, free_idx=np.arange(2 * m),
+                      params=(mu0, tx, tt, xi0, h, om))
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+    assert ref.status == 0 and ref.lam[m:].max() < 1e-120
+    # the structure the case is built for: d2 ell / d theta_m^2 = -1/theta_m^2 for every source
+    assert np.allclose(ref.hess_theta_diag[:m], -1.0 / theta[:m] ** 2, rtol=1e-9)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_ALL & ~hp.WANT_HESS_CROSS)
+    assert st == 0
+    compare_all(ev, r, lam, ref, cross=False)

@@ -153,8 +153,7 @@ def test_skip_long_time_axis(torch):
 def test_skip_space_only_background(torch):
     """Paper-literal S mode through the lists."""
     ev = synth.config(0)
-    with oracle.background_mode("S"):
-        ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS, bg="S")
     ctx = hp.HawkesContext(ev.n, ev.dim)
     ctx.set_background_mode(hp.BG_SPACE_ONLY)
     r, st, lam, g, hd, stats, _ = run_skip(torch, ev, ctx=ctx)
