@@ -248,19 +248,128 @@ def whole_job_value(world: int, steps: int, total_ms_max: float) -> float:
     return world * steps / (total_ms_max * 1e-3)
 
 
-def ncu_traffic(kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full
-    summary (profiles/traffic.csv: kernel,dram_bytes_per_launch; profiles/traffic.md names the command), or None."""
+def ncu_record(kernel: str, n: int) -> dict:
+    """What the committed `ncu --set full` capture of `kernel` at N = n says (profiles/traffic.csv: kernel, n_events,
+    dram_bytes_per_launch, fp64_pipe_pct_active, fp64_pipe_pct_elapsed, source; profiles/traffic.md names the
+    commands): DRAM bytes per launch and the FP64-pipe utilisation.  Every value is None when there is no capture of
+    this kernel at this N -- a number profiled at another size is not reported."""
+    none = {"traffic": None, "ncu_fp64_pipe_pct_active": None, "ncu_fp64_pipe_pct_elapsed": None, "ncu_source": None}
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(path) as fh:
             for line in fh:
-                parts = [p.strip() for p in line.split(",")]
-                if len(parts) >= 2 and parts[0] == kernel:
-                    return float(parts[1])
+                f = [p.strip() for p in line.split(",")]
+                if len(f) >= 6 and f[0] == kernel and f[1].isdigit() and int(f[1]) == int(n):
+                    return {"traffic": float(f[2]), "ncu_fp64_pipe_pct_active": float(f[3]),
+                            "ncu_fp64_pipe_pct_elapsed": float(f[4]), "ncu_source": "profiles/" + f[5]}
     except Exception:
         pass
-    return None
+    return none
+
+
+def roofline_records(n: int, p1_ms: float, p2_ms: float, sym: bool, peak_nominal: float, peak_dfma, instr_peak: float):
+    """`roofline` (pass 1, the dominant kernel) and `roofline_pass2` from the kernels' mean launch durations.
+    achieved = algorithmic flops of SURVEY 8(d) per launch / duration; the executed count and the FP64 issue fraction
+    depend on which pass-1 form ran (`sym`: background once per unordered pair)."""
+    a1 = pass1_flops(n) / (p1_ms * 1e-3) / 1e12
+    a2 = pass2_flops(n) / (p2_ms * 1e-3) / 1e12
+    if sym:
+        kernel1, key1 = "pass1s_kernel<R=2, LEVEL=1> (symmetric background)", "pass1s_kernel"
+        x1 = pass1_flops_executed(n)
+        i1 = 0.5 * n * (n - 1) * P1_SYM_INSTR
+    else:   # dense ordered-pair kernel: executes what SURVEY 8(d) counts (18 / 13 FP64 instructions per term)
+        kernel1, key1 = "pass1_kernel<R=2, LEVEL=1> (dense ordered pairs)", "pass1_kernel"
+        x1 = pass1_flops(n)
+        i1 = float(n) * n * 18 + 0.5 * n * (n - 1) * 13
+    a1x = x1 / (p1_ms * 1e-3) / 1e12
+    r1 = {"bound": "alu", "kernel": kernel1, "achieved": a1, "peak": peak_nominal, "unit": "TFLOP/s",
+          "frac": a1 / peak_nominal,
+          "flops_basis": "SURVEY 8(d): N^2 background + N(N-1)/2 excitation terms of Eq. 1, 28 / 22 flops each",
+          "achieved_executed": a1x, "frac_executed": a1x / peak_nominal, "flops_executed_per_launch": x1,
+          "peak_source": "derived: SMs x 64 FP64 FMA lanes x 2 x clocks.max.sm; MEASURED_PEAKS.json has no FP64 entry",
+          "peak_measured_dfma": peak_dfma, "frac_of_measured_dfma": a1 / peak_dfma if peak_dfma else None,
+          "fp64_pipe_issue_frac": i1 / (p1_ms * 1e-3) / instr_peak,
+          "ms_per_launch": p1_ms, "flops_per_launch": pass1_flops(n)}
+    r1.update(ncu_record(key1, n))
+    r2 = {"bound": "alu", "kernel": "pass2_kernel", "achieved": a2, "peak": peak_nominal, "unit": "TFLOP/s",
+          "frac": a2 / peak_nominal, "frac_of_measured_dfma": a2 / peak_dfma if peak_dfma else None,
+          "fp64_pipe_issue_frac": 0.5 * n * (n - 1) * 13 / (p2_ms * 1e-3) / instr_peak,
+          "ms_per_launch": p2_ms, "flops_per_launch": pass2_flops(n)}
+    r2.update(ncu_record("pass2_kernel", n))
+    return r1, r2
+
+
+def parity_sample(hp, ctx, ev, out, rows: int) -> dict:
+    """Parity in this very run: `rows` evenly strided rows of lambda_n and d lambda_n/dp and the same columns of c_m
+    against the oracle (scaled as tests/test_parity_gpu.py does)."""
+    import numpy as np
+    import oracle
+    n = ev.n
+    sidx = sample_idx(n, rows)
+    thr = oracle.max_threads()
+    lam_gpu = ctx.get_lambda(n).cpu().numpy()
+    d1_gpu = ctx.get_row_moments(n).cpu().numpy()[sidx]
+    lam_ref, d1_ref = oracle.rows(ev.x, ev.t, ev.theta, ev.params, sidx, derivs=True, threads=thr)
+    c_ref, _ = oracle.cols(ev.x, ev.t, ev.params, lam_gpu, sidx, threads=thr)
+    mu0, tx, tt, xi0, h, om = ev.params
+    D = ev.dim
+    cp = np.array([1 / mu0, D / tx, 1 / tt, 1 / xi0, D / h, 1 / om])
+    s1 = np.abs(d1_ref) + cp[None, :] * lam_ref[:, None]
+    integ = xi0 * (-np.expm1(-om * (ev.t[-1] - ev.t[sidx])))
+    g_gpu = out.grad_theta.cpu().numpy()[sidx]
+    return {"rows": int(len(sidx)),
+            "max_rel_err_lambda": float(np.max(np.abs(lam_gpu[sidx] - lam_ref) / lam_ref)),
+            "max_scaled_err_dlambda_dhyper": float(np.max(np.abs(d1_gpu - d1_ref) / s1)),
+            "max_scaled_err_grad_theta": float(np.max(np.abs(g_gpu - (c_ref - integ)) / (np.abs(c_ref) + integ + 1e-300))),
+            "tolerance": 1e-10}
+
+
+def timed_steps(torch, dev, call, steps, flush):
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for e0, e1 in evs:
+        flush.zero_()
+        e0.record()
+        call()
+        e1.record()
+    torch.cuda.synchronize(dev)
+    return [e0.elapsed_time(e1) for e0, e1 in evs]
+
+
+def sweep_entry(torch, hp, dev, local, n, seed, flush, peaks, with_parity: bool) -> dict:
+    """One size of BASELINE.json configs[4]: 3 warm-up + 5 timed hawkes_grad steps on a fresh context."""
+    import numpy as np
+    from paper_2103_03348_b200 import synth
+    ev = synth.config(4, n=n, seed=seed)
+    ctx = hp.HawkesContext(n, ev.dim, local)
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    x, t, th = f(ev.x), f(ev.t), f(ev.theta)
+    out = ctx.new_outputs(n, hp.WANT_GRAD, dev)
+    step = lambda: ctx.grad(x, t, th, ev.params, out=out)
+    timed_steps(torch, dev, step, 3, flush)
+    assert ctx.last_status() == 0
+    sampler = ClockSampler(local).start()
+    ctx.profile_enable(True)
+    ms = timed_steps(torch, dev, step, 5, flush)
+    prof = ctx.profile_read()
+    ctx.profile_enable(False)
+    clocks = sampler.stop()
+    cnt = max(prof["evals"], 1)
+    p1_ms, p2_ms = prof["pass1_ms"] / cnt, prof["pass2_ms"] / cnt
+    sym = ctx.pass1_is_symmetric(1)
+    r1, r2 = roofline_records(n, p1_ms, p2_ms, sym, *peaks)
+    ms_step = float(sum(ms)) / len(ms)
+    e = {"n_events": n, "steps": 5, "warmup": 3, "ms_per_step": ms_step, "evals_per_s": 1e3 / ms_step,
+         "gpairs_per_s": float(n) * n / (ms_step * 1e-3) / 1e9,
+         "pass1": {k: r1[k] for k in ("kernel", "ms_per_launch", "frac", "frac_executed", "fp64_pipe_issue_frac",
+                                      "traffic", "ncu_fp64_pipe_pct_elapsed")},
+         "pass2": {k: r2[k] for k in ("ms_per_launch", "frac", "fp64_pipe_issue_frac", "traffic",
+                                      "ncu_fp64_pipe_pct_elapsed")},
+         "step_frac_of_fp64_peak": (pass1_flops(n) + pass2_flops(n)) / (ms_step * 1e-3) / 1e12 / peaks[0],
+         "ll": float(out.ll.item()), "clocks": clocks}
+    if with_parity:
+        e["parity_sample"] = parity_sample(hp, ctx, ev, out, 128)
+    ctx.close()
+    return e
 
 
 def run_b200(args, ev, workload: str) -> dict:
@@ -292,15 +401,7 @@ def run_b200(args, ev, workload: str) -> dict:
     out = ctx.new_outputs(n, hp.WANT_GRAD, dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # 2x the 126 MB L2
 
-    def timed(call, steps):
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        for e0, e1 in evs:
-            flush.zero_()
-            e0.record()
-            call()
-            e1.record()
-        torch.cuda.synchronize(dev)
-        return [e0.elapsed_time(e1) for e0, e1 in evs]
+    timed = lambda call, steps: timed_steps(torch, dev, call, steps, flush)
 
     step = lambda: ctx.grad(x, t, th, ev.params, out=out)
     # -- device-resident leg ----------------------------------------------------------------------
@@ -347,14 +448,11 @@ def run_b200(args, ev, workload: str) -> dict:
     p1_ms = prof["pass1_ms"] / max(prof["evals"], 1)
     p2_ms = prof["pass2_ms"] / max(prof["evals"], 1)
     inner_ms = prof["total_ms"] / max(prof["evals"], 1)
-    a1 = pass1_flops(n) / (p1_ms * 1e-3) / 1e12
-    a2 = pass2_flops(n) / (p2_ms * 1e-3) / 1e12
-    # FP64-pipe instructions as the kernels issue them (SASS count): symmetric pass 1 34 per unordered
-    # pair (background 21 incl. both sets of sums, excitation 13), pass 2 13 per causal pair (factorised time decay)
-    a1x = pass1_flops_executed(n) / (p1_ms * 1e-3) / 1e12
-    p1_instr = 0.5 * n * (n - 1) * P1_SYM_INSTR
-    p2_instr = 0.5 * n * (n - 1) * 13
     instr_peak = props.multi_processor_count * FP64_LANES_PER_SM * sm_max * 1e6
+    peaks = (peak_nominal, peak_dfma, instr_peak)
+    roof1, roof2 = roofline_records(n, p1_ms, p2_ms, ctx.pass1_is_symmetric(1), *peaks)
+    roof1["peak_source"] = (f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
+                            f"{sm_max} MHz (clocks.max.sm); MEASURED_PEAKS.json has no FP64 entry")
     res = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -370,23 +468,8 @@ def run_b200(args, ev, workload: str) -> dict:
         "e2e": {"value": e_value, "unit": UNIT, "ms_per_step": e_total / K,
                 "h2d_bytes_per_step": int((ev.dim + 2) * n * 8), "d2h_bytes_per_step": int((1 + n + 6) * 8),
                 "call": "hawkes_eval_host (pinned host buffers)"},
-        "roofline": {"bound": "alu", "kernel": "pass1s_kernel<R=2, LEVEL=1> (symmetric background)", "achieved": a1,
-                     "peak": peak_nominal, "unit": "TFLOP/s", "frac": a1 / peak_nominal,
-                     "flops_basis": "SURVEY 8(d): N^2 background + N(N-1)/2 excitation terms of Eq. 1, 28 / 22 flops each",
-                     "achieved_executed": a1x, "frac_executed": a1x / peak_nominal,
-                     "flops_executed_per_launch": pass1_flops_executed(n),
-                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
-                                    f"{sm_max} MHz (clocks.max.sm); MEASURED_PEAKS.json has no FP64 entry",
-                     "peak_measured_dfma": peak_dfma, "frac_of_measured_dfma": a1 / peak_dfma if peak_dfma else None,
-                     "fp64_pipe_issue_frac": p1_instr / (p1_ms * 1e-3) / instr_peak,
-                     "ms_per_launch": p1_ms, "flops_per_launch": pass1_flops(n),
-                     "traffic": ncu_traffic("pass1s_kernel")},
-        "roofline_pass2": {"bound": "alu", "kernel": "pass2_kernel", "achieved": a2, "peak": peak_nominal,
-                           "unit": "TFLOP/s", "frac": a2 / peak_nominal,
-                           "frac_of_measured_dfma": a2 / peak_dfma if peak_dfma else None,
-                           "fp64_pipe_issue_frac": p2_instr / (p2_ms * 1e-3) / instr_peak,
-                           "ms_per_launch": p2_ms, "flops_per_launch": pass2_flops(n),
-                           "traffic": ncu_traffic("pass2_kernel")},
+        "roofline": roof1,
+        "roofline_pass2": roof2,
         "kernel_share": {"pass1": p1_ms / inner_ms, "pass2": p2_ms / inner_ms,
                          "o_n_and_gaps": 1.0 - (p1_ms + p2_ms) / inner_ms, "first_to_last_kernel_ms": inner_ms},
         "ll": ll_dev,
@@ -438,20 +521,9 @@ def run_b200(args, ev, workload: str) -> dict:
                           "frac": on_bytes / (on_ms * 1e-3) / 1e9 / hbm_peak,
                           "note": "launch-latency-bound by nature; the data they touch is L2-resident"}
     if world == 1 and not args.no_cpu_baseline:
-        # parity on a sample, in this very run: 256 rows of lambda_n and 256 columns of c_m against the oracle
-        import oracle
-        sidx = sample_idx(n, 256)
-        lam_gpu = ctx.get_lambda(n).cpu().numpy()
-        lam_ref, _ = oracle.rows(ev.x, ev.t, ev.theta, ev.params, sidx, derivs=False, threads=oracle.max_threads())
-        c_ref, _ = oracle.cols(ev.x, ev.t, ev.params, lam_gpu, sidx, threads=oracle.max_threads())
-        xi0, om = ev.params[3], ev.params[5]
-        integ = xi0 * (-np.expm1(-om * (ev.t[-1] - ev.t[sidx])))
-        g_gpu = out.grad_theta.cpu().numpy()[sidx]
-        res["parity_sample"] = {
-            "rows": int(len(sidx)),
-            "max_rel_err_lambda": float(np.max(np.abs(lam_gpu[sidx] - lam_ref) / lam_ref)),
-            "max_scaled_err_grad_theta": float(np.max(np.abs(g_gpu - (c_ref - integ)) / (np.abs(c_ref) + integ + 1e-300))),
-            "tolerance": 1e-10}
+        # parity on a sample, in this very run: 256 rows of lambda_n / d lambda_n/dp and 256 columns of c_m
+        timed(step, 1)
+        res["parity_sample"] = parity_sample(hp, ctx, ev, out, 256)
         res["cpu_baseline"] = cpu_baseline(ev, args.cpu_budget)
     if world == 1:
         # SURVEY 8(f)-4, reported apart from the dense numbers above (the paper's method visits every pair): the same
@@ -478,6 +550,15 @@ def run_b200(args, ev, workload: str) -> dict:
                                       "grad_hyper": float((sout.grad_hyper - out.grad_hyper).abs().max()
                                                           / out.grad_hyper.abs().max())},
             "note": "data-dependent: only terms that are exactly +0.0 in fp64 are left out; not the headline"}
+    if world == 1 and args.n is None and args.config == 1 and not args.no_sweep:
+        # BASELINE.json configs[4] / north_star's second size: N = 50,000 / 100,000 / 250,000 from the same generator,
+        # 3 warm-up + 5 timed steps each, with the clocks sampled during each entry's timed region and (unless
+        # --no-cpu-baseline) 128 rows and columns of each against the oracle
+        ctx.close()
+        del ctx
+        torch.cuda.empty_cache()
+        res["sweep"] = [sweep_entry(torch, hp, dev, local, nn, args.seed, flush, peaks, not args.no_cpu_baseline)
+                        for nn in (50000, 100000, 250000)]
     if dist is not None:
         dist.destroy_process_group()
     return res
@@ -592,19 +673,17 @@ def run_hmc(args) -> dict:
     x, t, idx = to(ev.x), to(ev.t), to(ev.free_idx)
     s2, tau0, L, every = synth.TREE_SIGMA2, synth.TREE_TAU0, 20, 10
     eps, floor = args.hmc_step, 1.0
-    res_var = {}
+    pp = tr.precision_diag(s2, tau0)
     sampler = ClockSampler(0).start()
-    launches = 0
-    for name, cache in (("recompute_all_pairs", 0), ("cached_background", 1), ("cached_kernel_matrix", 2),
-                        ("skip_lists_recompute", 3), ("skip_lists_cached_background", 4),
-                        ("sparse_kernel_matrix", 5)):
+
+    def run_variant(cache, step, prior_prec):
         if cache == 3:   # the exact-zero-skipping variants need the plan of these events and hyperparameters
             ctx.skip_plan(x, t, ev.params)
         z, mass = to(z0.copy()), to(np.ones(M))
         nrm = to(synth.normals(args.seed, 500, (W + K) * M).reshape(W + K, M))
         uni = to(synth.uniforms(args.seed, 501, W + K))
-        kw = dict(n_leapfrog=L, step=eps, precond_every=every, mass=mass, mass_floor=floor, cache_background=cache,
-                  prior_prec=tr.precision_diag(s2, tau0))
+        kw = dict(n_leapfrog=L, step=step, precond_every=every, mass=mass, mass_floor=floor, cache_background=cache,
+                  prior_prec=prior_prec)
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record()
         ctx.hmc_run(tr, x, t, idx, z, 0.0, ev.params, s2, tau0, n_iter=W, normals=nrm[:W].contiguous(),
@@ -617,27 +696,58 @@ def run_hmc(args) -> dict:
         torch.cuda.synchronize(dev)
         launches = ctx.launch_count() + tr.launch_count() - l0
         tr_h = trace.cpu().numpy()
-        res_var[name] = {"seconds_per_iteration": e1.elapsed_time(e2) * 1e-3 / K, "accept_rate": float(tr_h[:, 3].mean()),
-                         "log_posterior_last": float(tr_h[-1, 0]), "gpu_launches": int(launches),
-                         "evals_per_s_implied": (K * L + K // every + 1) / (e1.elapsed_time(e2) * 1e-3)}
+        n_refresh = len([it for it in range(K) if it % every == 0])
+        return {"seconds_per_iteration": e1.elapsed_time(e2) * 1e-3 / K, "accept_rate": float(tr_h[:, 3].mean()),
+                "step": step, "preconditioner": "A + P (DESIGN R20)" if prior_prec is not None else "A (PAPER.md:143-145)",
+                "log_posterior_last": float(tr_h[-1, 0]), "gpu_launches": int(launches),
+                "gpu_launches_per_iteration": launches / K,
+                "evals_per_s_implied": (K * L + n_refresh + 1) / (e1.elapsed_time(e2) * 1e-3)}
+
+    # headline: the paper's method (every pair recomputed at every leapfrog step) with the paper's
+    # preconditioner (the running average of the likelihood's Hessian diagonal alone); the time per
+    # iteration does not depend on the step size, the acceptance rate does (DESIGN R20: this preconditioner needs a
+    # far smaller step on a tree with very short branches)
+    head = run_variant(0, args.hmc_step_paper, None)
+    res_var = {"recompute_all_pairs__paper_preconditioner": head}
+    for name, cache in (("recompute_all_pairs", 0), ("cached_background", 1), ("cached_kernel_matrix", 2),
+                        ("skip_lists_recompute", 3), ("skip_lists_cached_background", 4),
+                        ("sparse_kernel_matrix", 5)):
+        res_var[name + "__plus_prior_curvature"] = run_variant(cache, eps, pp)
+    res_var["sparse_kernel_matrix__paper_preconditioner"] = run_variant(5, args.hmc_step_paper, None)
     clocks = sampler.stop()
-    # headline = the fastest variant (all compute the same sums; "recompute_all_pairs" is the paper's method; the
-    # skip_lists variants leave out tile pairs whose every term is an exact fp64 zero: data-dependent)
-    best_name = min(res_var, key=lambda k: res_var[k]["seconds_per_iteration"])
-    best = res_var[best_name]
-    return {"metric": "hmc_seconds_per_iteration", "value": best["seconds_per_iteration"], "unit": "s/iteration",
-            "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": best["seconds_per_iteration"] * 1e3,
-            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "BASELINE.json configs[3]: N=23,422, M=1,610 (configs[2] inputs), HMC on z: 20 leapfrog "
-                                   "steps per iteration, Hessian preconditioner refreshed every 10 iterations (plus the constant diagonal curvature of the prior)",
-                       "n_events": n, "n_tips": M, "step": eps, "mass_floor": floor, "call": "hawkes_hmc_run",
-                       "variant_of_value": best_name,
-                       "l2": "working set (0.75 MB) is L2-resident by design: every evaluation re-reads the same events",
-                       "parallelism": "1 GPU"},
-            "variants": res_var, "gpu_launches": best["gpu_launches"], "clocks": clocks,
-            "e2e": {"value": best["seconds_per_iteration"], "unit": "s/iteration", "h2d_bytes_per_step": 0,
-                    "d2h_bytes_per_step": 32, "note": "the chain state lives on the device; per iteration only the 4-double "
-                    "trace row leaves it (read back once at the end)"}}
+    res = {"metric": "hmc_seconds_per_iteration", "value": head["seconds_per_iteration"], "unit": "s/iteration",
+           "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": head["seconds_per_iteration"] * 1e3,
+           "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": "BASELINE.json configs[3]: N=23,422, M=1,610 (configs[2] inputs), HMC on z: 20 leapfrog "
+                                  "steps per iteration, Hessian preconditioner refreshed every 10 iterations",
+                      "n_events": n, "n_tips": M, "step": head["step"], "mass_floor": floor, "call": "hawkes_hmc_run",
+                      "variant_of_value": "recompute_all_pairs__paper_preconditioner (cache_background = 0, prior_prec = NULL)",
+                      "l2": "working set (0.75 MB) is L2-resident by design: every evaluation re-reads the same events",
+                      "parallelism": "1 GPU"},
+           "variants": res_var, "gpu_launches": head["gpu_launches"], "clocks": clocks,
+           "e2e": {"value": head["seconds_per_iteration"], "unit": "s/iteration", "h2d_bytes_per_step": 0,
+                   "d2h_bytes_per_step": 32, "note": "the chain state lives on the device; per iteration only the 4-double "
+                   "trace row leaves it (read back once at the end)"}}
+    if not args.no_cpu_baseline:
+        # the oracle's leapfrog (oracle/hmc.py on the likelihood and prior oracles): a bounded sample of one trajectory
+        import oracle
+        from oracle import hmc as ohmc
+        from oracle import tree as otree
+        threads = oracle.max_threads()
+        V = otree.vg(tree.parent, tree.branch, M, tau0)
+        target = ohmc.hawkes_target(ev.x, ev.t, ev.free_idx, 0.0, ev.params, V, s2, threads=threads)
+        lp0, g0, _ = target(z0, False)
+        n_steps = 4
+        t0_ = time.perf_counter()
+        ohmc.leapfrog(target, z0, np.sqrt(np.ones(M)) * synth.normals(args.seed, 500, M), g0, np.ones(M),
+                      args.hmc_step_paper, n_steps)
+        secs = time.perf_counter() - t0_
+        res["cpu_baseline"] = {"value": secs * L / n_steps, "unit": "s/iteration", "cores": threads, "kind": "oracle",
+                               "sample": f"{n_steps} of the {L} leapfrog steps of one trajectory (oracle/hmc.py: full "
+                                         f"likelihood oracle + dense Cholesky prior oracle per step), {secs:.1f} s on "
+                                         f"{threads} OpenMP threads, scaled by {L}/{n_steps}; the preconditioner refresh "
+                                         f"(1 Hessian evaluation per 10 iterations) is left out"}
+    return res
 
 
 def workload_of(args):
@@ -659,7 +769,7 @@ def workload_of(args):
 def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default 50; --config 3: 200 HMC iterations)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=1)
@@ -667,10 +777,14 @@ def main() -> int:
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--extras", action="store_true", help="also time the Hessian and the theta-only evaluation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] sizes in the default line")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
-    ap.add_argument("--hmc-step", type=float, default=0.2, help="leapfrog step size of --config 3")
+    ap.add_argument("--hmc-step", type=float, default=0.2, help="leapfrog step size of --config 3 with the prior curvature in the mass (R20)")
+    ap.add_argument("--hmc-step-paper", type=float, default=0.01, help="step size of --config 3 with the paper's preconditioner")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
+    if args.steps is None:
+        args.steps = 200 if (args.config == 3 and args.n is None) else 50
     rank, world, _ = dist_env()
     if args.impl == "reference":
         if rank != 0:
