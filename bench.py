@@ -479,6 +479,15 @@ def run_b200(args, ev, workload: str) -> dict:
         hstep = lambda: ctx.hessian(x, t, th, ev.params, out=hout_all)
         timed(hstep, 2)
         hms = timed(hstep, max(3, K // 4))
+        # the whole Hessian of configs[0]'s reading: theta-diagonal + 6x6 + the N x 6 cross block (csrc/cross.cuh)
+        xout = ctx.new_outputs(n, hp.WANT_HESS_THETA | hp.WANT_HESS_HYPER | hp.WANT_HESS_CROSS, dev)
+        xstep = lambda: ctx.hessian(x, t, th, ev.params, cross=True, out=xout)
+        timed(xstep, 2)
+        xms = timed(xstep, max(3, K // 4))
+        conly = ctx.new_outputs(n, hp.WANT_HESS_CROSS, dev)
+        cstep = lambda: ctx.eval(x, t, th, ev.params, hp.WANT_HESS_CROSS, out=conly)
+        timed(cstep, 2)
+        cms = timed(cstep, max(3, K // 4))
         lstep = lambda: ctx.eval(x, t, th, ev.params, hp.WANT_LL | hp.WANT_GRAD_THETA, out=out)
         timed(lstep, 2)
         lms = timed(lstep, max(3, K // 4))
@@ -496,6 +505,8 @@ def run_b200(args, ev, workload: str) -> dict:
         t2sms = timed(t2skip, max(3, K // 4))
         timed(step, 1)   # leave `out` holding the configs[1] result
         res["extras"] = {"hessian_ms": statistics.median(hms), "ll_grad_theta_only_ms": statistics.median(lms),
+                         "hessian_with_cross_block_ms": statistics.median(xms),
+                         "cross_block_only_ms": statistics.median(cms),
                          "step_ms_min": min(ms), "step_ms_median": statistics.median(ms),
                          "table2_scales_step_ms": statistics.median(t2ms),
                          "table2_scales_skip_step_ms": statistics.median(t2sms),

@@ -554,13 +554,14 @@ __device__ __forceinline__ double norm_cdf(double z) { return 0.5 * erfc(-z * 0.
 //   k = 31..33   sum theta (1-E),  sum theta T E,  sum theta T^2 E        (T = t_N - t_n, E = e^{-omega T})
 // rowd1[n*6 + p] = d lambda_n / dp (LEVEL >= 1, when `rowd1` != NULL: feeds the cross block and hawkes_get_row_moments);
 // rowd2[n*21 + k] = d2 lambda_n / dp dq, upper triangle row-major (LEVEL 2, when `rowd2` != NULL: diagnostics only).
+// crec: target records of the cross-block pass (csrc/cross.cuh), LEVEL >= 1, when != NULL.
 template <int LEVEL, bool DIM3>
 __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict__ rec, int64_t n, int64_t ld,
                                                         DevConsts c, const double* __restrict__ part,
                                                         Split sp, double* __restrict__ lam,
                                                         double* __restrict__ trec, double* __restrict__ trec2,
                                                         double* __restrict__ rowd1, double* __restrict__ rowd2,
-                                                        double* __restrict__ blockpart,
+                                                        double* __restrict__ crec, double* __restrict__ blockpart,
                                                         unsigned* __restrict__ status, double* __restrict__ bgcache,
                                                         int bg_mode, const double* __restrict__ partc, int sym_tiles,
                                                         int sym_tile, const double* __restrict__ tn_ptr) {
@@ -671,6 +672,19 @@ __global__ void __launch_bounds__(RED_T) reduce1_kernel(const double* __restrict
             if (rowd1 != nullptr) {
 #pragma unroll
                 for (int p = 0; p < 6; ++p) rowd1[i * 6 + p] = d1[p];
+            }
+            if (crec != nullptr) {   // target stream of the cross-block pass: the pass-2 record + rho_p = lambda_{n,p} / lambda_n
+                double2* o2 = reinterpret_cast<double2*>(crec) + (RS / 2 + 3) * i;
+                if (!DIM3) {
+                    o2[0] = make_double2(e.x, e.y);
+                    o2[1] = make_double2(e.t, iL);
+                } else {
+                    o2[0] = make_double2(e.x, e.y);
+                    o2[1] = make_double2(e.z, e.t);
+                    o2[2] = make_double2(iL, 0.0);
+                }
+#pragma unroll
+                for (int k = 0; k < 3; ++k) o2[RS / 2 + k] = make_double2(d1[2 * k] * iL, d1[2 * k + 1] * iL);
             }
             if (LEVEL >= 2) {
                 const double SBr4 = c.CBS * b[3], SBr2d2 = c.CBS * b[4], SBd4 = c.CBS * b[5];
@@ -976,38 +990,7 @@ __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__
     if (hess_theta_diag) hess_theta_diag[o] = -(c.CSS * c.CSS) * ds;
 }
 
-// ------------------------------------------------------------------------------------------------
-// Cross block (optional output, not tuned): thread per source m loops over all later targets.
-//   cross[m][p] = sum_n k_nm [ (dlog k_nm/dp) / lambda_n - lambda_{n,p} / lambda_n^2 ] - dLambda/(dtheta_m dp)
-template <bool DIM3>
-__global__ void __launch_bounds__(RED_T) cross_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
-                                                      const double* __restrict__ rowd1, int64_t n, DevConsts c,
-                                                      double* __restrict__ cross) {
-    constexpr int RS = DIM3 ? 6 : 4;
-    const int64_t m = (int64_t)blockIdx.x * RED_T + threadIdx.x;
-    if (m >= n) return;
-    const Ev<DIM3> g = read_rec<DIM3>(rec + m * RS);
-    double acc[6] = {0, 0, 0, 0, 0, 0};
-    const double D = (double)c.dim;
-    for (int64_t i = m + 1; i < n; ++i) {
-        const Ev<DIM3> s = read_rec<DIM3>(trec + i * RS);
-        const double dt = s.t - g.t;
-        if (!(dt > 0.0)) continue;
-        const double dx = s.x - g.x, dy = s.y - g.y, dz = s.z - g.z;
-        const double u = dx * dx + dy * dy + (DIM3 ? dz * dz : 0.0);
-        const double k = c.CS * exp(-c.omega * dt - u / (2.0 * c.h * c.h));
-        const double a = k * s.w;
-        const double gl[3] = {1.0 / c.xi0, u / (c.h * c.h * c.h) - D / c.h, 1.0 / c.omega - dt};
-#pragma unroll
-        for (int p = 0; p < 6; ++p) acc[p] += a * (p >= 3 ? gl[p - 3] : 0.0) - a * (rowd1[i * 6 + p] * s.w);
-    }
-    const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
-    const double T = tN - g.t;
-    acc[3] -= -expm1(-c.omega * T);
-    acc[5] -= c.xi0 * T * exp(-c.omega * T);
-#pragma unroll
-    for (int p = 0; p < 6; ++p) cross[m * 6 + p] = acc[p];
-}
+#include "cross.cuh"
 
 // Dense theta-theta block (correctness only): H[m][m'] = - sum_n k_nm k_nm' / lambda_n^2.
 template <bool DIM3>
@@ -1201,7 +1184,8 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, 
 namespace {
 struct Plan {
     Split sp1, sp2;   // decomposition of pass 1 / pass 2 (chunk = 0: not planned)
-    int grid1, grid2;
+    Split spx;        // ... and of the cross-block pass
+    int grid1, grid2, gridx;
     int64_t ld;
     int nblk;         // O(N) kernels
 };
@@ -1231,6 +1215,10 @@ struct hawkes_ctx {
     double* d_lam;        // n_max
     double* d_rowd1;      // n_max * 6: d lambda_n / dp of the last evaluation at LEVEL >= 1
     double* d_rowd2;      // n_max * 21 or NULL: d2 lambda_n / dp dq (hawkes_row_moments_enable)
+    double* d_crec;       // n_max * (RS + 6): target records of the cross-block pass
+    double* d_partx;      // its partial slots
+    size_t partx_doubles;
+    int occx;
     int force_dense;      // hawkes_set_pass1_mode: 1 = dense ordered-pair pass 1 even where the symmetric form applies
     double* d_blockpart;  // nblk_max * NRED
     double* d_scal;       // 2 (sum log lambda, Lambda) + peak scratch
@@ -1306,6 +1294,10 @@ constexpr int P2_R = HAWKES_P2_R;   // sources per thread in pass 2
 #ifndef HAWKES_P2_G1
 #define HAWKES_P2_G1 4
 #endif
+#ifndef HAWKES_PX_G
+#define HAWKES_PX_G 4
+#endif
+constexpr int PX_R = 2, PX_G = HAWKES_PX_G;   // cross-block pass: sources per thread, work groups per CTA
 constexpr int P1_G[3] = {HAWKES_P1_G0, HAWKES_P1_G1, HAWKES_P1_G2};
 constexpr int P2_G[2] = {HAWKES_P2_G0, HAWKES_P2_G1};
 
@@ -1407,6 +1399,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         ctx->plan_sym = sym;
         q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, sms * ctx->occ2[level2], q.ld, 2,
                              ctx->part2_doubles);
+        q.gridx = plan_split(&q.spx, n, NT * PX_R, 1, 0, 1, sms * ctx->occx, q.ld, XM, ctx->partx_doubles);
         ctx->plan_n = n; ctx->plan_l1 = level1; ctx->plan_l2 = level2;
     }
     const Plan& pl = ctx->plan;
@@ -1418,6 +1411,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
     const unsigned g1 = (unsigned)((pl.grid1 + P1_G[level1] - 1) / P1_G[level1]);
     double* const rowd1 = level1 >= 1 ? ctx->d_rowd1 : nullptr;
     double* const rowd2 = level1 >= 2 ? ctx->d_rowd2 : nullptr;
+    double* const crec = (want & HAWKES_WANT_HESS_CROSS) ? ctx->d_crec : nullptr;
     if (pe) CK(cudaEventRecord(pe[1], st));
     switch (level1) {
         case 0:
@@ -1428,7 +1422,7 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
+            reduce1_kernel<0, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, crec, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
         case 1:
             if (sym)
@@ -1436,12 +1430,12 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
             else
             pass1_kernel<P1_R, 1, DIM3, P1_G[1]><<<g1, NT * P1_G[1], smem_request(P1_G[1] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
+            reduce1_kernel<1, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, crec, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
         default:
             pass1_kernel<P1_R, 2, DIM3, P1_G[2]><<<g1, NT * P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_tab, ctx->d_part1, pl.sp1);
             if (pe) cudaEventRecord(pe[2], st);
-            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
+            reduce1_kernel<2, DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_part1, pl.sp1, ctx->d_lam, ctx->d_trec, ctx->d_trec2, rowd1, rowd2, crec, ctx->d_blockpart, ctx->d_status, ctx->d_bgcache, bg_mode, sym ? ctx->d_partc : nullptr, pl.sp1.n_tiles, NT * P1_R, nullptr);
             break;
     }
     ctx->launches += 2;
@@ -1479,8 +1473,11 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         CK(cudaEventRecord(pe[4], st));
     }
     if (want & HAWKES_WANT_HESS_CROSS) {
-        cross_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, ctx->d_trec, ctx->d_rowd1, n, c, hess_cross);
-        ctx->launches++;
+        const unsigned gx = (unsigned)((pl.gridx + PX_G - 1) / PX_G);
+        cross_pass_kernel<PX_R, DIM3, PX_G><<<gx, NT * PX_G, smem_request(PX_G * cross_group_bytes<DIM3>()), st>>>(
+            ctx->d_rec, ctx->d_crec, n, pl.ld, c, ctx->d_tab, ctx->d_partx, pl.spx);
+        cross_finish_kernel<DIM3><<<pl.nblk, RED_T, 0, st>>>(ctx->d_rec, n, pl.ld, c, ctx->d_partx, pl.spx, hess_cross);
+        ctx->launches += 2;
     }
     if (scal_aside) CK(cudaStreamWaitEvent(st, ctx->ev_join, 0));
     if (pe) {
@@ -1514,6 +1511,7 @@ int query_occupancy(hawkes_ctx* ctx) {
     if ((rc = setup_kernel(pass1_kernel<P1_R, 2, DIM3, P1_G[2]>, P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), &ctx->occ1[2]))) return rc;
     if ((rc = setup_kernel(pass2_kernel<P2_R, 0, DIM3, P2_G[0]>, P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), &ctx->occ2[0]))) return rc;
     if ((rc = setup_kernel(pass2_kernel<P2_R, 1, DIM3, P2_G[1]>, P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), &ctx->occ2[1]))) return rc;
+    if ((rc = setup_kernel(cross_pass_kernel<PX_R, DIM3, PX_G>, PX_G, smem_request(PX_G * cross_group_bytes<DIM3>()), &ctx->occx))) return rc;
     return HAWKES_OK;
 }
 
@@ -1590,6 +1588,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     for (int k = 0; k < 2; ++k) occ2 = c->occ2[k] > occ2 ? c->occ2[k] : occ2;
     c->part1_doubles = part_bound(n_max, c->sm_count * occ1, NT * P1_R, 12);
     c->part2_doubles = part_bound(n_max, c->sm_count * occ2, NT * P2_R, 2);
+    c->partx_doubles = part_bound(n_max, c->sm_count * c->occx, NT * PX_R, XM);
     c->cub_bytes = 0;
     cub::DeviceRadixSort::SortPairs(nullptr, c->cub_bytes, (const double*)nullptr, (double*)nullptr,
                                     (const int64_t*)nullptr, (int64_t*)nullptr, (int)n_max);
@@ -1601,7 +1600,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     bool ok = true;
     auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_trec2, (void**)&c->d_part1, (void**)&c->d_part2,
-                     (void**)&c->d_lam, (void**)&c->d_rowd1, (void**)&c->d_rowd2, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
+                     (void**)&c->d_lam, (void**)&c->d_rowd1, (void**)&c->d_rowd2, (void**)&c->d_crec, (void**)&c->d_partx, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
                      (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_kmat, (void**)&c->d_kmisc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
     for (auto p : ptrs) *p = nullptr;
     alloc((void**)&c->d_tab, sizeof(double) * TAB_N);
@@ -1612,6 +1611,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_part2, sizeof(double) * c->part2_doubles);
     alloc((void**)&c->d_lam, sizeof(double) * (size_t)c->ld_max);
     alloc((void**)&c->d_rowd1, sizeof(double) * 6 * (size_t)c->ld_max);
+    alloc((void**)&c->d_crec, sizeof(double) * (RS + 6) * (size_t)c->ld_max);
+    alloc((void**)&c->d_partx, sizeof(double) * c->partx_doubles);
     alloc((void**)&c->d_blockpart, sizeof(double) * NRED * (size_t)nblk);
     alloc((void**)&c->d_scal, sizeof(double) * 8);
     alloc((void**)&c->d_in, sizeof(double) * (size_t)(dim + 2) * (size_t)n_max);
@@ -1654,7 +1655,7 @@ void hawkes_destroy(hawkes_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     skip_plan_free(c);
-    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_rowd1, c->d_rowd2, c->d_blockpart,
+    void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_rowd1, c->d_rowd2, c->d_crec, c->d_partx, c->d_blockpart,
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
     for (void* p : ptrs)
         if (p) cudaFree(p);

@@ -786,7 +786,7 @@ int enqueue_eval_skip(hawkes_ctx* ctx, int64_t n, const double* x, const double*
     pass1_list_kernel<P1_R, L, DIM3, G1><<<g1, NT * G1, SM1, st>>>(ctx->d_rec, n, ld, c, ctx->d_tab, part1,              \
                                                                    items1, w1start, w1first, workers1);                   \
     reduce1_kernel<L, DIM3><<<nblk, RED_T, 0, st>>>(ctx->d_rec, n, ld, c, part1, s1, ctx->d_lam, ctx->d_trec,             \
-                                                    ctx->d_trec2, (L) >= 1 ? ctx->d_rowd1 : nullptr, (L) >= 2 ? ctx->d_rowd2 : nullptr, ctx->d_blockpart, ctx->d_status,               \
+                                                    ctx->d_trec2, (L) >= 1 ? ctx->d_rowd1 : nullptr, (L) >= 2 ? ctx->d_rowd2 : nullptr, nullptr, ctx->d_blockpart, ctx->d_status,               \
                                                     ctx->d_bgcache, bg_mode, sym ? sp.d_partc : nullptr, s1.n_tiles,      \
                                                     NT * P1_R, sp.d_tn)
     if (level1 == 0) { SKIP_PASS1(0); }

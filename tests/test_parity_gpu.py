@@ -139,7 +139,7 @@ def test_config0_table2_scales(torch):
 @pytest.fixture(scope="module")
 def cfg1_ref():
     ev = synth.config(1)
-    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
     return ev, ref
 
 
@@ -151,12 +151,15 @@ def test_config1_n23422_loglik_gradient_hessian(torch, cfg1_ref):
     r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD, ctx)
     assert st == ref.status == 0
     res = compare_all(ev, r, lam, ref, cross=False)
-    r2, st2, lam2, _ = run_gpu(torch, ev, hp.WANT_ALL & ~hp.WANT_HESS_CROSS, ctx)
+    r2, st2, lam2, _ = run_gpu(torch, ev, hp.WANT_ALL, ctx)
     assert st2 == 0
-    compare_all(ev, r2, lam2, ref, cross=False)
+    res2 = compare_all(ev, r2, lam2, ref, cross=True)       # the N x 6 cross block at full size (csrc/cross.cuh)
     # the two levels of the pass-1 kernel agree on what they share
     assert np.allclose(lam, lam2, rtol=1e-13, atol=0)
-    print("max scaled errors", res)
+    # the cross block alone (pass 1 at the gradient level, no pass 2) gives the same block
+    r3 = ctx.eval(*dev(torch, ev), ev.params, hp.WANT_HESS_CROSS)
+    assert np.allclose(r3.hess_cross.cpu().numpy(), r2.hess_cross.cpu().numpy(), rtol=1e-11, atol=1e-300)
+    print("max scaled errors", res, res2)
 
 
 def test_entry_points_agree_and_are_deterministic(torch, cfg1_ref):
@@ -267,19 +270,20 @@ def _full_oracle_case(torch, n):
     print(f"N={n}, full oracle: max scaled errors", res)
 
 
-def test_scaling_sweep_full_oracle_n50000(torch):
-    """The whole oracle (every row and column, all outputs but the cross block) at the first size of configs[4]."""
-    _full_oracle_case(torch, 50000)
+@pytest.mark.parametrize("n", [50000, 100000])
+def test_scaling_sweep_full_oracle(torch, n):
+    """The whole oracle (every row and column, all outputs but the cross block) at the first two sizes of configs[4]
+    (15 s and 50 s of 16-thread oracle time)."""
+    _full_oracle_case(torch, n)
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("n", [100000, 250000])
-def test_scaling_sweep_full_oracle_slow(torch, n):
-    """The same at N = 100,000 and N = 250,000: minutes of 16-thread oracle time each (250,000: 6.25e10 pairs), so
-    these run only with HAWKES_SLOW_TESTS=1; the log of the run that was made is profiles/r02_full_oracle_250k.txt."""
+def test_scaling_sweep_full_oracle_n250000_slow(torch):
+    """The same at N = 250,000 (north_star's second size; 6.25e10 pairs): five minutes of 16-thread oracle time, so it
+    runs only with HAWKES_SLOW_TESTS=1; the log of the run that was made is profiles/r02_full_oracle_250k.txt."""
     if os.environ.get("HAWKES_SLOW_TESTS") != "1":
-        pytest.skip("set HAWKES_SLOW_TESTS=1 (several minutes of oracle time)")
-    _full_oracle_case(torch, n)
+        pytest.skip("set HAWKES_SLOW_TESTS=1 (five minutes of oracle time)")
+    _full_oracle_case(torch, 250000)
 
 
 # ---------------------------------------------------------------------------------------------
