@@ -61,11 +61,15 @@ def compare_all(ev, r, lam, ref, cross=True):
         mu0, tx, tt, xi0, h, om = ev.params
         T = ev.t[-1] - ev.t
         c_m = np.abs(ref.grad_theta + xi0 * (-np.expm1(-om * T)))
-        rr = np.max(np.abs(ref.row_d1 / ref.lam[:, None]), axis=0)
-        # |d log k / dh| = |r^2/h^3 - D/h| on the pairs that are not exact zeros: exp(-r^2/2h^2) > 0 needs
-        # r^2/2h^2 < 1075 ln 2 = 745.2, so r^2/h^3 < 1490.3 / h
+        # Scale of entry (m, p): c_m times the largest magnitude a pair's bracket can have.  Its second part,
+        # lambda_{n,p}/lambda_n, is a difference of moment sums whose terms are bounded by
+        # |d lambda_n/dp| / lambda_n + c_p with c_p = (1/mu0, D/tau_x, 1/tau_t, 1/xi0, D/h, 1/omega), as in the row checks;
+        # its first part is |d log k / dp|: 1/xi0; |r^2/h^3 - D/h| on the pairs that are not exact zeros
+        # (exp(-r^2/2h^2) > 0 needs r^2/2h^2 < 1075 ln 2 = 745.2, so r^2/h^3 < 1490.3/h); |1/omega - dt|.
         D = ev.dim
-        colB = rr + np.array([0, 0, 0, 1 / xi0, max(D, 1490.3 - D) / h, 1 / om + (ev.t[-1] - ev.t[0])])
+        rr = np.max(np.abs(ref.row_d1 / ref.lam[:, None]), axis=0)
+        cp = np.array([1 / mu0, D / tx, 1 / tt, 1 / xi0, D / h, 1 / om])
+        colB = rr + cp + np.array([0, 0, 0, 1 / xi0, max(D, 1490.3 - D) / h, 1 / om + (ev.t[-1] - ev.t[0])])
         out["hess_cross"] = check("hess_cross", C, O, c_m[:, None] * colB[None, :] + np.array([0, 0, 0, 1, 0, xi0 * np.max(T)])[None, :], floor=1e-280)
         for p in range(6):
             assert np.max(np.abs(C[:, p] - O[:, p])) <= TOL * max(np.max(np.abs(O[:, p])), 1e-280)
