@@ -7,7 +7,10 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "hawkes_ref.cpp")
 SOURCES = [SRC, os.path.join(HERE, "tree_ref.cpp")]
-LIB = os.path.join(HERE, "libhawkes_ref.so")
+# HAWKES_ORACLE_SANITIZE=1: an AddressSanitizer + UBSan build in a library of its own (run the pins under
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so); profiles/r02_sanitizers.md)
+SANITIZE = os.environ.get("HAWKES_ORACLE_SANITIZE") == "1"
+LIB = os.path.join(HERE, "libhawkes_ref_asan.so" if SANITIZE else "libhawkes_ref.so")
 
 
 STAMP = LIB + ".srchash"   # sha256 of the sources the library was built from (mtimes do not survive a copy)
@@ -30,6 +33,8 @@ def build(force: bool = False) -> str:
     tmp = LIB + f".tmp{os.getpid()}"
     cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra",
            "-o", tmp] + SOURCES
+    if SANITIZE:
+        cmd[1:1] = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
     with open(STAMP, "w") as fh:
