@@ -224,8 +224,10 @@ int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stre
 int hawkes_row_moments_enable(hawkes_ctx* ctx, int enable);
 int hawkes_get_row_moments(hawkes_ctx* ctx, int64_t n, double* d1_out, double* d2_out, void* stream);
 
-/* Launch bookkeeping for benchmarks: number of kernels this context has launched since creation. */
+/* Launch bookkeeping for benchmarks: number of kernels this context has run since creation (kernels replayed from a
+ * CUDA graph included), and the number of graph launches among the host's launch calls (hawkes_hmc_run). */
 int64_t hawkes_launch_count(const hawkes_ctx* ctx);
+int64_t hawkes_graph_launch_count(const hawkes_ctx* ctx);
 
 /* Per-kernel device timing for benchmarks.  While enabled, every evaluation queued on the context
  * records CUDA events on its stream around pass 1, pass 2 (a4) and the whole
@@ -326,8 +328,10 @@ int hawkes_posterior_z_skip(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const
  *   prior (hawkes_tree_precision_diag) or NULL for M = mass (reading R20: without it the dynamics are
  *   unstable on trees with very short branches).
  *
- * The random numbers are inputs.  Everything is enqueued on `stream`; the accept decision is taken on the device,
- * the call never synchronises.  n_leapfrog posterior evaluations per iteration (the gradient at the current state
+ * The random numbers are inputs.  The work runs on a stream of the context that is forked from `stream` when the call
+ * starts and joined to it before the call returns (work queued on `stream` before / after the call is ordered before /
+ * after it, as for every other entry point); the accept decision is taken on the device, the call never synchronises
+ * (variant 5 excepted, see below).  It instantiates up to two CUDA graphs per call (which allocates driver memory).  n_leapfrog posterior evaluations per iteration (the gradient at the current state
  * is carried over), plus one Hessian-level evaluation per refresh and one evaluation before the first iteration.
  */
 typedef struct {
@@ -354,8 +358,12 @@ typedef struct {
                                     compressed by row and by column, in index order, and an evaluation reads those
                                     lists only.  Synchronises `stream` once per call, during this set-up (the number
                                     of non-zeros sizes the arrays, allocated on first use and kept); dim <= 2. */
-    int32_t reserved;
+    int32_t flags;           /* 0, or HAWKES_HMC_NO_GRAPH: enqueue every kernel of every iteration directly.  By default an
+                                iteration (its [refresh,] momentum draw, n_leapfrog evaluations and accept test) is captured
+                                once into a CUDA graph -- one for iterations with a preconditioner refresh, one for those
+                                without -- and replayed: one host launch per iteration.  Same kernels, same results. */
 } hawkes_hmc_opts;
+enum { HAWKES_HMC_NO_GRAPH = 1 };
 
 /* z [m] in-out, mass [m] in-out, normals [n_iter*m], uniforms [n_iter], trace [n_iter*4] or NULL
  * (per iteration: log pi of the state after the iteration, H_old, H_new, accepted 0/1): all DEVICE.

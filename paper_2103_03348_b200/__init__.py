@@ -18,6 +18,7 @@ WANT_GRAD = WANT_LL | WANT_GRAD_THETA | WANT_GRAD_HYPER
 WANT_ALL = 63
 BG_SPACE_TIME, BG_SPACE_ONLY = 0, 1
 PASS1_AUTO, PASS1_DENSE = 0, 1
+HMC_NO_GRAPH = 1
 
 
 class HawkesError(RuntimeError):
@@ -331,9 +332,9 @@ class HawkesContext:
 
     def hmc_run(self, tree: "HawkesTree", x, t, idx, z, beta: float, params, sigma2: float, tau0: float, *, n_iter: int,
                 n_leapfrog: int, step: float, precond_every: int, mass, mass_floor: float, normals, uniforms,
-                n_refresh_done: int = 0, cache_background: int = 0, prior_prec=None, trace=None):
+                n_refresh_done: int = 0, cache_background: int = 0, prior_prec=None, trace=None, graph: bool = True):
         """hawkes_hmc_run: z [m] and mass [m] are updated in place (device tensors); normals [n_iter, m] and
-        uniforms [n_iter] are device tensors; returns the trace [n_iter, 4] (device)."""
+        uniforms [n_iter] are device tensors; returns the trace [n_iter, 4] (device).  graph=False: HAWKES_HMC_NO_GRAPH."""
         torch = self._torch
         n, m = int(t.shape[0]), int(idx.shape[0])
         if normals.shape != (n_iter, m) or uniforms.shape != (n_iter,) or not normals.is_contiguous():
@@ -350,7 +351,7 @@ class HawkesContext:
         self._check_dev(prior_prec, "prior_prec", (m,), optional=True)
         self._check_dev(trace, "trace", (n_iter, 4))
         o = HmcOpts(int(n_iter), int(n_leapfrog), int(precond_every), int(n_refresh_done), float(step),
-                    float(mass_floor), int(cache_background), 0)
+                    float(mass_floor), int(cache_background), 0 if graph else HMC_NO_GRAPH)
         p = _params(params)
         rc = self._lib.hawkes_hmc_run(self._h, tree._h, n, _ptr(x), _ptr(t), m, _ptr(idx), _ptr(z), float(beta),
                                       ctypes.byref(p), float(sigma2), float(tau0), ctypes.byref(o), _ptr(normals),
@@ -402,6 +403,9 @@ class HawkesContext:
 
     def launch_count(self) -> int:
         return int(self._lib.hawkes_launch_count(self._h))
+
+    def graph_launch_count(self) -> int:
+        return int(self._lib.hawkes_graph_launch_count(self._h))
 
     def profile_enable(self, enable: bool = True):
         rc = self._lib.hawkes_profile_enable(self._h, 1 if enable else 0)

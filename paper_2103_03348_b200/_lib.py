@@ -24,7 +24,7 @@ PP = ctypes.POINTER(Params)
 class HmcOpts(ctypes.Structure):
     _fields_ = [("n_iter", ctypes.c_int32), ("n_leapfrog", ctypes.c_int32), ("precond_every", ctypes.c_int32),
                 ("n_refresh_done", ctypes.c_int32), ("step", ctypes.c_double), ("mass_floor", ctypes.c_double),
-                ("cache_background", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("cache_background", ctypes.c_int32), ("flags", ctypes.c_int32)]
 SYMBOLS = {
     "hawkes_create": (cint, [ctypes.POINTER(vp), i64, cint, cint]),
     "hawkes_destroy": (None, [vp]),
@@ -49,6 +49,7 @@ SYMBOLS = {
     "hawkes_set_background_mode": (cint, [vp, cint]),
     "hawkes_hessian_theta_block": (cint, [vp, i64, _dp, _dp, _dp, PP, i64, vp, _dp, vp]),
     "hawkes_launch_count": (i64, [vp]),
+    "hawkes_graph_launch_count": (i64, [vp]),
     "hawkes_profile_enable": (cint, [vp, cint]),
     "hawkes_profile_read": (cint, [vp, ctypes.POINTER(ctypes.c_double)]),
     "hawkes_fp64_peak": (cint, [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]),

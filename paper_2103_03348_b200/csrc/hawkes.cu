@@ -34,6 +34,9 @@
 
 #include "exp2_consts.inc"
 
+// tree.cu: counts kernels of a tree that ran inside a replayed CUDA graph (not part of the C ABI)
+extern "C" void hk_tree_count_launches(hawkes_tree* t, int64_t k);
+
 namespace {
 
 constexpr int NT = 128;        // threads per work group in the pairwise kernels (one stream-K worker)
@@ -1083,8 +1086,16 @@ __global__ void __launch_bounds__(1024) grad_beta_kernel(int64_t m, const int64_
 
 // ------------------------------------------------------------------------------------------------
 // HMC on z: three single-CTA kernels around the posterior evaluations.  hs = scalar scratch:
-// hs[0] = K_old; state scalars o3c[3] / o3p[3] = (ell, log prior, log pi) of the current / proposed state.
+// hs[0] = K_old; state scalars o3c[3] / o3p[3] = (ell, log prior, log pi) of the current / proposed state; hs[12], hs[13]
+// hold (as int64) the iteration of the call that is running and the preconditioner refreshes averaged so far -- on the
+// device, so that one captured CUDA graph serves every iteration (its kernels find their random numbers, their trace row
+// and the averaging weight through these counters).
 constexpr int HMC_T = 1024;
+constexpr int HS_IT = 12, HS_REFRESH = 13;
+__global__ void hmc_init_kernel(double* __restrict__ hs, int64_t n_refresh_done) {
+    reinterpret_cast<int64_t*>(hs)[HS_IT] = 0;
+    reinterpret_cast<int64_t*>(hs)[HS_REFRESH] = n_refresh_done;
+}
 __device__ __forceinline__ double hmc_block_sum(double a, double* sm /*[32]*/) {
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
@@ -1098,10 +1109,13 @@ __device__ __forceinline__ double hmc_block_sum(double a, double* sm /*[32]*/) {
 // p = sqrt(mass) normal;  K_old = 1/2 sum p^2/mass;  zp = z;  p += eps/2 grad;  zp += eps p / mass
 __global__ void __launch_bounds__(HMC_T) hmc_begin_kernel(int64_t m, const double* __restrict__ z, const double* __restrict__ grad,
                                                           const double* __restrict__ mass, const double* __restrict__ pp,
-                                                          const double* __restrict__ nrm,
+                                                          const double* __restrict__ normals,
                                                           double eps, double* __restrict__ zp, double* __restrict__ p,
-                                                          double* __restrict__ hs) {
+                                                          double* __restrict__ hs, int bump_refresh) {
     __shared__ double sm[32];
+    const int64_t it = reinterpret_cast<const int64_t*>(hs)[HS_IT];
+    const double* __restrict__ nrm = normals + it * m;
+    if (threadIdx.x == 0 && bump_refresh) reinterpret_cast<int64_t*>(hs)[HS_REFRESH] += 1;   // after hmc_mass_kernel read it
     double k = 0.0;
     for (int64_t i = threadIdx.x; i < m; i += HMC_T) {
         const double mi = pp ? mass[i] + pp[i] : mass[i];
@@ -1126,12 +1140,15 @@ __global__ void hmc_leap_kernel(int64_t m, const double* __restrict__ grad, cons
 // last half kick, energies, accept test, conditional copy of the state, trace
 __global__ void __launch_bounds__(HMC_T) hmc_end_kernel(int64_t m, const double* __restrict__ gradp, const double* __restrict__ mass,
                                                         const double* __restrict__ pp, double eps, const double* __restrict__ zp, const double* __restrict__ p,
-                                                        const double* __restrict__ o3p, const double* __restrict__ hs,
-                                                        const double* __restrict__ u, double* __restrict__ z,
+                                                        const double* __restrict__ o3p, double* __restrict__ hs,
+                                                        const double* __restrict__ uniforms, double* __restrict__ z,
                                                         double* __restrict__ grad, double* __restrict__ o3c,
-                                                        double* __restrict__ trace) {
+                                                        double* __restrict__ trace_all) {
     __shared__ double sm[32];
     __shared__ int acc;
+    const int64_t it = reinterpret_cast<const int64_t*>(hs)[HS_IT];
+    const double* u = uniforms + it;
+    double* trace = trace_all ? trace_all + it * 4 : nullptr;
     double k = 0.0;
     for (int64_t i = threadIdx.x; i < m; i += HMC_T) {
         const double pi = fma(0.5 * eps, gradp[i], p[i]);
@@ -1148,12 +1165,14 @@ __global__ void __launch_bounds__(HMC_T) hmc_end_kernel(int64_t m, const double*
     __syncthreads();
     if (acc)
         for (int64_t i = threadIdx.x; i < m; i += HMC_T) { z[i] = zp[i]; grad[i] = gradp[i]; }
+    if (threadIdx.x == 0) reinterpret_cast<int64_t*>(hs)[HS_IT] = it + 1;
 }
 // running average of the clamped negative Hessian diagonal: mass += (max(-hess_z, floor) - mass) / k
-__global__ void hmc_mass_kernel(int64_t m, const double* __restrict__ hess_z, double floor_, double inv_k,
+__global__ void hmc_mass_kernel(int64_t m, const double* __restrict__ hess_z, double floor_, const double* __restrict__ hs,
                                 double* __restrict__ mass) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m) return;
+    const double inv_k = 1.0 / (double)(reinterpret_cast<const int64_t*>(hs)[HS_REFRESH] + 1);   // this refresh included
     const double h = fmax(-hess_z[i], floor_), mi = mass[i];
     mass[i] = mi + (h - mi) * inv_k;
 }
@@ -1242,6 +1261,10 @@ struct hawkes_ctx {
     void* d_ksp_b;        // ... and the non-zeros by row and by column (allocated on first use, kept)
     size_t ksp_b_bytes;
     cudaStream_t side;    // small single-CTA kernels (scalars, tree prior) run here beside the big passes
+    cudaStream_t work;    // hawkes_hmc_run's own stream (forked from / joined to the caller's): stream capture needs a
+                          // non-default stream, and the caller may hand in the legacy default stream
+    cudaEvent_t ev_in, ev_out;
+    int64_t graph_launches;
     cudaEvent_t ev_fork, ev_join;
     cudaEvent_t ev_fork2, ev_tree;   // hawkes_posterior_z_skip: tree prior on the side stream
     bool side_ready;
@@ -1556,6 +1579,7 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->n_max = n_max;
     c->ld_max = round_up(n_max, 256);
     c->launches = 0;
+    c->graph_launches = 0;
     c->prof_on = false;
     c->prof_count = 0;
     c->prof_ev = nullptr;
@@ -1641,7 +1665,10 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork2, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&c->ev_tree, cudaEventDisableTiming) != cudaSuccess) {
+        cudaEventCreateWithFlags(&c->ev_tree, cudaEventDisableTiming) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->work, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming) != cudaSuccess) {
         hawkes_destroy(c);
         cudaGetLastError();
         return HAWKES_ERR_CUDA;
@@ -1666,6 +1693,9 @@ void hawkes_destroy(hawkes_ctx* c) {
         cudaEventDestroy(c->ev_join);
         cudaEventDestroy(c->ev_fork2);
         cudaEventDestroy(c->ev_tree);
+        cudaEventDestroy(c->ev_in);
+        cudaEventDestroy(c->ev_out);
+        cudaStreamDestroy(c->work);
         cudaStreamDestroy(c->side);
     }
     if (c->prof_ev) {
@@ -1837,9 +1867,11 @@ int hawkes_z_chain(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, co
     return HAWKES_OK;
 }
 
+// fill = false: theta already holds 1 at every non-sequenced event (an earlier call of this trajectory wrote them)
 static int posterior_z_impl(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
                             const int64_t* idx, const double* z, double beta, const hawkes_params* p, double sigma2,
-                            double tau0, double* out3, double* grad_z, double* hess_z, void* stream, bool skip) {
+                            double tau0, double* out3, double* grad_z, double* hess_z, void* stream, bool skip,
+                            bool fill = true) {
     if (!ctx || !tree || !x || !t || !idx || !z || !p) return HAWKES_ERR_ARG;
     if (n < 1 || n > ctx->n_max || m < 1 || m > n) return HAWKES_ERR_ARG;
     if (!out3 && !grad_z && !hess_z) return HAWKES_ERR_ARG;
@@ -1848,8 +1880,16 @@ static int posterior_z_impl(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const
     double* ht = gt + ctx->n_max;
     double* pg = ht + ctx->n_max;
     double* sc = ctx->d_post;   // sc[0] = ell, sc[1] = log prior
-    int rc = hawkes_theta_from_z(ctx, n, m, idx, z, beta, t, th, stream);
-    if (rc) return rc;
+    int rc = HAWKES_OK;
+    if (fill) {
+        rc = hawkes_theta_from_z(ctx, n, m, idx, z, beta, t, th, stream);
+        if (rc) return rc;
+    } else {
+        if (!std::isfinite(beta)) return HAWKES_ERR_PARAM;
+        CK(cudaSetDevice(ctx->device));
+        theta_scatter_kernel<<<(unsigned)((m + 255) / 256), 256, 0, (cudaStream_t)stream>>>(m, idx, z, beta, t, th);
+        ctx->launches++;
+    }
     const uint32_t want = (out3 ? HAWKES_WANT_LL : 0u) | ((grad_z || hess_z) ? HAWKES_WANT_GRAD_THETA : 0u) |
                           (hess_z ? HAWKES_WANT_HESS_THETA : 0u);
     // the O(M) tree prior (one latency-bound CTA) runs on the side stream beside the pairwise passes, which leave it
@@ -1905,7 +1945,18 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     if (use_skip && !ctx->skip) return HAWKES_ERR_ARG;
     if (!(o->step > 0.0) || !std::isfinite(o->step) || !(o->mass_floor > 0.0) || !std::isfinite(o->mass_floor))
         return HAWKES_ERR_PARAM;
-    cudaStream_t st = (cudaStream_t)stream;
+    // Everything runs on the context's own stream, forked from the caller's and joined to it at the end: the
+    // iterations are replayed from captured CUDA graphs, and capture needs a stream other than the legacy default one.
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t caller = (cudaStream_t)stream;
+    CK(cudaEventRecord(ctx->ev_in, caller));
+    CK(cudaStreamWaitEvent(ctx->work, ctx->ev_in, 0));
+    struct Join {
+        hawkes_ctx* c; cudaStream_t caller;
+        ~Join() { cudaEventRecord(c->ev_out, c->work); cudaStreamWaitEvent(caller, c->ev_out, 0); }
+    } join{ctx, caller};
+    cudaStream_t st = ctx->work;
+    stream = (void*)st;
     double* hs = ctx->d_hmc;            // [0] K_old, [4..6] o3 current, [8..10] o3 proposal
     double* o3c = hs + 4;
     double* o3p = hs + 8;
@@ -2018,8 +2069,8 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
             nblk_c = 1;                                        // one partial per column (kmat_finish_kernel)
         }
     }
-    auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess) -> int {
-        if (!kmat) return posterior_z_impl(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream, use_skip);
+    auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess, bool fill) -> int {
+        if (!kmat) return posterior_z_impl(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream, use_skip, fill);
         // the O(M) tree prior (one latency-bound CTA) runs on a side stream beside the two passes over K
         if (cudaEventRecord(ctx->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0) != cudaSuccess)
             return HAWKES_ERR_CUDA;
@@ -2049,35 +2100,72 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
         return HAWKES_OK;
     };
     // cache_background == 1: the first evaluation fills the background cache, every later one (all at LEVEL 0) uses it
+    hmc_init_kernel<<<1, 1, 0, st>>>(hs, (int64_t)o->n_refresh_done);
+    ctx->launches++;
     ctx->bg_mode = cache_bg ? 1 : 0;
-    rc = eval_post(z, o3c, gc, nullptr);
+    rc = eval_post(z, o3c, gc, nullptr, true);
     ctx->bg_mode = cache_bg ? 2 : 0;
     if (rc) return rc;
-    int n_refresh = o->n_refresh_done;
-    for (int it = 0; it < o->n_iter; ++it) {
-        if (o->precond_every > 0 && it % o->precond_every == 0) {
-            rc = eval_post(z, nullptr, nullptr, hz);
-            if (rc) return rc;
-            ++n_refresh;
-            CK(cudaSetDevice(ctx->device));
-            hmc_mass_kernel<<<mb, 256, 0, st>>>(m, hz, o->mass_floor, 1.0 / (double)n_refresh, mass);
+    // one iteration: [refresh of the preconditioner,] momentum draw, n_leapfrog evaluations, accept test.  The kernels
+    // find the iteration number and the refresh count on the device (hs), so the same enqueue serves every iteration
+    auto enqueue_iteration = [&](bool refresh) -> int {
+        int r;
+        if (refresh) {
+            if ((r = eval_post(z, nullptr, nullptr, hz, false))) return r;
+            if (cudaSetDevice(ctx->device) != cudaSuccess) return HAWKES_ERR_CUDA;
+            hmc_mass_kernel<<<mb, 256, 0, st>>>(m, hz, o->mass_floor, hs, mass);
             ctx->launches++;
         }
-        CK(cudaSetDevice(ctx->device));
-        hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, prior_prec, normals + (int64_t)it * m, eps, zp, pm, hs);
+        if (cudaSetDevice(ctx->device) != cudaSuccess) return HAWKES_ERR_CUDA;
+        hmc_begin_kernel<<<1, HMC_T, 0, st>>>(m, z, gc, mass, prior_prec, normals, eps, zp, pm, hs, refresh ? 1 : 0);
         ctx->launches++;
         for (int s = 0; s < o->n_leapfrog; ++s) {
             // the energies are needed at the end of the trajectory only
-            rc = eval_post(zp, s + 1 == o->n_leapfrog ? o3p : nullptr, gp, nullptr);
-            if (rc) return rc;
+            if ((r = eval_post(zp, s + 1 == o->n_leapfrog ? o3p : nullptr, gp, nullptr, false))) return r;
             if (s + 1 < o->n_leapfrog) {
                 hmc_leap_kernel<<<mb, 256, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm);
                 ctx->launches++;
             }
         }
-        hmc_end_kernel<<<1, HMC_T, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm, o3p, hs, uniforms + it, z, gc, o3c,
-                                            trace ? trace + (int64_t)it * 4 : nullptr);
+        hmc_end_kernel<<<1, HMC_T, 0, st>>>(m, gp, mass, prior_prec, eps, zp, pm, o3p, hs, uniforms, z, gc, o3c, trace);
         ctx->launches++;
+        return cudaGetLastError() == cudaSuccess ? HAWKES_OK : HAWKES_ERR_CUDA;
+    };
+    // The two kinds of iteration (with / without a refresh) are captured once each into a CUDA graph and replayed: one
+    // host launch per iteration instead of ~120-250 (HAWKES_HMC_NO_GRAPH in opts->flags: enqueue every kernel directly).
+    const bool use_graph = (o->flags & HAWKES_HMC_NO_GRAPH) == 0;
+    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    int64_t g_ctx[2] = {0, 0}, g_tree[2] = {0, 0};
+    struct GraphFree { cudaGraphExec_t* g; ~GraphFree() { for (int k = 0; k < 2; ++k) if (g[k]) cudaGraphExecDestroy(g[k]); } } gfree{gexec};
+    for (int it = 0; it < o->n_iter; ++it) {
+        const int kind = (o->precond_every > 0 && it % o->precond_every == 0) ? 1 : 0;
+        if (!use_graph) {
+            if ((rc = enqueue_iteration(kind == 1))) return rc;
+            continue;
+        }
+        if (!gexec[kind]) {
+            const int64_t l0 = ctx->launches, t0 = hawkes_tree_launch_count(tree);
+            CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed));
+            rc = enqueue_iteration(kind == 1);
+            cudaGraph_t graph = nullptr;
+            const cudaError_t ce = cudaStreamEndCapture(st, &graph);   // always ends the capture, also after an error
+            if (rc || ce != cudaSuccess || !graph) {
+                if (graph) cudaGraphDestroy(graph);
+                cudaGetLastError();
+                return rc ? rc : HAWKES_ERR_CUDA;
+            }
+            const cudaError_t ci = cudaGraphInstantiate(&gexec[kind], graph, 0);
+            cudaGraphDestroy(graph);
+            if (ci != cudaSuccess) { gexec[kind] = nullptr; cudaGetLastError(); return HAWKES_ERR_CUDA; }
+            g_ctx[kind] = ctx->launches - l0;
+            g_tree[kind] = hawkes_tree_launch_count(tree) - t0;
+            ctx->launches = l0;                                        // captured, not run: counted per replay below
+            hk_tree_count_launches(tree, -g_tree[kind]);
+        }
+        CK(cudaGraphLaunch(gexec[kind], st));
+        ctx->launches += g_ctx[kind];
+        hk_tree_count_launches(tree, g_tree[kind]);
+        ctx->graph_launches++;
     }
     CK(cudaGetLastError());
     return HAWKES_OK;
@@ -2165,6 +2253,7 @@ int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stre
 }
 
 int64_t hawkes_launch_count(const hawkes_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int64_t hawkes_graph_launch_count(const hawkes_ctx* ctx) { return ctx ? ctx->graph_launches : 0; }
 
 int hawkes_profile_enable(hawkes_ctx* ctx, int enable) {
     if (!ctx) return HAWKES_ERR_ARG;

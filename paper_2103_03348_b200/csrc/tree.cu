@@ -360,4 +360,7 @@ int hawkes_tree_precision_diag(hawkes_tree* t, double sigma2, double tau0, doubl
 int32_t hawkes_tree_levels(const hawkes_tree* t) { return t ? t->n_levels : 0; }
 int64_t hawkes_tree_launch_count(const hawkes_tree* t) { return t ? t->launches : 0; }
 
+/* Counts kernels of this tree that ran inside a replayed CUDA graph (hawkes_hmc_run launches them k at a time). */
+void hk_tree_count_launches(hawkes_tree* t, int64_t k) { if (t) t->launches += k; }
+
 }  // extern "C"

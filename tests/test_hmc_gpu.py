@@ -77,6 +77,60 @@ def test_hmc_matches_oracle_trajectory(torch, cache_bg, with_prior_prec):
     assert np.max(np.abs(trace[:, :3] - ref["trace"][:, :3])) <= 1e-8 * escale
     assert np.max(np.abs(z.cpu().numpy() - ref["z"])) <= 1e-8 * np.max(np.abs(ref["z"]))
     assert np.max(np.abs(mass.cpu().numpy() - ref["mass"]) / ref["mass"]) <= 1e-8
+    # the call replays captured CUDA graphs (one host launch per iteration); enqueuing every kernel directly
+    # (HAWKES_HMC_NO_GRAPH) runs the same kernels in the same order: bit-identical state, preconditioner and trace
+    assert ctx.graph_launch_count() == n_iter
+    z2, mass2 = dev(torch, z0.copy()), dev(torch, mass0.copy())
+    l0 = ctx.launch_count()
+    trace2 = ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z2, beta, ev.params, s2, tau0,
+                         n_iter=n_iter, n_leapfrog=L, step=eps, precond_every=every, mass=mass2, mass_floor=floor,
+                         normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=cache_bg,
+                         prior_prec=pp_d, graph=False)
+    torch.cuda.synchronize()
+    assert ctx.graph_launch_count() == n_iter
+    assert torch.equal(z2, z) and torch.equal(mass2, mass) and np.array_equal(trace2.cpu().numpy(), trace)
+    # ... and the launch bookkeeping counts the replayed kernels: a second graph run adds as many as the direct run did
+    direct = ctx.launch_count() - l0
+    z3, mass3 = dev(torch, z0.copy()), dev(torch, mass0.copy())
+    l1 = ctx.launch_count()
+    ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z3, beta, ev.params, s2, tau0,
+                n_iter=n_iter, n_leapfrog=L, step=eps, precond_every=every, mass=mass3, mass_floor=floor,
+                normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=cache_bg, prior_prec=pp_d)
+    torch.cuda.synchronize()
+    assert ctx.launch_count() - l1 == direct
+    assert torch.equal(z3, z)
+
+
+def test_hmc_full_size_single_iteration(torch):
+    """BASELINE.json configs[3] inputs (N = 23,422, M = 1,610): one iteration of hawkes_hmc_run -- a preconditioner
+    refresh, the momentum draw, 6 leapfrog steps, the accept test -- against oracle/hmc.py on the full likelihood
+    oracle and the dense Cholesky prior oracle (8 oracle evaluations), with the paper's preconditioner
+    (prior_prec = NULL) and the recompute-every-pair variant bench.py reports as the headline."""
+    import paper_2103_03348_b200 as hp
+    ev, tree, z0 = synth.config_tree(0)
+    idx = ev.free_idx
+    M = len(idx)
+    s2, tau0 = synth.TREE_SIGMA2, synth.TREE_TAU0
+    n_iter, L, eps, every, floor = 1, 6, 0.01, 1, 1.0
+    normals = synth.normals(0, 500, n_iter * M).reshape(n_iter, M)
+    uniforms = synth.uniforms(0, 501, n_iter)
+    V = otree.vg(tree.parent, tree.branch, M, tau0)
+    target = ohmc.hawkes_target(ev.x, ev.t, idx, 0.0, ev.params, V, s2, threads=THREADS)
+    ref = ohmc.run(target, z0, normals, uniforms, n_iter, L, eps, every, np.ones(M), floor)
+    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
+    tr = hp.HawkesTree(tree.parent, tree.branch, 0)
+    z, mass = dev(torch, z0.copy()), dev(torch, np.ones(M))
+    trace = ctx.hmc_run(tr, dev(torch, ev.x), dev(torch, ev.t), dev(torch, idx), z, 0.0, ev.params, s2, tau0,
+                        n_iter=n_iter, n_leapfrog=L, step=eps, precond_every=every, mass=mass, mass_floor=floor,
+                        normals=dev(torch, normals), uniforms=dev(torch, uniforms), cache_background=0)
+    torch.cuda.synchronize()
+    assert ctx.last_status() == 0
+    trace = trace.cpu().numpy()
+    assert np.array_equal(trace[:, 3], ref["trace"][:, 3])
+    escale = np.max(np.abs(ref["trace"][:, 1:3]))
+    assert np.max(np.abs(trace[:, :3] - ref["trace"][:, :3])) <= 1e-8 * escale
+    assert np.max(np.abs(z.cpu().numpy() - ref["z"])) <= 1e-8 * np.max(np.abs(ref["z"]))
+    assert np.max(np.abs(mass.cpu().numpy() - ref["mass"]) / ref["mass"]) <= 1e-8
 
 
 def test_hmc_rejects_bad_options(torch):
