@@ -205,6 +205,45 @@ enum { HAWKES_PASS1_AUTO = 0, HAWKES_PASS1_DENSE = 1 };
 int hawkes_set_pass1_mode(hawkes_ctx* ctx, int mode);
 int hawkes_pass1_is_symmetric(const hawkes_ctx* ctx, int level);
 
+/* ---- One evaluation sharded across several GPUs ---------------------------------
+ * One process per GPU, every rank holding all events.  The pair space of each pairwise pass (Eq. 1; Eq. 4,
+ * PAPER.md:137) is cut into world x W pieces of equal modelled cost, rank r evaluating pieces [r W, (r+1) W); a rank
+ * produces PARTIAL sums per event, which the caller exchanges between the phases with one all-gather per pass (the
+ * binding uses torch.distributed / NCCL) and which the next phase adds in rank order:
+ *
+ *   hawkes_shard_pass1   (rank, world)  events -> part_out[hawkes_shard_part_doubles(n, want, 1)]: the rank's partial moment
+ *                                       sums of lambda_n (background and self-excitation sums, and their r^2 / dt moments
+ *                                       when hyperparameter derivatives are wanted)
+ *   -- all-gather: parts_all = [world][that many doubles], rank-major --
+ *   hawkes_shard_reduce1 (world)        parts_all -> lambda_n (kept by the context), ll, grad_hyper, hess_hyper.  Every rank
+ *                                       runs it on the same numbers in the same order: replicated, bit-identical results.
+ *   hawkes_shard_pass2   (rank, world)  -> part2_out[hawkes_shard_part_doubles(n, want, 2)]: the rank's partial c_m (and d_m)
+ *   -- all-gather: parts2_all = [world][that many doubles] --
+ *   hawkes_shard_finish  (world)        parts2_all -> grad_theta[n], hess_theta_diag[n] (Eq. 4, Eq. 5), replicated.
+ *
+ * `want`: bits LL .. HESS_HYPER of hawkes_eval (no cross block), the same in all four calls and on all ranks; x, t, theta,
+ * p as for hawkes_eval; world <= 64.  All pointers DEVICE; the calls enqueue on `stream` and never synchronise; device
+ * status as hawkes_eval (hawkes_last_status after hawkes_shard_reduce1).  With world = 1 the four calls compute what
+ * hawkes_eval computes (another summation order).  Results are bit-identical run to run for a given world.
+ * hawkes_shard_workers: W of the two passes for this context and `want` (diagnostics).
+ * hawkes_plan_segments: HOST-only, needs no device.  The cut itself, for tests and tools: for the workers
+ *   [w_begin, w_end) of a pass (1 or 2) cut into workers_total pieces at moment level `level` (0..2; `symmetric` = the
+ *   once-per-unordered-pair form of pass 1) it writes up to `cap` rows (worker, tile, j_begin, j_end, partial slot) into
+ *   seg[cap*5] -- worker w evaluates, for the 256 events of `tile`, the streamed events [j_begin, j_end) -- and returns
+ *   the number of rows there are (call again with a larger buffer if it exceeds cap), or a negative status. */
+int64_t hawkes_shard_part_doubles(int64_t n, uint32_t want, int phase);
+int hawkes_shard_pass1(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                       const hawkes_params* p /*HOST*/, uint32_t want, int rank, int world, double* part_out, void* stream);
+int hawkes_shard_reduce1(hawkes_ctx* ctx, int64_t n, const hawkes_params* p /*HOST*/, uint32_t want, int world,
+                         const double* parts_all, double* ll, double* grad_hyper, double* hess_hyper, void* stream);
+int hawkes_shard_pass2(hawkes_ctx* ctx, int64_t n, const hawkes_params* p /*HOST*/, uint32_t want, int rank, int world,
+                       double* part2_out, void* stream);
+int hawkes_shard_finish(hawkes_ctx* ctx, int64_t n, const hawkes_params* p /*HOST*/, uint32_t want, int world,
+                        const double* parts2_all, double* grad_theta, double* hess_theta_diag, void* stream);
+int hawkes_shard_workers(const hawkes_ctx* ctx, uint32_t want, int* workers_pass1 /*HOST*/, int* workers_pass2 /*HOST*/);
+int64_t hawkes_plan_segments(int64_t n, int pass, int level, int symmetric, int workers_total, int w_begin, int w_end,
+                             int64_t* seg /*HOST*/, int64_t cap);
+
 /* After an evaluation queued on this context has been enqueued: copies of the per-event rates
  * lambda_n (n doubles) into a caller buffer, on `stream`.  For tests and diagnostics. */
 int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stream);

@@ -366,6 +366,50 @@ class HawkesContext:
         if rc != 0:
             raise HawkesError(rc, "hawkes_set_background_mode")
 
+    # -- one evaluation sharded across GPUs (include/hawkes.h, "One evaluation sharded ...") ---------------------
+    def shard_part_doubles(self, n: int, want: int, phase: int) -> int:
+        return int(self._lib.hawkes_shard_part_doubles(n, want, phase))
+
+    def shard_pass1(self, x, t, theta, params, want: int, rank: int, world: int, part_out):
+        n = self._check_inputs(x, t, theta)
+        self._check_dev(part_out, "part_out", (self.shard_part_doubles(n, want, 1),))
+        p = _params(params)
+        rc = self._lib.hawkes_shard_pass1(self._h, n, _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), want, rank, world,
+                                          _ptr(part_out), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_shard_pass1")
+
+    def shard_reduce1(self, n: int, params, want: int, world: int, parts_all, out: EvalResult):
+        self._check_dev(parts_all, "parts_all", (world, self.shard_part_doubles(n, want, 1)))
+        self._check_out(out, n)
+        p = _params(params)
+        rc = self._lib.hawkes_shard_reduce1(self._h, n, ctypes.byref(p), want, world, _ptr(parts_all), _ptr(out.ll),
+                                            _ptr(out.grad_hyper), _ptr(out.hess_hyper), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_shard_reduce1")
+
+    def shard_pass2(self, n: int, params, want: int, rank: int, world: int, part2_out):
+        self._check_dev(part2_out, "part2_out", (self.shard_part_doubles(n, want, 2),))
+        p = _params(params)
+        rc = self._lib.hawkes_shard_pass2(self._h, n, ctypes.byref(p), want, rank, world, _ptr(part2_out), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_shard_pass2")
+
+    def shard_finish(self, n: int, params, want: int, world: int, parts2_all, out: EvalResult):
+        self._check_dev(parts2_all, "parts2_all", (world, self.shard_part_doubles(n, want, 2)))
+        p = _params(params)
+        rc = self._lib.hawkes_shard_finish(self._h, n, ctypes.byref(p), want, world, _ptr(parts2_all),
+                                           _ptr(out.grad_theta), _ptr(out.hess_theta_diag), self._stream())
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_shard_finish")
+
+    def shard_workers(self, want: int):
+        a, b = ctypes.c_int(0), ctypes.c_int(0)
+        rc = self._lib.hawkes_shard_workers(self._h, want, ctypes.byref(a), ctypes.byref(b))
+        if rc != 0:
+            raise HawkesError(rc, "hawkes_shard_workers")
+        return int(a.value), int(b.value)
+
     def set_pass1_mode(self, mode: int):
         """hawkes_set_pass1_mode: PASS1_AUTO (background once per unordered pair where it applies) or PASS1_DENSE."""
         rc = self._lib.hawkes_set_pass1_mode(self._h, int(mode))
@@ -492,3 +536,46 @@ class HawkesTree:
 
     def launch_count(self) -> int:
         return int(self._lib.hawkes_tree_launch_count(self._h))
+
+
+def plan_segments(n: int, pass_: int, level: int, symmetric: bool, workers_total: int, w_begin: int, w_end: int):
+    """hawkes_plan_segments (host-only, no GPU): int64 array [rows, 5] = (worker, tile, j_begin, j_end, partial slot)."""
+    import numpy as np
+    lib = load()
+    cap = 1024
+    while True:
+        seg = np.zeros((cap, 5), dtype=np.int64)
+        cnt = int(lib.hawkes_plan_segments(n, pass_, level, 1 if symmetric else 0, workers_total, w_begin, w_end,
+                                           seg.ctypes.data, cap))
+        if cnt < 0:
+            raise HawkesError(cnt, "hawkes_plan_segments")
+        if cnt <= cap:
+            return seg[:cnt]
+        cap = cnt
+
+
+def shard_eval(ctx, dist, rank: int, world: int, x, t, theta, params, want: int = WANT_GRAD, out: EvalResult | None = None):
+    """One evaluation sharded across the `world` processes of `dist` (torch.distributed, one process per GPU; or None
+    with world == 1): the four hawkes_shard_* phases of `ctx` with one all-gather between pass and reduction.  Every rank
+    returns the full, replicated outputs.  Orchestration only: `ctx` does the arithmetic."""
+    import torch
+    n = int(t.shape[0])
+    r = out if out is not None else ctx.new_outputs(n, want)
+    mk = lambda k: torch.empty(k, dtype=torch.float64, device=t.device)
+
+    def gather(part):
+        allp = mk(world * part.numel()).view(world, part.numel())
+        if dist is None or world == 1:
+            allp.copy_(part.view(1, -1))
+        else:
+            dist.all_gather_into_tensor(allp.view(-1), part)
+        return allp
+
+    part1 = mk(ctx.shard_part_doubles(n, want, 1))
+    ctx.shard_pass1(x, t, theta, params, want, rank, world, part1)
+    ctx.shard_reduce1(n, params, want, world, gather(part1), r)
+    if want & (WANT_GRAD_THETA | WANT_HESS_THETA):
+        part2 = mk(ctx.shard_part_doubles(n, want, 2))
+        ctx.shard_pass2(n, params, want, rank, world, part2)
+        ctx.shard_finish(n, params, want, world, gather(part2), r)
+    return r

@@ -48,6 +48,13 @@ SYMBOLS = {
     "hawkes_skip_perm": (cint, [vp, i64, vp]),
     "hawkes_set_background_mode": (cint, [vp, cint]),
     "hawkes_hessian_theta_block": (cint, [vp, i64, _dp, _dp, _dp, PP, i64, vp, _dp, vp]),
+    "hawkes_shard_part_doubles": (i64, [i64, u32, cint]),
+    "hawkes_shard_pass1": (cint, [vp, i64, _dp, _dp, _dp, PP, u32, cint, cint, _dp, vp]),
+    "hawkes_shard_reduce1": (cint, [vp, i64, PP, u32, cint, _dp, _dp, _dp, _dp, vp]),
+    "hawkes_shard_pass2": (cint, [vp, i64, PP, u32, cint, cint, _dp, vp]),
+    "hawkes_shard_finish": (cint, [vp, i64, PP, u32, cint, _dp, _dp, _dp, vp]),
+    "hawkes_shard_workers": (cint, [vp, u32, ctypes.POINTER(cint), ctypes.POINTER(cint)]),
+    "hawkes_plan_segments": (i64, [i64, cint, cint, cint, cint, cint, cint, vp, i64]),
     "hawkes_launch_count": (i64, [vp]),
     "hawkes_graph_launch_count": (i64, [vp]),
     "hawkes_profile_enable": (cint, [vp, cint]),

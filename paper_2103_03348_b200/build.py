@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhawkes_b200.so")
 SOURCES = [os.path.join(CSRC, "hawkes.cu"), os.path.join(CSRC, "tree.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("exp2_consts.inc", "pass1_sym.cuh", "hmc_kmat.cuh", "hmc_ksparse.cuh", "skip.cuh", "cross.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("exp2_consts.inc", "pass1_sym.cuh", "hmc_kmat.cuh", "hmc_ksparse.cuh", "skip.cuh", "cross.cuh", "shard.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "hawkes.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]

@@ -97,14 +97,14 @@ __global__ void __launch_bounds__(NT * G, 1) cross_pass_kernel(const double* __r
     __syncthreads();
 
     const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
-    const int64_t vcta = (int64_t)blockIdx.x * G + grp;
+    const int64_t vcta = (int64_t)blockIdx.x * G + grp + sp.w_begin;
     double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
     double* const sbuf1 = sbuf0 + TS * RSX;
     const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
 
     const int64_t total = split_prefix(sp, sp.n_tiles);
     const int64_t lo = vcta * sp.chunk;
-    if (lo >= total) return;
+    if (lo >= total || vcta >= sp.w_end) return;
     const int64_t hi = min(lo + sp.chunk, total);
     const P1C pc = pinned_consts(smagic, c);
 
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(NT * G, 1) cross_pass_kernel(const double* __r
             a = a2;
             b = b2;
         }
-        const int slot = (int)(vcta - base / sp.chunk);
+        const int slot = split_slot_of(sp, vcta, base);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int64_t i = m0 + r * NT + tid;

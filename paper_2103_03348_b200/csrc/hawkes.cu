@@ -391,6 +391,9 @@ struct Split {
     int w_head;      // extra cost of the streamed events with index < tile end     (pass 1: excitation)
     int tri;         // 1: only streamed events with index >= tile begin are visited (pass 2)
     const int* slot_tab;   // device table of slots per tile (list-driven passes of skip.cuh); NULL: closed form
+    int fixed_slots;       // > 0: every tile has this many slots (the gathered per-rank sums of the sharded evaluation)
+    int w_begin, w_end;    // workers [w_begin, w_end) of the cut run on this device (all of them unless the evaluation
+                           // is sharded across GPUs: shard.cuh); partial slots are numbered from the first of them
 };
 
 __host__ __device__ inline int64_t split_prefix(const Split& s, int64_t I) {   // cost of tiles [0, I)
@@ -418,10 +421,18 @@ __host__ __device__ inline int64_t split_pos(const Split& s, int64_t I, int64_t 
 }
 // first CTA and number of CTAs (= partial slots) that hold a segment of tile I
 __host__ __device__ inline void split_slots(const Split& s, int64_t I, int* first, int* count) {
+    if (s.fixed_slots > 0) { *first = 0; *count = s.fixed_slots; return; }
     if (s.slot_tab != nullptr) { *first = 0; *count = s.slot_tab[I]; return; }
-    const int64_t a = split_prefix(s, I) / s.chunk, b = (split_prefix(s, I + 1) - 1) / s.chunk;
+    int64_t a = split_prefix(s, I) / s.chunk, b = (split_prefix(s, I + 1) - 1) / s.chunk;
+    if (a < s.w_begin) a = s.w_begin;
+    if (b > (int64_t)s.w_end - 1) b = (int64_t)s.w_end - 1;
     *first = (int)a;
-    *count = (int)(b - a + 1);
+    *count = b >= a ? (int)(b - a + 1) : 0;
+}
+// partial slot of worker `w` in the tile whose cost axis starts at `base`
+__host__ __device__ inline int split_slot_of(const Split& s, int64_t w, int64_t base) {
+    const int64_t first = base / s.chunk;
+    return (int)(w - (first > s.w_begin ? first : (int64_t)s.w_begin));
 }
 
 // a1: one CTA per SM, G independent work groups of NT threads; group (blockIdx.x * G + g) is worker
@@ -444,14 +455,14 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_kernel(const double* __restri
     __syncthreads();   // the only CTA-wide barrier; the groups are independent from here on
 
     const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
-    const int64_t vcta = (int64_t)blockIdx.x * G + grp;
+    const int64_t vcta = (int64_t)blockIdx.x * G + grp + sp.w_begin;
     double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
     double* const sbuf1 = sbuf0 + TS * RS;
     const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
 
     const int64_t total = split_prefix(sp, sp.n_tiles);
     const int64_t lo = vcta * sp.chunk;
-    if (lo >= total) return;
+    if (lo >= total || vcta >= sp.w_end) return;
     const int64_t hi = min(lo + sp.chunk, total);
     const P1C pc = pinned_consts(smagic, c);
 
@@ -504,7 +515,7 @@ __global__ void __launch_bounds__(NT * G, 1) pass1_kernel(const double* __restri
             a = a2;
             b = b2;
         }
-        const int slot = (int)(vcta - base / sp.chunk);
+        const int slot = split_slot_of(sp, vcta, base);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int64_t i = i0 + r * NT + tid;
@@ -866,14 +877,14 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
     __syncthreads();
 
     const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
-    const int64_t vcta = (int64_t)blockIdx.x * G + grp;
+    const int64_t vcta = (int64_t)blockIdx.x * G + grp + sp.w_begin;
     double* const sbuf0 = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
     double* const sbuf1 = sbuf0 + TS * RS;
     const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
 
     const int64_t total = split_prefix(sp, sp.n_tiles);
     const int64_t lo = vcta * sp.chunk;
-    if (lo >= total) return;
+    if (lo >= total || vcta >= sp.w_end) return;
     const int64_t hi = min(lo + sp.chunk, total);
     const P1C pc_ = pinned_consts(smagic, c);
     // warp-uniform, fixed for the whole evaluation: bit 0 (prep_kernel) a streamed tile spans too much time, bit 1
@@ -943,7 +954,7 @@ __global__ void __launch_bounds__(NT * G, 1) pass2_kernel(const double* __restri
             a = a2;
             b = b2;
         }
-        const int slot = (int)(vcta - base / sp.chunk);
+        const int slot = split_slot_of(sp, vcta, base);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int64_t i = m0 + r * NT + tid;
@@ -1340,6 +1351,9 @@ int plan_split(Split* sp, int64_t n, int tile, int w_all, int w_head, int tri, i
     sp->w_head = w_head;
     sp->tri = tri;
     sp->slot_tab = nullptr;
+    sp->fixed_slots = 0;
+    sp->w_begin = 0;
+    sp->w_end = 0x7fffffff;
     const int64_t total = split_prefix(*sp, sp->n_tiles);
     const int64_t min_chunk = (int64_t)(tri ? 1 : w_all + w_head) * 32;   // >= ~32 streamed events per CTA
     int64_t chunk = (total + ctas - 1) / ctas;
@@ -1361,7 +1375,7 @@ int plan_split(Split* sp, int64_t n, int tile, int w_all, int w_head, int tri, i
 size_t part_bound(int64_t n_max, int ctas_max, int tile, int n_mom) {
     // slots x ld  <~  1.3 ctas x tile + 2 ld  (see plan_split); generous, and plan_split() coarsens the cut
     // if an actual plan would not fit
-    return (size_t)n_mom * ((size_t)2 * ctas_max * tile + 4 * (size_t)round_up(n_max, 256));
+    return (size_t)n_mom * ((size_t)2 * ctas_max * tile + 10 * (size_t)round_up(n_max, 256));
 }
 
 int make_consts(const hawkes_params* p, int dim, int s_mode, DevConsts* c) {
@@ -1548,6 +1562,10 @@ int check_common(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
 }  // namespace
 
 #include "skip.cuh"
+
+namespace {
+#include "shard.cuh"
+}  // namespace
 
 extern "C" {
 
@@ -2200,6 +2218,110 @@ int hawkes_hessian_theta_block(hawkes_ctx* ctx, int64_t n, const double* x, cons
     hess_block_kernel<<<dim3(nt, nt), 256, 0, st>>>(ctx->d_kmat, n, m, hess_block);
     ctx->launches += 3;
     CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+
+// ---- one evaluation sharded across GPUs (csrc/shard.cuh) ------------------------------------------------------------
+static int shard_check(hawkes_ctx* ctx, int64_t n, const hawkes_params* p, uint32_t want, int rank, int world, DevConsts* c) {
+    if (!ctx || !p || n < 1 || n > ctx->n_max) return HAWKES_ERR_ARG;
+    if (want == 0 || (want & ~31u)) return HAWKES_ERR_ARG;            // no cross block in the sharded evaluation
+    if (world < 1 || world > 64 || rank < 0 || rank >= world) return HAWKES_ERR_ARG;
+    int rc = make_consts(p, ctx->dim, ctx->s_mode, c);
+    if (rc) return rc;
+    CK(cudaSetDevice(ctx->device));
+    return HAWKES_OK;
+}
+
+int64_t hawkes_shard_part_doubles(int64_t n, uint32_t want, int phase) {
+    if (n < 1 || (phase != 1 && phase != 2)) return 0;
+    const int level1 = (want & HAWKES_WANT_HESS_HYPER) ? 2 : ((want & HAWKES_WANT_GRAD_HYPER) ? 1 : 0);
+    const int nb = level1 == 0 ? 1 : (level1 == 1 ? 3 : 6);
+    return (phase == 1 ? 2 * nb : 2) * round_up(n, 256);
+}
+
+int hawkes_shard_pass1(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, const double* theta,
+                       const hawkes_params* p, uint32_t want, int rank, int world, double* part_out, void* stream) {
+    DevConsts c;
+    int rc = shard_check(ctx, n, p, want, rank, world, &c);
+    if (rc) return rc;
+    if (!x || !t || !theta || !part_out) return HAWKES_ERR_ARG;
+    const ShardLevels L = shard_levels(ctx, want);
+    if (ctx->dim == 3) return shard_pass1_impl<true>(ctx, n, x, t, theta, c, L, rank, world, part_out, (cudaStream_t)stream);
+    return shard_pass1_impl<false>(ctx, n, x, t, theta, c, L, rank, world, part_out, (cudaStream_t)stream);
+}
+
+int hawkes_shard_reduce1(hawkes_ctx* ctx, int64_t n, const hawkes_params* p, uint32_t want, int world,
+                         const double* parts_all, double* ll, double* grad_hyper, double* hess_hyper, void* stream) {
+    DevConsts c;
+    int rc = shard_check(ctx, n, p, want, 0, world, &c);
+    if (rc) return rc;
+    if (!parts_all || ((want & HAWKES_WANT_LL) && !ll) || ((want & HAWKES_WANT_GRAD_HYPER) && !grad_hyper) ||
+        ((want & HAWKES_WANT_HESS_HYPER) && !hess_hyper)) return HAWKES_ERR_ARG;
+    const ShardLevels L = shard_levels(ctx, want);
+    if (ctx->dim == 3) return shard_reduce1_impl<true>(ctx, n, c, want, L, world, parts_all, ll, grad_hyper, hess_hyper, (cudaStream_t)stream);
+    return shard_reduce1_impl<false>(ctx, n, c, want, L, world, parts_all, ll, grad_hyper, hess_hyper, (cudaStream_t)stream);
+}
+
+int hawkes_shard_pass2(hawkes_ctx* ctx, int64_t n, const hawkes_params* p, uint32_t want, int rank, int world,
+                       double* part2_out, void* stream) {
+    DevConsts c;
+    int rc = shard_check(ctx, n, p, want, rank, world, &c);
+    if (rc) return rc;
+    if (!part2_out) return HAWKES_ERR_ARG;
+    const ShardLevels L = shard_levels(ctx, want);
+    if (ctx->dim == 3) return shard_pass2_impl<true>(ctx, n, c, L, rank, world, part2_out, (cudaStream_t)stream);
+    return shard_pass2_impl<false>(ctx, n, c, L, rank, world, part2_out, (cudaStream_t)stream);
+}
+
+int hawkes_shard_finish(hawkes_ctx* ctx, int64_t n, const hawkes_params* p, uint32_t want, int world,
+                        const double* parts2_all, double* grad_theta, double* hess_theta_diag, void* stream) {
+    DevConsts c;
+    int rc = shard_check(ctx, n, p, want, 0, world, &c);
+    if (rc) return rc;
+    if (!parts2_all || ((want & HAWKES_WANT_GRAD_THETA) && !grad_theta) || ((want & HAWKES_WANT_HESS_THETA) && !hess_theta_diag))
+        return HAWKES_ERR_ARG;
+    if (ctx->dim == 3) return shard_finish_impl<true>(ctx, n, c, want, world, parts2_all, grad_theta, hess_theta_diag, (cudaStream_t)stream);
+    return shard_finish_impl<false>(ctx, n, c, want, world, parts2_all, grad_theta, hess_theta_diag, (cudaStream_t)stream);
+}
+
+int64_t hawkes_plan_segments(int64_t n, int pass, int level, int symmetric, int workers_total, int w_begin, int w_end,
+                             int64_t* seg, int64_t cap) {
+    if (n < 1 || (pass != 1 && pass != 2) || level < 0 || level > 2 || workers_total < 1 || w_begin < 0 || w_end < w_begin)
+        return HAWKES_ERR_ARG;
+    if (cap > 0 && !seg) return HAWKES_ERR_ARG;
+    Split sp;
+    const int64_t ld = round_up(n, 256);
+    if (pass == 1) plan_split(&sp, n, NT * P1_R, symmetric ? 0 : W_ALL[level], W_HEAD[level], 0, workers_total, ld, 12, (size_t)-1);
+    else plan_split(&sp, n, NT * P2_R, 1, 0, 1, workers_total, ld, 2, (size_t)-1);
+    sp.w_begin = w_begin;
+    sp.w_end = w_end;
+    const int64_t total = split_prefix(sp, sp.n_tiles);
+    int64_t count = 0;
+    for (int64_t w = w_begin; w < w_end; ++w) {       // what worker w of the pairwise kernels does, restated on the host
+        const int64_t lo = w * sp.chunk;
+        if (lo >= total) break;
+        const int64_t hi = std::min(lo + sp.chunk, total);
+        for (int I = split_tile_of(sp, lo); I < sp.n_tiles; ++I) {
+            const int64_t base = split_prefix(sp, I);
+            if (base >= hi) break;
+            const int64_t cost_I = split_prefix(sp, I + 1) - base;
+            const int64_t jb = split_pos(sp, I, std::max(lo - base, (int64_t)0));
+            const int64_t je = split_pos(sp, I, std::min(hi - base, cost_I));
+            if (count < cap) {
+                int64_t* o = seg + 5 * count;
+                o[0] = w; o[1] = I; o[2] = jb; o[3] = je; o[4] = split_slot_of(sp, w, base);
+            }
+            ++count;
+        }
+    }
+    return count;
+}
+
+int hawkes_shard_workers(const hawkes_ctx* ctx, uint32_t want, int* workers_pass1, int* workers_pass2) {
+    if (!ctx || !workers_pass1 || !workers_pass2) return HAWKES_ERR_ARG;
+    const ShardLevels L = shard_levels(ctx, want);
+    *workers_pass1 = ctx->sm_count * ctx->occ1[L.level1];
+    *workers_pass2 = ctx->sm_count * ctx->occ2[L.level2];
     return HAWKES_OK;
 }
 

@@ -186,7 +186,7 @@ __global__ void HAWKES_SYM_BOUNDS pass1s_kernel(const double* __restrict__ rec, 
     __syncthreads();
 
     const int grp = threadIdx.x / NT, tid = threadIdx.x % NT, lane = threadIdx.x & 31, wrp = tid >> 5;
-    const int64_t vcta = (int64_t)blockIdx.x * G + grp;
+    const int64_t vcta = (int64_t)blockIdx.x * G + grp + sp.w_begin;
     double* const gbuf = reinterpret_cast<double*>(smem + plan.buf_off + grp * GB);
     double* const sbuf0 = gbuf;
     double* const sbuf1 = gbuf + NA * TS;
@@ -196,7 +196,7 @@ __global__ void HAWKES_SYM_BOUNDS pass1s_kernel(const double* __restrict__ rec, 
 
     const int64_t total = split_prefix(sp, sp.n_tiles);
     const int64_t lo = vcta * sp.chunk;
-    if (lo >= total) return;
+    if (lo >= total || vcta >= sp.w_end) return;
     const int64_t hi = min(lo + sp.chunk, total);
     // every loop constant through shared memory: held in vector registers, never re-loaded inside the loops
     P1C pc;
@@ -274,7 +274,7 @@ __global__ void HAWKES_SYM_BOUNDS pass1s_kernel(const double* __restrict__ rec, 
             a = a2;
             b = b2;
         }
-        const int slot = (int)(vcta - base / sp.chunk);
+        const int slot = split_slot_of(sp, vcta, base);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int64_t i = i0 + r * NT + tid;

@@ -59,6 +59,65 @@ def test_two_replicas_max_over_ranks_and_seeds(tmp_path):
     assert res[0]["seed"] == 7 and res[1]["seed"] == 8 and res[0]["t0"] != res[1]["t0"]
 
 
+SHARD_WORKER = textwrap.dedent("""
+    import json, os, sys
+    sys.path.insert(0, %r)
+    sys.path.insert(0, os.path.join(%r, "tests"))
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import oracle
+    import paper_2103_03348_b200 as hp
+    from paper_2103_03348_b200 import synth
+    from shard_stub import StubShardContext
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    dist.init_process_group("gloo")
+    ev = synth.small_random(700, seed=5, ties=True, duplicates=True)
+    ev.x *= 6.0
+    ev.t *= 15.0
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a))
+    res = []
+    for sym in (True, False):
+        ctx = StubShardContext(workers_per_rank=5, symmetric=sym)
+        r = hp.shard_eval(ctx, dist, rank, world, f(ev.x), f(ev.t), f(ev.theta), ev.params, hp.WANT_LL | hp.WANT_GRAD_THETA)
+        ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params)
+        res.append({"rank": rank, "sym": sym,
+                    "lam_err": float(np.max(np.abs(ctx.lam - ref.lam) / ref.lam)),
+                    "ll_err": abs(r.ll.item() - ref.integral - ref.ll) / abs(ref.ll),
+                    "grad_err": float(np.max(np.abs(r.grad_theta.numpy() - ref.grad_theta)) / np.max(np.abs(ref.grad_theta))),
+                    "lam_sum": float(ctx.lam.sum())})
+    gathered = [None] * world
+    dist.all_gather_object(gathered, res)
+    if rank == 0:
+        print(json.dumps(gathered), flush=True)
+    dist.destroy_process_group()
+""") % (ROOT, ROOT)
+
+
+def test_two_ranks_shard_one_evaluation(tmp_path):
+    """paper_2103_03348_b200.shard_eval (the orchestration the GPU path uses: phase, all-gather, phase, ...) over gloo with
+    two processes.  The phases are a numpy stand-in (tests/shard_stub.py) that evaluates exactly the pieces of the pair
+    space hawkes_plan_segments gives each rank, so the test covers the cut, the exchange and the rank-ordered sums: the
+    assembled lambda, ell and d ell/d theta must be the oracle's, identically on both ranks."""
+    script = tmp_path / "shard_worker.py"
+    script.write_text(SHARD_WORKER)
+    port = free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), GLOO_SOCKET_IFNAME="lo")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=300) for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
+    res = json.loads(outs[0][0].strip().splitlines()[-1])
+    for a, b in zip(res[0], res[1]):                       # per pass-1 form: rank 0's and rank 1's record
+        assert a["rank"] == 0 and b["rank"] == 1 and a["sym"] == b["sym"]
+        for r in (a, b):
+            assert r["lam_err"] < 1e-12 and r["ll_err"] < 1e-13 and r["grad_err"] < 1e-12, r
+        assert a["lam_sum"] == b["lam_sum"]                # replicated: the same bits on both ranks
+
+
 def test_single_process_helpers():
     sys.path.insert(0, ROOT)
     import bench
