@@ -404,6 +404,10 @@ def run_b200(args, ev, workload: str) -> dict:
     timed = lambda call, steps: timed_steps(torch, dev, call, steps, flush)
 
     step = lambda: ctx.grad(x, t, th, ev.params, out=out)
+    if args.shard:
+        # ONE evaluation cut across the ranks (hawkes_shard_*): every rank holds the same events,
+        # evaluates its share of both pairwise passes and all-gathers the partial sums (NCCL) -- "scaling": "strong"
+        step = lambda: hp.shard_eval(ctx, dist, rank, world, x, t, th, ev.params, hp.WANT_GRAD, out=out)
     # -- device-resident leg ----------------------------------------------------------------------
     timed(step, W)
     assert ctx.last_status() == 0, "evaluation reported a data error"
@@ -416,13 +420,21 @@ def run_b200(args, ev, workload: str) -> dict:
     barrier()
     wall = time.perf_counter() - wall0
     launches = ctx.launch_count() - l0
-    prof = ctx.profile_read()
+    prof = ctx.profile_read() if not args.shard else None
     ctx.profile_enable(False)
     total_ms = float(sum(ms))
     # -- end-to-end leg: HOST buffers through hawkes_eval_host (H2D of inputs + D2H of results inside) ----
     hx, ht, hth = (a.cpu().pin_memory() for a in (x, t, th))
     hout = ctx.new_outputs(n, hp.WANT_GRAD, "cpu", pinned=True)
     estep = lambda: ctx.eval_host(hx, ht, hth, ev.params, hp.WANT_GRAD, out=hout)
+    if args.shard:
+        def estep():   # host buffers in, sharded evaluation, replicated results back to the host on every rank
+            x.copy_(hx, non_blocking=True); t.copy_(ht, non_blocking=True); th.copy_(hth, non_blocking=True)
+            hp.shard_eval(ctx, dist, rank, world, x, t, th, ev.params, hp.WANT_GRAD, out=out)
+            hout.ll.copy_(out.ll, non_blocking=True)
+            hout.grad_theta.copy_(out.grad_theta, non_blocking=True)
+            hout.grad_hyper.copy_(out.grad_hyper, non_blocking=True)
+            torch.cuda.current_stream(dev).synchronize()
     timed(estep, W)
     barrier()
     e_ms = timed(estep, K)
@@ -439,12 +451,27 @@ def run_b200(args, ev, workload: str) -> dict:
     ll_dev = float(out.ll.item())
     ll_host = float(hout.ll.item())
     assert ll_dev == ll_host, "device-resident and host-buffer evaluations must be bit-identical"
-    value = whole_job_value(world, K, total_ms)
-    e_value = whole_job_value(world, K, e_total)
+    # replicas: every rank did K evaluations of its own problem; sharded: the ranks did K evaluations together
+    value = whole_job_value(1 if args.shard else world, K, total_ms)
+    e_value = whole_job_value(1 if args.shard else world, K, e_total)
     props = torch.cuda.get_device_properties(dev)
     sm_max = clocks.get("sm_max_mhz") or 1965
     peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     peak_dfma = ctx.fp64_peak(200.0)
+    if args.shard:   # the per-kernel ring belongs to hawkes_eval; a sharded step reports the whole step only
+        if dist is not None:
+            dist.destroy_process_group()
+        return {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload, "n_events": n, "dim": ev.dim, "call": "hawkes_shard_pass1/reduce1/pass2/finish",
+                           "parallelism": f"one evaluation sharded across {world} ranks (2 all-gathers per evaluation)",
+                           "l2": "256 MiB memset between timed steps, outside the per-step event pairs"},
+                "gpairs_per_s": float(n) * n * value / 1e9, "gpu_launches": int(launches), "clocks": clocks,
+                "e2e": {"value": e_value, "unit": UNIT, "ms_per_step": e_total / K,
+                        "h2d_bytes_per_step": int((ev.dim + 2) * n * 8), "d2h_bytes_per_step": int((1 + n + 6) * 8),
+                        "call": "pinned host buffers -> shard_eval -> pinned host buffers, on every rank"},
+                "ll": ll_dev}
     p1_ms = prof["pass1_ms"] / max(prof["evals"], 1)
     p2_ms = prof["pass2_ms"] / max(prof["evals"], 1)
     inner_ms = prof["total_ms"] / max(prof["evals"], 1)
@@ -455,11 +482,13 @@ def run_b200(args, ev, workload: str) -> dict:
                             f"{sm_max} MHz (clocks.max.sm); MEASURED_PEAKS.json has no FP64 entry")
     res = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload, "n_events": n, "dim": ev.dim, "outputs": "ll + grad_theta[N] + grad_hyper[6]",
                    "call": "hawkes_grad", "l2": "256 MiB memset between timed steps, outside the per-step event pairs",
-                   "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)"},
+                   "parallelism": ("1 GPU" if world == 1 and not args.shard else
+                                   f"one evaluation sharded across {world} ranks (2 all-gathers per evaluation)" if args.shard
+                                   else f"{world} independent replicas (no collective)")},
         "gpairs_per_s": float(n) * n * value / 1e9,
         "kernel_terms_per_s": (float(n) * n + float(n) * (n - 1)) * value,
         "wall_s_timed_region": wall,
@@ -764,7 +793,7 @@ def run_hmc(args) -> dict:
 def workload_of(args):
     from paper_2103_03348_b200 import synth
     rank, world, _ = dist_env()
-    if world > 1 and args.impl != "reference":
+    if world > 1 and args.impl != "reference" and not getattr(args, "shard", False):   # sharded: the same events on every rank
         args = argparse.Namespace(**{**vars(args), "seed": replica_seed(args.seed, rank)})
     if args.n is not None:
         ev = synth.make_events(args.n, args.seed)
@@ -789,6 +818,8 @@ def main() -> int:
     ap.add_argument("--extras", action="store_true", help="also time the Hessian and the theta-only evaluation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] sizes in the default line")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: cut ONE evaluation across the ranks (hawkes_shard_*) instead of running N replicas")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--hmc-step", type=float, default=0.2, help="leapfrog step size of --config 3 with the prior curvature in the mass (R20)")
     ap.add_argument("--hmc-step-paper", type=float, default=0.01, help="step size of --config 3 with the paper's preconditioner")

@@ -109,7 +109,9 @@ def test_sharded_argument_errors(torch):
         with pytest.raises(hp.HawkesError) as e:
             ctx.shard_pass1(x, t, th, ev.params, hp.WANT_GRAD, rank, world, part)
         assert e.value.status == hp.ERR_ARG
-    with pytest.raises(hp.HawkesError):                     # the cross block is not part of the sharded evaluation
-        ctx.shard_pass1(x, t, th, ev.params, hp.WANT_ALL, 0, 2, part)
+    big = torch.empty(ctx.shard_part_doubles(ev.n, hp.WANT_ALL, 1), dtype=torch.float64, device="cuda")
+    with pytest.raises(hp.HawkesError) as e:                # the cross block is not part of the sharded evaluation
+        ctx.shard_pass1(x, t, th, ev.params, hp.WANT_ALL, 0, 2, big)
+    assert e.value.status == hp.ERR_ARG
     w1, w2 = ctx.shard_workers(hp.WANT_GRAD)
     assert w1 > 0 and w2 > 0
