@@ -389,17 +389,25 @@ struct Split {
     int n_tiles;
     int w_all;       // cost of a streamed event every owned event pairs with       (pass 1: background)
     int w_head;      // extra cost of the streamed events with index < tile end     (pass 1: excitation)
-    int tri;         // 1: only streamed events with index >= tile begin are visited (pass 2)
+    int tri;         // 1: only streamed events with index >= tile begin are visited (pass 2).  Then w_all is the cost of a
+                     // streamed event past the tile's own (plain pieces), w_head that of one of the tile's own events
+                     // (masked, unfactorised pieces) and w_tile a fixed cost per tile (loading the owners, two barriers,
+                     // writing the partials): the last workers of the axis hold many short, mostly masked tiles
+    int w_tile;
     const int* slot_tab;   // device table of slots per tile (list-driven passes of skip.cuh); NULL: closed form
+    int align;             // > 1: segment ends are rounded to a multiple of this many streamed events (the symmetric pass 1
+                           // walks whole blocks of 32: a cut inside a block would cost both workers the whole block)
     int fixed_slots;       // > 0: every tile has this many slots (the gathered per-rank sums of the sharded evaluation)
     int w_begin, w_end;    // workers [w_begin, w_end) of the cut run on this device (all of them unless the evaluation
                            // is sharded across GPUs: shard.cuh); partial slots are numbered from the first of them
 };
 
 __host__ __device__ inline int64_t split_prefix(const Split& s, int64_t I) {   // cost of tiles [0, I)
-    if (s.tri) return s.n * I - (int64_t)s.tile * (I * (I - 1) / 2);
     const int64_t nf = s.n / s.tile;                 // full tiles
     const int64_t If = I < nf ? I : nf;
+    if (s.tri)
+        return If * ((int64_t)s.w_tile + (int64_t)s.w_head * s.tile) + (int64_t)s.w_all * (s.n * If - (int64_t)s.tile * (If * (If + 1) / 2)) +
+               (I > nf ? (int64_t)s.w_tile + (int64_t)s.w_head * (s.n - nf * s.tile) : 0);
     return (int64_t)s.w_all * s.n * I + (int64_t)s.w_head * ((int64_t)s.tile * (If * (If + 1) / 2) + (I > nf ? s.n : 0));
 }
 __host__ __device__ inline int split_tile_of(const Split& s, int64_t c) {      // largest I with prefix(I) <= c
@@ -412,10 +420,17 @@ __host__ __device__ inline int split_tile_of(const Split& s, int64_t c) {      /
 }
 // streamed-event index reached after `c` cost units of tile I (monotone; 0 -> first visited, cost(I) -> n)
 __host__ __device__ inline int64_t split_pos(const Split& s, int64_t I, int64_t c) {
-    if (s.tri) { const int64_t j = I * s.tile + c; return j < s.n ? j : s.n; }
     int64_t i1 = (I + 1) * s.tile; if (i1 > s.n) i1 = s.n;
+    if (s.tri) {
+        const int64_t i0 = I * s.tile, own = (int64_t)s.w_head * (i1 - i0);
+        c -= s.w_tile;
+        if (c <= 0) return i0;
+        const int64_t j = c < own ? i0 + c / s.w_head : i1 + (c - own) / s.w_all;
+        return j < s.n ? j : s.n;
+    }
     const int64_t wh = s.w_all + s.w_head;
     int64_t j = (c < wh * i1 || s.w_all == 0) ? c / wh : i1 + (c - wh * i1) / s.w_all;
+    if (s.align > 1 && j < i1) j = (j + s.align / 2) / s.align * s.align;   // the tile's end itself is never moved
     if (s.w_all == 0 && j > i1) j = i1;   // excitation-only pass: nothing is visited past the tile's end
     return j < s.n ? j : s.n;
 }
@@ -1337,6 +1352,9 @@ constexpr int P2_G[2] = {HAWKES_P2_G0, HAWKES_P2_G1};
 
 // cost weights of the pass-1 cost axis per LEVEL: modelled issue cycles of a
 // background term (every streamed source) and of an excitation term (sources before the tile's end)
+// ... and of pass 2 (and the cross pass): a pair of a plain piece (factorised, 13 FP64 instructions) against one of the
+// tile's own, masked piece (unfactorised + the per-pair time test): 32.5 : 41 modelled cycles
+constexpr int W2_PLAIN = 4, W2_OWN = 5;
 constexpr int W_ALL[3] = {40, 46, 57};
 constexpr int W_HEAD[3] = {26, 33, 44};
 
@@ -1350,12 +1368,14 @@ int plan_split(Split* sp, int64_t n, int tile, int w_all, int w_head, int tri, i
     sp->w_all = w_all;
     sp->w_head = w_head;
     sp->tri = tri;
+    sp->w_tile = tri ? 16 * w_all : 0;
     sp->slot_tab = nullptr;
     sp->fixed_slots = 0;
+    sp->align = (!tri && w_all == 0) ? 32 : 1;
     sp->w_begin = 0;
     sp->w_end = 0x7fffffff;
     const int64_t total = split_prefix(*sp, sp->n_tiles);
-    const int64_t min_chunk = (int64_t)(tri ? 1 : w_all + w_head) * 32;   // >= ~32 streamed events per CTA
+    const int64_t min_chunk = (int64_t)(tri ? w_all : w_all + w_head) * 32;   // >= ~32 streamed events per CTA
     int64_t chunk = (total + ctas - 1) / ctas;
     if (chunk < min_chunk) chunk = min_chunk;
     for (;;) {
@@ -1434,9 +1454,9 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
                              sms * ctx->occ1[level1], q.ld, 12, ctx->part1_doubles);
         ctx->plan_bg = no_bg;
         ctx->plan_sym = sym;
-        q.grid2 = plan_split(&q.sp2, n, NT * P2_R, 1, 0, 1, sms * ctx->occ2[level2], q.ld, 2,
+        q.grid2 = plan_split(&q.sp2, n, NT * P2_R, W2_PLAIN, W2_OWN, 1, sms * ctx->occ2[level2], q.ld, 2,
                              ctx->part2_doubles);
-        q.gridx = plan_split(&q.spx, n, NT * PX_R, 1, 0, 1, sms * ctx->occx, q.ld, XM, ctx->partx_doubles);
+        q.gridx = plan_split(&q.spx, n, NT * PX_R, W2_PLAIN, W2_OWN, 1, sms * ctx->occx, q.ld, XM, ctx->partx_doubles);
         ctx->plan_n = n; ctx->plan_l1 = level1; ctx->plan_l2 = level2;
     }
     const Plan& pl = ctx->plan;
@@ -2292,7 +2312,7 @@ int64_t hawkes_plan_segments(int64_t n, int pass, int level, int symmetric, int 
     Split sp;
     const int64_t ld = round_up(n, 256);
     if (pass == 1) plan_split(&sp, n, NT * P1_R, symmetric ? 0 : W_ALL[level], W_HEAD[level], 0, workers_total, ld, 12, (size_t)-1);
-    else plan_split(&sp, n, NT * P2_R, 1, 0, 1, workers_total, ld, 2, (size_t)-1);
+    else plan_split(&sp, n, NT * P2_R, W2_PLAIN, W2_OWN, 1, workers_total, ld, 2, (size_t)-1);
     sp.w_begin = w_begin;
     sp.w_end = w_end;
     const int64_t total = split_prefix(sp, sp.n_tiles);

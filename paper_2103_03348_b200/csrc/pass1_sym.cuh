@@ -136,7 +136,11 @@ __device__ __forceinline__ void p1s_block(const double* __restrict__ sb, int j0,
             }
         }
 #pragma unroll
-        for (int k = 0; k < NB; ++k) cc[k] = __shfl_sync(0xffffffffu, cc[k], src);
+        for (int k = 0; k < NB; ++k)   // in place: the accumulator keeps its register pair across the rotation
+            asm volatile("{\n\t.reg .b32 lo, hi;\n\tmov.b64 {lo, hi}, %0;\n\t"
+                         "shfl.sync.idx.b32 lo, lo, %1, 0x1f, 0xffffffff;\n\t"
+                         "shfl.sync.idx.b32 hi, hi, %1, 0x1f, 0xffffffff;\n\tmov.b64 %0, {lo, hi};\n\t}"
+                         : "+d"(cc[k]) : "r"(src));
         idx = (idx + 1) & 31;
     }
     // lane l now holds the column sums of streamed event j0 + l

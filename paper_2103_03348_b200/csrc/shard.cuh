@@ -101,7 +101,7 @@ inline void shard_plan(const hawkes_ctx* ctx, int64_t n, const ShardLevels& L, i
     const int64_t ld = round_up(n, 256);
     plan_split(sp1, n, NT * P1_R, L.sym ? 0 : W_ALL[L.level1], W_HEAD[L.level1], 0, world * workers_per_rank1, ld, 12,
                ctx ? ctx->part1_doubles : (size_t)-1);
-    plan_split(sp2, n, NT * P2_R, 1, 0, 1, world * workers_per_rank2, ld, 2, ctx ? ctx->part2_doubles : (size_t)-1);
+    plan_split(sp2, n, NT * P2_R, W2_PLAIN, W2_OWN, 1, world * workers_per_rank2, ld, 2, ctx ? ctx->part2_doubles : (size_t)-1);
 }
 
 template <bool DIM3>
