@@ -167,12 +167,14 @@ int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
  * exact zeros is left out, so each output differs from hawkes_eval's by summation order alone (same tolerance).
  *
  * hawkes_skip_plan: x (dim x n, coordinate-major) and t (n) are HOST or DEVICE pointers; the events may be in any
- *   order (time-sorted input is not required by this variant).  Synchronous: copies the events to the host, builds
- *   the plan there (O(n log n) + one box test per tile pair) and uploads it; the context owns it until the next
- *   hawkes_skip_plan or hawkes_destroy.  The plan depends on the events, the hyperparameters and the background mode
+ *   order (time-sorted input is not required by this variant).  Synchronous, and it allocates.  The first plan of a set
+ *   of events copies them to the host once for the k-d order and the boxes (O(n log n)); the work lists (one box test
+ *   per tile pair, count / scan / fill) and their cut into workers are built by kernels.  The context owns the plan
+ *   until the next hawkes_skip_plan or hawkes_destroy.  The plan depends on the events, the hyperparameters and the background mode
  *   -- not on theta -- so one plan serves every evaluation of an HMC trajectory.  Planning the same events again for
  *   other hyperparameters (what an MCMC sweep does between HMC updates) keeps the order and the boxes as long as
- *   every cut-off radius stays within a factor 2 of the one the order was built for, and rebuilds only the lists.
+ *   every cut-off radius stays within a factor 2 of the one the order was built for, and rebuilds only the lists: the
+ *   events are recognised by a comparison on the device and are not brought to the host again.
  *   Errors: HAWKES_ERR_ARG, HAWKES_ERR_PARAM, HAWKES_ERR_NONFINITE (events), HAWKES_ERR_NOMEM, HAWKES_ERR_CUDA,
  *   HAWKES_ERR_UNSUPPORTED (work lists do not fit the context's partial buffers).
  * hawkes_eval_skip: arguments, outputs (in the caller's event order), stream semantics and device status as

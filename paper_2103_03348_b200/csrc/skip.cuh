@@ -382,6 +382,9 @@ struct SkipPlan {
     hawkes_params p;
     int s_mode;
     int64_t* d_perm;       // record i of the tree order is the caller's event perm[i]
+    int2* d_pool_items;    // one allocation for the four item lists (the d_items* pointers point into it)
+    int* d_pool_cut;       // ... and one for their cuts (d_w*start, d_w*first, d_slots*, ...)
+    double* d_ev;          // the planned events as the caller gave them (x, then t): a re-plan recognises them on the device
     double* d_tn;          // t_N = max t
     int2* d_items1;        // pass-1 work list and its cut
     int* d_w1start;
@@ -424,19 +427,6 @@ struct SkipPlan {
 
 namespace {
 
-void skip_plan_free(hawkes_ctx* c) {
-    SkipPlan* s = c->skip;
-    if (!s) return;
-    void* ptrs[] = {s->d_perm, s->d_tn, s->d_items1, s->d_w1start, s->d_w1first, s->d_slots1,
-                    s->d_items1s, s->d_w1sstart, s->d_w1sfirst, s->d_slots1s, s->d_itemsb, s->d_wbstart, s->d_wbfirst,
-                    s->d_w1sfirst_sym, s->d_slots_sym, s->d_partc, s->d_part_sym, s->d_items2, s->d_w2start, s->d_w2first, s->d_slots2};
-    for (void* q : ptrs)
-        if (q) cudaFree(q);
-    delete s->host;
-    delete s;
-    c->skip = nullptr;
-}
-
 // One SM is left free: hawkes_posterior_z_skip runs the single-CTA tree prior on the side stream beside the list
 // kernels, and a CTA of theirs that had to wait for that SM would hold up the whole pass.
 inline int skip_sms(const hawkes_ctx* ctx) { return ctx->sm_count > 1 ? ctx->sm_count - 1 : 1; }
@@ -452,6 +442,192 @@ struct SkipHost {
     double cutoff[4];
 };
 namespace {
+
+void skip_plan_free(hawkes_ctx* c) {
+    SkipPlan* s = c->skip;
+    if (!s) return;
+    void* ptrs[] = {s->d_ev, s->d_perm, s->d_tn, s->d_pool_items, s->d_pool_cut, s->d_partc, s->d_part_sym};
+    for (void* q : ptrs)
+        if (q) cudaFree(q);
+    delete s->host;
+    delete s;
+    c->skip = nullptr;
+}
+
+
+// The box tests, one definition for the host and the device.  (targets T, sources S)
+struct SkipGeom {
+    int dim, s_mode;
+    double tau_x, tau_t, h, omega;
+};
+__host__ __device__ inline double skip_gap2(const SkipBox& A, const SkipBox& B, int dim) {   // squared distance of the spatial boxes
+    double s = 0.0;
+    for (int a = 0; a < dim; ++a) {
+        const double g = fmax(0.0, fmax(A.lo[a] - B.hi[a], B.lo[a] - A.hi[a]));
+        s += g * g;
+    }
+    return s;
+}
+// background: smallest exponent r^2/2tau_x^2 + dt^2/2tau_t^2 any pair of the boxes can have
+__host__ __device__ inline bool skip_live_b(const SkipBox& T, const SkipBox& S, const SkipGeom& q) {
+    double z = skip_gap2(T, S, q.dim) / (2.0 * q.tau_x * q.tau_x);
+    if (!q.s_mode) {
+        const double g = fmax(0.0, fmax(T.lo[q.dim] - S.hi[q.dim], S.lo[q.dim] - T.hi[q.dim]));
+        z += g * g / (2.0 * q.tau_t * q.tau_t);
+    }
+    return !(z >= SKIP_Z0);
+}
+// excitation of targets T by sources S: some pair must be causal (t_n > t_m); smallest exponent r^2/2h^2 + omega dt
+__host__ __device__ inline bool skip_live_s(const SkipBox& T, const SkipBox& S, const SkipGeom& q) {
+    if (!(T.hi[q.dim] > S.lo[q.dim])) return false;
+    const double z = skip_gap2(T, S, q.dim) / (2.0 * q.h * q.h) + q.omega * fmax(0.0, T.lo[q.dim] - S.hi[q.dim]);
+    return !(z >= SKIP_Z0);
+}
+
+// The four work lists on the device: one thread per (tile I, tile Jt) pair tests the tile boxes, then the CPT chunks of
+// Jt against tile I.  Pass A counts (cnt[l][I*nt + Jt], l = 0: pass-1 items of either kind, 1: with a live excitation,
+// 2: unordered background items (Jt <= I), 3: pass-2 items of source tile I and target tile Jt); an exclusive scan of
+// each count array gives the offsets; pass B (FILL) writes the items there -- sorted by I, then J, as the host loops
+// of round 1 produced them.
+constexpr int SKIP_CPT = (NT * P1_R) / TS;   // chunks per tile
+template <bool FILL>
+__global__ void __launch_bounds__(256) skip_lists_kernel(int nt, int nc, const SkipBox* __restrict__ tile,
+                                                         const SkipBox* __restrict__ chunk, SkipGeom q,
+                                                         int* __restrict__ cnt, const int* __restrict__ off,
+                                                         int2* __restrict__ items1, int2* __restrict__ items1s,
+                                                         int2* __restrict__ itemsb, int2* __restrict__ items2) {
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t np = (int64_t)nt * nt;
+    if (idx >= np) return;
+    const int I = (int)(idx / nt), Jt = (int)(idx % nt);
+    const SkipBox TI = tile[I], TJ = tile[Jt];
+    const bool tb = skip_live_b(TI, TJ, q), ts = skip_live_s(TI, TJ, q), t2 = skip_live_s(TJ, TI, q);
+    int c1 = 0, c1s = 0, cb = 0, c2 = 0;
+    int o1 = 0, o1s = 0, ob = 0, o2 = 0;
+    if (FILL) { o1 = off[idx]; o1s = off[np + idx]; ob = off[2 * np + idx]; o2 = off[3 * np + idx]; }
+    if (tb || ts || t2) {
+        for (int J = Jt * SKIP_CPT; J < min(nc, (Jt + 1) * SKIP_CPT); ++J) {
+            const SkipBox C = chunk[J];
+            const bool lb = tb && skip_live_b(TI, C, q), ls = ts && skip_live_s(TI, C, q);
+            const int kind = (lb ? SK_B : 0) | (ls ? SK_S : 0);
+            if (kind) {
+                if (FILL) items1[o1 + c1] = make_int2(I, J * 4 + kind);
+                ++c1;
+            }
+            if (ls) {
+                if (FILL) items1s[o1s + c1s] = make_int2(I, J * 4 + SK_S);
+                ++c1s;
+            }
+            if (lb && Jt <= I) {
+                if (FILL) itemsb[ob + cb] = make_int2(I, J);
+                ++cb;
+            }
+            if (t2 && skip_live_s(C, TI, q)) {      // pass 2: sources = tile I, targets = chunk J
+                if (FILL) items2[o2 + c2] = make_int2(I, J * 4 + SK_S);
+                ++c2;
+            }
+        }
+    }
+    if (!FILL) { cnt[idx] = c1; cnt[np + idx] = c1s; cnt[2 * np + idx] = cb; cnt[3 * np + idx] = c2; }
+}
+
+// Device-side cut of a work list (sorted by tile) into `workers` consecutive ranges of about equal cost, in units of
+// 32-record blocks (4 per item; cost[k] = cost of one block of item k, NULL: 1; C = exclusive prefix sum of cost, NULL: k).
+// wstart[w], w = 0..workers: first block of worker w (workers at the end of a short list may be empty); tile_start[I],
+// I = 0..n_tiles: first item of tile I.  The same cut whatever the launch: it depends on the list alone.
+__device__ __forceinline__ long long skip_before(const long long* C, int k) { return C ? 4 * C[k] : 4ll * k; }
+__global__ void skip_cut_kernel(const int2* __restrict__ items, int K, const int* __restrict__ cost,
+                                const long long* __restrict__ C, int workers, int n_tiles, int* __restrict__ wstart,
+                                int* __restrict__ tile_start) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = K > 0 ? skip_before(C, K - 1) + 4ll * (cost ? cost[K - 1] : 1) : 0;
+    const long long chunk = (total + workers - 1) / workers > 0 ? (total + workers - 1) / workers : 1;
+    if (i <= workers) {
+        int v;
+        const long long T = (long long)i * chunk;          // worker i starts once the cost before it reaches T
+        if (i == 0 || K == 0) v = 0;
+        else if (T >= total) v = 4 * K;
+        else {
+            int lo = 0, hi = K - 1;                          // largest k with skip_before(k) < T
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (skip_before(C, mid) < T) lo = mid; else hi = mid - 1;
+            }
+            const long long ck = cost ? cost[lo] : 1;
+            long long b = (T - skip_before(C, lo) + ck - 1) / ck - 1;   // block of item lo at whose end T is reached
+            if (b < 0) b = 0;
+            if (b > 3) b = 3;
+            v = 4 * lo + (int)b + 1;
+            if (v > 4 * K) v = 4 * K;
+        }
+        if (i == workers) v = 4 * K;
+        wstart[i] = v;
+    }
+    if (i <= n_tiles) {
+        int lo = 0, hi = K;                                  // first item with tile >= i
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (items[mid].x < i) lo = mid + 1; else hi = mid;
+        }
+        tile_start[i] = lo;
+    }
+}
+// Workers that came out empty (two thresholds inside one block of a short list) move to the end: every tile's workers
+// are then consecutive and non-empty, as the partial-slot numbering (worker - first worker of the tile) assumes.
+__global__ void skip_compact_kernel(int workers, int nblocks, int* __restrict__ wstart) {
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    int used = 0;                                            // wstart[0..used] strictly increasing so far
+    for (int w = 1; w <= workers; ++w)
+        if (wstart[w] > wstart[used]) wstart[++used] = wstart[w];
+    for (int w = used + 1; w <= workers; ++w) wstart[w] = nblocks;
+}
+// per tile: the first worker that holds one of its blocks and the number of workers that do (= partial slots)
+__global__ void skip_slots_kernel(int n_tiles, int workers, const int* __restrict__ wstart, const int* __restrict__ tile_start,
+                                  int* __restrict__ wfirst, int* __restrict__ slots, int* __restrict__ worst) {
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    if (I >= n_tiles) return;
+    const int k0 = tile_start[I], k1 = tile_start[I + 1];
+    int first = 0, count = 0;
+    if (k1 > k0) {
+        auto worker_of = [&](int q) {                        // the worker w with wstart[w] <= q < wstart[w + 1]
+            int lo = 0, hi = workers - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (wstart[mid] <= q) lo = mid; else hi = mid - 1;
+            }
+            return lo;
+        };
+        first = worker_of(4 * k0);
+        count = worker_of(4 * k1 - 1) - first + 1;
+    }
+    wfirst[I] = first;
+    slots[I] = count;
+    atomicMax(worst, count);
+}
+__global__ void skip_cost1_kernel(int K, const int2* __restrict__ items, int wb, int ws, int* __restrict__ cost,
+                                  unsigned long long* __restrict__ n_b) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= K) return;
+    const int kind = items[k].y & 3;
+    cost[k] = ((kind & SK_B) ? wb : 0) + ((kind & SK_S) ? ws : 0);
+    if (kind & SK_B) atomicAdd(n_b, 1ull);
+}
+// symmetric form: the S items' slots follow the unordered background items' in every tile
+__global__ void skip_sym_kernel(int n_tiles, const int* __restrict__ wf_s, const int* __restrict__ sl_s,
+                                const int* __restrict__ sl_b, int* __restrict__ wfs_sym, int* __restrict__ sl_sym,
+                                int* __restrict__ worst) {
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    if (I >= n_tiles) return;
+    wfs_sym[I] = wf_s[I] - sl_b[I];
+    sl_sym[I] = sl_b[I] + sl_s[I];
+    atomicMax(worst, sl_b[I] + sl_s[I]);
+}
+
+// 1 into *flag if the caller's events differ from the planned ones (bitwise)
+__global__ void skip_same_events_kernel(int64_t m, const double* __restrict__ a, const double* __restrict__ b, int* flag) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m && __double_as_longlong(a[i]) != __double_as_longlong(b[i])) *flag = 1;
+}
 
 // Cut a list (sorted by tile) into at most `workers` non-empty consecutive ranges of about equal cost.  The unit
 // of the cut is a block of 32 streamed records, 4 per item (cost[k] is the cost of one block of item k): wstart
@@ -499,14 +675,15 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     if (!hs) return HAWKES_ERR_NOMEM;
     struct Guard { SkipHost*& h; ~Guard() { delete h; } } guard{hs};   // owned here until the plan takes it
     std::vector<double>&hx = hs->hx, &ht = hs->ht;
-    hx.resize((size_t)dim * n);
-    ht.resize((size_t)n);
-    CK(cudaMemcpy(hx.data(), x, sizeof(double) * dim * n, cudaMemcpyDefault));
-    CK(cudaMemcpy(ht.data(), t, sizeof(double) * n, cudaMemcpyDefault));
-    for (int64_t i = 0; i < n; ++i)
-        if (!std::isfinite(ht[i])) return HAWKES_ERR_NONFINITE;
-    for (size_t i = 0; i < hx.size(); ++i)
-        if (!std::isfinite(hx[i])) return HAWKES_ERR_NONFINITE;
+    // The caller's events (host or device pointers) are staged on the device: x, then t.  The new plan keeps this copy;
+    // a later plan of the same events -- what an MCMC sweep asks for after every hyperparameter move -- recognises
+    // them by a device-side comparison and never brings them to the host again.
+    const size_t ev_doubles = (size_t)nd * (size_t)n;
+    double* d_ev = nullptr;
+    if (cudaMalloc((void**)&d_ev, ev_doubles * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+    struct EvGuard { double*& p; ~EvGuard() { if (p) cudaFree(p); } } ev_guard{d_ev};   // owned here until the plan takes it
+    CK(cudaMemcpy(d_ev, x, sizeof(double) * dim * n, cudaMemcpyDefault));
+    CK(cudaMemcpy(d_ev + (size_t)dim * n, t, sizeof(double) * n, cudaMemcpyDefault));
     auto val = [&](int a, int64_t i) { return a < dim ? hx[(size_t)a * n + i] : ht[i]; };
 
     // cut-off radii: a term is an exact zero beyond them whatever the other coordinates are
@@ -518,12 +695,32 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     // Tiles and chunks are then the leaves of the tree: compact boxes that end where the runs end.
     double cutoff[4] = {0, 0, 0, 0};
     for (int a = 0; a < nd; ++a) cutoff[a] = a < dim ? std::min(rs, rb) : std::min(ts_, tb);
-    bool reuse = old && old->host && old->n == n && old->host->hx.size() == hx.size() &&
-                 std::memcmp(old->host->hx.data(), hx.data(), hx.size() * sizeof(double)) == 0 &&
-                 std::memcmp(old->host->ht.data(), ht.data(), ht.size() * sizeof(double)) == 0;
+    bool reuse = old && old->host && old->n == n && old->d_ev != nullptr && old->host->ht.size() == (size_t)n;
     for (int a = 0; a < nd && reuse; ++a) {
         const double r = cutoff[a] / old->host->cutoff[a];
         if (!(r >= 0.5 && r <= 2.0) && !(std::isinf(cutoff[a]) && std::isinf(old->host->cutoff[a]))) reuse = false;
+    }
+    if (reuse) {   // the same events, bit for bit?
+        int* d_flag = reinterpret_cast<int*>(ctx->d_status + 1);   // status[1] is rewritten by the next evaluation's prep
+        CK(cudaMemset(d_flag, 0, sizeof(int)));
+        skip_same_events_kernel<<<(unsigned)((ev_doubles + 255) / 256), 256>>>((int64_t)ev_doubles, d_ev, old->d_ev, d_flag);
+        int differ = 1;
+        CK(cudaMemcpy(&differ, d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+        CK(cudaMemset(d_flag, 0, sizeof(int)));
+        if (differ) reuse = false;
+    }
+    if (reuse) {
+        hx.swap(old->host->hx);
+        ht.swap(old->host->ht);
+    } else {
+        hx.resize((size_t)dim * n);
+        ht.resize((size_t)n);
+        CK(cudaMemcpy(hx.data(), d_ev, sizeof(double) * dim * n, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(ht.data(), d_ev + (size_t)dim * n, sizeof(double) * n, cudaMemcpyDeviceToHost));
+        for (int64_t i = 0; i < n; ++i)
+            if (!std::isfinite(ht[i])) return HAWKES_ERR_NONFINITE;
+        for (size_t i = 0; i < hx.size(); ++i)
+            if (!std::isfinite(hx[i])) return HAWKES_ERR_NONFINITE;
     }
     std::vector<int64_t>& perm = hs->perm;
     if (reuse) {
@@ -581,30 +778,7 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
         hs->chunk = boxes(TS);
         hs->tile = boxes(NT * P1_R);
     }
-    const std::vector<SkipBox>&chunk = hs->chunk, &tile1 = hs->tile, &tile2 = hs->tile;
-    auto gap2 = [&](const SkipBox& A, const SkipBox& B) {   // squared distance between the spatial boxes
-        double s = 0.0;
-        for (int a = 0; a < dim; ++a) {
-            const double g = std::max(0.0, std::max(A.lo[a] - B.hi[a], B.lo[a] - A.hi[a]));
-            s += g * g;
-        }
-        return s;
-    };
-    // background of (targets T, sources S): min exponent r^2/2tau_x^2 + dt^2/2tau_t^2
-    auto live_b = [&](const SkipBox& T, const SkipBox& S) {
-        double z = gap2(T, S) / (2.0 * p->tau_x * p->tau_x);
-        if (!ctx->s_mode) {
-            const double g = std::max(0.0, std::max(T.lo[dim] - S.hi[dim], S.lo[dim] - T.hi[dim]));
-            z += g * g / (2.0 * p->tau_t * p->tau_t);
-        }
-        return !(z >= SKIP_Z0);
-    };
-    // excitation of targets T by sources S: some pair must be causal (t_n > t_m), min exponent r^2/2h^2 + omega dt
-    auto live_s = [&](const SkipBox& T, const SkipBox& S) {
-        if (!(T.hi[dim] > S.lo[dim])) return false;
-        const double z = gap2(T, S) / (2.0 * p->h * p->h) + p->omega * std::max(0.0, T.lo[dim] - S.hi[dim]);
-        return !(z >= SKIP_Z0);
-    };
+    const std::vector<SkipBox>&chunk = hs->chunk, &tile1 = hs->tile;
 
     SkipPlan* sp = new (std::nothrow) SkipPlan();
     if (!sp) return HAWKES_ERR_NOMEM;
@@ -613,92 +787,129 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
     sp->host = hs;
     hs = nullptr;          // the plan owns it now (freed by skip_plan_free)
     sp->order_reused = reuse ? 1 : 0;
+    sp->d_ev = d_ev;
+    d_ev = nullptr;        // the plan owns the device copy of the events now
     sp->n = n;
     sp->p = *p;
     sp->s_mode = ctx->s_mode;
-    const int nc = (int)chunk.size(), nt1 = (int)tile1.size(), nt2 = (int)tile2.size();
-    std::vector<int2> items1, items1s, items2;
-    std::vector<int> cost1, cost1s, cost2;
-    // a chunk's box lies inside its tile's: a pair of tiles that is dead leaves nothing to test below it
-    constexpr int CPT = (NT * P1_R) / TS;   // chunks per tile
-    for (int I = 0; I < nt1; ++I)
-        for (int Jt = 0; Jt < nt1; ++Jt) {
-            const bool tb_live = live_b(tile1[I], tile1[Jt]), ts_live = live_s(tile1[I], tile1[Jt]);
-            if (!tb_live && !ts_live) continue;
-            for (int J = Jt * CPT; J < std::min(nc, (Jt + 1) * CPT); ++J) {
-            const int kind = ((tb_live && live_b(tile1[I], chunk[J])) ? SK_B : 0) |
-                             ((ts_live && live_s(tile1[I], chunk[J])) ? SK_S : 0);
-            if (!kind) continue;
-            items1.push_back(make_int2(I, J * 4 + kind));
-            cost1.push_back(((kind & SK_B) ? W_ALL[1] : 0) + ((kind & SK_S) ? W_HEAD[1] + 4 : 0));
-            sp->items_b += (kind & SK_B) ? 1 : 0;
-            sp->items_s += (kind & SK_S) ? 1 : 0;
-            if (kind & SK_S) {
-                items1s.push_back(make_int2(I, J * 4 + SK_S));
-                cost1s.push_back(1);
-            }
-            }
-        }
-    for (int M = 0; M < nt2; ++M)
-        for (int Jt = 0; Jt < nt2; ++Jt) {
-            if (!live_s(tile2[Jt], tile2[M])) continue;
-            for (int J = Jt * CPT; J < std::min(nc, (Jt + 1) * CPT); ++J)
-                if (live_s(chunk[J], tile2[M])) {
-                    items2.push_back(make_int2(M, J * 4 + SK_S));
-                    cost2.push_back(1);
-                }
-        }
-    sp->items_p2 = (int64_t)items2.size();
-    sp->items_dense1 = (int64_t)nt1 * nc;
-    sp->items_dense2 = (int64_t)nt2 * nc;
-
-    // cut into workers; halve the worker count while the fullest tile's slots do not fit the partial buffers
+    const int nc = (int)chunk.size(), nt1 = (int)tile1.size(), nt2 = nt1;
+    // ---- the four work lists and their cuts, all on the device (round 2; the host loops of round 1 took 39 ms per
+    // re-plan at N = 250,000) ------------------------------------------------------------------------------------
     const int64_t ld = round_up(n, 256);
-    std::vector<int> ws, wf, sl;
-    auto cut = [&](const std::vector<int2>& items, const std::vector<int>& cost, int n_tiles, int workers, int n_mom,
-                   size_t cap, int* used) {
+    const SkipGeom geom{dim, ctx->s_mode, p->tau_x, p->tau_t, p->h, p->omega};
+    const int64_t np = (int64_t)nt1 * nt1;
+    if (4 * np >= ((int64_t)1 << 31)) return HAWKES_ERR_UNSUPPORTED;
+    struct DevTmp {
+        void* p[8] = {};
+        ~DevTmp() { for (void* q : p) if (q) cudaFree(q); }
+    } tmp;
+    auto dalloc = [&](int slot, void** dst, size_t bytes) {
+        if (cudaMalloc(dst, bytes ? bytes : 8) != cudaSuccess) { cudaGetLastError(); *dst = nullptr; return false; }
+        if (slot >= 0) tmp.p[slot] = *dst;
+        return true;
+    };
+    SkipBox *d_tile = nullptr, *d_chunk = nullptr;
+    int *d_cnt = nullptr, *d_off = nullptr;
+    void* d_scan = nullptr;
+    size_t scan_bytes = 0, scan_bytes64 = 0;
+    cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, (const int*)nullptr, (int*)nullptr, (int)np);
+    if (!dalloc(0, (void**)&d_tile, sizeof(SkipBox) * nt1) || !dalloc(1, (void**)&d_chunk, sizeof(SkipBox) * nc) ||
+        !dalloc(2, (void**)&d_cnt, sizeof(int) * 4 * np) || !dalloc(3, (void**)&d_off, sizeof(int) * 4 * np) ||
+        !dalloc(4, &d_scan, scan_bytes)) return HAWKES_ERR_NOMEM;
+    CK(cudaMemcpy(d_tile, tile1.data(), sizeof(SkipBox) * nt1, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(d_chunk, chunk.data(), sizeof(SkipBox) * nc, cudaMemcpyHostToDevice));
+    const unsigned gl = (unsigned)((np + 255) / 256);
+    skip_lists_kernel<false><<<gl, 256>>>(nt1, nc, d_tile, d_chunk, geom, d_cnt, nullptr, nullptr, nullptr, nullptr, nullptr);
+    for (int l = 0; l < 4; ++l)
+        CK(cub::DeviceScan::ExclusiveSum(d_scan, scan_bytes, d_cnt + l * np, d_off + l * np, (int)np));
+    int total[4];
+    {
+        int tails[8];   // last count and last offset of each list
+        for (int l = 0; l < 4; ++l) {
+            CK(cudaMemcpyAsync(&tails[2 * l], d_cnt + (l + 1) * np - 1, sizeof(int), cudaMemcpyDeviceToHost, 0));
+            CK(cudaMemcpyAsync(&tails[2 * l + 1], d_off + (l + 1) * np - 1, sizeof(int), cudaMemcpyDeviceToHost, 0));
+        }
+        CK(cudaStreamSynchronize(0));
+        for (int l = 0; l < 4; ++l) total[l] = tails[2 * l] + tails[2 * l + 1];
+    }
+    // plan-owned pools: the items of the four lists; the cuts (ints)
+    const int W1 = skip_sms(ctx) * P1_G[0], W2 = skip_sms(ctx) * P2_G[0], Wmax = std::max(W1, W2);
+    int2* d_it[4];
+    {
+        size_t all = 0;
+        for (int l = 0; l < 4; ++l) all += (size_t)total[l] + 1;
+        if (!dalloc(-1, (void**)&sp->d_pool_items, sizeof(int2) * all)) return HAWKES_ERR_NOMEM;
+        int2* base = sp->d_pool_items;
+        for (int l = 0; l < 4; ++l) { d_it[l] = base; base += (size_t)total[l] + 1; }
+    }
+    const size_t per_list = (size_t)(Wmax + 1) + 3 * (size_t)nt1 + 1;     // wstart, tile_start, wfirst, slots
+    const size_t pool_ints = 4 * per_list + 2 * (size_t)nt1 + 16;
+    if (!dalloc(-1, (void**)&sp->d_pool_cut, sizeof(int) * pool_ints)) return HAWKES_ERR_NOMEM;
+    int* cw[4]; int* ct[4]; int* cf[4]; int* cs[4];
+    for (int l = 0; l < 4; ++l) {
+        int* b0 = sp->d_pool_cut + l * per_list;
+        cw[l] = b0; ct[l] = b0 + (Wmax + 1); cf[l] = ct[l] + nt1 + 1; cs[l] = cf[l] + nt1;
+    }
+    int* const d_wfs_sym = sp->d_pool_cut + 4 * per_list;
+    int* const d_sl_sym = d_wfs_sym + nt1;
+    int* const d_worst = d_sl_sym + nt1;                                  // + the count of B items (2 ints)
+    skip_lists_kernel<true><<<gl, 256>>>(nt1, nc, d_tile, d_chunk, geom, nullptr, d_off, d_it[0], d_it[1], d_it[2], d_it[3]);
+    CK(cudaGetLastError());
+    // block costs of the pass-1 list (46 per background block, 37 per masked excitation block: DESIGN.md section 5's
+    // issue model) and their prefix sums; the other lists have unit costs
+    int* d_cost1 = nullptr;
+    long long* d_C1 = nullptr;
+    cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes64, (const int*)nullptr, (long long*)nullptr, total[0] + 1);
+    void* d_scan64 = nullptr;
+    if (!dalloc(5, (void**)&d_cost1, sizeof(int) * ((size_t)total[0] + 1)) ||
+        !dalloc(6, (void**)&d_C1, sizeof(long long) * ((size_t)total[0] + 1)) || !dalloc(7, &d_scan64, scan_bytes64))
+        return HAWKES_ERR_NOMEM;
+    CK(cudaMemset(d_worst, 0, 4 * sizeof(int)));
+    if (total[0] > 0) {
+        skip_cost1_kernel<<<(unsigned)((total[0] + 255) / 256), 256>>>(total[0], d_it[0], W_ALL[1], W_HEAD[1] + 4, d_cost1,
+                                                                      reinterpret_cast<unsigned long long*>(d_worst + 2));
+        CK(cub::DeviceScan::ExclusiveSum(d_scan64, scan_bytes64, d_cost1, d_C1, total[0]));
+    }
+    // cut into workers; halve the worker count while the fullest tile's slots do not fit the partial buffers
+    auto dcut = [&](int l, const int* cost, const long long* C, int workers, int n_mom, size_t cap, int* used) -> int {
+        const int K = total[l], span = std::max(workers, nt1) + 1;
         for (;; workers = (workers + 1) / 2) {
-            *used = skip_cut(items, cost, n_tiles, workers, &ws, &wf, &sl);
+            if (cudaMemset(d_worst, 0, sizeof(int)) != cudaSuccess) return HAWKES_ERR_CUDA;
+            skip_cut_kernel<<<(unsigned)((span + 255) / 256), 256>>>(d_it[l], K, cost, C, workers, nt1, cw[l], ct[l]);
+            skip_compact_kernel<<<1, 1>>>(workers, 4 * K, cw[l]);
+            skip_slots_kernel<<<(unsigned)((nt1 + 255) / 256), 256>>>(nt1, workers, cw[l], ct[l], cf[l], cs[l], d_worst);
             int worst = 0;
-            for (int v : sl) worst = std::max(worst, v);
-            if ((size_t)worst * n_mom * (size_t)ld <= cap) return HAWKES_OK;
+            if (cudaMemcpy(&worst, d_worst, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return HAWKES_ERR_CUDA;
+            if ((size_t)worst * n_mom * (size_t)ld <= cap) { *used = workers; return HAWKES_OK; }
             if (workers == 1) return HAWKES_ERR_UNSUPPORTED;
         }
     };
     int rc;
-    if ((rc = cut(items1, cost1, nt1, skip_sms(ctx) * P1_G[0], 12, ctx->part1_doubles, &sp->workers1))) return rc;
-    if ((rc = skip_upload(&sp->d_items1, items1)) || (rc = skip_upload(&sp->d_w1start, ws)) ||
-        (rc = skip_upload(&sp->d_w1first, wf)) || (rc = skip_upload(&sp->d_slots1, sl))) return rc;
-    if ((rc = cut(items1s, cost1s, nt1, skip_sms(ctx) * P1_G[0], 12, ctx->part1_doubles, &sp->workers1s))) return rc;
-    if ((rc = skip_upload(&sp->d_items1s, items1s)) || (rc = skip_upload(&sp->d_w1sstart, ws)) ||
-        (rc = skip_upload(&sp->d_w1sfirst, wf)) || (rc = skip_upload(&sp->d_slots1s, sl))) return rc;
+    if ((rc = dcut(0, d_cost1, d_C1, W1, 12, ctx->part1_doubles, &sp->workers1))) return rc;
+    if ((rc = dcut(1, nullptr, nullptr, W1, 12, ctx->part1_doubles, &sp->workers1s))) return rc;
+    if ((rc = dcut(3, nullptr, nullptr, W2, 2, ctx->part2_doubles, &sp->workers2))) return rc;
+    sp->d_items1 = d_it[0]; sp->d_w1start = cw[0]; sp->d_w1first = cf[0]; sp->d_slots1 = cs[0];
+    sp->d_items1s = d_it[1]; sp->d_w1sstart = cw[1]; sp->d_w1sfirst = cf[1]; sp->d_slots1s = cs[1];
+    sp->d_items2 = d_it[3]; sp->d_w2start = cw[3]; sp->d_w2first = cf[3]; sp->d_slots2 = cs[3];
+    sp->items_s = total[1];
+    sp->items_p2 = total[3];
+    sp->items_dense1 = (int64_t)nt1 * nc;
+    sp->items_dense2 = (int64_t)nt2 * nc;
+    {
+        unsigned long long nb = 0;
+        CK(cudaMemcpy(&nb, d_worst + 2, sizeof(nb), cudaMemcpyDeviceToHost));
+        sp->items_b = (int64_t)nb;
+    }
     {   // symmetric background: off unless it fits (hawkes_set_pass1_mode(DENSE) switches it off as in the dense path)
-        const std::vector<int> wf_s = wf, sl_s = sl;          // cut of the S items, just made
-        std::vector<int2> itemsb;
-        for (int I = 0; I < nt1; ++I)
-            for (int Jt = 0; Jt <= I; ++Jt) {
-                if (!live_b(tile1[I], tile1[Jt])) continue;
-                for (int J = Jt * CPT; J < std::min(nc, (Jt + 1) * CPT); ++J)
-                    if (live_b(tile1[I], chunk[J])) itemsb.push_back(make_int2(I, J));
-            }
-        sp->items_bsym = (int64_t)itemsb.size();
-        const int64_t Q = 4 * (int64_t)itemsb.size();
-        const int W = (int)std::min<int64_t>(skip_sms(ctx) * P1_G[0], Q);
-        std::vector<int> wb(W + 1), wbf(nt1, 0), slb(nt1, 0), wbl(nt1, -1);
-        for (int w = 0; w <= W; ++w) wb[w] = (int)(Q * w / W);
-        for (int w = 0; w < W; ++w)
-            for (int k = wb[w] / 4; k <= (wb[w + 1] - 1) / 4 && wb[w] < wb[w + 1]; ++k) {
-                const int I = itemsb[k].x;
-                if (wbl[I] < 0) wbf[I] = w;
-                wbl[I] = w;
-            }
-        int worst = 0;
-        std::vector<int> wfs_sym(nt1), sl_sym(nt1);
-        for (int I = 0; I < nt1; ++I) {
-            slb[I] = wbl[I] < 0 ? 0 : wbl[I] - wbf[I] + 1;
-            wfs_sym[I] = wf_s[I] - slb[I];
-            sl_sym[I] = slb[I] + sl_s[I];
-            worst = std::max(worst, sl_sym[I]);
+        sp->items_bsym = total[2];
+        const int64_t Q = 4 * (int64_t)total[2];
+        int Wb = 0, worst = 0;
+        rc = Q > 0 ? dcut(2, nullptr, nullptr, W1, 0, (size_t)-1, &Wb) : HAWKES_OK;   // no capacity bound of its own ...
+        if (rc) return rc;
+        if (Q > 0) {                                                                  // ... the combined slots have
+            CK(cudaMemset(d_worst, 0, sizeof(int)));
+            skip_sym_kernel<<<(unsigned)((nt1 + 255) / 256), 256>>>(nt1, cf[1], cs[1], cs[2], d_wfs_sym, d_sl_sym, d_worst);
+            CK(cudaMemcpy(&worst, d_worst, sizeof(int), cudaMemcpyDeviceToHost));
         }
         const size_t pcd = (size_t)colpart_doubles(nt1, NT * P1_R, 3);
         const size_t prd = (size_t)worst * 12 * (size_t)ld;
@@ -718,25 +929,26 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
             if (!sp->partc_doubles) sp->partc_doubles = pcd;
             if (!sp->part_sym_doubles) sp->part_sym_doubles = prd;
             sp->partc_level = -1;
-            sp->workersb = W;
-            CK(cudaMemset(sp->d_partc, 0, sp->partc_doubles * sizeof(double)));
-            if ((rc = skip_upload(&sp->d_itemsb, itemsb)) || (rc = skip_upload(&sp->d_wbstart, wb)) ||
-                (rc = skip_upload(&sp->d_wbfirst, wbf)) || (rc = skip_upload(&sp->d_w1sfirst_sym, wfs_sym)) ||
-                (rc = skip_upload(&sp->d_slots_sym, sl_sym))) return rc;
+            sp->workersb = Wb;
+            CK(cudaMemsetAsync(sp->d_partc, 0, sp->partc_doubles * sizeof(double), 0));
+            sp->d_itemsb = d_it[2]; sp->d_wbstart = cw[2]; sp->d_wbfirst = cf[2];
+            sp->d_w1sfirst_sym = d_wfs_sym; sp->d_slots_sym = d_sl_sym;
         } else {
             cudaGetLastError();
             if (sp->d_partc) cudaFree(sp->d_partc);
             sp->d_partc = nullptr;
         }
     }
-    if ((rc = cut(items2, cost2, nt2, skip_sms(ctx) * P2_G[0], 2, ctx->part2_doubles, &sp->workers2))) return rc;
-    if ((rc = skip_upload(&sp->d_items2, items2)) || (rc = skip_upload(&sp->d_w2start, ws)) ||
-        (rc = skip_upload(&sp->d_w2first, wf)) || (rc = skip_upload(&sp->d_slots2, sl))) return rc;
-    if ((rc = skip_upload(&sp->d_perm, perm))) return rc;
-    double tn = -inf;
-    for (int64_t i = 0; i < n; ++i) tn = std::max(tn, ht[i]);
-    std::vector<double> tnv(1, tn);
-    if ((rc = skip_upload(&sp->d_tn, tnv))) return rc;
+    // the order on the device: taken over from the previous plan when it is the same
+    if (reuse && old->d_perm) { sp->d_perm = old->d_perm; old->d_perm = nullptr; sp->d_tn = old->d_tn; old->d_tn = nullptr; }
+    else {
+        if ((rc = skip_upload(&sp->d_perm, perm))) return rc;
+        double tn = -inf;
+        for (int64_t i = 0; i < n; ++i) tn = std::max(tn, ht[i]);
+        std::vector<double> tnv(1, tn);
+        if ((rc = skip_upload(&sp->d_tn, tnv))) return rc;
+    }
+    CK(cudaDeviceSynchronize());
     return HAWKES_OK;
 }
 
