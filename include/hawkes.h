@@ -390,7 +390,11 @@ typedef struct {
                                     and kept: the one entry point that may allocate), plus lambda0 = everything that does
                                     not involve a sequenced rate; an evaluation is then two passes over K (row sums ->
                                     lambda, column sums -> d ell/d theta): HBM-bound instead of FP64-bound.  Same sums in
-                                    another order.  dim <= 2 only (HAWKES_ERR_UNSUPPORTED otherwise).
+                                    another order.  dim <= 2 only (HAWKES_ERR_UNSUPPORTED otherwise).  Variants 2 and 5
+                                    cache every constant of the call, the prior included: log p(z) = log p(0) + 1/2 z^T G z
+                                    with G = -V_G^-1/sigma2 formed once per (tree, sigma2, tau0) by the O(M) algorithm at
+                                    the M unit vectors (M x M doubles kept by the tree; trees of more than ~3,100 tips
+                                    keep the O(M) walk), a dense matrix-vector product per evaluation.
                                  3, 4: variants 0 and 1 with every evaluation over the work lists of hawkes_skip_plan
                                     (exact zeros left out; the caller has planned these events and hyperparameters,
                                     HAWKES_ERR_ARG otherwise).  Same sums in another order.

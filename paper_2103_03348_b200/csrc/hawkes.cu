@@ -36,6 +36,9 @@
 
 // tree.cu: counts kernels of a tree that ran inside a replayed CUDA graph (not part of the C ABI)
 extern "C" void hk_tree_count_launches(hawkes_tree* t, int64_t k);
+// tree.cu: the prior as a cached dense quadratic form (cached-matrix variants of hawkes_hmc_run)
+extern "C" int hk_tree_dense_prepare(hawkes_tree* t, double sigma2, double tau0, void* stream);
+extern "C" int hk_tree_dense_prior(hawkes_tree* t, const double* z, double* logp, double* grad_z, void* stream);
 
 namespace {
 
@@ -2107,12 +2110,22 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
             nblk_c = 1;                                        // one partial per column (kmat_finish_kernel)
         }
     }
+    bool dense_prior = false;
+    if (kmat) {
+        rc = hk_tree_dense_prepare(tree, sigma2, tau0, stream);
+        if (rc && rc != HAWKES_ERR_UNSUPPORTED) return rc;
+        dense_prior = rc == HAWKES_OK;
+        CK(cudaSetDevice(ctx->device));
+    }
     auto eval_post = [&](const double* zin, double* out3, double* grad, double* hess, bool fill) -> int {
         if (!kmat) return posterior_z_impl(ctx, tree, n, x, t, m, idx, zin, beta, p, sigma2, tau0, out3, grad, hess, stream, use_skip, fill);
         // the O(M) tree prior (one latency-bound CTA) runs on a side stream beside the two passes over K
         if (cudaEventRecord(ctx->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0) != cudaSuccess)
             return HAWKES_ERR_CUDA;
-        int r2 = hawkes_tree_prior(tree, zin, sigma2, tau0, lp, grad ? pg : nullptr, (void*)ctx->side);
+        // these variants cache every constant of the call: the prior too, as its dense quadratic form (20 MB out of L2 at
+        // M = 1,610) instead of a walk of the tree's ~150 levels; trees that do not fit shared memory keep the walk
+        int r2 = dense_prior ? hk_tree_dense_prior(tree, zin, out3 ? lp : nullptr, grad ? pg : nullptr, (void*)ctx->side)
+                             : hawkes_tree_prior(tree, zin, sigma2, tau0, lp, grad ? pg : nullptr, (void*)ctx->side);
         if (r2) return r2;
         if (cudaSetDevice(ctx->device) != cudaSuccess || cudaEventRecord(ctx->ev_join, ctx->side) != cudaSuccess)
             return HAWKES_ERR_CUDA;

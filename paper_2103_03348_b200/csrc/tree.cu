@@ -90,7 +90,10 @@ __global__ void __launch_bounds__(TREE_T) tree_prior_kernel(int n_tips, int n_le
         for (int l = threadIdx.x; l <= n_levels; l += TREE_T) s_ls[l] = g_level_start[l];
         tq = s_tq; level_start = s_ls;
     }
-    for (int i = threadIdx.x; i < n_tips; i += TREE_T) nm[i] = z[i];
+    // z == NULL (SMEM only, one CTA per tip): z = the unit vector of tip blockIdx.x; the gradient goes to row blockIdx.x
+    // of grad_z -- the rows of -V_G^-1 / sigma^2, the Hessian of the quadratic log prior (tree_dense_* below)
+    for (int i = threadIdx.x; i < n_tips; i += TREE_T) nm[i] = z ? z[i] : (i == (int)blockIdx.x ? 1.0 : 0.0);
+    if (!z) grad_z += (size_t)blockIdx.x * n_tips;
     __syncthreads();
     const double inv_s2 = 1.0 / sigma2;
     double quad = 0.0;
@@ -190,6 +193,44 @@ __global__ void __launch_bounds__(TREE_T) tree_precision_kernel(int n_tips, int 
     for (int i = threadIdx.x; i < n_tips; i += TREE_T) prec_diag[i] = 1.0 / (sigma2 * vout[i]);
 }
 
+// The log prior is quadratic: log p(z) = log p(0) + 1/2 z^T G z with G = -V_G^-1 / sigma^2, grad = G z.  For the variants of
+// hawkes_hmc_run that cache every constant of a call (the kernel matrix), G is formed once (its rows are the gradients
+// at the unit vectors: M CTAs of tree_prior_kernel) and a prior evaluation becomes one dense symmetric matrix-vector
+// product out of L2 (20 MB at M = 1,610) instead of a latency-bound walk of the tree's ~150 levels.
+// One warp per row, lane-strided, fixed shuffle tree: bit-identical run to run.
+constexpr int DENSE_ROWS = 8;   // rows (warps) per CTA
+__global__ void __launch_bounds__(32 * DENSE_ROWS) tree_dense_gemv_kernel(int m, const double* __restrict__ G,
+                                                                          const double* __restrict__ z,
+                                                                          double* __restrict__ grad, double* __restrict__ zy) {
+    const int row = blockIdx.x * DENSE_ROWS + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (row >= m) return;
+    const double* g = G + (size_t)row * m;
+    double a = 0.0;
+    for (int k = lane; k < m; k += 32) a = fma(g[k], z[k], a);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
+    if (lane == 0) {
+        if (grad) grad[row] = a;
+        zy[row] = z[row] * a;
+    }
+}
+// log p = log p(0) + 1/2 sum_i z_i (G z)_i: one CTA, thread j takes i = j, j + 1024, ..., then a fixed tree
+__global__ void __launch_bounds__(1024) tree_dense_logp_kernel(int m, const double* __restrict__ zy, double logp0,
+                                                               double* __restrict__ logp) {
+    __shared__ double red[32];
+    double a = 0.0;
+    for (int i = threadIdx.x; i < m; i += 1024) a += zy[i];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) a += __shfl_down_sync(0xffffffffu, a, off);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double r = 0.0;
+        for (int w = 0; w < 32; ++w) r += red[w];
+        *logp = logp0 + 0.5 * r;
+    }
+}
+
 }  // namespace
 
 struct hawkes_tree {
@@ -202,6 +243,9 @@ struct hawkes_tree {
     bool smem;
     size_t smem_bytes;
     int64_t launches;
+    double* d_G;          // dense -V_G^-1 / sigma^2 (tree_dense_*), built on first use for (G_sigma2, G_tau0), or NULL
+    double* d_zy;         // M products z_i (G z)_i + 1
+    double G_sigma2, G_tau0, G_logp0;
 };
 
 extern "C" {
@@ -262,6 +306,7 @@ int hawkes_tree_create(hawkes_tree** out, int32_t n_tips, const int32_t* parent,
     hawkes_tree* t = new (std::nothrow) hawkes_tree();
     if (!t) return HAWKES_ERR_NOMEM;
     t->device = device; t->n_tips = M; t->n_levels = n_levels; t->root = root; t->launches = 0;
+    t->d_G = nullptr; t->d_zy = nullptr; t->G_sigma2 = t->G_tau0 = t->G_logp0 = 0.0;
     // first level from which every level holds at most 32 nodes (walked by a single warp)
     t->narrow_from = n_levels;
     while (t->narrow_from > 0 && level_start[t->narrow_from] - level_start[t->narrow_from - 1] <= 32) t->narrow_from--;
@@ -320,7 +365,7 @@ void hawkes_tree_destroy(hawkes_tree* t) {
     if (!t) return;
     cudaSetDevice(t->device);
     void* ptrs[] = {t->d_level_start, t->d_order, t->d_child_a, t->d_child_b, t->d_branch, t->d_scratch,
-                    t->d_tq};
+                    t->d_tq, t->d_G, t->d_zy};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     delete t;
@@ -359,6 +404,58 @@ int hawkes_tree_precision_diag(hawkes_tree* t, double sigma2, double tau0, doubl
 
 int32_t hawkes_tree_levels(const hawkes_tree* t) { return t ? t->n_levels : 0; }
 int64_t hawkes_tree_launch_count(const hawkes_tree* t) { return t ? t->launches : 0; }
+
+/* Internal (hawkes_hmc_run, cached-matrix variants; not part of the C ABI).  hk_tree_dense_prepare: forms G for
+ * (sigma2, tau0) unless the tree holds it already; may allocate M x M doubles and synchronises `stream` once (log p(0)).
+ * HAWKES_ERR_UNSUPPORTED if the tree does not fit shared memory (M > ~3,100): the caller then walks the tree.
+ * hk_tree_dense_prior: log p(z) into *logp (may be NULL) and G z into grad_z (may be NULL), enqueued on `stream`. */
+int hk_tree_dense_prepare(hawkes_tree* t, double sigma2, double tau0, void* stream) {
+    if (!t || !(sigma2 > 0.0) || !std::isfinite(sigma2) || !(tau0 >= 0.0) || !std::isfinite(tau0)) return HAWKES_ERR_PARAM;
+    if (!t->smem) return HAWKES_ERR_UNSUPPORTED;
+    if (t->d_G && t->G_sigma2 == sigma2 && t->G_tau0 == tau0) return HAWKES_OK;
+    CKT(cudaSetDevice(t->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M = t->n_tips;
+    if (!t->d_G) {
+        if (cudaMalloc((void**)&t->d_G, sizeof(double) * (size_t)M * M) != cudaSuccess ||
+            cudaMalloc((void**)&t->d_zy, sizeof(double) * ((size_t)M + 1)) != cudaSuccess) {
+            cudaGetLastError();
+            if (t->d_G) cudaFree(t->d_G);
+            t->d_G = nullptr;
+            return HAWKES_ERR_NOMEM;
+        }
+    }
+    tree_prior_kernel<true><<<M, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_tq,
+                                                             t->logs_tree, t->v_root, t->root, nullptr, sigma2, tau0,
+                                                             t->d_scratch, nullptr, t->d_G);
+    // log p(0): the kernel at z = 0 (d_zy serves as the zero vector, then receives the scalar)
+    CKT(cudaMemsetAsync(t->d_zy, 0, sizeof(double) * ((size_t)M + 1), st));
+    tree_prior_kernel<true><<<1, TREE_T, t->smem_bytes, st>>>(t->n_tips, t->n_levels, t->narrow_from, t->d_level_start, t->d_tq,
+                                                             t->logs_tree, t->v_root, t->root, t->d_zy, sigma2, tau0,
+                                                             t->d_scratch, t->d_zy + M, nullptr);
+    t->launches += 2;
+    CKT(cudaMemcpyAsync(&t->G_logp0, t->d_zy + M, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CKT(cudaStreamSynchronize(st));
+    CKT(cudaGetLastError());
+    t->G_sigma2 = sigma2;
+    t->G_tau0 = tau0;
+    return HAWKES_OK;
+}
+
+int hk_tree_dense_prior(hawkes_tree* t, const double* z, double* logp, double* grad_z, void* stream) {
+    if (!t || !t->d_G || !z) return HAWKES_ERR_ARG;
+    CKT(cudaSetDevice(t->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M = t->n_tips;
+    tree_dense_gemv_kernel<<<(unsigned)((M + DENSE_ROWS - 1) / DENSE_ROWS), 32 * DENSE_ROWS, 0, st>>>(M, t->d_G, z, grad_z, t->d_zy);
+    t->launches++;
+    if (logp) {
+        tree_dense_logp_kernel<<<1, 1024, 0, st>>>(M, t->d_zy, t->G_logp0, logp);
+        t->launches++;
+    }
+    CKT(cudaGetLastError());
+    return HAWKES_OK;
+}
 
 /* Counts kernels of this tree that ran inside a replayed CUDA graph (hawkes_hmc_run launches them k at a time). */
 void hk_tree_count_launches(hawkes_tree* t, int64_t k) { if (t) t->launches += k; }
