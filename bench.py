@@ -532,7 +532,30 @@ def run_b200(args, ev, workload: str) -> dict:
         t2skip = lambda: ctx.eval_skip(x, t, th, _synth.TABLE2_PARAMS, hp.WANT_GRAD, out=out)
         timed(t2skip, 2)
         t2sms = timed(t2skip, max(3, K // 4))
+        # SURVEY 8(e) on one GPU: the phases of every rank of a sharded evaluation timed one after the other (no exchange,
+        # no overlap): what each GPU of an N-GPU job would compute; the two all-gathers come on top
+        shard = {}
+        for wd in (2, 4, 8):
+            mk = lambda *sh: torch.empty(*sh, dtype=torch.float64, device=dev)
+            parts = mk(wd, ctx.shard_part_doubles(n, hp.WANT_GRAD, 1))
+            parts2 = mk(wd, ctx.shard_part_doubles(n, hp.WANT_GRAD, 2))
+            sout = ctx.new_outputs(n, hp.WANT_GRAD, dev)
+            per = {"pass1": [], "pass2": []}
+            for rep in range(2):                      # first repetition = warm-up
+                per = {"pass1": [], "pass2": []}
+                for r in range(wd):
+                    per["pass1"].append(_event_timed(torch, dev, lambda: ctx.shard_pass1(x, t, th, ev.params, hp.WANT_GRAD, r, wd, parts[r]), 1)[0])
+                red = _event_timed(torch, dev, lambda: ctx.shard_reduce1(n, ev.params, hp.WANT_GRAD, wd, parts, sout), 1)[0]
+                for r in range(wd):
+                    per["pass2"].append(_event_timed(torch, dev, lambda: ctx.shard_pass2(n, ev.params, hp.WANT_GRAD, r, wd, parts2[r]), 1)[0])
+                fin = _event_timed(torch, dev, lambda: ctx.shard_finish(n, ev.params, hp.WANT_GRAD, wd, parts2, sout), 1)[0]
+            slowest = max(per["pass1"]) + red + max(per["pass2"]) + fin
+            shard[str(wd)] = {"pass1_ms_per_rank": per["pass1"], "pass2_ms_per_rank": per["pass2"], "reduce1_ms": red,
+                              "finish_ms": fin, "slowest_rank_compute_ms": slowest,
+                              "all_gather_bytes_per_rank": [int(parts[0].numel() * 8), int(parts2[0].numel() * 8)],
+                              "ll_matches_one_gpu": abs(sout.ll.item() - out.ll.item()) <= 1e-12 * abs(out.ll.item())}
         timed(step, 1)   # leave `out` holding the configs[1] result
+        res["shard_emulation_one_gpu"] = shard
         res["extras"] = {"hessian_ms": statistics.median(hms), "ll_grad_theta_only_ms": statistics.median(lms),
                          "hessian_with_cross_block_ms": statistics.median(xms),
                          "cross_block_only_ms": statistics.median(cms),
@@ -556,7 +579,10 @@ def run_b200(args, ev, workload: str) -> dict:
                 + n * (32 + 32 + 8 + 34 * 8 / 64.0)                           #          two record streams, lambda, block sums
                 + (n + w2 * tile) * 8.0 + n * 16.0)                           # theta: pass-2 slots in, gradient out
     on_ms = (prof["prep_ms"] + prof["mid_ms"] + prof["tail_ms"]) / max(prof["evals"], 1)
-    res["o_n_kernels"] = {"ms_with_launch_gaps": on_ms, "bytes_per_eval_estimate": on_bytes,
+    cnt_ = max(prof["evals"], 1)
+    res["o_n_kernels"] = {"ms_with_launch_gaps": on_ms, "prep_ms": prof["prep_ms"] / cnt_,
+                          "reduce1_to_pass2_ms": prof["mid_ms"] / cnt_, "theta_ms": prof["tail_ms"] / cnt_,
+                          "bytes_per_eval_estimate": on_bytes,
                           "achieved_gb_s": on_bytes / (on_ms * 1e-3) / 1e9, "hbm_peak_gb_s": hbm_peak,
                           "frac": on_bytes / (on_ms * 1e-3) / 1e9 / hbm_peak,
                           "note": "launch-latency-bound by nature; the data they touch is L2-resident"}

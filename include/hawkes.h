@@ -265,6 +265,12 @@ int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stre
 int hawkes_row_moments_enable(hawkes_ctx* ctx, int enable);
 int hawkes_get_row_moments(hawkes_ctx* ctx, int64_t n, double* d1_out, double* d2_out, void* stream);
 
+/* Debug builds only (`python -m paper_2103_03348_b200.build --guard`, loaded when HAWKES_B200_GUARD=1 is set for the
+ * binding): every scratch buffer of the context lies between two 4 KB bands of a known byte pattern; this call
+ * synchronises the device and returns the number of band bytes that no longer hold it (0 = no out-of-bounds write so
+ * far).  HAWKES_ERR_UNSUPPORTED in the normal build (no bands).  The pool's stand-in for compute-sanitizer memcheck. */
+int64_t hawkes_debug_guard_check(hawkes_ctx* ctx);
+
 /* Launch bookkeeping for benchmarks: number of kernels this context has run since creation (kernels replayed from a
  * CUDA graph included), and the number of graph launches among the host's launch calls (hawkes_hmc_run). */
 int64_t hawkes_launch_count(const hawkes_ctx* ctx);

@@ -445,6 +445,13 @@ class HawkesContext:
     def last_status(self) -> int:
         return int(self._lib.hawkes_last_status(self._h, self._stream()))
 
+    def debug_guard_check(self) -> int:
+        """hawkes_debug_guard_check: corrupted guard-band bytes (guard build, HAWKES_B200_GUARD=1), else raises."""
+        rc = int(self._lib.hawkes_debug_guard_check(self._h))
+        if rc < 0:
+            raise HawkesError(rc, "hawkes_debug_guard_check")
+        return rc
+
     def launch_count(self) -> int:
         return int(self._lib.hawkes_launch_count(self._h))
 

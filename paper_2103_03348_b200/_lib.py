@@ -55,6 +55,7 @@ SYMBOLS = {
     "hawkes_shard_finish": (cint, [vp, i64, PP, u32, cint, _dp, _dp, _dp, vp]),
     "hawkes_shard_workers": (cint, [vp, u32, ctypes.POINTER(cint), ctypes.POINTER(cint)]),
     "hawkes_plan_segments": (i64, [i64, cint, cint, cint, cint, cint, cint, vp, i64]),
+    "hawkes_debug_guard_check": (i64, [vp]),
     "hawkes_launch_count": (i64, [vp]),
     "hawkes_graph_launch_count": (i64, [vp]),
     "hawkes_profile_enable": (cint, [vp, cint]),
@@ -86,10 +87,11 @@ def load():
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB
-    if not _build.up_to_date():
+    guard = os.environ.get("HAWKES_B200_GUARD") == "1"   # the debug build with guard bands (hawkes_debug_guard_check)
+    path = _build.LIB_GUARD if guard else _build.LIB
+    if not _build.up_to_date(guard):
         try:
-            _build.build()
+            _build.build(guard=guard)
         except Exception as exc:   # no nvcc on this machine, or compile error: never run a stale library silently
             what = "is older than its sources" if os.path.exists(path) else "is missing"
             raise ImportError(

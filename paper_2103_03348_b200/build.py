@@ -8,6 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhawkes_b200.so")
+LIB_GUARD = os.path.join(HERE, "libhawkes_b200_guard.so")   # debug build: -DHAWKES_GUARD (hawkes_debug_guard_check)
 SOURCES = [os.path.join(CSRC, "hawkes.cu"), os.path.join(CSRC, "tree.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("exp2_consts.inc", "pass1_sym.cuh", "hmc_kmat.cuh", "hmc_ksparse.cuh", "skip.cuh", "cross.cuh", "shard.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "hawkes.h")]
@@ -36,25 +37,29 @@ def source_hash() -> str:
     return h.hexdigest()
 
 
-def up_to_date() -> bool:
-    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
+def up_to_date(guard: bool = False) -> bool:
+    lib = LIB_GUARD if guard else LIB
+    if not (os.path.exists(lib) and os.path.exists(lib + ".srchash")):
         return False
-    with open(STAMP) as fh:
+    with open(lib + ".srchash") as fh:
         return fh.read().strip() == source_hash()
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and up_to_date():
-        return LIB
+def build(force: bool = False, verbose: bool = False, guard: bool = False) -> str:
+    if not force and up_to_date(guard):
+        return LIB_GUARD if guard else LIB
+    LIB = LIB_GUARD if guard else globals()["LIB"]
+    STAMP = LIB + ".srchash"
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc()] + NVCC_FLAGS + ["-o", tmp] + SOURCES
+    cmd = [nvcc()] + NVCC_FLAGS + (["-DHAWKES_GUARD"] if guard else []) + ["-o", tmp] + SOURCES
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    with open(os.path.join(HERE, "ptxas_info.log"), "w") as fh:
-        fh.write(res.stderr)
+    if not guard:
+        with open(os.path.join(HERE, "ptxas_info.log"), "w") as fh:
+            fh.write(res.stderr)
     os.replace(tmp, LIB)
     with open(STAMP, "w") as fh:
         fh.write(source_hash() + "\n")
@@ -62,4 +67,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, guard="--guard" in sys.argv))

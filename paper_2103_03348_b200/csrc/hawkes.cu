@@ -29,6 +29,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <vector>
 #include <cstdlib>
 #include <new>
 
@@ -1242,7 +1243,18 @@ struct Plan {
 
 // =================================================================================================
 // host side
+// -DHAWKES_GUARD (python -m paper_2103_03348_b200.build --guard): every scratch buffer of hawkes_create sits between two
+// 4 KB bands of a known pattern that hawkes_debug_guard_check verifies -- this pool's stand-in for compute-sanitizer's
+// memcheck (closed here): an out-of-bounds write of a partial slot, a record or a staging area lands in a band.
+#ifdef HAWKES_GUARD
+constexpr size_t GUARD_BYTES = 4096;
+#else
+constexpr size_t GUARD_BYTES = 0;
+#endif
+struct GuardRec { char* user; size_t bytes; };
+
 struct hawkes_ctx {
+    std::vector<GuardRec> guards;
     int device;
     int dim;
     int64_t n_max;
@@ -1663,7 +1675,18 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
         if (scan_bytes > c->cub_bytes) c->cub_bytes = scan_bytes;
     }
     bool ok = true;
-    auto alloc = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 8) != cudaSuccess) { ok = false; *p = nullptr; } };
+    auto alloc = [&](void** p, size_t bytes) {
+        if (!ok) return;
+        if (!bytes) bytes = 8;
+        char* base = nullptr;
+        if (cudaMalloc((void**)&base, bytes + 2 * GUARD_BYTES) != cudaSuccess) { ok = false; *p = nullptr; return; }
+        if (GUARD_BYTES) {
+            if (cudaMemset(base, 0xA5, GUARD_BYTES) != cudaSuccess ||
+                cudaMemset(base + GUARD_BYTES + bytes, 0xA5, GUARD_BYTES) != cudaSuccess) ok = false;
+            c->guards.push_back(GuardRec{base + GUARD_BYTES, bytes});
+        }
+        *p = base + GUARD_BYTES;
+    };
     void** ptrs[] = {(void**)&c->d_tab, (void**)&c->d_rec, (void**)&c->d_trec, (void**)&c->d_trec2, (void**)&c->d_part1, (void**)&c->d_part2,
                      (void**)&c->d_lam, (void**)&c->d_rowd1, (void**)&c->d_rowd2, (void**)&c->d_crec, (void**)&c->d_partx, (void**)&c->d_blockpart, (void**)&c->d_scal, (void**)&c->d_in,
                      (void**)&c->d_out, (void**)&c->d_post, (void**)&c->d_hmc, (void**)&c->d_kmat, (void**)&c->d_kmisc, (void**)&c->d_bgcache, (void**)&c->d_partc, (void**)&c->d_status, (void**)&c->d_cub, (void**)&c->d_sort_keys, (void**)&c->d_sort_idx};
@@ -1725,8 +1748,12 @@ void hawkes_destroy(hawkes_ctx* c) {
     skip_plan_free(c);
     void* ptrs[] = {c->d_tab, c->d_rec, c->d_trec, c->d_trec2, c->d_part1, c->d_part2, c->d_lam, c->d_rowd1, c->d_rowd2, c->d_crec, c->d_partx, c->d_blockpart,
                     c->d_scal, c->d_in, c->d_out, c->d_post, c->d_hmc, c->d_kmat, c->d_kmisc, c->d_bgcache, c->d_partc, c->d_status, c->d_cub, c->d_sort_keys, c->d_sort_idx};
-    for (void* p : ptrs)
-        if (p) cudaFree(p);
+    for (void* p : ptrs) {
+        if (!p) continue;
+        bool guarded = false;
+        for (const GuardRec& g : c->guards) guarded = guarded || g.user == (char*)p;
+        cudaFree(guarded ? (char*)p - GUARD_BYTES : (char*)p);
+    }
     if (c->d_ksp_a) cudaFree(c->d_ksp_a);
     if (c->d_ksp_b) cudaFree(c->d_ksp_b);
     if (c->side_ready) {
@@ -2405,6 +2432,22 @@ int hawkes_get_lambda(hawkes_ctx* ctx, int64_t n, double* lambda_out, void* stre
     if (!ctx || !lambda_out || n < 1 || n > ctx->n_max) return HAWKES_ERR_ARG;
     CK(cudaMemcpyAsync(lambda_out, ctx->d_lam, sizeof(double) * n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return HAWKES_OK;
+}
+
+int64_t hawkes_debug_guard_check(hawkes_ctx* ctx) {
+    if (!ctx) return HAWKES_ERR_ARG;
+    if (!GUARD_BYTES) return HAWKES_ERR_UNSUPPORTED;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaDeviceSynchronize());
+    std::vector<unsigned char> h(GUARD_BYTES ? GUARD_BYTES : 1);
+    int64_t bad = 0;
+    for (const GuardRec& g : ctx->guards)
+        for (int side = 0; side < 2; ++side) {
+            const char* src = side == 0 ? g.user - GUARD_BYTES : g.user + g.bytes;
+            CK(cudaMemcpy(h.data(), src, GUARD_BYTES, cudaMemcpyDeviceToHost));
+            for (size_t k = 0; k < GUARD_BYTES; ++k) bad += h[k] != 0xA5;
+        }
+    return bad;
 }
 
 int64_t hawkes_launch_count(const hawkes_ctx* ctx) { return ctx ? ctx->launches : 0; }

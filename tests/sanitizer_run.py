@@ -3,7 +3,8 @@
     compute-sanitizer --tool memcheck  --error-exitcode 9 python tests/sanitizer_run.py
     compute-sanitizer --tool racecheck --error-exitcode 9 python tests/sanitizer_run.py
 
-Not a pytest file (the sanitizers slow every kernel 10-100x, so this is run on demand and its tails are kept in
+With the guard-band build (`python -m paper_2103_03348_b200.build --guard`, then HAWKES_B200_GUARD=1) the run ends with
+hawkes_debug_guard_check on its contexts.  Not a pytest file (the sanitizers slow every kernel 10-100x, so this is run on demand and its tails are kept in
 profiles/r02_sanitizers.md).  It only calls the C ABI through the binding and checks that the results are finite;
 parity is the job of the test-suite proper.  Families touched: prep / pass1s (levels 0, 1, masked and plain blocks,
 ragged tile) / dense pass 1 (level 2 and PASS1_DENSE) / reduce1 / scalars / pass 2 (factorised and not, levels 0, 1) /
@@ -97,6 +98,10 @@ def main():
         finite(trace, z, mass)
     torch.cuda.synchronize()
     assert ctx.last_status() == 0
+    if os.environ.get("HAWKES_B200_GUARD") == "1":     # the guard-band build: no scratch buffer was overrun
+        bad = ctx.debug_guard_check() + c3.debug_guard_check()
+        assert bad == 0, f"{bad} guard-band bytes overwritten"
+        print("guard bands intact: 0 bytes overwritten around the scratch buffers of both contexts")
     print("sanitizer_run ok: n=%d, %d + %d launches" % (ev.n, ctx.launch_count() + c3.launch_count(), tr.launch_count()))
 
 
