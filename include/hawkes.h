@@ -224,7 +224,8 @@ int hawkes_pass1_is_symmetric(const hawkes_ctx* ctx, int level);
  *   hawkes_shard_finish  (world)        parts2_all -> grad_theta[n], hess_theta_diag[n] (Eq. 4, Eq. 5), replicated.
  *
  * `want`: bits LL .. HESS_HYPER of hawkes_eval (no cross block), the same in all four calls and on all ranks; x, t, theta,
- * p as for hawkes_eval; world <= 64.  All pointers DEVICE; the calls enqueue on `stream` and never synchronise; device
+ * p as for hawkes_eval; world <= 64.  All pointers DEVICE; the calls enqueue on `stream` and never synchronise (the two
+ * pass calls allocate their partial-slot buffers on first use and when a cut needs larger ones); device
  * status as hawkes_eval (hawkes_last_status after hawkes_shard_reduce1).  With world = 1 the four calls compute what
  * hawkes_eval computes (another summation order).  Results are bit-identical run to run for a given world.
  * hawkes_shard_workers: W of the two passes for this context and `want` (diagnostics).

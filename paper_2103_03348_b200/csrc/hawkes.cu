@@ -1275,6 +1275,9 @@ struct hawkes_ctx {
     double* d_lam;        // n_max
     double* d_rowd1;      // n_max * 6: d lambda_n / dp of the last evaluation at LEVEL >= 1
     double* d_rowd2;      // n_max * 21 or NULL: d2 lambda_n / dp dq (hawkes_row_moments_enable)
+    double* d_shpart1;    // partial slots of the sharded phases (shard.cuh): allocated on first use, grown on demand
+    double* d_shpart2;
+    size_t shpart1_doubles, shpart2_doubles;
     double* d_crec;       // n_max * (RS + 6): target records of the cross-block pass
     double* d_partx;      // its partial slots
     size_t partx_doubles;
@@ -1644,6 +1647,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->bg_mode = 0;
     c->s_mode = 0;
     c->force_dense = 0;
+    c->d_shpart1 = c->d_shpart2 = nullptr;
+    c->shpart1_doubles = c->shpart2_doubles = 0;
     c->kmat_doubles = c->kmisc_doubles = 0;
     c->d_ksp_a = c->d_ksp_b = nullptr;
     c->ksp_a_bytes = c->ksp_b_bytes = 0;
@@ -1754,6 +1759,8 @@ void hawkes_destroy(hawkes_ctx* c) {
         for (const GuardRec& g : c->guards) guarded = guarded || g.user == (char*)p;
         cudaFree(guarded ? (char*)p - GUARD_BYTES : (char*)p);
     }
+    if (c->d_shpart1) cudaFree(c->d_shpart1);
+    if (c->d_shpart2) cudaFree(c->d_shpart2);
     if (c->d_ksp_a) cudaFree(c->d_ksp_a);
     if (c->d_ksp_b) cudaFree(c->d_ksp_b);
     if (c->side_ready) {

@@ -100,8 +100,32 @@ inline void shard_plan(const hawkes_ctx* ctx, int64_t n, const ShardLevels& L, i
                        int workers_per_rank2, Split* sp1, Split* sp2) {
     const int64_t ld = round_up(n, 256);
     plan_split(sp1, n, NT * P1_R, L.sym ? 0 : W_ALL[L.level1], W_HEAD[L.level1], 0, world * workers_per_rank1, ld, 12,
-               ctx ? ctx->part1_doubles : (size_t)-1);
-    plan_split(sp2, n, NT * P2_R, W2_PLAIN, W2_OWN, 1, world * workers_per_rank2, ld, 2, ctx ? ctx->part2_doubles : (size_t)-1);
+               (size_t)-1);
+    plan_split(sp2, n, NT * P2_R, W2_PLAIN, W2_OWN, 1, world * workers_per_rank2, ld, 2, (size_t)-1);
+    (void)ctx;
+}
+
+// Partial slots of the sharded cut.  With world x W workers on the axis a tile may be shared by up to min(its workers, W)
+// workers of one rank -- world times what the one-GPU cut needs -- so the sharded phases keep partial buffers of their
+// own, sized for the cut at hand and grown on demand (the one allocation of these calls; kept by the context).
+inline int shard_slots_bound(const Split& sp, int workers_per_rank) {
+    int worst = 0;
+    for (int I = 0; I < sp.n_tiles; ++I) {
+        int first, count;
+        split_slots(sp, I, &first, &count);            // sp.w_begin / w_end still span the whole axis here
+        if (count > workers_per_rank) count = workers_per_rank;
+        if (count > worst) worst = count;
+    }
+    return worst;
+}
+inline int shard_ensure(double** buf, size_t* have, size_t need) {
+    if (need <= *have) return HAWKES_OK;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr;
+    *have = 0;
+    if (cudaMalloc((void**)buf, need * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return HAWKES_ERR_NOMEM; }
+    *have = need;
+    return HAWKES_OK;
 }
 
 template <bool DIM3>
@@ -110,9 +134,13 @@ int shard_pass1_impl(hawkes_ctx* ctx, int64_t n, const double* x, const double* 
     const int W1 = ctx->sm_count * ctx->occ1[L.level1], W2 = ctx->sm_count * ctx->occ2[L.level2];
     Split sp1, sp2;
     shard_plan(ctx, n, L, world, W1, W2, &sp1, &sp2);
+    const int64_t ld = round_up(n, 256);
+    {
+        const int rc = shard_ensure(&ctx->d_shpart1, &ctx->shpart1_doubles, (size_t)shard_slots_bound(sp1, W1) * 12 * (size_t)ld);
+        if (rc) return rc;
+    }
     sp1.w_begin = rank * W1;
     sp1.w_end = (rank + 1) * W1;
-    const int64_t ld = round_up(n, 256);
     const int nblk = (int)((n + RED_T - 1) / RED_T);
     CK(cudaMemsetAsync(ctx->d_status, 0, 2 * sizeof(unsigned), st));
     prep_kernel<<<nblk, RED_T, 0, st>>>(n, ctx->dim, x, t, theta, ctx->d_rec, ctx->d_status, c.omega);
@@ -122,11 +150,11 @@ int shard_pass1_impl(hawkes_ctx* ctx, int64_t n, const double* x, const double* 
     if (L.sym)                                                                                                              \
         pass1s_kernel<P1_R, (LV) <= 1 ? (LV) : 1, DIM3, P1_G[(LV) <= 1 ? (LV) : 1]>                                         \
             <<<g1, NT * P1_G[LV], smem_request(P1_G[LV] * sym_group_bytes<DIM3>((LV) == 0 ? 1 : 3)), st>>>(                 \
-                ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_part1, ctx->d_partc, sp1);                                         \
+                ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_shpart1, ctx->d_partc, sp1);                                         \
     else                                                                                                                    \
         pass1_kernel<P1_R, LV, DIM3, P1_G[LV]><<<g1, NT * P1_G[LV], smem_request(P1_G[LV] * group_buf_bytes<DIM3>()), st>>>( \
-            ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_part1, sp1);                                                           \
-    shard_sum1_kernel<LV><<<nblk, RED_T, 0, st>>>(n, ld, ctx->d_part1, sp1, L.sym ? ctx->d_partc : nullptr, NT * P1_R, part_out)
+            ctx->d_rec, n, ld, c, ctx->d_tab, ctx->d_shpart1, sp1);                                                           \
+    shard_sum1_kernel<LV><<<nblk, RED_T, 0, st>>>(n, ld, ctx->d_shpart1, sp1, L.sym ? ctx->d_partc : nullptr, NT * P1_R, part_out)
     if (lv == 0) { SHARD_P1(0); }
     else if (lv == 1) { SHARD_P1(1); }
     else { SHARD_P1(2); }
@@ -174,18 +202,22 @@ int shard_pass2_impl(hawkes_ctx* ctx, int64_t n, const DevConsts& c, const Shard
     const int W1 = ctx->sm_count * ctx->occ1[L.level1], W2 = ctx->sm_count * ctx->occ2[L.level2];
     Split sp1, sp2;
     shard_plan(ctx, n, L, world, W1, W2, &sp1, &sp2);
+    const int64_t ld = round_up(n, 256);
+    {
+        const int rc = shard_ensure(&ctx->d_shpart2, &ctx->shpart2_doubles, (size_t)shard_slots_bound(sp2, W2) * 2 * (size_t)ld);
+        if (rc) return rc;
+    }
     sp2.w_begin = rank * W2;
     sp2.w_end = (rank + 1) * W2;
-    const int64_t ld = round_up(n, 256);
     const int nblk = (int)((n + RED_T - 1) / RED_T);
     const unsigned g2 = (unsigned)ctx->sm_count;
     if (L.level2)
         pass2_kernel<P2_R, 1, DIM3, P2_G[1]><<<g2, NT * P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), st>>>(
-            ctx->d_rec, ctx->d_trec, ctx->d_trec2, ctx->d_status, n, ld, c, ctx->d_tab, ctx->d_part2, sp2);
+            ctx->d_rec, ctx->d_trec, ctx->d_trec2, ctx->d_status, n, ld, c, ctx->d_tab, ctx->d_shpart2, sp2);
     else
         pass2_kernel<P2_R, 0, DIM3, P2_G[0]><<<g2, NT * P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), st>>>(
-            ctx->d_rec, ctx->d_trec, ctx->d_trec2, ctx->d_status, n, ld, c, ctx->d_tab, ctx->d_part2, sp2);
-    shard_sum2_kernel<<<nblk, RED_T, 0, st>>>(n, ld, ctx->d_part2, sp2, L.level2, part2_out);
+            ctx->d_rec, ctx->d_trec, ctx->d_trec2, ctx->d_status, n, ld, c, ctx->d_tab, ctx->d_shpart2, sp2);
+    shard_sum2_kernel<<<nblk, RED_T, 0, st>>>(n, ld, ctx->d_shpart2, sp2, L.level2, part2_out);
     ctx->launches += 2;
     CK(cudaGetLastError());
     return HAWKES_OK;
