@@ -93,10 +93,17 @@ def load():
         try:
             _build.build(guard=guard)
         except Exception as exc:   # no nvcc on this machine, or compile error: never run a stale library silently
-            what = "is older than its sources" if os.path.exists(path) else "is missing"
-            raise ImportError(
-                f"paper_2103_03348_b200: CUDA library {path} {what} and could not be rebuilt "
-                f"({exc}); run `python -m paper_2103_03348_b200.build` on a machine with nvcc") from exc
+            stamp = path + ".srchash"
+            if os.path.exists(path) and not os.path.exists(stamp):
+                # a library without its source stamp (copied without it): staleness unknown -- say so, loudly, and use it
+                import warnings
+                warnings.warn(f"paper_2103_03348_b200: {path} has no source stamp and could not be rebuilt ({exc}); "
+                              f"loading it as it is -- it may not match csrc/", RuntimeWarning)
+            else:
+                what = "is older than its sources" if os.path.exists(path) else "is missing"
+                raise ImportError(
+                    f"paper_2103_03348_b200: CUDA library {path} {what} and could not be rebuilt "
+                    f"({exc}); run `python -m paper_2103_03348_b200.build` on a machine with nvcc") from exc
     lib = ctypes.CDLL(path)
     for name, (res, args) in SYMBOLS.items():
         fn = getattr(lib, name)   # AttributeError if the symbol is not exported
