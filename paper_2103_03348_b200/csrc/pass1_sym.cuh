@@ -71,7 +71,7 @@ __device__ __forceinline__ void p1s_block(const double* __restrict__ sb, int j0,
     for (int k = 0; k < NB; ++k) cc[k] = 0.0;
     int idx = lane;
     const int src = (lane + 1) & 31;
-#pragma unroll (LEVEL == 0 ? 4 : SYM_UNROLL)   // level 0: 0.686 -> 0.656 ms at N=23,422 with 4; level 1: 2 (4: 0.757 against 0.733)
+#pragma unroll ((LEVEL == 0 || !S_ON) ? 4 : SYM_UNROLL)   // level 0: 0.686 -> 0.656 ms at N=23,422 with 4; level 1: 2 (4: 0.757 against 0.733)
     for (int s = 0; s < 32; ++s) {
         const double* p = sb + j0 + idx;
         Ev<DIM3> e;
