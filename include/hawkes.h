@@ -66,6 +66,7 @@ enum {
     HAWKES_ERR_NOMEM = -5,       /* scratch allocation failed                                       */
     HAWKES_ERR_UNSUPPORTED = -6, /* dim not in {1,2,3}; dense Hessian with n > 4096                 */
     HAWKES_ERR_NONFINITE = -7,   /* device-detected: NaN/Inf in x, t or theta, or theta < 0         */
+    HAWKES_ERR_TOO_LARGE = -8,   /* hawkes_loglik_static: n exceeds HAWKES_STATIC_N_MAX             */
     HAWKES_WARN_ZERO_RATE = 1    /* device-detected: some lambda_n == 0 => ll = -inf, entries that
                                     divide by that lambda_n are NaN (always so for n == 1)          */
 };
@@ -131,6 +132,40 @@ int hawkes_eval_host(hawkes_ctx* ctx, int64_t n, const double* x /*HOST*/, const
 int hawkes_hessian_theta_dense(hawkes_ctx* ctx, int64_t n, const double* x, const double* t,
                                const double* theta, const hawkes_params* p /*HOST*/,
                                double* hess_theta, void* stream);
+
+/* ---- Log-likelihood without any device allocation -------------------------------------------------------------------
+ * Every other evaluation needs a hawkes_ctx, and hawkes_create obtains its scratch with cudaMalloc.  Some programs that
+ * want ell (Eq. 1, PAPER.md:76-78 -- e.g. the Metropolis-Hastings updates of the hyperparameters, which use likelihood
+ * evaluations only) cannot do that: a host application whose own pool has already claimed the whole
+ * device, so that a cudaMalloc from a library fails or is forbidden by its memory accounting; a sampler thread that
+ * must not stall the other streams of the process (cudaMalloc / cudaFree serialise the device); a plug-in loaded
+ * into a process that hands it input and output buffers and nothing else.  This one call serves them.  It needs no
+ * context and calls no cudaMalloc, cudaFree or other allocating routine: the intermediates of the evaluation (packed
+ * event records, pass-1 partial sums, lambda_n, block sums) live in a fixed array that is part of the library image --
+ * about 9 MB of device memory on every GPU on which the library is loaded, held until the process exits -- which is why
+ * the problem size is capped:
+ *
+ *     n <= HAWKES_STATIC_N_MAX (32,768 events; the paper's 23,422 cases fit);  larger n: HAWKES_ERR_TOO_LARGE, nothing
+ *     is enqueued or written.
+ *
+ * It is hawkes_loglik with the ordered-pair pass 1 (the kernels are the same ones; only where their scratch lives
+ * differs), for the default space-time background.  Arguments as for hawkes_loglik, all on the CURRENT device of the
+ * calling thread: x [dim*n], t [n], theta [n], ll [1] DEVICE; p HOST; dim in {1,2,3}.  status_out: DEVICE, one uint32,
+ * or NULL -- receives the data-dependent status of this evaluation as a bit set (HAWKES_STATIC_BIT_*; 0 = clean), the
+ * counterpart of hawkes_last_status for a caller without a context; it is written on `stream` like ll.
+ *
+ *  - The first call on each device sets that device up: it looks up the device address of the array, raises the
+ *    shared-memory limit of the pairwise kernel and copies the 2 KB exponential table into the array with a blocking
+ *    cudaMemcpy.  Make that first call outside any stream capture; later calls only enqueue work on `stream`.
+ *  - All calls in the process share the one array per device, and the array keeps whatever the previous call left in
+ *    it.  Each call clears the status words it accumulates into and overwrites everything else before reading it, so
+ *    calls that run one after the other on the GPU are independent of each other.  Two calls whose kernels can overlap
+ *    on the GPU (different streams without an ordering between them, or two host threads) race on the array and give
+ *    wrong results: order them.  The contexts of hawkes_create have their own scratch and are not affected. */
+#define HAWKES_STATIC_N_MAX 32768
+enum { HAWKES_STATIC_BIT_UNSORTED = 1, HAWKES_STATIC_BIT_NONFINITE = 2, HAWKES_STATIC_BIT_ZERO_RATE = 4 };
+int hawkes_loglik_static(int64_t n, int dim, const double* x, const double* t, const double* theta,
+                         const hawkes_params* p /*HOST*/, double* ll, uint32_t* status_out, void* stream);
 
 /* Helper, not on the hot path: stable argsort of the events by time and gather into SoA outputs
  * (x_out[dim*n], t_out[n], theta_out[n]); perm[i] = input index of output event i (int64).

@@ -12,6 +12,9 @@ from ._lib import HmcOpts, Params, load, lib_path  # noqa: F401
 
 OK = 0
 ERR_ARG, ERR_PARAM, ERR_UNSORTED, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = -1, -2, -3, -4, -5, -6, -7
+ERR_TOO_LARGE = -8
+STATIC_N_MAX = 32768   # HAWKES_STATIC_N_MAX: the largest problem loglik_static() takes
+STATIC_BIT_UNSORTED, STATIC_BIT_NONFINITE, STATIC_BIT_ZERO_RATE = 1, 2, 4
 WARN_ZERO_RATE = 1
 WANT_LL, WANT_GRAD_THETA, WANT_GRAD_HYPER, WANT_HESS_THETA, WANT_HESS_HYPER, WANT_HESS_CROSS = 1, 2, 4, 8, 16, 32
 WANT_GRAD = WANT_LL | WANT_GRAD_THETA | WANT_GRAD_HYPER
@@ -47,6 +50,36 @@ def _params(p) -> Params:
 
 def _ptr(t):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def loglik_static(x, t, theta, params, out, status_out=None):
+    """hawkes_loglik_static: the log-likelihood for callers that cannot allocate GPU memory -- no HawkesContext (whose
+    creation cudaMallocs its scratch) is involved, and neither this wrapper nor the C call behind it allocates: the
+    intermediates sit in a fixed array inside the library, which limits the problem to STATIC_N_MAX events
+    (HawkesError with ERR_TOO_LARGE beyond that).  Meant for code running inside a host application that owns all
+    device memory, or that must not trigger the device-wide stall of an allocation.
+
+    x [dim, n], t [n], theta [n]: float64 CUDA tensors on the current device; `out`: a float64 CUDA tensor of one
+    element that receives ell (the caller provides it, for the same reason); `status_out`: optional int32 CUDA tensor of
+    one element for the STATIC_BIT_* flags of this evaluation.  Asynchronous on the current stream.  The first call on
+    a device does a one-off set-up with a small blocking copy, so make it before any stream capture.  All calls share
+    the library's one array: do not let two of them run on the GPU at the same time (two streams, two threads)."""
+    import torch
+    for name, a, dt in (("x", x, torch.float64), ("t", t, torch.float64), ("theta", theta, torch.float64),
+                        ("out", out, torch.float64), ("status_out", status_out, torch.int32)):
+        if a is None and name == "status_out":
+            continue
+        if not a.is_cuda or a.device.index != torch.cuda.current_device() or a.dtype != dt or not a.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous {dt} CUDA tensor on the current device")
+    n = t.shape[0]
+    if x.dim() != 2 or x.shape[1] != n or theta.shape != (n,) or out.numel() != 1 or (status_out is not None and status_out.numel() != 1):
+        raise ValueError("expected x [dim, n] (SoA), t [n], theta [n], out [1], status_out [1]")
+    p = _params(params)
+    rc = load().hawkes_loglik_static(n, x.shape[0], _ptr(x), _ptr(t), _ptr(theta), ctypes.byref(p), _ptr(out), _ptr(status_out),
+                                     ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != 0:
+        raise HawkesError(rc, "hawkes_loglik_static")
+    return out
 
 
 class HawkesContext:

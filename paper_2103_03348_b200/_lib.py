@@ -31,6 +31,7 @@ SYMBOLS = {
     "hawkes_strerror": (ctypes.c_char_p, [cint]),
     "hawkes_last_status": (cint, [vp, vp]),
     "hawkes_loglik": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, vp]),
+    "hawkes_loglik_static": (cint, [i64, cint, _dp, _dp, _dp, PP, _dp, vp, vp]),
     "hawkes_grad": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, _dp, _dp, vp]),
     "hawkes_hessian": (cint, [vp, i64, _dp, _dp, _dp, PP, _dp, _dp, _dp, vp]),
     "hawkes_eval": (cint, [vp, i64, _dp, _dp, _dp, PP, u32, _dp, _dp, _dp, _dp, _dp, _dp, vp]),

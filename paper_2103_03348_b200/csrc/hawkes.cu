@@ -32,6 +32,7 @@
 #include <vector>
 #include <cstdlib>
 #include <new>
+#include <mutex>
 
 #include "exp2_consts.inc"
 
@@ -1617,6 +1618,7 @@ const char* hawkes_strerror(int status) {
         case HAWKES_ERR_NOMEM: return "out of device memory";
         case HAWKES_ERR_UNSUPPORTED: return "unsupported dimension or size";
         case HAWKES_ERR_NONFINITE: return "non-finite input or negative theta";
+        case HAWKES_ERR_TOO_LARGE: return "more events than the fixed scratch of hawkes_loglik_static holds (HAWKES_STATIC_N_MAX)";
         case HAWKES_WARN_ZERO_RATE: return "some lambda_n is zero (ll = -inf)";
         default: return "unknown status";
     }
@@ -2532,3 +2534,113 @@ int hawkes_fp64_peak(hawkes_ctx* ctx, double millis, double* tflops, void* strea
 }
 
 }  // extern "C"
+
+// =================================================================================================
+// hawkes_loglik_static: ell for callers that may not allocate device memory (include/hawkes.h gives the who and why).
+// The evaluation is the one hawkes_loglik runs in its ordered-pair form -- prep_kernel, pass1_kernel<LEVEL 0>,
+// reduce1_kernel<0>, scalars_kernel, unchanged -- but every intermediate those kernels pass to each other lives in the
+// file-scope array below instead of in a context's cudaMalloc'ed buffers.  The array is part of the module image: each
+// GPU on which this library is loaded holds STATIC_DOUBLES * 8 bytes (about 9 MB) for it until the process exits.
+namespace {
+constexpr int64_t STATIC_LD = HAWKES_STATIC_N_MAX;                 // records per buffer (a multiple of 256)
+static_assert(STATIC_LD % 256 == 0, "the record buffers are addressed with ld = n rounded up to 256");
+constexpr size_t STATIC_NBLK = STATIC_LD / RED_T;                  // CTAs of the O(N) kernels at the largest n
+// offsets in doubles; every buffer starts on a 256-byte boundary (multiples of 32 doubles)
+constexpr size_t SO_TAB = 0;                                       // TAB_N entries of the exponential table (read-only after set-up)
+constexpr size_t SO_STATUS = SO_TAB + TAB_N;                       // 2 status words, cleared by every call
+constexpr size_t SO_SCAL = SO_STATUS + 32;                         // sum log lambda, Lambda
+constexpr size_t SO_BLOCKPART = SO_SCAL + 32;                      // NRED sums per CTA of reduce1_kernel
+constexpr size_t SO_LAM = SO_BLOCKPART + (STATIC_NBLK * NRED + 31) / 32 * 32;
+constexpr size_t SO_REC = SO_LAM + STATIC_LD;                      // packed records (6 doubles each when dim = 3)
+constexpr size_t SO_TREC = SO_REC + 6 * STATIC_LD;                 // reduce1_kernel always writes the two pass-2 target
+constexpr size_t SO_TREC2 = SO_TREC + 6 * STATIC_LD;               // streams; nothing here reads them
+constexpr size_t SO_PART = SO_TREC2 + 6 * STATIC_LD;               // pass-1 partial slots
+constexpr size_t STATIC_PART_DOUBLES = (size_t)1 << 19;            // plan_split coarsens the cut if a plan needs more
+constexpr size_t STATIC_DOUBLES = SO_PART + STATIC_PART_DOUBLES;
+}  // namespace
+
+// Device code may name this array directly.  In host code the name is only a handle for the runtime's symbol calls, not
+// a device address (a kernel handed `hawkes_static_scratch` by the host would fault, or on a system where the GPU can
+// reach host memory quietly use the wrong bytes): static_setup() below asks the runtime for the address on each device.
+static __device__ __align__(256) double hawkes_static_scratch[STATIC_DOUBLES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDev {
+    double* base;    // device address of hawkes_static_scratch on this device
+    int sm_count;
+    bool ready;
+};
+StaticDev g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+
+// Once per device, with that device current: address of the array, launch attributes of the pairwise kernel, table.
+// Nothing here allocates device memory; the cudaMemcpy is a blocking 2 KB copy (hence: not under stream capture).
+int static_setup(int dev, const StaticDev** out) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDev& sd = g_static_dev[dev];
+    if (!sd.ready) {
+        double* base = nullptr;
+        if (cudaGetSymbolAddress((void**)&base, hawkes_static_scratch) != cudaSuccess || base == nullptr) {
+            cudaGetLastError();
+            return HAWKES_ERR_CUDA;
+        }
+        int sms = 0, groups = 0, rc;
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if ((rc = setup_kernel(pass1_kernel<P1_R, 0, false, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<false>()), &groups))) return rc;
+        if ((rc = setup_kernel(pass1_kernel<P1_R, 0, true, P1_G[0]>, P1_G[0], smem_request(P1_G[0] * group_buf_bytes<true>()), &groups))) return rc;
+        CK(cudaMemcpy(base + SO_TAB, hawkes_exp2_table_host, sizeof(double) * TAB_N, cudaMemcpyHostToDevice));
+        sd.base = base;
+        sd.sm_count = sms;
+        sd.ready = true;
+    }
+    *out = &sd;
+    return HAWKES_OK;
+}
+
+template <bool DIM3>
+int enqueue_loglik_static(const StaticDev& sd, int64_t n, int dim, const double* x, const double* t, const double* theta,
+                          const DevConsts& c, double* ll, uint32_t* status_out, cudaStream_t st) {
+    double* const base = sd.base;
+    unsigned* const status = reinterpret_cast<unsigned*>(base + SO_STATUS);
+    const int64_t ld = round_up(n, 256);
+    const int nblk = (int)((n + RED_T - 1) / RED_T);
+    // the same cut of the pair space as a context's dense pass 1 (stream-K over sm_count x P1_G[0] workers), bounded by
+    // the partial slots the array has room for
+    Split sp;
+    const int workers = plan_split(&sp, n, NT * P1_R, W_ALL[0], W_HEAD[0], 0, sd.sm_count * P1_G[0], ld, 2, STATIC_PART_DOUBLES);
+    // The array still holds the previous call's data.  The status words are OR-ed into, so they must start at zero;
+    // records, partial slots, lambda and block sums are each written in full (for this n) before the next kernel reads them.
+    CK(cudaMemsetAsync(status, 0, 2 * sizeof(unsigned), st));
+    prep_kernel<<<nblk, RED_T, 0, st>>>(n, dim, x, t, theta, base + SO_REC, status, c.omega);
+    const unsigned g1 = (unsigned)((workers + P1_G[0] - 1) / P1_G[0]);
+    pass1_kernel<P1_R, 0, DIM3, P1_G[0]><<<g1, NT * P1_G[0], smem_request(P1_G[0] * group_buf_bytes<DIM3>()), st>>>(
+        base + SO_REC, n, ld, c, base + SO_TAB, base + SO_PART, sp);
+    reduce1_kernel<0, DIM3><<<nblk, RED_T, 0, st>>>(base + SO_REC, n, ld, c, base + SO_PART, sp, base + SO_LAM, base + SO_TREC,
+                                                    base + SO_TREC2, nullptr, nullptr, nullptr, base + SO_BLOCKPART, status,
+                                                    nullptr, 0, nullptr, sp.n_tiles, NT * P1_R, nullptr);
+    scalars_kernel<<<1, SCAL_T, 0, st>>>(base + SO_BLOCKPART, nblk, c, ll, nullptr, nullptr, base + SO_SCAL);
+    if (status_out) CK(cudaMemcpyAsync(status_out, status, sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
+    CK(cudaGetLastError());
+    return HAWKES_OK;
+}
+}  // namespace
+
+extern "C" int hawkes_loglik_static(int64_t n, int dim, const double* x, const double* t, const double* theta,
+                                    const hawkes_params* p, double* ll, uint32_t* status_out, void* stream) {
+    static_assert(ST_UNSORTED == HAWKES_STATIC_BIT_UNSORTED && ST_NONFINITE == HAWKES_STATIC_BIT_NONFINITE &&
+                  ST_ZERO_RATE == HAWKES_STATIC_BIT_ZERO_RATE, "status_out carries the kernels' status bits as they are");
+    if (!x || !t || !theta || !p || !ll || n < 1) return HAWKES_ERR_ARG;
+    if (dim < 1 || dim > 3) return HAWKES_ERR_UNSUPPORTED;
+    if (n > HAWKES_STATIC_N_MAX) return HAWKES_ERR_TOO_LARGE;   // the array has room for this many events and no more
+    DevConsts c;
+    int rc = make_consts(p, dim, 0, &c);
+    if (rc) return rc;
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return HAWKES_ERR_UNSUPPORTED;
+    const StaticDev* sd = nullptr;
+    if ((rc = static_setup(dev, &sd))) return rc;
+    return dim == 3 ? enqueue_loglik_static<true>(*sd, n, dim, x, t, theta, c, ll, status_out, (cudaStream_t)stream)
+                    : enqueue_loglik_static<false>(*sd, n, dim, x, t, theta, c, ll, status_out, (cudaStream_t)stream);
+}
