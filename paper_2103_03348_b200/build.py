@@ -46,11 +46,10 @@ def up_to_date(guard: bool = False) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False, guard: bool = False) -> str:
+    lib = LIB_GUARD if guard else LIB
     if not force and up_to_date(guard):
-        return LIB_GUARD if guard else LIB
-    LIB = LIB_GUARD if guard else globals()["LIB"]
-    STAMP = LIB + ".srchash"
-    tmp = LIB + f".tmp{os.getpid()}"
+        return lib
+    tmp = lib + f".tmp{os.getpid()}"
     cmd = [nvcc()] + NVCC_FLAGS + (["-DHAWKES_GUARD"] if guard else []) + ["-o", tmp] + SOURCES
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
@@ -60,10 +59,10 @@ def build(force: bool = False, verbose: bool = False, guard: bool = False) -> st
     if not guard:
         with open(os.path.join(HERE, "ptxas_info.log"), "w") as fh:
             fh.write(res.stderr)
-    os.replace(tmp, LIB)
-    with open(STAMP, "w") as fh:
+    os.replace(tmp, lib)
+    with open(lib + ".srchash", "w") as fh:
         fh.write(source_hash() + "\n")
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

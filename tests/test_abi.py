@@ -67,3 +67,11 @@ def test_product_package_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".h", ".cuh", ".inc")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text and "hawkes_ref" not in text, f
+
+
+def test_build_returns_the_library_path_when_nothing_is_stale():
+    """build() with an up-to-date library takes its early return (it used to raise UnboundLocalError there)."""
+    from paper_2103_03348_b200 import build as b
+    hp.load()                       # builds if needed
+    assert b.up_to_date()
+    assert b.build() == b.LIB
