@@ -211,7 +211,10 @@ int hawkes_set_background_mode(hawkes_ctx* ctx, int mode);
  *   every cut-off radius stays within a factor 2 of the one the order was built for, and rebuilds only the lists: the
  *   events are recognised by a comparison on the device and are not brought to the host again.
  *   Errors: HAWKES_ERR_ARG, HAWKES_ERR_PARAM, HAWKES_ERR_NONFINITE (events), HAWKES_ERR_NOMEM, HAWKES_ERR_CUDA,
- *   HAWKES_ERR_UNSUPPORTED (work lists do not fit the context's partial buffers).
+ *   HAWKES_ERR_UNSUPPORTED (work lists do not fit the context's partial buffers, or a list has 2^29 items or more).
+ *   A call that fails leaves the context WITHOUT a plan: the previous plan, if there was one, has been released too
+ *   (its buffers are handed to the new plan while that is being built), so hawkes_eval_skip, hawkes_posterior_z_skip
+ *   and hawkes_hmc_run variants 3 / 4 return HAWKES_ERR_ARG until a later hawkes_skip_plan succeeds.
  * hawkes_eval_skip: arguments, outputs (in the caller's event order), stream semantics and device status as
  *   hawkes_eval, without the cross block (`want` bits 0..4).  HAWKES_ERR_ARG if there is no plan or it was built
  *   for another n, other hyperparameters or another background mode; the caller guarantees x and t are the planned
@@ -259,8 +262,10 @@ int hawkes_pass1_is_symmetric(const hawkes_ctx* ctx, int level);
  *   hawkes_shard_finish  (world)        parts2_all -> grad_theta[n], hess_theta_diag[n] (Eq. 4, Eq. 5), replicated.
  *
  * `want`: bits LL .. HESS_HYPER of hawkes_eval (no cross block), the same in all four calls and on all ranks; x, t, theta,
- * p as for hawkes_eval; world <= 64.  All pointers DEVICE; the calls enqueue on `stream` and never synchronise (the two
- * pass calls allocate their partial-slot buffers on first use and when a cut needs larger ones); device
+ * p as for hawkes_eval; world <= 64.  All pointers DEVICE; the calls enqueue on `stream`.  hawkes_shard_reduce1 and
+ * hawkes_shard_finish never synchronise or allocate.  The two pass calls do both on occasion: they cudaMalloc their partial-slot
+ * buffers on first use, and when a cut needs larger ones they cudaFree the old buffer first, which waits for all work on the
+ * device (the first evaluation of a given (n, want, world), in practice; later ones only enqueue).  Device
  * status as hawkes_eval (hawkes_last_status after hawkes_shard_reduce1).  With world = 1 the four calls compute what
  * hawkes_eval computes (another summation order).  Results are bit-identical run to run for a given world.
  * hawkes_shard_workers: W of the two passes for this context and `want` (diagnostics).

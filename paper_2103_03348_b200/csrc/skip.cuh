@@ -832,6 +832,9 @@ int skip_build(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, con
         CK(cudaStreamSynchronize(0));
         for (int l = 0; l < 4; ++l) total[l] = tails[2 * l] + tails[2 * l + 1];
     }
+    // the cut kernels index the quarter-blocks of a list as 4 * K in int (skip_cut_kernel, skip_compact_kernel, wstart)
+    for (int l = 0; l < 4; ++l)
+        if (total[l] < 0 || total[l] >= (1 << 29)) return HAWKES_ERR_UNSUPPORTED;
     // plan-owned pools: the items of the four lists; the cuts (ints)
     const int W1 = skip_sms(ctx) * P1_G[0], W2 = skip_sms(ctx) * P2_G[0], Wmax = std::max(W1, W2);
     int2* d_it[4];
