@@ -419,7 +419,8 @@ int hawkes_posterior_z_skip(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const
  * The random numbers are inputs.  The work runs on a stream of the context that is forked from `stream` when the call
  * starts and joined to it before the call returns (work queued on `stream` before / after the call is ordered before /
  * after it, as for every other entry point); the accept decision is taken on the device, the call never synchronises
- * (variant 5 excepted, see below).  It instantiates up to two CUDA graphs per call (which allocates driver memory).  n_leapfrog posterior evaluations per iteration (the gradient at the current state
+ * (variant 5 excepted, see below).  It instantiates up to two CUDA graphs per call (which allocates driver memory; none when every
+ * kind of iteration runs fewer than 3 times, e.g. n_iter = 1).  n_leapfrog posterior evaluations per iteration (the gradient at the current state
  * is carried over), plus one Hessian-level evaluation per refresh and one evaluation before the first iteration.
  */
 typedef struct {
@@ -453,7 +454,10 @@ typedef struct {
     int32_t flags;           /* 0, or HAWKES_HMC_NO_GRAPH: enqueue every kernel of every iteration directly.  By default an
                                 iteration (its [refresh,] momentum draw, n_leapfrog evaluations and accept test) is captured
                                 once into a CUDA graph -- one for iterations with a preconditioner refresh, one for those
-                                without -- and replayed: one host launch per iteration.  Same kernels, same results. */
+                                without -- and replayed: one host launch per iteration.  Same kernels, same results.  A kind of
+                                iteration that this call runs fewer than 3 times is enqueued directly (capture costs more than
+                                it saves), and so is everything while hawkes_profile_enable is on (the timing events must be
+                                recorded per evaluation, not frozen into a graph). */
 } hawkes_hmc_opts;
 enum { HAWKES_HMC_NO_GRAPH = 1 };
 

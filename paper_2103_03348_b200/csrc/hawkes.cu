@@ -2220,13 +2220,21 @@ int hawkes_hmc_run(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* 
     };
     // The two kinds of iteration (with / without a refresh) are captured once each into a CUDA graph and replayed: one
     // host launch per iteration instead of ~120-250 (HAWKES_HMC_NO_GRAPH in opts->flags: enqueue every kernel directly).
-    const bool use_graph = (o->flags & HAWKES_HMC_NO_GRAPH) == 0;
+    // Capturing and instantiating the ~120-250 nodes of an iteration costs more than enqueueing them once or twice, so a
+    // kind is captured only if this call runs it at least HMC_GRAPH_MIN_REPLAYS times (n_iter = 1 per MCMC sweep, the
+    // paper's HMC-within-Gibbs use, therefore enqueues directly).  While the timing ring is on, nothing is captured: its
+    // event records would be frozen into the graph and the ring's bookkeeping would count the capture only.
+    constexpr int HMC_GRAPH_MIN_REPLAYS = 3;
+    const bool use_graph = (o->flags & HAWKES_HMC_NO_GRAPH) == 0 && !ctx->prof_on;
+    int n_kind[2] = {0, 0};
+    n_kind[1] = o->precond_every > 0 ? (o->n_iter + o->precond_every - 1) / o->precond_every : 0;
+    n_kind[0] = o->n_iter - n_kind[1];
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     int64_t g_ctx[2] = {0, 0}, g_tree[2] = {0, 0};
     struct GraphFree { cudaGraphExec_t* g; ~GraphFree() { for (int k = 0; k < 2; ++k) if (g[k]) cudaGraphExecDestroy(g[k]); } } gfree{gexec};
     for (int it = 0; it < o->n_iter; ++it) {
         const int kind = (o->precond_every > 0 && it % o->precond_every == 0) ? 1 : 0;
-        if (!use_graph) {
+        if (!use_graph || n_kind[kind] < HMC_GRAPH_MIN_REPLAYS) {
             if ((rc = enqueue_iteration(kind == 1))) return rc;
             continue;
         }
