@@ -1,8 +1,8 @@
 """GPU parity of the sharded evaluation (hawkes_shard_*; include/hawkes.h): the four phases of every rank run one
-after the other on ONE GPU -- the ranks' kernels never wait on one another, so nothing is lost by the emulation but
-the overlap -- with the all-gathers replaced by a concatenation; results against the oracle, against the one-GPU
+after the other on ONE GPU, each rank on a context of its own -- the ranks' kernels never wait on one another, so nothing
+is lost by the emulation but the overlap -- with the all-gathers replaced by a concatenation; results against the oracle, against the one-GPU
 path, and run to run.  The two-process orchestration itself (torch.distributed all-gather between the phases) is
-covered on CPU by tests/test_multiproc.py."""
+covered on CPU by tests/test_multiproc.py and, with the real kernels in two processes, by tests/test_shard_procs_gpu.py."""
 import os
 
 import numpy as np
@@ -31,21 +31,35 @@ def dev(torch, ev):
 
 
 def shard_eval_one_gpu(torch, ctx, world, x, t, th, params, want):
-    """world ranks, one after the other, on this GPU and this context."""
+    """world ranks, one after the other, on this GPU -- EACH RANK WITH ITS OWN CONTEXT, as on real hardware: a rank that
+    read records, column partials or partial slots it did not produce itself would find another context's (or no) data
+    there, not a neighbour's valid numbers of the same evaluation.  `ctx` is rank 0's context; the others are made here.
+    Every rank runs the replicated phases on the gathered partials; their outputs must agree to the bit."""
     n = int(t.shape[0])
     mk = lambda *s: torch.empty(*s, dtype=torch.float64, device="cuda")
-    out = ctx.new_outputs(n, want)
+    ctxs = [ctx] + [hp.HawkesContext(ctx.n_max, ctx.dim) for _ in range(world - 1)]
+    outs = [c.new_outputs(n, want) for c in ctxs]
     parts = mk(world, ctx.shard_part_doubles(n, want, 1))
-    for r in range(world):
-        ctx.shard_pass1(x, t, th, params, want, r, world, parts[r])
-    ctx.shard_reduce1(n, params, want, world, parts, out)
+    for r, c in enumerate(ctxs):
+        c.shard_pass1(x, t, th, params, want, r, world, parts[r])
+    for c, o in zip(ctxs, outs):
+        c.shard_reduce1(n, params, want, world, parts, o)
     if want & (hp.WANT_GRAD_THETA | hp.WANT_HESS_THETA):
         parts2 = mk(world, ctx.shard_part_doubles(n, want, 2))
-        for r in range(world):
-            ctx.shard_pass2(n, params, want, r, world, parts2[r])
-        ctx.shard_finish(n, params, want, world, parts2, out)
-    st = ctx.last_status()
-    return out, st, ctx.get_lambda(n).cpu().numpy()
+        for r, c in enumerate(ctxs):
+            c.shard_pass2(n, params, want, r, world, parts2[r])
+        for c, o in zip(ctxs, outs):
+            c.shard_finish(n, params, want, world, parts2, o)
+    sts = [c.last_status() for c in ctxs]
+    lams = [c.get_lambda(n) for c in ctxs]
+    for o, lam_r, st_r in zip(outs[1:], lams[1:], sts[1:]):
+        assert st_r == sts[0] and torch.equal(lam_r, lams[0])
+        for f in ("ll", "grad_theta", "grad_hyper", "hess_theta_diag", "hess_hyper"):
+            a, b = getattr(outs[0], f), getattr(o, f)
+            assert (a is None and b is None) or torch.equal(a, b), f
+    for c in ctxs[1:]:
+        c.close()
+    return outs[0], sts[0], lams[0].cpu().numpy()
 
 
 def compare(ev, r, lam, ref):
