@@ -95,13 +95,15 @@ def load():
             _build.build(guard=guard)
         except Exception as exc:   # no nvcc on this machine, or compile error: never run a stale library silently
             stamp = path + ".srchash"
-            if os.path.exists(path) and not os.path.exists(stamp):
-                # a library without its source stamp (copied without it): staleness unknown -- say so, loudly, and use it
+            unstamped = os.path.exists(path) and not os.path.exists(stamp)
+            if unstamped and os.environ.get("HAWKES_B200_ALLOW_UNSTAMPED") == "1":
+                # a library copied without its source stamp: staleness unknown.  Loaded only on this explicit request.
                 import warnings
                 warnings.warn(f"paper_2103_03348_b200: {path} has no source stamp and could not be rebuilt ({exc}); "
-                              f"loading it as it is -- it may not match csrc/", RuntimeWarning)
+                              f"loading it because HAWKES_B200_ALLOW_UNSTAMPED=1 -- it may not match csrc/", RuntimeWarning)
             else:
-                what = "is older than its sources" if os.path.exists(path) else "is missing"
+                what = ("has no source stamp (it cannot be checked against csrc/; set HAWKES_B200_ALLOW_UNSTAMPED=1 to load it anyway)"
+                        if unstamped else "is older than its sources" if os.path.exists(path) else "is missing")
                 raise ImportError(
                     f"paper_2103_03348_b200: CUDA library {path} {what} and could not be rebuilt "
                     f"({exc}); run `python -m paper_2103_03348_b200.build` on a machine with nvcc") from exc

@@ -75,3 +75,25 @@ def test_build_returns_the_library_path_when_nothing_is_stale():
     hp.load()                       # builds if needed
     assert b.up_to_date()
     assert b.build() == b.LIB
+
+
+def test_loader_refuses_a_library_without_its_source_stamp(tmp_path, monkeypatch):
+    """A .so whose .srchash is missing and that cannot be rebuilt is an ImportError (it used to load with a warning that
+    no test run turns into a failure); HAWKES_B200_ALLOW_UNSTAMPED=1 is the explicit override."""
+    import shutil
+    import warnings
+    from paper_2103_03348_b200 import build as b
+    real = hp.lib_path()
+    fake = str(tmp_path / "libhawkes_b200.so")
+    shutil.copy(real, fake)                                   # copied without its stamp
+    monkeypatch.setattr(b, "LIB", fake)
+    monkeypatch.setattr(b, "nvcc", lambda: (_ for _ in ()).throw(RuntimeError("nvcc not found")))
+    monkeypatch.setattr(_lib, "_lib", None)
+    with pytest.raises(ImportError, match="no source stamp"):
+        _lib.load()
+    monkeypatch.setenv("HAWKES_B200_ALLOW_UNSTAMPED", "1")
+    with warnings.catch_warnings(record=True) as w:
+        warnings.simplefilter("always")
+        lib = _lib.load()
+    assert lib.hawkes_strerror(0) == b"ok" and any("HAWKES_B200_ALLOW_UNSTAMPED" in str(x.message) for x in w)
+    monkeypatch.setattr(_lib, "_lib", None)                   # the next load() takes the real library again
