@@ -234,8 +234,11 @@ int hawkes_skip_perm(hawkes_ctx* ctx, int64_t n, int64_t* perm_host);
 /* Pass-1 form of the context.  Eq. 1's double sum holds the background term of
  * every ORDERED pair, and B_{nn'} = B_{n'n}:
  *   HAWKES_PASS1_AUTO (default): log-likelihood- and gradient-level evaluations compute each background exponential
- *     once per UNORDERED pair and add it to both events' sums (when the context holds the column-partial buffer:
- *     problems of up to ~290,000 events);
+ *     once per UNORDERED pair and add it to both events' sums.  This form keeps one column partial per (event, later
+ *     target tile): 3072 * T * (T + 1) bytes of scratch for T = ceil(n_max / 256) tiles -- quadratic in n_max: 26 MB at
+ *     n_max = 23,422, 2.9 GB at 250,000.  hawkes_create allocates it up to 16 GiB (n_max <= 605,184 events); a larger
+ *     context has no such buffer and every evaluation falls back to the ordered-pair kernel, about 30 % slower at these
+ *     levels (hawkes_pass1_is_symmetric tells which form a context uses);
  *   HAWKES_PASS1_DENSE: every evaluation uses the ordered-pair kernel.
  * Same sums in another order.  Applies to every later evaluation and to later hawkes_skip_plan calls.
  * hawkes_pass1_is_symmetric: 1 if an evaluation whose pass 1 runs at `level` (0: ll / theta-gradient, 1: + hyper-

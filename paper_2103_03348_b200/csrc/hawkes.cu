@@ -1715,7 +1715,9 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     alloc((void**)&c->d_post, sizeof(double) * (size_t)(8 + 4 * n_max));
     alloc((void**)&c->d_hmc, sizeof(double) * (size_t)(16 + 5 * n_max));
     alloc((void**)&c->d_bgcache, sizeof(double) * (size_t)n_max);
-    {   // column partials of the symmetric pass 1 (levels 0 and 1: NB <= 3); above 16 GB the dense kernel runs instead
+    {   // column partials of the symmetric pass 1 (levels 0 and 1: NB <= 3): 3 * 256 * T (T + 1) / 2 doubles = 3072 T (T + 1)
+        // bytes for T = ceil(n_max / 256) tiles (26 MB at 23,422; 2.9 GB at 250,000).  Above 16 GiB (n_max > 605,184) the
+        // buffer is not allocated and the dense ordered-pair kernel runs instead (hawkes_pass1_is_symmetric reports it)
         const int nt = (int)((n_max + NT * P1_R - 1) / (NT * P1_R));
         c->partc_doubles = (size_t)colpart_doubles(nt, NT * P1_R, 3);
         if (c->partc_doubles * sizeof(double) > ((size_t)16 << 30)) c->partc_doubles = 0;

@@ -10,7 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
-    config.addinivalue_line("markers", "slow: minutes of oracle time; runs only with HAWKES_SLOW_TESTS=1")
+    config.addinivalue_line("markers", "slow: minutes of oracle time; left out with HAWKES_SKIP_SLOW_TESTS=1")
 
 
 @pytest.fixture(scope="session")

@@ -291,10 +291,11 @@ def test_scaling_sweep_full_oracle(torch, n):
 
 @pytest.mark.slow
 def test_scaling_sweep_full_oracle_n250000_slow(torch):
-    """The same at N = 250,000 (north_star's second size; 6.25e10 pairs): five minutes of 16-thread oracle time, so it
-    runs only with HAWKES_SLOW_TESTS=1; the log of the run that was made is profiles/r02_full_oracle_250k.txt."""
-    if os.environ.get("HAWKES_SLOW_TESTS") != "1":
-        pytest.skip("set HAWKES_SLOW_TESTS=1 (five minutes of oracle time)")
+    """The same at N = 250,000 (north_star's second size; 6.25e10 pairs): about five minutes of 16-thread oracle time.  It
+    runs by default -- north_star asks for oracle-matching outputs at this size, so the default suite must carry them;
+    HAWKES_SKIP_SLOW_TESTS=1 leaves it out while iterating (profiles/r02_full_oracle_250k.txt is the log of an earlier run)."""
+    if os.environ.get("HAWKES_SKIP_SLOW_TESTS") == "1":
+        pytest.skip("HAWKES_SKIP_SLOW_TESTS=1")
     _full_oracle_case(torch, 250000)
 
 
@@ -395,6 +396,80 @@ def test_dense_pass1_kernel_agrees_with_symmetric_pass1(torch):
                 assert np.max(np.abs(hs - hd) / np.maximum(np.abs(hd), 1e-300)) <= 1e-9
     with pytest.raises(hp.HawkesError):
         ctx.set_pass1_mode(5)
+
+
+def test_context_above_the_symmetric_scratch_cap_uses_the_dense_kernel(torch):
+    """The column partials of the once-per-unordered-pair pass 1 take 3072 T (T + 1) bytes for T = ceil(n_max / 256) tiles;
+    hawkes_create allocates them up to 16 GiB, i.e. n_max <= 605,184 (include/hawkes.h).  One event more and the context
+    has no such buffer: it reports the ordered-pair form at every level and its results (the dense kernel, not a
+    mode switch) match the oracle."""
+    small = hp.HawkesContext(605184 // 64, 2)      # well below the cap: symmetric
+    assert small.pass1_is_symmetric(0) and small.pass1_is_symmetric(1)
+    small.close()
+    ctx = hp.HawkesContext(605185, 2)
+    assert not ctx.pass1_is_symmetric(0) and not ctx.pass1_is_symmetric(1) and not ctx.pass1_is_symmetric(2)
+    ev = synth.small_random(1500, seed=31, ties=True, duplicates=True)
+    ev.x *= math.sqrt(ev.n / 16.0)
+    ev.t *= ev.n / 40.0
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, row_d1=True, threads=THREADS)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_ALL & ~hp.WANT_HESS_CROSS, ctx=ctx)
+    assert st == ref.status == 0
+    compare_all(ev, r, lam, ref, cross=False)
+    ctx.close()
+
+
+@pytest.mark.parametrize("case", ["theta_zero", "t_minus_1000", "t_plus_1e6"])
+def test_zero_rates_and_shifted_time_origin(torch, case):
+    """Two readings DESIGN.md records that no other parity case exercises.  R10: theta_m = 0 is accepted (PAPER.md:62 has
+    theta_n > 0) -- here for the earliest event, the last one, a run inside a tile and a few scattered events.  R8: times
+    of any sign and far from the origin -- the integral term runs over [0, t_N], so b_n = -t_n / tau_t of
+    SURVEY 8(c) A3 is large and positive for t < 0 and hugely negative for t ~ 1e6.  Every path: the default evaluation
+    (symmetric pass 1 at the gradient level, dense at the Hessian level), PASS1_DENSE, the work lists of
+    hawkes_skip_plan, and the evaluation cut across two ranks."""
+    from test_shard_gpu import shard_eval_one_gpu
+    ev = synth.small_random(777, seed=52, ties=True, duplicates=True)
+    ev.x *= math.sqrt(ev.n / 16.0)
+    ev.t *= ev.n / 40.0
+    if case == "theta_zero":
+        ev.theta[[0, 5, 300, 301, 302, 303, 511, 512, ev.n - 1]] = 0.0
+    elif case == "t_minus_1000":
+        ev.t = ev.t - 1000.0
+    else:
+        ev.t = ev.t + 1.0e6
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=THREADS)
+    assert ref.status == 0 and np.all(np.isfinite(ref.grad_theta)) and np.isfinite(ref.ll)
+    x, t, th = dev(torch, ev)
+    ctx = hp.HawkesContext(ev.n, ev.dim)
+    want = hp.WANT_ALL & ~hp.WANT_HESS_CROSS
+    # default path, all outputs including the cross block; then the gradient level (symmetric pass 1)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_ALL, ctx=ctx)
+    assert st == 0
+    compare_all(ev, r, lam, ref)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD, ctx=ctx)
+    assert st == 0 and ctx.pass1_is_symmetric(1)
+    compare_all(ev, r, lam, ref, cross=False)
+    ctx.set_pass1_mode(hp.PASS1_DENSE)
+    r, st, lam, _ = run_gpu(torch, ev, hp.WANT_GRAD, ctx=ctx)
+    assert st == 0
+    compare_all(ev, r, lam, ref, cross=False)
+    ctx.set_pass1_mode(hp.PASS1_AUTO)
+    # exact-zero skipping: outputs in the caller's order
+    ctx.skip_plan(x, t, ev.params)
+    for w in (hp.WANT_GRAD, want):
+        rs = ctx.eval_skip(x, t, th, ev.params, w)
+        assert ctx.last_status() == 0
+        s = scales(ev, ref)
+        check("ll (skip)", rs.ll.item(), ref.ll, s["ll"])
+        check("grad_theta (skip)", rs.grad_theta.cpu().numpy(), ref.grad_theta, s["grad_theta"])
+        check("grad_hyper (skip)", rs.grad_hyper.cpu().numpy(), ref.grad_hyper, s["grad_hyper"])
+        if rs.hess_theta_diag is not None:
+            check("hess_theta_diag (skip)", rs.hess_theta_diag.cpu().numpy(), ref.hess_theta_diag, floor=1e-280)
+            check("hess_hyper (skip)", rs.hess_hyper.cpu().numpy(), ref.hess_hyper, hess_hyper_scale(ref.hess_hyper))
+    # one evaluation cut across two ranks (a context each)
+    for w in (hp.WANT_GRAD, want):
+        rsh, st, lam = shard_eval_one_gpu(torch, ctx, 2, x, t, th, ev.params, w)
+        assert st == 0
+        compare_all(ev, rsh, lam, ref, cross=False)
 
 
 @pytest.mark.parametrize("n,seed,dim", [(3, 41, 2), (300, 42, 2), (777, 43, 3), (1000, 44, 2)])
