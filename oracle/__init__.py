@@ -127,6 +127,25 @@ def integral(t, theta, params, dim: int, *, bg: str = "ST"):
     return float(lam[0]), d1, d2.reshape(6, 6)
 
 
+def cross_abs(x, t, params, lam, row_d1, *, threads: int = 1):
+    """Error scale of the cross block (tests only): abs[m, p] = sum_{t_m<t_n} (k_nm/lambda_n) (T_p + |lambda_{n,p}|/lambda_n),
+    T = (0, 0, 0, 1/xi0, r^2/h^3 + D/h, 1/omega + dt) -- the magnitudes of the terms of entry (m, p), SURVEY.md 8(c) B16."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    prm = np.asarray(params, dtype=np.float64)
+    lam = np.ascontiguousarray(lam, dtype=np.float64)
+    rd1 = np.ascontiguousarray(row_d1, dtype=np.float64)
+    dim, n = x.shape
+    out = np.zeros(n * 6)
+    fn = lib().hawkes_ref_cross_abs
+    fn.restype = ctypes.c_int
+    fn.argtypes = [ctypes.c_int64, ctypes.c_int] + [_dp] * 6 + [ctypes.c_int]
+    st = fn(n, dim, _p(x), _p(t), _p(prm), _p(lam), _p(rd1), _p(out), threads)
+    if st != 0:
+        raise ValueError(f"hawkes_ref_cross_abs: status {st}")
+    return out.reshape(n, 6)
+
+
 def cols(x, t, params, lam, idx, *, threads: int = 1):
     """c_m = sum_{t_m<t_n} k_nm / lambda_n and d_m = sum (k_nm/lambda_n)^2 for the listed columns."""
     x = np.ascontiguousarray(x, dtype=np.float64)

@@ -388,6 +388,37 @@ int hawkes_ref_cols(int64_t n, int dim, const double* x, const double* t, const 
     return 0;
 }
 
+// Error scale of the cross block d2 ell / d theta_m dp ("the sum of the magnitudes of the terms"),
+// for the parity tests only -- it is not an output of the method.  Entry (m, p) of the block is
+//   sum_{n: t_n > t_m} a_nm [ d log k_nm / dp - lambda_{n,p} / lambda_n ] - Lambda_{theta_m p},   a_nm = k_nm / lambda_n,
+// and this routine sums, over the same pairs, a_nm times the magnitudes of what the bracket is made of:
+//   abs[m*6 + p] = sum_n a_nm ( T_p(n, m) + |lambda_{n,p}| / lambda_n ),
+//   T = (0, 0, 0, 1/xi0, r^2/h^3 + D/h, 1/omega + dt)    -- the terms of d log k / d(xi0, h, omega), taken positive.
+// row_d1[n*6 + p] = lambda_{n,p} as returned by hawkes_ref_eval.  The integral part and the terms inside lambda_{n,p}
+// are added by the test.
+int hawkes_ref_cross_abs(int64_t n, int dim, const double* x, const double* t, const double* params,
+                         const double* lambda, const double* row_d1, double* abs_out, int threads) {
+    if (n < 1 || dim < 1 || dim > 3 || !lambda || !row_d1 || !abs_out) return -1;
+    const P p = make_params(params, dim, 0);
+    (void)threads;
+#ifdef _OPENMP
+    const int nthreads = threads > 0 ? threads : 1;
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
+#endif
+    for (int64_t m = 0; m < n; ++m) {
+        ld s[6] = {0, 0, 0, 0, 0, 0};
+        for (int64_t i = 0; i < n; ++i) {
+            const Pair q = make_pair(dim, n, x, t, i, m);   // target i, source m
+            if (!q.causal) continue;
+            const ld a = (ld)excitation(p, q.r2, q.dt) / (ld)lambda[i];
+            const ld T[6] = {0, 0, 0, (ld)1 / p.xi0, (ld)q.r2 / ((ld)p.h * p.h * p.h) + (ld)dim / p.h, (ld)1 / p.omega + q.dt};
+            for (int b = 0; b < 6; ++b) s[b] += a * (T[b] + std::fabs((ld)row_d1[i * 6 + b]) / (ld)lambda[i]);
+        }
+        for (int b = 0; b < 6; ++b) abs_out[m * 6 + b] = (double)s[b];
+    }
+    return 0;
+}
+
 // Lambda(t_N) and its hyperparameter derivatives alone (O(N)): integral[1], d1[6], d2[36] row-major.
 int hawkes_ref_integral(int64_t n, int dim, const double* t, const double* theta, const double* params,
                         double* integral, double* d1, double* d2, int bg_mode) {

@@ -420,3 +420,33 @@ def test_s_mode_background_is_the_leave_one_out_kde():
         kde = KernelDensity(kernel="gaussian", bandwidth=tx).fit(others)
         dens = math.exp(kde.score_samples(X[n:n + 1])[0])      # mean of the kernels
         assert abs(r.lam[n] - mu0 * len(others) * dens) <= 1e-10 * r.lam[n]
+
+
+def test_cross_abs_scale_brute_force_and_triangle_inequality():
+    """oracle.cross_abs, the entry-wise error scale of the cross block (used by the GPU parity tests,
+    not an output of the method): typed out here as a double loop from its definition, bounded below by the block itself
+    (triangle inequality) and equal to it where no term changes sign (column mu0: the bracket is -SB_n / (mu0 lambda_n))."""
+    ev = synth.small_random(40, seed=77, ties=True, duplicates=True)
+    ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, cross=True, row_d1=True)
+    A = oracle.cross_abs(ev.x, ev.t, ev.params, ref.lam, ref.row_d1)
+    mu0, tx, tt, xi0, h, om = ev.params
+    n, D = ev.n, ev.dim
+    B = np.zeros((n, 6))
+    for m in range(n):
+        for i in range(n):
+            dt = ev.t[i] - ev.t[m]
+            if not dt > 0:
+                continue
+            r2 = float(np.sum((ev.x[:, i] - ev.x[:, m]) ** 2))
+            k = xi0 * om * (2 * np.pi) ** (-D / 2) * h ** (-D) * np.exp(-om * dt - r2 / (2 * h * h))
+            a = k / ref.lam[i]
+            T = np.array([0, 0, 0, 1 / xi0, r2 / h ** 3 + D / h, 1 / om + dt])
+            B[m] += a * (T + np.abs(ref.row_d1[i]) / ref.lam[i])
+    assert np.allclose(A, B, rtol=1e-12, atol=0)
+    Tm = ev.t[-1] - ev.t
+    S = ref.hess_cross.copy()                     # the pair sums alone: add the integral part back
+    S[:, 3] += -np.expm1(-om * Tm)
+    S[:, 5] += xi0 * Tm * np.exp(-om * Tm)
+    assert np.all(np.abs(S) <= A * (1 + 1e-12) + 1e-300)
+    assert np.allclose(np.abs(S[:, 0]), A[:, 0], rtol=1e-12, atol=1e-300)
+    assert np.all(A[:, 3:] > np.abs(S[:, 3:])[:, :] - 1e-300) and A[:-2].min() >= 0

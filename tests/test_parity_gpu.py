@@ -49,16 +49,19 @@ def check_cross(ev, C, ref):
     # c_m = sum_n k_nm / lambda_n from the oracle's column routine: recovering it from grad_theta (c_m minus an O(1)
     # integral term) would lose every c_m below 1e-16
     c_m, _ = oracle.cols(ev.x, ev.t, ev.params, ref.lam, np.arange(ev.n), threads=THREADS)
-    # Scale of entry (m, p): c_m times the largest magnitude a pair's bracket can have.  Its second part,
-    # lambda_{n,p}/lambda_n, is a difference of moment sums whose terms are bounded by
-    # |d lambda_n/dp| / lambda_n + c_p with c_p = (1/mu0, D/tau_x, 1/tau_t, 1/xi0, D/h, 1/omega), as in the row checks;
-    # its first part is |d log k / dp|: 1/xi0; |r^2/h^3 - D/h| on the pairs that are not exact zeros
-    # (exp(-r^2/2h^2) > 0 needs r^2/2h^2 < 1075 ln 2 = 745.2, so r^2/h^3 < 1490.3/h); |1/omega - dt|.
+    # Scale of entry (m, p) = the sum of the magnitudes of its terms, from oracle quantities only:
+    #   sum_n a_nm (T_p + |lambda_{n,p}| / lambda_n)    oracle.cross_abs: T_p = the terms of d log k / dp taken positive,
+    #   + 2 c_p c_m                                     lambda_{n,p} / lambda_n is itself a difference of two moment sums
+    #                                                   (SURVEY 8(c) A6), each at most c_p = (1/mu0, D/tau_x, 1/tau_t,
+    #                                                   1/xi0, D/h, 1/omega) above |lambda_{n,p}| / lambda_n, as in the row checks
+    #   + |Lambda_{theta_m p}|                          1 - E_m for xi0, xi0 T_m E_m for omega.
     D = ev.dim
-    rr = np.max(np.abs(ref.row_d1 / ref.lam[:, None]), axis=0)
+    A = oracle.cross_abs(ev.x, ev.t, ev.params, ref.lam, ref.row_d1, threads=THREADS)
     cp = np.array([1 / mu0, D / tx, 1 / tt, 1 / xi0, D / h, 1 / om])
-    colB = rr + cp + np.array([0, 0, 0, 1 / xi0, max(D, 1490.3 - D) / h, 1 / om + (ev.t[-1] - ev.t[0])])
-    worst = check("hess_cross", C, O, c_m[:, None] * colB[None, :] + np.array([0, 0, 0, 1, 0, xi0 * np.max(T)])[None, :], floor=1e-280)
+    lam_terms = np.zeros((ev.n, 6))
+    lam_terms[:, 3] = -np.expm1(-om * T)
+    lam_terms[:, 5] = xi0 * T * np.exp(-om * T)
+    worst = check("hess_cross", C, O, A + 2.0 * c_m[:, None] * cp[None, :] + lam_terms, floor=1e-280)
     for p in range(6):
         assert np.max(np.abs(C[:, p] - O[:, p])) <= TOL * max(np.max(np.abs(O[:, p])), 1e-280)
     return worst
