@@ -625,6 +625,7 @@ def run_b200(args, ev, workload: str) -> dict:
         torch.cuda.empty_cache()
         res["sweep"] = [sweep_entry(torch, hp, dev, local, nn, args.seed, flush, peaks, not args.no_cpu_baseline)
                         for nn in (50000, 100000, 250000)]
+        res["configs"] = other_configs(args)
     if dist is not None:
         dist.destroy_process_group()
     return res
@@ -725,9 +726,10 @@ def run_posterior(args) -> dict:
     return res
 
 
-def run_hmc(args) -> dict:
+def run_hmc(args, only=None) -> dict:
     """configs[3]: preconditioned HMC on z, 20 leapfrog steps per iteration, preconditioner refreshed every 10
-    iterations; --steps = timed iterations (BASELINE: 200)."""
+    iterations; --steps = timed iterations (BASELINE: 200).  only: names of the extra variants to run beside the
+    headline (None = all)."""
     import numpy as np
     import torch
     import paper_2103_03348_b200 as hp
@@ -778,8 +780,10 @@ def run_hmc(args) -> dict:
     for name, cache in (("recompute_all_pairs", 0), ("cached_background", 1), ("cached_kernel_matrix", 2),
                         ("skip_lists_recompute", 3), ("skip_lists_cached_background", 4),
                         ("sparse_kernel_matrix", 5)):
-        res_var[name + "__plus_prior_curvature"] = run_variant(cache, eps, pp)
-    res_var["sparse_kernel_matrix__paper_preconditioner"] = run_variant(5, args.hmc_step_paper, None)
+        if only is None or name + "__plus_prior_curvature" in only:
+            res_var[name + "__plus_prior_curvature"] = run_variant(cache, eps, pp)
+    if only is None or "sparse_kernel_matrix__paper_preconditioner" in only:
+        res_var["sparse_kernel_matrix__paper_preconditioner"] = run_variant(5, args.hmc_step_paper, None)
     clocks = sampler.stop()
     res = {"metric": "hmc_seconds_per_iteration", "value": head["seconds_per_iteration"], "unit": "s/iteration",
            "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": head["seconds_per_iteration"] * 1e3,
@@ -814,6 +818,69 @@ def run_hmc(args) -> dict:
                                          f"{threads} OpenMP threads, scaled by {L}/{n_steps}; the preconditioner refresh "
                                          f"(1 Hessian evaluation per 10 iterations) is left out"}
     return res
+
+
+def run_config0(args) -> dict:
+    """configs[0]: N = 1,000, log-lik, full gradient and Hessian -- hawkes_eval with every output (theta-diagonal, 6 x 6,
+    N x 6 cross block) plus the dense theta-theta block; every output against the full oracle on the spot."""
+    import numpy as np
+    import torch
+    import paper_2103_03348_b200 as hp
+    from paper_2103_03348_b200 import synth
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    ev = synth.config(0, args.seed)
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    x, t, th = to(ev.x), to(ev.t), to(ev.theta)
+    ctx = hp.HawkesContext(ev.n, ev.dim, 0)
+    out = ctx.eval(x, t, th, ev.params, hp.WANT_ALL)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    step = lambda: ctx.eval(x, t, th, ev.params, hp.WANT_ALL, out=out)
+    _event_timed(torch, dev, step, args.warmup, flush)
+    l0 = ctx.launch_count()
+    ms = _event_timed(torch, dev, step, args.steps, flush)
+    launches = ctx.launch_count() - l0
+    dense_ms = _event_timed(torch, dev, lambda: ctx.hessian_theta_dense(x, t, th, ev.params), args.steps, flush)
+    st = ctx.last_status()
+    res = {"workload": "BASELINE.json configs[0]: N=1,000, log-lik + full gradient + Hessian (theta diagonal, 6x6, Nx6 cross block)",
+           "call": "hawkes_eval(WANT_ALL)", "steps": args.steps, "warmup": args.warmup, "ms_per_step": statistics.median(ms),
+           "evals_per_s": args.steps / (float(sum(ms)) * 1e-3), "gpu_launches_per_step": launches / args.steps,
+           "dense_theta_block_ms": statistics.median(dense_ms), "device_status": int(st)}
+    if not args.no_cpu_baseline:
+        import oracle
+        ref = oracle.evaluate(ev.x, ev.t, ev.theta, ev.params, hess=True, cross=True, row_d1=True, threads=oracle.max_threads())
+        rel = lambda g, o: float(np.max(np.abs(g.cpu().numpy().reshape(np.shape(o)) - o)) / np.max(np.abs(o)))
+        res["parity_vs_full_oracle_max_rel_to_largest_entry"] = {
+            "ll": abs(out.ll.item() - ref.ll) / abs(ref.ll), "grad_theta": rel(out.grad_theta, ref.grad_theta),
+            "grad_hyper": rel(out.grad_hyper, ref.grad_hyper), "hess_theta_diag": rel(out.hess_theta_diag, ref.hess_theta_diag),
+            "hess_hyper": rel(out.hess_hyper, ref.hess_hyper), "hess_cross_per_column": [
+                rel(out.hess_cross[:, k], ref.hess_cross[:, k]) for k in range(6) if np.max(np.abs(ref.hess_cross[:, k])) > 0],
+            "tolerance": 1e-10}
+    ctx.close()
+    return res
+
+
+def other_configs(args) -> dict:
+    """BASELINE.json configs[0], [2], [3] inside the default line (configs[1] is the line itself, configs[4] its `sweep`):
+    the same measurements `--config 0 | 2 | 3` print on their own, with short step counts and without the oracle-timing legs."""
+    sub = lambda **kw: argparse.Namespace(**{**vars(args), **kw})
+    c0 = run_config0(sub(steps=20, warmup=5))
+    post = run_posterior(sub(steps=20, warmup=5, no_cpu_baseline=True))
+    fastest = "sparse_kernel_matrix__plus_prior_curvature"
+    hmc = run_hmc(sub(steps=200, warmup=5, no_cpu_baseline=True), only=(fastest,))
+    pick = lambda d, keys: {k: d[k] for k in keys if k in d}
+    return {
+        "configs[0]": c0,
+        "configs[2]": {**pick(post, ("metric", "value", "unit", "steps", "warmup", "ms_per_step", "gpu_launches", "breakdown_ms",
+                                     "out3", "clocks")),
+                       "workload": post["config"]["workload"], "call": post["config"]["call"], "e2e": post["e2e"],
+                       "parity": "tests/test_tree_gpu.py::test_posterior_z_config2_full_size (full likelihood oracle + dense Cholesky prior oracle)"},
+        "configs[3]": {**pick(hmc, ("metric", "value", "unit", "steps", "warmup", "higher_is_better", "clocks")),
+                       "workload": hmc["config"]["workload"], "call": hmc["config"]["call"],
+                       "variant_of_value": hmc["config"]["variant_of_value"],
+                       "paper_method": hmc["variants"]["recompute_all_pairs__paper_preconditioner"],
+                       "fastest_exact_variant": {"name": fastest, **hmc["variants"][fastest]},
+                       "parity": "tests/test_hmc_gpu.py (oracle trajectory incl. accept decisions; full-size single iteration)"}}
 
 
 def workload_of(args):
