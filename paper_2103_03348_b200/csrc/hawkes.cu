@@ -1024,6 +1024,126 @@ __global__ void __launch_bounds__(RED_T) theta_kernel(const double* __restrict__
     if (hess_theta_diag) hess_theta_diag[o] = -(c.CSS * c.CSS) * ds;
 }
 
+// ------------------------------------------------------------------------------------------------
+// a4 restricted to a subset of the sources ("computing the entire vector ... (d ell/d theta_1, ...,
+// d ell/d theta_M) requires time O(NM)"; Alg. 2 step 2: "parfor n in {1, ..., M}").  Only the M sequenced
+// events have a free rate; hawkes_posterior_z and the HMC update read c_m, d_m at those M indices only, so the pass visits
+// the pairs (target n, source idx[k]) alone: M N / 2 causal pairs instead of N^2 / 2.
+// CTA (bx, by): the SUB_TILE sources idx[by * SUB_TILE ...) (R per thread; all G work groups hold the same ones) against
+// the G * TS targets [bx * G * TS, ...), group g taking the g-th TS of them.  Every pair carries the dt > 0 test
+// (p2_tile<MASKED>), so idx needs no order; a CTA none of whose targets comes after the tile's earliest source writes
+// zeros without filling the table.  The groups' sums are added in group order and written to
+// part[((bx * gridDim.y + by) * 2 + k) * SUB_TILE + local]; theta_sub_kernel adds the bx slots in order: fixed cut,
+// fixed order, no atomics -- bit-identical run to run.
+constexpr int SUB_G = 4;
+#ifndef HAWKES_SUB_R
+#define HAWKES_SUB_R 1
+#endif
+constexpr int SUB_R = HAWKES_SUB_R;   // sources per thread: 1 halves the work of a CTA (finer, better balanced over the SMs)
+template <int R> constexpr int sub_tile() { return NT * R; }
+
+template <int R, int LEVEL, bool DIM3, int G>
+__global__ void __launch_bounds__(NT * G, 1) pass2_sub_kernel(const double* __restrict__ rec, const double* __restrict__ trec,
+                                                              int64_t n, DevConsts c, const double* __restrict__ tab_g,
+                                                              const int64_t* __restrict__ idx, int64_t m,
+                                                              double* __restrict__ part) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    constexpr unsigned BUF = group_buf_bytes<DIM3>();
+    static_assert(smem_request(G * BUF) <= SMEM_MAX, "table + streaming buffers must fit shared memory");
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double smagic;
+    __shared__ long long s_min[NT * G / 32];
+    __shared__ double comb[G - 1][2 * R][NT];
+    const int grp = threadIdx.x / NT, tid = threadIdx.x % NT;
+    const int64_t k0 = (int64_t)blockIdx.y * (NT * R);
+    int64_t src[R];
+    long long mn = 0x7fffffffffffffffLL;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int64_t k = k0 + r * NT + tid;
+        src[r] = idx[k < m ? k : m - 1];     // a tail thread repeats the last source; its sums are not written
+        mn = src[r] < mn ? src[r] : mn;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const long long o = __shfl_xor_sync(0xffffffffu, mn, off);
+        mn = o < mn ? o : mn;
+    }
+    if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = mn;
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < NT * G / 32; ++w) mn = s_min[w] < mn ? s_min[w] : mn;   // earliest source of the tile
+
+    double cm[R], dm[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { cm[r] = 0.0; dm[r] = 0.0; }
+    const int64_t j0 = (int64_t)blockIdx.x * (G * TS);
+    const int64_t j1 = min(j0 + (int64_t)G * TS, n);
+    // times are non-decreasing: a target with index <= mn is not later than any source of the tile
+    if (j1 - 1 > mn) {   // CTA-uniform
+        const unsigned smem_base = (unsigned)__cvta_generic_to_shared(smem);
+        const SmemPlan plan = smem_plan(smem_base, G * BUF);
+        fill_table(reinterpret_cast<double*>(smem + plan.tab_off), tab_g);
+        stash_consts(smagic);
+        __syncthreads();
+        const P1C pc = pinned_consts(smagic, c);
+        const unsigned lane_base = (smem_base + plan.tab_off) | (8u * (threadIdx.x & 31));
+        const int64_t a = j0 + (int64_t)grp * TS;
+        const int cnt = (int)max((int64_t)0, min((int64_t)TS, n - a));
+        if (cnt > 0 && a + cnt - 1 > mn) {   // group-uniform
+            double* const sbuf = reinterpret_cast<double*>(smem + plan.buf_off + grp * BUF);
+            RecIO<DIM3> io;
+            io.load(trec, a, cnt, tid);
+            io.store(sbuf, tid);
+            group_sync(grp);
+            Ev<DIM3> g[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) g[r] = read_rec<DIM3>(rec + src[r] * RS);
+            p2_tile<R, LEVEL, true, DIM3>(sbuf, cnt, g, cm, dm, pc, lane_base);
+        }
+    }
+    if (grp > 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) { comb[grp - 1][r][tid] = cm[r]; comb[grp - 1][R + r][tid] = dm[r]; }
+    }
+    __syncthreads();
+    if (grp == 0) {
+        double* o = part + ((int64_t)blockIdx.x * gridDim.y + blockIdx.y) * 2 * (NT * R);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+#pragma unroll
+            for (int q = 0; q < G - 1; ++q) { cm[r] += comb[q][r][tid]; dm[r] += comb[q][R + r][tid]; }
+            o[r * NT + tid] = cm[r];
+            if (LEVEL >= 1) o[NT * R + r * NT + tid] = dm[r];
+        }
+    }
+}
+
+// a5 for the subset: grad_theta[idx[k]], hess_theta_diag[idx[k]] from the n_chunks partial slots of source k, in slot order.
+// Entries of the two arrays outside idx are not written.
+template <bool DIM3>
+__global__ void theta_sub_kernel(const double* __restrict__ rec, int64_t n, DevConsts c, const double* __restrict__ part,
+                                 int n_chunks, int n_tiles, int tile, const int64_t* __restrict__ idx, int64_t m,
+                                 double* __restrict__ grad_theta, double* __restrict__ hess_theta_diag) {
+    constexpr int RS = DIM3 ? 6 : 4;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const int64_t by = k / tile, local = k % tile;
+    double cs = 0.0, ds = 0.0;
+    for (int j = 0; j < n_chunks; ++j) {
+        const double* o = part + ((int64_t)j * n_tiles + by) * 2 * tile + local;
+        cs += o[0];
+        if (hess_theta_diag) ds += o[tile];
+    }
+    const int64_t i = idx[k];
+    if (grad_theta) {
+        const double tN = rec[(n - 1) * RS + (DIM3 ? 3 : 2)];
+        const double ti = rec[i * RS + (DIM3 ? 3 : 2)];
+        grad_theta[i] = c.CSS * cs - c.xi0 * (-expm1(-c.omega * (tN - ti)));
+    }
+    if (hess_theta_diag) hess_theta_diag[i] = -(c.CSS * c.CSS) * ds;
+}
+
 #include "cross.cuh"
 
 // Dense theta-theta block (correctness only): H[m][m'] = - sum_n k_nm k_nm' / lambda_n^2.
@@ -1294,6 +1414,8 @@ struct hawkes_ctx {
     size_t partc_doubles;
     int plan_sym;
     int reserve_sm;       // SMs the pairwise passes leave free (hawkes_posterior_z: the tree prior runs beside them)
+    const int64_t* sub_idx;   // != NULL: the evaluation's pass 2 is wanted at these sub_m sources only (set by posterior_z_impl
+    int64_t sub_m;            // around its hawkes_eval, O(NM)); grad_theta / hess_theta_diag are written at idx only
     int plan_reserve;
     int bg_mode;          // 0 normal, 1 store the cache, 2 use it (set by hawkes_hmc_run only)
     int s_mode;           // hawkes_set_background_mode
@@ -1531,7 +1653,27 @@ int enqueue_eval(hawkes_ctx* ctx, int64_t n, const double* x, const double* t, c
         if (scal_aside) CK(cudaEventRecord(ctx->ev_join, ctx->side));
         ctx->launches++;
     }
-    if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
+    // pass 2 over a subset of the sources when the caller reads only those (and the subset is small enough to pay, and its
+    // partial slots fit): M N / 2 pairs instead of N^2 / 2
+    const int sub_chunks = (int)((n + SUB_G * TS - 1) / (SUB_G * TS));
+    const int sub_tiles = ctx->sub_m > 0 ? (int)((ctx->sub_m + sub_tile<SUB_R>() - 1) / sub_tile<SUB_R>()) : 0;
+    const bool sub = ctx->sub_idx != nullptr && ctx->sub_m > 0 && 2 * ctx->sub_m <= n && !(want & HAWKES_WANT_HESS_CROSS) &&
+                     (size_t)sub_chunks * sub_tiles * 2 * sub_tile<SUB_R>() <= ctx->part2_doubles && sub_tiles <= 65535;
+    if (sub && (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA))) {
+        const dim3 gs((unsigned)sub_chunks, (unsigned)sub_tiles);
+        if (pe) CK(cudaEventRecord(pe[3], st));
+        if (want & HAWKES_WANT_HESS_THETA)
+            pass2_sub_kernel<SUB_R, 1, DIM3, SUB_G><<<gs, NT * SUB_G, smem_request(SUB_G * group_buf_bytes<DIM3>()), st>>>(
+                ctx->d_rec, ctx->d_trec, n, c, ctx->d_tab, ctx->sub_idx, ctx->sub_m, ctx->d_part2);
+        else
+            pass2_sub_kernel<SUB_R, 0, DIM3, SUB_G><<<gs, NT * SUB_G, smem_request(SUB_G * group_buf_bytes<DIM3>()), st>>>(
+                ctx->d_rec, ctx->d_trec, n, c, ctx->d_tab, ctx->sub_idx, ctx->sub_m, ctx->d_part2);
+        if (pe) CK(cudaEventRecord(pe[4], st));
+        theta_sub_kernel<DIM3><<<(unsigned)((ctx->sub_m + 255) / 256), 256, 0, st>>>(
+            ctx->d_rec, n, c, ctx->d_part2, sub_chunks, sub_tiles, sub_tile<SUB_R>(), ctx->sub_idx, ctx->sub_m,
+            (want & HAWKES_WANT_GRAD_THETA) ? grad_theta : nullptr, (want & HAWKES_WANT_HESS_THETA) ? hess_theta_diag : nullptr);
+        ctx->launches += 2;
+    } else if (want & (HAWKES_WANT_GRAD_THETA | HAWKES_WANT_HESS_THETA)) {
         const unsigned g2 = (unsigned)((pl.grid2 + P2_G[level2] - 1) / P2_G[level2]);
         if (pe) CK(cudaEventRecord(pe[3], st));
         if (want & HAWKES_WANT_HESS_THETA)
@@ -1587,6 +1729,8 @@ int query_occupancy(hawkes_ctx* ctx) {
     if ((rc = setup_kernel(pass1_kernel<P1_R, 2, DIM3, P1_G[2]>, P1_G[2], smem_request(P1_G[2] * group_buf_bytes<DIM3>()), &ctx->occ1[2]))) return rc;
     if ((rc = setup_kernel(pass2_kernel<P2_R, 0, DIM3, P2_G[0]>, P2_G[0], smem_request(P2_G[0] * group_buf_bytes<DIM3>()), &ctx->occ2[0]))) return rc;
     if ((rc = setup_kernel(pass2_kernel<P2_R, 1, DIM3, P2_G[1]>, P2_G[1], smem_request(P2_G[1] * group_buf_bytes<DIM3>()), &ctx->occ2[1]))) return rc;
+    if ((rc = setup_kernel(pass2_sub_kernel<SUB_R, 0, DIM3, SUB_G>, SUB_G, smem_request(SUB_G * group_buf_bytes<DIM3>()), &dummy))) return rc;
+    if ((rc = setup_kernel(pass2_sub_kernel<SUB_R, 1, DIM3, SUB_G>, SUB_G, smem_request(SUB_G * group_buf_bytes<DIM3>()), &dummy))) return rc;
     if ((rc = setup_kernel(cross_pass_kernel<PX_R, DIM3, PX_G>, PX_G, smem_request(PX_G * cross_group_bytes<DIM3>()), &ctx->occx))) return rc;
     return HAWKES_OK;
 }
@@ -1658,6 +1802,8 @@ int hawkes_create(hawkes_ctx** out, int64_t n_max, int dim, int device) {
     c->plan_bg = -1;
     c->plan_sym = -1;
     c->reserve_sm = 0;
+    c->sub_idx = nullptr;
+    c->sub_m = 0;
     c->plan_reserve = -1;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess ||
@@ -1985,8 +2131,12 @@ static int posterior_z_impl(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const
                               hess_z ? ht : nullptr, nullptr, stream);
     } else {
         ctx->reserve_sm = 1;
+        ctx->sub_idx = idx;   // only gt[idx[k]], ht[idx[k]] are read below: pass 2 over the M sequenced sources
+        ctx->sub_m = m;
         rc = hawkes_eval(ctx, n, x, t, th, p, want, sc, (grad_z || hess_z) ? gt : nullptr, nullptr, hess_z ? ht : nullptr,
                          nullptr, nullptr, stream);
+        ctx->sub_idx = nullptr;
+        ctx->sub_m = 0;
         ctx->reserve_sm = 0;
     }
     if (rc) return rc;

@@ -220,6 +220,33 @@ def test_posterior_z_small_problem(torch):
     posterior_case(torch, ev, tree, z, 0.25, 0.1, beta=0.001)
 
 
+def subset_events(n, m, shuffle, seed=61):
+    """A dense little problem (ties, duplicated locations) whose sequenced set is an arbitrary subset of m events that
+    always holds the first event and, for m >= 2, the last one; shuffle: idx in no particular order."""
+    ev = synth.small_random(n, seed=seed, ties=True, duplicates=True)
+    ev.x *= np.sqrt(n / 16.0)
+    ev.t *= n / 40.0
+    rest = np.argsort(synth.uniforms(seed, 700, n), kind="stable")
+    rest = rest[(rest != 0) & (rest != n - 1)]
+    idx = np.concatenate([[0, n - 1][:min(m, 2)], rest[:max(m - 2, 0)]]).astype(np.int64)
+    if not shuffle:
+        idx = np.sort(idx)
+    ev.free_idx = idx
+    return ev
+
+
+@pytest.mark.parametrize("m,shuffle", [(1, False), (2, True), (97, True), (256, False), (257, True), (750, True), (751, False),
+                                       (1500, False)])
+def test_posterior_z_source_subsets(torch, m, shuffle):
+    """Pass 2 runs over the m sequenced sources only when 2 m <= n (the O(NM) gradient; Alg. 2 step 2), over
+    all n otherwise: m = 1, one and two source tiles, a ragged tile, both sides of the switch, m = n; idx sorted and not;
+    the subset holds event 0 and event n - 1; ties in time and duplicated locations.  Every output against the oracle."""
+    ev = subset_events(1500, m, shuffle)
+    tree = synth.make_tree(ev.t[ev.free_idx], 61)
+    z = synth.draw_z(tree, 0.25, 0.1, 61)
+    posterior_case(torch, ev, tree, z, 0.25, 0.1, beta=0.002)
+
+
 def test_posterior_z_config2_full_size(torch):
     """BASELINE.json configs[2] at full size: N = 23,422, M = 1,610."""
     ev, tree, z = synth.config_tree(0)
