@@ -1130,10 +1130,22 @@ __global__ void theta_sub_kernel(const double* __restrict__ rec, int64_t n, DevC
     if (k >= m) return;
     const int64_t by = k / tile, local = k % tile;
     double cs = 0.0, ds = 0.0;
-    for (int j = 0; j < n_chunks; ++j) {
-        const double* o = part + ((int64_t)j * n_tiles + by) * 2 * tile + local;
-        cs += o[0];
-        if (hess_theta_diag) ds += o[tile];
+    const int64_t stride = (int64_t)n_tiles * 2 * tile;
+    const double* o = part + by * 2 * tile + local;
+    int j = 0;
+    for (; j + 8 <= n_chunks; j += 8) {   // eight slots' loads in flight, adds in slot order
+        double vc[8], vd[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            vc[u] = o[(j + u) * stride];
+            vd[u] = hess_theta_diag ? o[(j + u) * stride + tile] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { cs += vc[u]; ds += vd[u]; }
+    }
+    for (; j < n_chunks; ++j) {
+        cs += o[j * stride];
+        if (hess_theta_diag) ds += o[j * stride + tile];
     }
     const int64_t i = idx[k];
     if (grad_theta) {
