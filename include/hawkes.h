@@ -392,7 +392,10 @@ int hawkes_z_chain(hawkes_ctx* ctx, int64_t n, int64_t m, const int64_t* idx, co
  *   chain rule.  out3[0] = ell, out3[1] = log p(z | V_G, sigma2, tau0), out3[2] = their sum;
  *   grad_z[m] = d(ell + log p)/dz;  hess_z[m] = likelihood part of the diagonal second derivative (see
  *   hawkes_z_chain; the prior's Hessian -V_G^-1/sigma2 is not added).  out3, grad_z, hess_z: DEVICE, each optional.
- * Uses context scratch for theta and the theta-derivatives; enqueues only. */
+ * Uses context scratch for theta and the theta-derivatives; enqueues only.  Only the m sequenced events have a free rate, so
+ * when 2 m <= n the second pairwise pass (Eq. 4 / Eq. 5) visits the pairs (target, source idx[k]) alone -- the O(NM) cost the
+ * paper states for the gradient (Alg. 2 step 2) instead of O(N^2 / 2); idx may be in any order.
+ * hawkes_hmc_run's recompute variants (cache_background 0 and 1) evaluate the posterior the same way. */
 int hawkes_posterior_z(hawkes_ctx* ctx, hawkes_tree* tree, int64_t n, const double* x, const double* t, int64_t m,
                        const int64_t* idx, const double* z, double beta, const hawkes_params* p /*HOST*/,
                        double sigma2, double tau0, double* out3, double* grad_z, double* hess_z, void* stream);
